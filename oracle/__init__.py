@@ -1,0 +1,409 @@
+"""fp64 CPU oracle for the MMC hot path of arXiv:2106.05593 -- TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s ``cpu_baseline`` / ``--impl reference``
+legs may import this package.  It shares no code with ``paper_2106_05593_b200`` (the CUDA path)
+and neither imports the other.  The arithmetic lives in ``mmc_oracle.c`` (plain C, fp64, one cell
+at a time, the paper's order); this module only builds it with gcc, marshals numpy arrays, does the
+per-class thermal set-up bookkeeping, and provides the zero-padded FFT convolution of Eq. (14) with
+``numpy.fft`` as the library step.
+
+Parity pins (tests/test_oracle_*.py, ``-m "not gpu"``): Philox known answers; thermal functions vs
+series / Curie-Weiss / SURVEY probe values; trial-move geometry; single-cell Langevin <cos> and
+length-distribution quadrature; local dF == global dE by brute force; detailed-balance ratio;
+colour-order independence; Newell invariants + independent 6-D quadrature; FFT == direct sum.
+Unpinned (stated in DESIGN.md): equilibrium of coupled meshes with exchange+DMI+demag against any
+external value -- "parity unpinned" for that item only.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass, field
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "mmc_oracle.c")
+_LIB = os.path.join(_HERE, "libmmc_oracle.so")
+
+KB = 1.380649e-23
+MU0 = 4e-7 * np.pi
+MUB = 9.2740100783e-24
+
+
+def build(force: bool = False) -> str:
+    """Compile mmc_oracle.c with gcc (-O2, OpenMP, libquadmath).  Building is not using."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=gnu11", "-fPIC", "-shared", "-fopenmp", "-ffp-contract=off",
+               _SRC, "-o", _LIB, "-lquadmath", "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+class _Problem(C.Structure):
+    _fields_ = [
+        ("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("pbc", C.c_uint32),
+        ("dx", C.c_double), ("dy", C.c_double), ("dz", C.c_double),
+        ("active", C.c_void_p), ("region", C.c_void_p), ("inter_region_exchange", C.c_int32),
+        ("Ms0", C.c_void_p), ("beta", C.c_void_p),
+        ("c2", C.c_void_p), ("c4", C.c_void_p), ("c0", C.c_void_p),
+        ("Kq", C.c_void_p), ("K1T", C.c_void_p),
+        ("ax", C.c_void_p), ("ay", C.c_void_p), ("az", C.c_void_p),
+        ("sigma", C.c_void_p),
+        ("A0", C.c_double), ("D0", C.c_double), ("Bext", C.c_double * 3),
+        ("bdx", C.c_void_p), ("bdy", C.c_void_p), ("bdz", C.c_void_p),
+        ("one_minus_cos_cone", C.c_double), ("seed", C.c_uint64),
+    ]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(build())
+        dp = C.POINTER(C.c_double)
+        L.orc_philox4x32_10.argtypes = [C.POINTER(C.c_uint32)] * 3
+        L.orc_u01.restype = C.c_double; L.orc_u01.argtypes = [C.c_uint32]
+        L.orc_cell_uniforms.argtypes = [C.c_uint64, C.c_uint64, C.c_uint64, dp]
+        for name in ("orc_langevin", "orc_langevin_prime"):
+            getattr(L, name).restype = C.c_double; getattr(L, name).argtypes = [C.c_double]
+        L.orc_me.restype = C.c_double; L.orc_me.argtypes = [C.c_double, C.c_double]
+        L.orc_chi_par.restype = C.c_double; L.orc_chi_par.argtypes = [C.c_double] * 4
+        L.orc_thermal.restype = C.c_int; L.orc_thermal.argtypes = [C.c_double] * 5 + [dp]
+        L.orc_trial.argtypes = [dp, dp, C.c_double, C.c_double, dp, dp]
+        L.orc_cell_dF.argtypes = [C.POINTER(_Problem), dp, dp, dp, C.c_int, C.c_int, C.c_int, dp, dp]
+        L.orc_colour_pass.restype = C.c_int64
+        L.orc_colour_pass.argtypes = [C.POINTER(_Problem), dp, dp, dp, C.c_int, C.c_uint64,
+                                      C.c_void_p, C.c_int64, C.c_int,
+                                      C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+        L.orc_observables.argtypes = [C.POINTER(_Problem), dp, dp, dp, dp, dp, C.POINTER(C.c_int64)]
+        L.orc_newell.argtypes = [C.c_double] * 6 + [dp]
+        L.orc_demag_tensor.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [C.c_int, dp]
+        L.orc_demag_direct.argtypes = [C.c_int] * 3 + [dp] * 7
+        _lib = L
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+# ----------------------------------------------------------------------------- scalar helpers
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr); k = (C.c_uint32 * 2)(*key); o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return tuple(int(x) for x in o)
+
+
+def u01(x: int) -> float:
+    return lib().orc_u01(x)
+
+
+def cell_uniforms(seed: int, sweep: int, cell: int):
+    u = np.zeros(4)
+    lib().orc_cell_uniforms(seed, sweep, cell, _dp(u))
+    return u
+
+
+def langevin(x): return lib().orc_langevin(float(x))
+def langevin_prime(x): return lib().orc_langevin_prime(float(x))
+def me_of_T(T, Tc): return lib().orc_me(float(T), float(Tc))
+def chi_par(T, Tc, mu, me): return lib().orc_chi_par(float(T), float(Tc), float(mu), float(me))
+
+
+def thermal(T, Tc, mu, V, Ms0):
+    """-> dict(me, chi, c2, c4, c0, sigma13); Eq. (7),(8),(9),(13)."""
+    o = np.zeros(6)
+    if lib().orc_thermal(float(T), float(Tc), float(mu), float(V), float(Ms0), _dp(o)) != 0:
+        raise ValueError("T must be > 0")
+    return dict(me=o[0], chi=o[1], c2=o[2], c4=o[3], c0=o[4], sigma13=o[5])
+
+
+def trial(m, u3, one_minus_cos_cone, sigma):
+    m = np.ascontiguousarray(m, dtype=np.float64); u3 = np.ascontiguousarray(u3, dtype=np.float64)
+    dm = np.zeros(3); f = C.c_double()
+    lib().orc_trial(_dp(m), _dp(u3), float(one_minus_cos_cone), float(sigma), _dp(dm), C.byref(f))
+    return dm, f.value
+
+
+def newell(X, Y, Z, dx, dy, dz):
+    o = np.zeros(6)
+    lib().orc_newell(float(X), float(Y), float(Z), float(dx), float(dy), float(dz), _dp(o))
+    return o
+
+
+def demag_tensor(nx, ny, nz, dx, dy, dz, r_near=32):
+    """Octant table [6, nz, ny, nx] (xx,yy,zz,xy,xz,yz) for offsets >= 0."""
+    out = np.zeros((6, nz, ny, nx))
+    lib().orc_demag_tensor(nx, ny, nz, float(dx), float(dy), float(dz), int(r_near), _dp(out))
+    return out
+
+
+def demag_direct(tab, Mx, My, Mz):
+    """B_d = -mu0 sum_j N(r_i-r_j) M_j by the O(N^2) sum (Eq. (14)); arrays shaped [nz, ny, nx]."""
+    _, nz, ny, nx = tab.shape
+    Mx, My, Mz = (np.ascontiguousarray(a, dtype=np.float64) for a in (Mx, My, Mz))
+    b = [np.zeros((nz, ny, nx)) for _ in range(3)]
+    lib().orc_demag_direct(nx, ny, nz, _dp(tab), _dp(Mx), _dp(My), _dp(Mz), _dp(b[0]), _dp(b[1]), _dp(b[2]))
+    return b
+
+
+def _full_kernel(tab):
+    """Place the octant table on the zero-padded periodic grid: offset o_d, |o_d|<N_d,
+    stored at index o_d mod P_d, P_d = 2 N_d (P_d = 1 when N_d = 1); index N_d left zero.  Diagonal
+    components are even in every coordinate, N_ab (a != b) is odd in coordinates a and b."""
+    _, nz, ny, nx = tab.shape
+    P = [1 if n == 1 else 2 * n for n in (nz, ny, nx)]
+    full = np.zeros((6, P[0], P[1], P[2]))
+    par = {0: (1, 1, 1), 1: (1, 1, 1), 2: (1, 1, 1), 3: (1, -1, -1), 4: (-1, 1, -1), 5: (-1, -1, 1)}  # (z,y,x) signs
+    for sz_ in ((1, -1) if nz > 1 else (1,)):
+        for sy_ in ((1, -1) if ny > 1 else (1,)):
+            for sx_ in ((1, -1) if nx > 1 else (1,)):
+                oz = np.arange(nz) if sz_ > 0 else np.arange(1, nz)
+                oy = np.arange(ny) if sy_ > 0 else np.arange(1, ny)
+                ox = np.arange(nx) if sx_ > 0 else np.arange(1, nx)
+                if oz.size == 0 or oy.size == 0 or ox.size == 0:
+                    continue
+                for q in range(6):
+                    pz, py, px = par[q]
+                    sgn = (pz if sz_ < 0 else 1) * (py if sy_ < 0 else 1) * (px if sx_ < 0 else 1)
+                    full[q][np.ix_((sz_ * oz) % P[0], (sy_ * oy) % P[1], (sx_ * ox) % P[2])] = sgn * tab[q][np.ix_(oz, oy, ox)]
+    return full
+
+
+class DemagFFT:
+    """Zero-padded FFT convolution of Eq. (14) in fp64 with numpy.fft."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, r_near=32):
+        self.shape = (nz, ny, nx)
+        self.tab = demag_tensor(nx, ny, nz, dx, dy, dz, r_near)
+        full = _full_kernel(self.tab)
+        self.P = full.shape[1:]
+        self.Khat = np.fft.rfftn(full, axes=(1, 2, 3))
+
+    def field(self, Mx, My, Mz):
+        """B_d (tesla), arrays [nz, ny, nx]; M = Ms0 m in A/m, zero in empty cells."""
+        nz, ny, nx = self.shape
+        Mh = []
+        for a in (Mx, My, Mz):
+            pad = np.zeros(self.P); pad[:nz, :ny, :nx] = a
+            Mh.append(np.fft.rfftn(pad))
+        K = self.Khat
+        Hx = -(K[0] * Mh[0] + K[3] * Mh[1] + K[4] * Mh[2])
+        Hy = -(K[3] * Mh[0] + K[1] * Mh[1] + K[5] * Mh[2])
+        Hz = -(K[4] * Mh[0] + K[5] * Mh[1] + K[2] * Mh[2])
+        return [MU0 * np.fft.irfftn(H, s=self.P, axes=(0, 1, 2))[:nz, :ny, :nx] for H in (Hx, Hy, Hz)]
+
+
+# ----------------------------------------------------------------------------- the MMC oracle
+@dataclass
+class Material:
+    Ms0: float = 0.0; A0: float = 0.0; K1: float = 0.0
+    ax: float = 0.0; ay: float = 0.0; az: float = 1.0
+    D0: float = 0.0; Tc: float = 1.0; mu_atom: float = MUB
+
+
+class OracleMMC:
+    """Step-by-step fp64 MMC.  State m is kept in float64; with
+    ``store_fp32=True`` accepted vectors are rounded to fp32, the GPU's storage format."""
+
+    def __init__(self, nx, ny, nz, dx, dy, dz, pbc_mask=0, store_fp32=True):
+        self.nx, self.ny, self.nz = nx, ny, nz
+        self.dx, self.dy, self.dz = dx, dy, dz
+        self.pbc = pbc_mask
+        for a, n in enumerate((nx, ny, nz)):
+            if (pbc_mask >> a) & 1 and n % 2:
+                raise ValueError("periodic dimension must have even length (O6)")
+        self.N = nx * ny * nz
+        self.V = dx * dy * dz
+        self.store_fp32 = store_fp32
+        self.regions = [Material()]
+        self.region_of_cell = np.zeros(self.N, dtype=np.int32)
+        self.inter_region_exchange = 1
+        self.T_cell = np.full(self.N, 300.0)
+        self.Bext = np.zeros(3)
+        self.cone_deg = 30.0
+        self.sigma_user = -1.0
+        self.adaptive = False
+        self.demag_enabled = False
+        self.demag_updates = 1
+        self.demag_r_near = 32
+        self._demag = None
+        self.seed = 0
+        self.sweep = 0
+        self.accepted = 0; self.trials = 0
+        self._win_acc = 0; self._win_tri = 0; self._win_sweeps = 0
+        self.m = [np.zeros(self.N) for _ in range(3)]
+        self.bd = None
+        self._dirty = True
+
+    # -- set-up ---------------------------------------------------------------------------
+    def set_material(self, regions, region_of_cell=None):
+        self.regions = list(regions)
+        self.region_of_cell = (np.zeros(self.N, dtype=np.int32) if region_of_cell is None
+                               else np.ascontiguousarray(region_of_cell, dtype=np.int32).ravel())
+        self._dirty = True
+
+    def set_exchange_coupling(self, inter_region_exchange):
+        self.inter_region_exchange = int(inter_region_exchange); self._dirty = True
+
+    def set_temperature(self, T_uniform, T_per_cell=None):
+        self.T_cell = (np.full(self.N, float(T_uniform)) if T_per_cell is None
+                       else np.ascontiguousarray(T_per_cell, dtype=np.float32).astype(np.float64).ravel())
+        self._dirty = True
+
+    def set_field(self, Bx, By, Bz):
+        self.Bext = np.array([Bx, By, Bz], dtype=np.float64)
+
+    def set_move(self, cone_deg, sigma=-1.0, adaptive_cone=False):
+        self.cone_deg = float(cone_deg); self.sigma_user = float(sigma); self.adaptive = bool(adaptive_cone)
+        self._dirty = True
+
+    def set_demag(self, enabled, updates_per_sweep=1, r_near=32):
+        self.demag_enabled = bool(enabled); self.demag_updates = int(updates_per_sweep)
+        self.demag_r_near = r_near
+
+    def set_seed(self, seed): self.seed = int(seed)
+    def set_sweep_counter(self, s): self.sweep = int(s)
+
+    def set_m(self, mx, my, mz):
+        self.m = [np.ascontiguousarray(np.asarray(a, dtype=np.float32).astype(np.float64).ravel()) for a in (mx, my, mz)]
+
+    def get_m(self):
+        return [a.copy() for a in self.m]
+
+    def _setup(self):
+        """O1: per-cell coefficients; one thermal solve per distinct (region, T) class."""
+        if not self._dirty:
+            return
+        N = self.N
+        reg = self.region_of_cell
+        Ms0r = np.array([r.Ms0 for r in self.regions])
+        self.active = np.ascontiguousarray((Ms0r[reg] > 0).astype(np.uint8))
+        act_regs = [r for r in self.regions if r.Ms0 > 0]
+        A0s = {r.A0 for r in act_regs}; D0s = {r.D0 for r in act_regs}
+        if len(A0s) > 1 or len(D0s) > 1:
+            raise ValueError("A0 and D0 must be uniform over non-empty regions")
+        self.A0 = A0s.pop() if A0s else 0.0
+        self.D0 = D0s.pop() if D0s else 0.0
+        names = ("Ms0", "beta", "c2", "c4", "c0", "Kq", "K1T", "ax", "ay", "az", "sigma", "me")
+        arr = {k: np.zeros(N) for k in names}
+        arr["az"][:] = 1.0; arr["beta"][:] = 1.0
+        key = reg.astype(np.int64) * (1 << 32) + self.T_cell.astype(np.float32).view(np.uint32).astype(np.int64)
+        uniq, inv = np.unique(key, return_inverse=True)
+        cls = {k: np.zeros(uniq.size) for k in names}
+        first = np.zeros(uniq.size, dtype=np.int64)
+        first[inv[::-1]] = np.arange(N - 1, -1, -1)
+        for q in range(uniq.size):
+            c = first[q]; r = self.regions[reg[c]]; T = self.T_cell[c]
+            cls["beta"][q] = 1.0 / (KB * T) if T > 0 else np.nan
+            if r.Ms0 <= 0:
+                cls["az"][q] = 1.0
+                continue
+            if not (T > 0):
+                raise ValueError("T <= 0")
+            th = thermal(T, r.Tc, r.mu_atom, self.V, r.Ms0)
+            al = np.sqrt(r.ax ** 2 + r.ay ** 2 + r.az ** 2) or 1.0
+            cls["Ms0"][q] = r.Ms0; cls["c2"][q] = th["c2"]; cls["c4"][q] = th["c4"]; cls["c0"][q] = th["c0"]
+            cls["Kq"][q] = r.K1 * th["me"]; cls["K1T"][q] = r.K1 * th["me"] ** 3
+            cls["ax"][q], cls["ay"][q], cls["az"][q] = r.ax / al, r.ay / al, r.az / al
+            cls["sigma"][q] = self.sigma_user if self.sigma_user >= 0 else th["sigma13"]
+            cls["me"][q] = th["me"]
+        for k in names:
+            arr[k] = np.ascontiguousarray(cls[k][inv])
+        self.coef = arr
+        self._dirty = False
+
+    def _problem(self):
+        self._setup()
+        p = _Problem()
+        p.nx, p.ny, p.nz, p.pbc = self.nx, self.ny, self.nz, self.pbc
+        p.dx, p.dy, p.dz = self.dx, self.dy, self.dz
+        p.active = self.active.ctypes.data
+        p.region = self.region_of_cell.ctypes.data
+        p.inter_region_exchange = self.inter_region_exchange
+        for k in ("Ms0", "beta", "c2", "c4", "c0", "Kq", "K1T", "ax", "ay", "az", "sigma"):
+            setattr(p, k, self.coef[k].ctypes.data)
+        p.A0, p.D0 = self.A0, self.D0
+        p.Bext = (C.c_double * 3)(*self.Bext)
+        if self.demag_enabled and self.bd is not None:
+            p.bdx, p.bdy, p.bdz = (b.ctypes.data for b in self.bd)
+        else:
+            p.bdx = p.bdy = p.bdz = None
+        p.one_minus_cos_cone = 2.0 * np.sin(0.5 * np.deg2rad(self.cone_deg)) ** 2
+        p.seed = self.seed
+        return p
+
+    # -- demag ----------------------------------------------------------------------------
+    def demag_field(self):
+        """B_d (tesla) of the current state, three flat arrays (Eq. (14))."""
+        self._setup()
+        if self._demag is None:
+            self._demag = DemagFFT(self.nx, self.ny, self.nz, self.dx, self.dy, self.dz, self.demag_r_near)
+        sh = (self.nz, self.ny, self.nx)
+        M = [(self.coef["Ms0"] * a).reshape(sh) for a in self.m]
+        return [np.ascontiguousarray(b.ravel()) for b in self._demag.field(*M)]
+
+    # -- iteration --------------------------------------------------------------------------
+    def colour_pass(self, colour, dump=False, order=None):
+        """One colour pass at the current sweep counter (does not advance it).  With dump=True
+        returns dict(dm[N,3], terms[N,6], margin[N], accepted[N])."""
+        p = self._problem()
+        N = self.N
+        d = None
+        ptrs = [None] * 4
+        if dump:
+            d = dict(dm=np.zeros((N, 3)), terms=np.zeros((N, 6)), margin=np.full(N, np.nan), accepted=np.zeros(N, dtype=np.uint8))
+            ptrs = [d["dm"].ctypes.data, d["terms"].ctypes.data, d["margin"].ctypes.data, d["accepted"].ctypes.data]
+        tri = C.c_int64()
+        if order is not None:
+            order = np.ascontiguousarray(order, dtype=np.int64)
+        acc = lib().orc_colour_pass(C.byref(p), _dp(self.m[0]), _dp(self.m[1]), _dp(self.m[2]), int(colour),
+                                    self.sweep, None if order is None else order.ctypes.data,
+                                    0 if order is None else order.size, int(self.store_fp32),
+                                    *ptrs, C.byref(tri))
+        self.accepted += acc; self.trials += tri.value
+        self._win_acc += acc; self._win_tri += tri.value
+        return d
+
+    def sweep_once(self):
+        """O6: [demag] -> red -> [demag iff updates_per_sweep == 2] -> black -> counter++; then S11."""
+        if self.demag_enabled:
+            self.bd = self.demag_field()
+        self.colour_pass(0)
+        if self.demag_enabled and self.demag_updates == 2:
+            self.bd = self.demag_field()
+        self.colour_pass(1)
+        self.sweep += 1
+        self._win_sweeps += 1
+        if self._win_sweeps == 100:
+            # PAPER.md:100 + reading G11: every 100 iterations, +-1 deg outside 0.5 +- 0.05, clamp [1, 180]
+            if self.adaptive and self._win_tri > 0:
+                rate = self._win_acc / self._win_tri
+                if rate > 0.55: self.cone_deg = min(180.0, self.cone_deg + 1.0)
+                elif rate < 0.45: self.cone_deg = max(1.0, self.cone_deg - 1.0)
+            self._win_acc = self._win_tri = self._win_sweeps = 0
+
+    def run(self, n_sweeps):
+        for _ in range(n_sweeps):
+            self.sweep_once()
+
+    def cell_dF(self, i, j, k, dm):
+        p = self._problem()
+        t = np.zeros(6); dm = np.ascontiguousarray(dm, dtype=np.float64)
+        lib().orc_cell_dF(C.byref(p), _dp(self.m[0]), _dp(self.m[1]), _dp(self.m[2]), i, j, k, _dp(dm), _dp(t))
+        return t
+
+    def observables(self):
+        """O8.  Energies in joule; E_demag uses the field of the *current* state."""
+        if self.demag_enabled:
+            self.bd = self.demag_field()
+        p = self._problem()
+        E = np.zeros(6); mean = np.zeros(4); na = C.c_int64()
+        lib().orc_observables(C.byref(p), _dp(self.m[0]), _dp(self.m[1]), _dp(self.m[2]), _dp(E), _dp(mean), C.byref(na))
+        return dict(mean_m=mean[:3].copy(), mean_len=mean[3], E_ex=E[0], E_an=E[1], E_zee=E[2], E_dmi=E[3],
+                    E_demag=E[4], E_long=E[5], accepted=self.accepted, trials=self.trials,
+                    sweeps_done=self.sweep, cone_deg=self.cone_deg, n_active=na.value)

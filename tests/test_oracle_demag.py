@@ -1,0 +1,155 @@
+"""Pins of the oracle's demagnetising path (Eq. (14))."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle as O
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rows(name):
+    with open(os.path.join(GOLD, name)) as f:
+        return [ln.split() for ln in f if ln.strip() and not ln.startswith("#")]
+
+
+def test_newell_probe_values():
+    for r in _rows("newell_probe.txt"):
+        v = [float(x) for x in r]
+        assert np.allclose(O.newell(*v[:6]), v[6:12], rtol=2e-11, atol=1e-15)
+
+
+def test_newell_trace_and_symmetry():
+    """Self term of a cube = 1/3 each, trace 1 at the origin and 0 elsewhere (div B = 0); off-diagonals vanish on
+    the coordinate planes; diagonal components even, N_ab odd in a and b."""
+    d = (1.0, 0.7, 1.9)
+    n0 = O.newell(0, 0, 0, *d)
+    assert n0[:3].sum() == pytest.approx(1.0, abs=1e-15) and np.all(np.abs(n0[3:]) < 1e-30)
+    assert np.allclose(O.newell(0, 0, 0, 2, 2, 2)[:3], 1 / 3, atol=1e-16)
+    rng = np.random.default_rng(0)
+    for _ in range(20):
+        o = rng.integers(-6, 7, 3)
+        if not o.any():
+            continue
+        X, Y, Z = o * np.array(d)
+        n = O.newell(X, Y, Z, *d)
+        assert abs(n[:3].sum()) < 1e-16
+        nm = O.newell(-X, Y, Z, *d)
+        assert np.allclose(nm, n * np.array([1, 1, 1, -1, -1, 1]), rtol=1e-13, atol=1e-30)
+        if o[2] == 0:
+            assert abs(n[4]) < 1e-30 and abs(n[5]) < 1e-30            # N_xz = N_yz = 0 at Z = 0
+
+
+def _quad_tensor(R, d, n=10):
+    """Independent definition: N_ab(R) = (1/V) int_cell int_cell K_ab(R + u - v) du dv,
+    K_ab = (1/4 pi)(delta_ab/r^3 - 3 r_a r_b/r^5); u - v has a triangular weight (d - |w|) per axis;
+    Gauss-Legendre on [-d, 0] and [0, d]."""
+    x, w = np.polynomial.legendre.leggauss(n)
+    axes = []
+    for da in d:
+        pts = np.concatenate([-da / 2 + da / 2 * x, da / 2 + da / 2 * x])
+        wts = np.concatenate([w, w]) * da / 2 * (da - np.abs(pts))
+        axes.append((pts, wts))
+    WX, WY, WZ = np.meshgrid(axes[0][0], axes[1][0], axes[2][0], indexing="ij")
+    wt = axes[0][1][:, None, None] * axes[1][1][None, :, None] * axes[2][1][None, None, :]
+    rx, ry, rz = R[0] + WX, R[1] + WY, R[2] + WZ
+    r2 = rx * rx + ry * ry + rz * rz; r5 = r2 ** 2.5
+    V = d[0] * d[1] * d[2]
+    f = lambda a, b, dl: ((dl * r2 - 3 * a * b) / r5 * wt).sum() / (4 * np.pi * V)
+    return np.array([f(rx, rx, 1), f(ry, ry, 1), f(rz, rz, 1), f(rx, ry, 0), f(rx, rz, 0), f(ry, rz, 0)])
+
+
+@pytest.mark.parametrize("off,d", [((3, 2, 1), (1, 1, 1)), ((2, 0, 0), (1, 1, 1)), ((0, 2, 1), (1, 1, 1)),
+                                   ((2, 1, 0), (1, 1, 2)), ((0, 0, 2), (1, 1, 2)), ((1, 2, 1), (1, 1, 2)),
+                                   ((4, -3, 2), (5e-9, 4e-9, 3e-9))])
+def test_newell_against_6d_quadrature(off, d):
+    R = np.array(off, float) * np.array(d)
+    ref = _quad_tensor(R, d, n=14)
+    got = O.newell(*R, *d)
+    assert np.allclose(got, ref, rtol=2e-7, atol=2e-9 * np.abs(ref).max())
+
+
+def test_newell_composition_identity():
+    """The mean of N over all cell pairs of a uniformly magnetised block equals the self term of the block taken
+    as one big cell (SURVEY pin: two stacked cubes 1/3 - 0.135017180544 = 0.198316152789; 6x5x2 block)."""
+    two = O.newell(0, 0, 0, 1, 1, 2)[2]
+    assert two == pytest.approx(1 / 3 + O.newell(0, 0, 1, 1, 1, 1)[2], rel=1e-13)
+    nx, ny, nz = 6, 5, 2
+    acc = np.zeros(6)
+    for ox in range(-nx + 1, nx):
+        for oy in range(-ny + 1, ny):
+            for oz in range(-nz + 1, nz):
+                cnt = (nx - abs(ox)) * (ny - abs(oy)) * (nz - abs(oz))
+                acc += cnt * O.newell(ox, oy, oz, 1, 1, 1)
+    acc /= nx * ny * nz
+    big = O.newell(0, 0, 0, nx, ny, nz)
+    assert np.allclose(acc, big, rtol=1e-12, atol=1e-15)
+    assert big[2] == pytest.approx(0.56805647309712, rel=1e-11)
+
+
+@pytest.mark.parametrize("d", [(5e-9, 5e-9, 5e-9), (5e-9, 5e-9, 10e-9)])
+def test_far_field_matches_newell_beyond_r_near(d):
+    """Sub-cube dipole average (O7) vs the binary128 Newell value where the two are stitched."""
+    tab_far = O.demag_tensor(40, 40, 3, *d, r_near=32)
+    tab_all = O.demag_tensor(40, 40, 3, *d, r_near=1000)
+    far = np.zeros((3, 40, 40), bool); far[:, 33:, :] = True; far[:, :, 33:] = True
+    scale = np.abs(tab_all[:3][:, far]).max()
+    assert np.abs(tab_far - tab_all)[:, far].max() < 3e-6 * scale
+    assert np.array_equal(tab_far[:, ~far], tab_all[:, ~far])
+
+
+@pytest.mark.parametrize("shape,d", [((8, 6, 1), (5e-9, 5e-9, 5e-9)), ((5, 4, 3), (3e-9, 3e-9, 3e-9)),
+                                     ((6, 7, 1), (5e-9, 5e-9, 10e-9)), ((4, 4, 2), (2e-9, 3e-9, 4e-9))])
+def test_fft_convolution_equals_direct_sum(shape, d):
+    nx, ny, nz = shape
+    rng = np.random.default_rng(nx * 100 + ny * 10 + nz)
+    M = rng.normal(size=(3, nz, ny, nx)) * 8e5
+    M[:, rng.uniform(size=(nz, ny, nx)) < 0.25] = 0.0                    # empty cells
+    conv = O.DemagFFT(nx, ny, nz, *d)
+    b_fft = conv.field(*M)
+    b_dir = O.demag_direct(conv.tab, *M)
+    scale = max(np.abs(b).max() for b in b_dir)
+    for a in range(3):
+        assert np.abs(b_fft[a] - b_dir[a]).max() < 1e-13 * scale
+    # the spectrum of the tensor is real (even/odd-odd symmetry of N)
+    assert np.abs(conv.Khat.imag).max() < 1e-13 * np.abs(conv.Khat.real).max()
+
+
+def test_uniform_block_field_is_minus_block_tensor_times_M():
+    """Thin-film limit check through the whole path: a uniformly magnetised 12x10x1 block of cubes has
+    mean H_d = -N_block M with N_block the Newell self term of the 12x10x1 cuboid; for M || z this is the
+    perpendicular-film shape anisotropy that Figs. 3-6 rely on."""
+    nx, ny, nz, h = 12, 10, 1, 5e-9
+    conv = O.DemagFFT(nx, ny, nz, h, h, h)
+    Nblk = O.newell(0, 0, 0, nx * h, ny * h, nz * h)
+    for a in range(3):
+        M = np.zeros((3, nz, ny, nx)); M[a] = 8e5
+        b = conv.field(*M)
+        for q in range(3):
+            expect = -O.MU0 * 8e5 * (Nblk[a] if q == a else 0.0)
+            assert b[q].mean() == pytest.approx(expect, abs=1e-12 * O.MU0 * 8e5)
+    assert Nblk[2] > 0.8 and Nblk[0] < 0.1
+
+
+def test_oracle_sweep_uses_frozen_field_once_per_iteration():
+    """field computed at the start of the iteration, not updated on accept; optional second
+    update before the black pass (updates_per_sweep = 2)."""
+    nx = ny = 8
+    rng = np.random.default_rng(3)
+    v = rng.normal(size=(3, nx * ny)); v /= np.linalg.norm(v, axis=0)
+    out = {}
+    for upd in (1, 2):
+        s = O.OracleMMC(nx, ny, 1, 5e-9, 5e-9, 5e-9, pbc_mask=0)
+        s.set_material([O.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)]); s.set_temperature(300.0)
+        s.set_move(20.0, -1.0, False); s.set_demag(True, upd); s.set_seed(5)
+        s.set_m(*(0.8675 * v).astype(np.float32))
+        b0 = s.demag_field()
+        s.sweep_once()
+        out[upd] = np.stack(s.m)
+        if upd == 1:
+            assert all(np.array_equal(s.bd[a], b0[a]) for a in range(3))     # still the start-of-iteration field
+        else:
+            assert not np.array_equal(s.bd[0], b0[0])
+    red = np.array([(c % nx + c // nx) % 2 == 0 for c in range(nx * ny)])
+    assert np.array_equal(out[1][:, red], out[2][:, red])                    # red pass saw the same field
