@@ -1,0 +1,280 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the MMC hot path (cell updates/s) on synthetic meshes shaped like BASELINE.json's configs.
+
+    python bench.py --gpus N --steps K --warmup W [--config 1..5] [--impl reference]
+
+A "step" is one whole MMC iteration of the hot path: demag pack/pad -> forward FFT -> tensor multiply ->
+inverse FFT + crop -> red colour pass -> black colour pass -> end-of-sweep bookkeeping (acceptance counters, running
+means, cone controller).  `value` = (non-empty cells x steps) / device time, inputs resident in HBM; `e2e` = the same
+through the C ABI with HOST buffers (pinned H2D of m before and D2H of m + observables after every step).
+Multi-GPU: every rank runs an independent replica (own seed), no data-path collective;
+value = total updates of all ranks / max-over-ranks device time.
+`--impl reference` times the fp64 CPU oracle as it stands on the host cores on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "cell_updates_per_sec"
+UNIT = "cell updates/s"
+# algorithmic (compulsory) bytes per cell update of the colour pass: own m read 12 + write 12,
+# B_d 12 (demag configs), mask 1 (cfg 4, 5), per-cell coefficients 28 (cfg 4)
+ALGO_BYTES_PER_UPDATE = {1: 24, 2: 36, 3: 36, 4: 65, 5: 37}
+
+
+def replica_seed(base_seed: int, rank: int) -> int:
+    """Independent replica per rank: distinct Philox key, same workload."""
+    return (int(base_seed) + 0x9E3779B97F4A7C15 * int(rank)) & 0xFFFFFFFFFFFFFFFF
+
+
+def aggregate_over_ranks(units: float, seconds: float, backend_device: str = "cuda") -> float:
+    """value = units of all ranks / max-over-ranks time (the contract's whole-job aggregate)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return units / seconds
+    t = torch.tensor([units], dtype=torch.float64, device=backend_device)
+    s = torch.tensor([seconds], dtype=torch.float64, device=backend_device)
+    dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    dist.all_reduce(s, op=dist.ReduceOp.MAX)
+    return float(t.item() / s.item())
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index=0):
+        self.rows = []; self.proc = None; self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                          "-i", str(self.gpu)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True); self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.rows.append(ln.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            p = [x.strip() for x in r.split(",")]
+            if len(p) < 9:
+                continue
+            try:
+                sm.append(float(p[1])); mx.append(float(p[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), p[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def _workload(cfg: int, small: bool):
+    import workloads as W
+    if small:
+        kw = {1: {}, 2: dict(nx=64, ny=64), 3: dict(nx=64, ny=64), 4: dict(nx=64, ny=64, nz=4), 5: dict(nx=140, ny=140)}[cfg]
+        return W.make(cfg, **kw)
+    return W.make(cfg)
+
+
+# ------------------------------------------------------------------------------------------------ oracle arm
+def oracle_sample(cfg: int):
+    """Bounded sample of config `cfg` for the CPU legs: same recipe, reduced mesh."""
+    import workloads as W
+    kw = {1: {}, 2: {}, 3: dict(nx=256, ny=256), 4: dict(nx=256, ny=256, nz=4), 5: dict(nx=560, ny=560)}[cfg]
+    return W.make(cfg, **kw), kw
+
+
+def time_oracle(cfg: int, steps: int, warmup: int):
+    import oracle as O
+    import workloads as W
+    wl, kw = oracle_sample(cfg)
+    wl.adaptive_cone = False
+    o = O.OracleMMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, store_fp32=True)
+    W.configure(o, wl, O.Material)
+    if wl.demag:
+        o.demag_field()                       # tensor set-up outside the timed region (as on the GPU side)
+    o.run(max(1, warmup))
+    t0 = time.perf_counter()
+    o.run(steps)
+    dt = time.perf_counter() - t0
+    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    sample = f"{wl.name} recipe on a {wl.nx}x{wl.ny}x{wl.nz} mesh ({wl.n_active} non-empty cells), {steps} iterations incl. numpy.fft demag"
+    return wl.n_active * steps / dt, dt, cores, sample
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    steps = max(1, args.steps); warm = max(1, args.warmup)
+    v, dt, cores, sample = time_oracle(args.config, steps, warm)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warm,
+            "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "config": {"workload": f"cfg{args.config} (oracle sample: {sample})"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1")); rank = int(os.environ.get("RANK", "0")); local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    import paper_2106_05593_b200 as P
+    import workloads as W
+    cfg = args.config
+    wl = _workload(cfg, args.small)
+    wl.adaptive_cone = False                      # fixed cone/sigma for throughput runs (SURVEY 8(d) timing protocol)
+    wl.seed = replica_seed(wl.seed, rank)
+    g = P.MMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, device=local)
+    W.configure(g, wl, P.Material)
+    K, Wm = max(1, args.steps), max(3, args.warmup)
+    dev = torch.device("cuda", local)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    g.sweep(Wm)                                   # warm-up (also builds the demag plan and tensor spectrum)
+    barrier()
+    sampler = ClockSampler(local); sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    phases = g.sweep_timed(K)                     # K iterations, per-phase CUDA events on the launching stream
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    units = float(wl.n_active) * K
+    value = aggregate_over_ranks(units, ms * 1e-3)
+    ob = g.observables()
+
+    # e2e through the C ABI with host buffers: pinned H2D of the step's m, one iteration, D2H of m + observables
+    nE = max(3, min(K, 20))
+    host_in = [torch.from_numpy(np.ascontiguousarray(wl.m0[a])).pin_memory() for a in range(3)]
+    host_out = [torch.empty(wl.N, dtype=torch.float32).pin_memory() for _ in range(3)]
+    dbuf = [torch.empty(wl.N, dtype=torch.float32, device=dev) for _ in range(3)]
+    L = P.lib()
+    obs = P.Obs()
+
+    def e2e_step():
+        for a in range(3):
+            dbuf[a].copy_(host_in[a], non_blocking=True)
+        g._ck(L.mmc_set_m(g._h, dbuf[0].data_ptr(), dbuf[1].data_ptr(), dbuf[2].data_ptr()))
+        g._ck(L.mmc_sweep(g._h, 1))
+        g._ck(L.mmc_get_m(g._h, dbuf[0].data_ptr(), dbuf[1].data_ptr(), dbuf[2].data_ptr()))
+        for a in range(3):
+            host_out[a].copy_(dbuf[a], non_blocking=True)
+        g._ck(L.mmc_get_observables(g._h, P.C.byref(obs)))      # synchronises; D2H of the read-out struct
+
+    e2e_step(); barrier()
+    t0 = time.perf_counter()
+    for _ in range(nE):
+        e2e_step()
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    e2e_val = aggregate_over_ranks(float(wl.n_active) * nE, e2e_s)
+    h2d = 3 * wl.N * 4; d2h = 3 * wl.N * 4 + P.C.sizeof(P.Obs)
+
+    if rank == 0:
+        peak, peak_src = _peaks()
+        step_ms = sum(phases.values()) / K
+        # dominant kernel among OUR kernels (the two cuFFT legs are library code in this round): the colour pass
+        own = {k: v for k, v in phases.items() if k not in ("fft_fwd", "fft_inv")}
+        pass_ms = (phases["red"] + phases["black"]) / (2 * K)
+        algo_bytes = ALGO_BYTES_PER_UPDATE[cfg] * (wl.n_active / 2.0)
+        achieved = algo_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{wl.name} {wl.nx}x{wl.ny}x{wl.nz} ({wl.n_active} non-empty cells)", "cfg": cfg,
+                       "step": "1 MMC iteration = demag FFT convolution + red + black colour pass + bookkeeping",
+                       "l2": "working set (state + coefficients + FFT buffers) exceeds the 126 MB L2" if wl.N >= 2 ** 22 else
+                             "working set fits L2 (small config); every iteration still streams the FFT buffers",
+                       "parallelism": "replicas" if world > 1 else "single GPU", "cone_deg": wl.cone_deg,
+                       "acceptance": ob["accepted"] / max(1, ob["trials"])},
+            "clocks": clocks,
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nE},
+            "gpu_launches": (6 if wl.demag else 3) * K,
+            "phases_ms_per_step": {k: v / K for k, v in phases.items()},
+            "sweep_only_updates_per_sec": wl.n_active / ((phases["red"] + phases["black"]) / K * 1e-3) if pass_ms > 0 else None,
+            "demag_convolutions_per_sec": (K / (sum(phases[k] for k in ("pack", "fft_fwd", "multiply", "fft_inv", "crop")) * 1e-3)) if wl.demag else None,
+            "roofline": {"kernel": "colour_pass_kernel (one colour pass)", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                         "algorithmic_bytes_per_update": ALGO_BYTES_PER_UPDATE[cfg], "updates_per_launch": wl.n_active / 2.0,
+                         "launch_ms": pass_ms, "share_of_step": (phases["red"] + phases["black"]) / K / step_ms if step_ms > 0 else None},
+        }
+        if not args.no_cpu_baseline and world == 1:
+            v, dt, cores, sample = time_oracle(cfg, 2, 1)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+        print(json.dumps(line))
+    g.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config (default 4: the largest fully magnetic mesh, 1024x1024x4)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--small", action="store_true", help="reduced mesh (debugging only; not a bench number)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

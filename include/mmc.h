@@ -1,0 +1,127 @@
+/*
+ * mmc.h -- C ABI of the B200-native micromagnetic Monte Carlo (MMC) hot path of
+ * arXiv:2106.05593 (S. Lepadatu, "Micromagnetic Monte Carlo method with variable magnetization
+ * length based on the LLB equation").  Citations are /root/reference/PAPER.md line numbers.
+ *
+ * What the library computes: n MMC iterations on a cuboidal mesh of cells of volume
+ * V = dx*dy*dz.  One iteration = [demagnetising field by zero-padded FFT convolution
+ * with the Newell tensor, Eq. (14), frozen for the iteration] -> red colour pass
+ * -> black colour pass (checkerboard).  In a colour pass every non-empty cell of that
+ * colour gets exactly one compound trial move (rotation inside a cone + length factor in
+ * [1-sigma, 1+sigma], PAPER.md:92 steps 1-2), scored by the local free-energy change
+ * (exchange Eq. (10), uniaxial anisotropy Eq. (11), applied field, interfacial DMI Eq. (15),
+ * demag Eq. (14), longitudinal term = exponent of Eq. (7)) and accepted with Eq. (5).
+ * Random numbers: Philox4x32-10, key = seed, counter = (cell index, sweep counter); one block of
+ * four uniforms per cell per sweep, so an oracle can replay the identical stream.
+ *
+ * Conventions
+ *  - every function returns 0 (MMC_OK) or a negative MMC_E_* code; nothing throws or aborts across
+ *    the ABI; mmc_last_error(ctx) gives a message for the last failing call on that ctx.
+ *  - cell index c = i + nx*(j + ny*k), x fastest; colour = (i+j+k) & 1 (0 = "red").
+ *  - m = M/Ms0, stored as three fp32 arrays; all arithmetic of the sweep is fp32
+ *    except the longitudinal bracket (fp64).  Fields in tesla, energies in joule.
+ *  - pointers documented "device" are plain device pointers valid on the ctx device (for example
+ *    torch.Tensor.data_ptr()); "host" pointers are ordinary host memory.  The caller owns every
+ *    buffer it passes; the library copies host inputs during the call and keeps no caller pointer.
+ *  - all device work is enqueued on the stream given at mmc_create; setters taking host arrays and
+ *    mmc_get_observables synchronise that stream, everything else is asynchronous.
+ *  - a ctx is not thread-safe; there is no global state.
+ */
+#ifndef MMC_H_
+#define MMC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MMC_OK              0
+#define MMC_E_INVALID      -1   /* bad argument (NULL, non-positive size, T <= 0, odd periodic length, ...) */
+#define MMC_E_ZERO_LENGTH  -2   /* a non-empty cell has |m| = 0: rotation undefined, length move cannot leave 0 */
+#define MMC_E_CUDA         -3   /* a CUDA runtime / cuFFT call failed; see mmc_last_error */
+#define MMC_E_NOMEM        -4   /* host or device allocation failed */
+#define MMC_E_UNSUPPORTED  -5   /* valid request outside what is built (e.g. A0 differing between regions) */
+#define MMC_E_STATE        -6   /* call order: m / material / temperature not set before sweeping */
+
+typedef struct mmc_ctx mmc_ctx;   /* opaque, owned by the library */
+
+/* Material of one region, SI units.  Ms0 == 0 marks an empty region (no trial, no bond, no demag source).
+ * A0: exchange stiffness at T=0 (A(T) = A0 me^2); K1 + unit axis (ax,ay,az): uniaxial
+ * anisotropy constant at T=0 (K1(T) = K1 me^3, Eq. (11)); D0: interfacial DMI at T=0
+ * (D(T) = D0 me^2, Eq. (15)); Tc: Curie temperature; mu_atom: atomic moment in J/T
+ * (Eq. (8)).  A0 and D0 must be equal in all non-empty regions (MMC_E_UNSUPPORTED). */
+typedef struct { double Ms0, A0, K1, ax, ay, az, D0, Tc, mu_atom; } mmc_material;
+
+/* Read-out (PAPER.md:100 acceptance rate; PAPER.md:135 average magnetisation; Appendix B energies).
+ * Means are over non-empty cells.  Energies in joule with pair terms counted once:
+ * E_ex = sum_bonds (A0 V/h^2)|m_i-m_j|^2, E_an = sum V[K1(T) - K1 me (m.e)^2], E_zee = -V sum Ms0 m.B_ext,
+ * E_dmi = -D0 V sum m.G, E_demag = -(V/2) sum Ms0 m.B_d (B_d of the current state), E_long = sum kB T F_l. */
+typedef struct {
+    double   mean_m[3], mean_len;
+    double   E_ex, E_an, E_zee, E_dmi, E_demag, E_long;
+    uint64_t accepted, trials, sweeps_done;      /* accepted/trials since creation or the last counter reset */
+    double   cone_deg, sigma_used;               /* sigma_used: the (first non-empty cell's) length half-width */
+    double   run_mean_m[3], run_mean_len;        /* average of the per-sweep means since mmc_reset_averages */
+    uint64_t run_sweeps;
+} mmc_obs;
+
+/* Create a context for an nx*ny*nz mesh of dx*dy*dz metre cells on CUDA device `device`.
+ * pbc_mask bit0/1/2 = periodic in x/y/z for exchange and DMI (a periodic length must be even and >= 2:
+ * the checkerboard needs it); the demag convolution is always open-boundary.  cuda_stream is a
+ * cudaStream_t (NULL = legacy default stream).  Defaults: one non-magnetic region, T unset, B = 0,
+ * cone 30 deg fixed, sigma from Eq. (13), demag off, seed 0, sweep counter 0. */
+int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, double dz,
+               unsigned pbc_mask, int device, void* cuda_stream);
+int mmc_destroy(mmc_ctx* ctx);
+
+/* regions: host array of n_regions records; region_of_cell: host int32[N] (NULL => every cell region 0). */
+int mmc_set_material(mmc_ctx* ctx, int n_regions, const mmc_material* regions, const int32_t* region_of_cell);
+/* 0 => bonds between cells of different regions carry no exchange and no DMI ("phase separation"). */
+int mmc_set_exchange_coupling(mmc_ctx* ctx, int inter_region_exchange);
+/* Uniform temperature, or per cell when T_per_cell (host float[N], kelvin) is not NULL.
+ * Recomputes me (Eq. (9), H_ext = 0), chi (Eq. (8)), the longitudinal coefficients (Eq. (7)) and sigma (Eq. (13)). */
+int mmc_set_temperature(mmc_ctx* ctx, double T_uniform, const float* T_per_cell);
+int mmc_set_field(mmc_ctx* ctx, double Bx, double By, double Bz);                 /* applied field, tesla */
+/* cone half-angle in degrees (0 < cone <= 180); sigma < 0 => Eq. (13) capped at 0.03, else the
+ * given half-width of the uniform length factor; adaptive_cone != 0 => every 100 iterations the cone changes by
+ * 1 degree when the acceptance rate leaves 0.5 +- 0.05, clamped to [1, 180]. */
+int mmc_set_move(mmc_ctx* ctx, double cone_deg, double sigma, int adaptive_cone);
+/* updates_per_sweep: 1 = once per iteration; 2 = also before the black pass. */
+int mmc_set_demag(mmc_ctx* ctx, int enabled, int updates_per_sweep);
+int mmc_set_seed(mmc_ctx* ctx, uint64_t seed);
+int mmc_set_sweep_counter(mmc_ctx* ctx, uint64_t sweep);
+/* device pointers, N floats each, natural cell order.  Fails with MMC_E_ZERO_LENGTH if a non-empty cell is 0. */
+int mmc_set_m(mmc_ctx* ctx, const float* mx, const float* my, const float* mz);
+int mmc_get_m(mmc_ctx* ctx, float* mx, float* my, float* mz);
+/* n iterations, asynchronous on the ctx stream. */
+int mmc_sweep(mmc_ctx* ctx, int n_sweeps);
+/* Same as mmc_sweep, but brackets every phase of every iteration with CUDA events on the ctx stream, synchronises, and
+ * returns the summed device time per phase in milliseconds: phase_ms[8] (host) = pack+pad, forward FFT, tensor multiply,
+ * inverse FFT, crop, red pass, black pass, end-of-sweep bookkeeping. */
+int mmc_sweep_timed(mmc_ctx* ctx, int n_sweeps, double* phase_ms);
+/* One demag convolution of the current state; bx/by/bz device float[N] (natural order) receive B_d = mu0 H_d
+ * in tesla; any of them may be NULL (then the field is only computed).  Works with demag disabled too. */
+int mmc_demag_field(mmc_ctx* ctx, float* bx, float* by, float* bz);
+int mmc_get_observables(mmc_ctx* ctx, mmc_obs* host_out);      /* synchronises */
+int mmc_reset_counters(mmc_ctx* ctx);                          /* accepted/trials := 0 */
+int mmc_reset_averages(mmc_ctx* ctx);                          /* run_mean_* := 0 */
+/* One colour pass (colour 0 or 1) at the current sweep counter with a per-cell dump, natural cell order, device
+ * pointers, any may be NULL: dm float[3N] (cell-major: dm[3c+a]), dF_terms float[6N] (ex, an, zee, dmi, demag,
+ * long in units of kB T), margin float[N] (= ln u - 4 ln f + dF; accept <=> margin < 0), accepted uint8[N].
+ * Cells of the other colour and empty cells are left untouched.  The pass updates m like a normal pass, uses the
+ * demag field of the last computation, and does not advance the sweep counter. */
+int mmc_debug_pass(mmc_ctx* ctx, int colour, float* dm, float* dF_terms, float* margin, uint8_t* accepted);
+/* Host-side thermal functions used by the set-up (for tests of the host logic): out[6] = me, chi (1/T), c2, c4,
+ * sigma of Eq. (13) with the cap, mu2 = -c2/(2 c4). */
+int mmc_thermal(double T, double Tc, double mu_atom, double V, double Ms0, double* out6);
+/* Host-side demag tensor used by the set-up: out[6] = N_xx, N_yy, N_zz, N_xy, N_xz, N_yz at integer cell offset. */
+int mmc_demag_tensor_at(double dx, double dy, double dz, int ox, int oy, int oz, double* out6);
+
+const char* mmc_strerror(int code);
+const char* mmc_last_error(const mmc_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MMC_H_ */

@@ -79,6 +79,7 @@ def lib():
         L.orc_colour_pass.argtypes = [C.POINTER(_Problem), dp, dp, dp, C.c_int, C.c_uint64,
                                       C.c_void_p, C.c_int64, C.c_int,
                                       C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_int64)]
+        L.orc_colour_terms_given_dm.argtypes = [C.POINTER(_Problem), dp, dp, dp, C.c_int, dp, dp]
         L.orc_observables.argtypes = [C.POINTER(_Problem), dp, dp, dp, dp, dp, C.POINTER(C.c_int64)]
         L.orc_newell.argtypes = [C.c_double] * 6 + [dp]
         L.orc_demag_tensor.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [C.c_int, dp]
@@ -390,6 +391,14 @@ class OracleMMC:
     def run(self, n_sweeps):
         for _ in range(n_sweeps):
             self.sweep_once()
+
+    def colour_terms_given_dm(self, colour, dm):
+        """O4 for every active cell of `colour` with caller-supplied trial vectors dm[N,3] -> terms[N,6] (NaN elsewhere)."""
+        p = self._problem()
+        dm = np.ascontiguousarray(dm, dtype=np.float64)
+        t = np.full((self.N, 6), np.nan)
+        lib().orc_colour_terms_given_dm(C.byref(p), _dp(self.m[0]), _dp(self.m[1]), _dp(self.m[2]), int(colour), _dp(dm), _dp(t))
+        return t
 
     def cell_dF(self, i, j, k, dm):
         p = self._problem()

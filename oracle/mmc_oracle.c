@@ -551,3 +551,21 @@ void orc_demag_direct(int nx, int ny, int nz, const double *tab,
         bx[ci] = ORC_MU0 * hx; by[ci] = ORC_MU0 * hy; bz[ci] = ORC_MU0 * hz;
     }
 }
+
+/*
+ * Parity plumbing (stage 2): O4 evaluated for every active cell of one colour with trial
+ * vectors supplied by the caller (dm_in[3c+a]) instead of O3's own, so that the energy arithmetic of another
+ * implementation can be judged separately from its trigonometry.  No new arithmetic: calls orc_cell_dF.
+ */
+void orc_colour_terms_given_dm(const orc_problem *p, const double *mx, const double *my, const double *mz,
+                               int colour, const double *dm_in, double *terms_out)
+{
+    #pragma omp parallel for collapse(2) schedule(static)
+    for (int k = 0; k < p->nz; ++k)
+        for (int j = 0; j < p->ny; ++j)
+            for (int i = (j + k + colour) & 1; i < p->nx; i += 2) {
+                int64_t c = orc_idx(p, i, j, k);
+                if (!p->active[c]) continue;
+                orc_cell_dF(p, mx, my, mz, i, j, k, dm_in + 3 * c, terms_out + 6 * c);
+            }
+}

@@ -1,0 +1,629 @@
+// api.cu -- the extern "C" boundary of include/mmc.h: context, host-side set-up (thermal classes, bond/active
+// mask, coefficient upload), the iteration loop (demag -> red -> black -> end_sweep) and the read-outs.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <unordered_map>
+
+#include "mmc_internal.h"
+
+using namespace mmc;
+
+struct mmc_ctx {
+    Geometry g{};
+    double dx = 0, dy = 0, dz = 0, V = 0;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    std::string err;
+    // problem description (host)
+    std::vector<mmc_material> regions;
+    std::vector<int32_t> region_of_cell;          // empty => all 0
+    int inter_region = 1;
+    double T_uniform = 0.0; std::vector<float> T_cell;   // T_cell empty => uniform
+    bool T_set = false, material_set = false, m_set = false;
+    double B[3] = { 0, 0, 0 };
+    double cone_deg = 30.0, sigma_user = -1.0; int adaptive = 0;
+    int demag_enabled = 0, demag_updates = 1;
+    uint64_t seed = 0;
+    // derived (host)
+    bool dirty = true, m_needs_check = false;
+    bool percell = false;
+    unsigned features = 0;
+    double A0 = 0, D0 = 0, sigma_first = 0;
+    Coef coef{};
+    float K1T_u = 0.f, c0_u = 0.f, Ms0_u = 0.f;
+    bool Ms0_uniform = true;
+    unsigned long long n_active = 0;
+    // device
+    float* m[3] = { nullptr, nullptr, nullptr };
+    float* bd[3] = { nullptr, nullptr, nullptr };
+    uint8_t* mask = nullptr;
+    float* Ms0_split = nullptr;
+    float* pc[12] = { nullptr };                  // invT,c4,mu2hi,mu2lo,bKq,bzee,sigma,ax,ay,az,K1T,c0adj
+    Control* ctl = nullptr;
+    double* run_sums = nullptr; int n_slots = 0;
+    double* obs_scratch = nullptr; int obs_blocks = 0;
+    Observables* d_obs = nullptr;
+    int* d_flag = nullptr;
+    float* stage = nullptr;                       // N floats, for natural-order outputs
+    DemagPlan* demag = nullptr;
+};
+
+namespace {
+
+int fail(mmc_ctx* c, int code, const std::string& msg) { if (c) c->err = msg; return code; }
+
+#define CU(c, x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return fail((c), MMC_E_CUDA, std::string(#x) + ": " + cudaGetErrorString(e_)); } while (0)
+
+struct DeviceGuard {
+    int prev = -1; bool ok;
+    explicit DeviceGuard(int dev) { ok = cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+inline long long split_index_h(const Geometry& g, int i, int j, int k)
+{
+    const int col = (i + j + k) & 1;
+    return (long long)col * g.H + ((long long)k * g.ny + j) * g.hx + (i >> 1);
+}
+
+template <class T>
+int upload(mmc_ctx* c, T** dptr, const std::vector<T>& h)
+{
+    if (!*dptr) CU(c, cudaMalloc(dptr, h.size() * sizeof(T)));
+    CU(c, cudaMemcpyAsync(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return MMC_OK;
+}
+
+// O1 + mask: everything the kernels need that depends on material, temperature, move and coupling settings.
+int ensure_setup(mmc_ctx* c)
+{
+    if (!c->dirty) return MMC_OK;
+    const Geometry& g = c->g;
+    const long long N = (long long)g.nx * g.ny * g.nz;
+    const size_t S = (size_t)(2 * g.H);
+    const bool have_reg = !c->region_of_cell.empty();
+    const int nreg = (int)c->regions.size();
+    // uniform exchange / DMI constants over non-empty regions
+    bool any = false; double A0 = 0, D0 = 0;
+    for (const auto& r : c->regions) {
+        if (!(r.Ms0 > 0)) continue;
+        if (!any) { A0 = r.A0; D0 = r.D0; any = true; }
+        else if (r.A0 != A0 || r.D0 != D0) return fail(c, MMC_E_UNSUPPORTED, "A0 and D0 must be equal in all non-empty regions");
+    }
+    c->A0 = A0; c->D0 = D0;
+    auto reg_of = [&](long long cell) -> int { return have_reg ? c->region_of_cell[cell] : 0; };
+    auto T_of = [&](long long cell) -> float { return c->T_cell.empty() ? (float)c->T_uniform : c->T_cell[cell]; };
+    // classes = distinct (region, T) pairs among active cells
+    struct Cls { int region; float T; ThermalCoef th; };
+    std::vector<Cls> classes;
+    std::unordered_map<uint64_t, int> cls_of_key;
+    std::vector<int> cls_of_cell((size_t)N, -1);
+    unsigned long long n_active = 0;
+    for (long long cell = 0; cell < N; ++cell) {
+        const int r = reg_of(cell);
+        if (!(c->regions[r].Ms0 > 0)) continue;
+        n_active++;
+        const float T = T_of(cell);
+        uint32_t tb; std::memcpy(&tb, &T, 4);
+        const uint64_t key = ((uint64_t)(uint32_t)r << 32) | tb;
+        auto it = cls_of_key.find(key);
+        int id;
+        if (it == cls_of_key.end()) {
+            if (!(T > 0.f) || !std::isfinite(T)) return fail(c, MMC_E_INVALID, "temperature must be > 0 in every non-empty cell");
+            Cls k; k.region = r; k.T = T;
+            const mmc_material& mt = c->regions[r];
+            if (!(mt.Tc > 0) || !(mt.mu_atom > 0)) return fail(c, MMC_E_INVALID, "Tc and mu_atom must be > 0 in non-empty regions");
+            int rc = thermal_coefficients((double)T, mt.Tc, mt.mu_atom, c->V, mt.Ms0, &k.th);
+            if (rc != MMC_OK) return fail(c, rc, "thermal_coefficients failed");
+            id = (int)classes.size(); classes.push_back(k); cls_of_key.emplace(key, id);
+        } else id = it->second;
+        cls_of_cell[(size_t)cell] = id;
+    }
+    c->n_active = n_active;
+    // per-cell mode iff more than one class differs in anything the kernel reads
+    c->percell = classes.size() > 1;
+    // mask (bit d: bonded neighbour in direction d; bit 6: active), Ms0
+    std::vector<uint8_t> mask(S, 0);
+    std::vector<float> ms0(S, 0.f);
+    bool need_mask = (g.nx % 8) != 0;
+    bool ms0_uniform = true; double ms0_first = -1;
+    const int nn[3] = { g.nx, g.ny, g.nz };
+    for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
+        const long long cell = (long long)i + (long long)g.nx * (j + (long long)g.ny * k);
+        const long long s = split_index_h(g, i, j, k);
+        if (cls_of_cell[(size_t)cell] < 0) { need_mask = true; continue; }
+        const int r = reg_of(cell);
+        const double Ms = c->regions[r].Ms0;
+        ms0[(size_t)s] = (float)Ms;
+        if (ms0_first < 0) ms0_first = Ms; else if (Ms != ms0_first) ms0_uniform = false;
+        unsigned mb = 0x40u;
+        const int q[3] = { i, j, k };
+        for (int d = 0; d < 6; ++d) {
+            const int a = d >> 1, step = (d & 1) ? -1 : 1;
+            if (nn[a] < 2) continue;
+            int v = q[a] + step;
+            if (v < 0 || v >= nn[a]) { if (!((g.pbc >> a) & 1u)) { need_mask = true; continue; } v = (v + nn[a]) % nn[a]; }
+            int p[3] = { i, j, k }; p[a] = v;
+            const long long nb = (long long)p[0] + (long long)g.nx * (p[1] + (long long)g.ny * p[2]);
+            if (cls_of_cell[(size_t)nb] < 0) { need_mask = true; continue; }
+            if (!c->inter_region && reg_of(nb) != r) { need_mask = true; continue; }
+            mb |= 1u << d;
+        }
+        mask[(size_t)s] = (uint8_t)mb;
+    }
+    c->Ms0_uniform = ms0_uniform && n_active == (unsigned long long)N;   // empty cells need per-cell weights to zero their M
+    c->Ms0_u = ms0_first > 0 ? (float)ms0_first : 0.f;
+    int rc = upload(c, &c->mask, mask); if (rc) return rc;
+    if (!c->Ms0_uniform) { rc = upload(c, &c->Ms0_split, ms0); if (rc) return rc; }
+    // coefficients
+    const double V = c->V, kB = kBoltzmann;
+    const double Jd[3] = { 2.0 * A0 * V / (c->dx * c->dx), 2.0 * A0 * V / (c->dy * c->dy), 2.0 * A0 * V / (c->dz * c->dz) };
+    Coef cf{};
+    cf.Bx = (float)c->B[0]; cf.By = (float)c->B[1]; cf.Bz = (float)c->B[2];
+    auto class_values = [&](const Cls& k, double beta, float out[12], double* mu2) {
+        const mmc_material& mt = c->regions[k.region];
+        double al = std::sqrt(mt.ax * mt.ax + mt.ay * mt.ay + mt.az * mt.az);
+        double ex = 0, ey = 0, ez = 1;
+        if (al > 0) { ex = mt.ax / al; ey = mt.ay / al; ez = mt.az / al; }
+        const double sig = c->sigma_user >= 0 ? c->sigma_user : k.th.sigma13;
+        *mu2 = k.th.mu2;
+        const float hi = (float)k.th.mu2;
+        out[0] = (float)(1.0 / (double)k.T); out[1] = (float)k.th.c4; out[2] = hi; out[3] = (float)(k.th.mu2 - (double)hi);
+        out[4] = (float)(beta * V * mt.K1 * k.th.me); out[5] = (float)(beta * V * mt.Ms0); out[6] = (float)sig;
+        out[7] = (float)ex; out[8] = (float)ey; out[9] = (float)ez;
+        out[10] = (float)(beta * V * mt.K1 * k.th.me * k.th.me * k.th.me);
+        out[11] = (float)((k.th.me > 0 || k.th.mu2 == 0) ? 0.0 : -k.th.c4 * k.th.mu2 * k.th.mu2);
+    };
+    if (!c->percell) {
+        if (!classes.empty()) {
+            const Cls& k = classes[0];
+            const double beta = 1.0 / (kB * (double)k.T);
+            float v[12]; double mu2;
+            class_values(k, beta, v, &mu2);
+            cf.kx = (float)(beta * Jd[0]); cf.ky = (float)(beta * Jd[1]); cf.kz = (float)(beta * Jd[2]);
+            cf.gx = (float)(beta * D0 * V / c->dx); cf.gy = (float)(beta * D0 * V / c->dy);
+            cf.c4 = v[1]; cf.mu2 = mu2; cf.bKq = v[4]; cf.bzee = v[5]; cf.sigma = v[6];
+            cf.ax = v[7]; cf.ay = v[8]; cf.az = v[9];
+            c->K1T_u = v[10]; c->c0_u = v[11];
+            c->sigma_first = v[6];
+        }
+    } else {
+        const double b1 = 1.0 / kB;                   // beta at T = 1 K; the kernel multiplies by the cell's 1/T
+        cf.kx = (float)(b1 * Jd[0]); cf.ky = (float)(b1 * Jd[1]); cf.kz = (float)(b1 * Jd[2]);
+        cf.gx = (float)(b1 * D0 * V / c->dx); cf.gy = (float)(b1 * D0 * V / c->dy);
+        std::vector<float> cv(classes.size() * 12);
+        for (size_t q = 0; q < classes.size(); ++q) { double mu2; class_values(classes[q], 1.0 / (kB * (double)classes[q].T), &cv[12 * q], &mu2); }
+        c->sigma_first = cv[6];
+        std::vector<float> arr(S);
+        for (int f = 0; f < 12; ++f) {
+            std::fill(arr.begin(), arr.end(), f == 0 ? 1.f : (f == 9 ? 1.f : 0.f));
+            for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
+                const long long cell = (long long)i + (long long)g.nx * (j + (long long)g.ny * k);
+                const int id = cls_of_cell[(size_t)cell];
+                if (id >= 0) arr[(size_t)split_index_h(g, i, j, k)] = cv[12 * (size_t)id + f];
+            }
+            rc = upload(c, &c->pc[f], arr); if (rc) return rc;
+        }
+    }
+    c->coef = cf;
+    unsigned f = 0;
+    if (need_mask) f |= F_MASK;
+    if (c->percell) f |= F_PERCELL;
+    if (g.nz > 1) f |= F_Z;
+    if (D0 != 0.0) f |= F_DMI;
+    if (c->demag_enabled) f |= F_DEMAG;
+    c->features = f;
+    c->dirty = false;
+    return MMC_OK;
+}
+
+int push_control(mmc_ctx* c, bool reset_window)
+{
+    Control h;
+    CU(c, cudaMemcpyAsync(&h, c->ctl, sizeof(Control), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    h.adaptive = c->adaptive; h.cone_deg = c->cone_deg;
+    const double s = std::sin(0.5 * c->cone_deg * 0.017453292519943295);
+    h.one_minus_cos_cone = (float)(2.0 * s * s);
+    if (reset_window) { h.accepted += h.win_accepted; h.trials += h.win_trials; h.win_accepted = h.win_trials = 0; h.win_sweeps = 0; }
+    CU(c, cudaMemcpyAsync(c->ctl, &h, sizeof(Control), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return MMC_OK;
+}
+
+SweepArgs make_args(mmc_ctx* c, int colour)
+{
+    SweepArgs a{};
+    a.g = c->g;
+    for (int q = 0; q < 3; ++q) { a.m[q] = c->m[q]; a.bd[q] = c->bd[q]; }
+    a.mask = c->mask; a.coef = c->coef;
+    a.coef.Bx = (float)c->B[0]; a.coef.By = (float)c->B[1]; a.coef.Bz = (float)c->B[2];
+    a.pc.invT = c->pc[0]; a.pc.c4 = c->pc[1]; a.pc.mu2hi = c->pc[2]; a.pc.mu2lo = c->pc[3]; a.pc.bKq = c->pc[4];
+    a.pc.bzee = c->pc[5]; a.pc.sigma = c->pc[6]; a.pc.ax = c->pc[7]; a.pc.ay = c->pc[8]; a.pc.az = c->pc[9];
+    a.ctl = c->ctl; a.seed_lo = (unsigned)c->seed; a.seed_hi = (unsigned)(c->seed >> 32);
+    a.colour = colour; a.run_sums = c->run_sums;
+    return a;
+}
+
+int ensure_demag(mmc_ctx* c)
+{
+    if (c->demag) return MMC_OK;
+    std::string e;
+    int rc = demag_create(&c->demag, c->g, c->dx, c->dy, c->dz, c->stream, &e);
+    if (rc != MMC_OK) { demag_destroy(c->demag); c->demag = nullptr; return fail(c, rc, "demag set-up: " + e); }
+    return MMC_OK;
+}
+
+int compute_demag(mmc_ctx* c, PhaseTimer* timer = nullptr)
+{
+    int rc = ensure_demag(c); if (rc) return rc;
+    std::string e;
+    rc = demag_compute(c->demag, c->m, c->Ms0_uniform ? nullptr : c->Ms0_split, c->Ms0_u, c->bd, c->stream, &e, timer);
+    if (rc != MMC_OK) return fail(c, rc, "demag: " + e);
+    return MMC_OK;
+}
+
+int check_m(mmc_ctx* c)
+{
+    CU(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream));
+    int rc = launch_check_zero(c->g, c->m, c->mask, c->d_flag, c->stream);
+    if (rc) return fail(c, rc, "check_zero launch failed");
+    int flag = 0;
+    CU(c, cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    c->m_needs_check = false;
+    if (flag) return fail(c, MMC_E_ZERO_LENGTH, "a non-empty cell has zero (or non-finite) magnetisation");
+    return MMC_OK;
+}
+
+int ready(mmc_ctx* c)
+{
+    if (!c) return MMC_E_INVALID;
+    if (!c->material_set || !c->T_set || !c->m_set) return fail(c, MMC_E_STATE, "set material, temperature and m before this call");
+    int rc = ensure_setup(c); if (rc) return rc;
+    if (c->m_needs_check) { rc = check_m(c); if (rc) return rc; }
+    return MMC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, double dz, unsigned pbc_mask, int device, void* cuda_stream)
+{
+    if (!out) return MMC_E_INVALID;
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || pbc_mask > 7u) return MMC_E_INVALID;
+    if ((long long)nx * ny * nz > (1ll << 31)) return MMC_E_INVALID;
+    const int nn[3] = { nx, ny, nz };
+    for (int a = 0; a < 3; ++a)
+        if (((pbc_mask >> a) & 1u) && (nn[a] < 2 || (nn[a] & 1))) return MMC_E_INVALID;   // checkerboard needs even periodic lengths
+    mmc_ctx* c = new (std::nothrow) mmc_ctx();
+    if (!c) return MMC_E_NOMEM;
+    c->g.nx = nx; c->g.ny = ny; c->g.nz = nz; c->g.pbc = pbc_mask;
+    c->g.hx = (((nx + 1) / 2) + 3) / 4 * 4;
+    c->g.H = (int64_t)c->g.hx * ny * nz;
+    c->dx = dx; c->dy = dy; c->dz = dz; c->V = dx * dy * dz;
+    c->device = device; c->stream = (cudaStream_t)cuda_stream;
+    c->regions.push_back(mmc_material{ 0, 0, 0, 0, 0, 1, 0, 1, 9.2740100783e-24 });
+    DeviceGuard dg(device);
+    auto bail = [&](int code) { mmc_destroy(c); return code; };
+    if (!dg.ok) return bail(MMC_E_CUDA);
+    const size_t S = (size_t)(2 * c->g.H);
+    for (int q = 0; q < 3; ++q) {
+        if (cudaMalloc(&c->m[q], S * sizeof(float)) != cudaSuccess) return bail(MMC_E_NOMEM);
+        if (cudaMalloc(&c->bd[q], S * sizeof(float)) != cudaSuccess) return bail(MMC_E_NOMEM);
+        cudaMemsetAsync(c->m[q], 0, S * sizeof(float), c->stream);
+        cudaMemsetAsync(c->bd[q], 0, S * sizeof(float), c->stream);
+    }
+    c->n_slots = sweep_grid_blocks(c->g, true);
+    c->obs_blocks = 148 * 4;
+    if (cudaMalloc(&c->ctl, sizeof(Control)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaMalloc(&c->run_sums, (size_t)c->n_slots * 4 * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaMalloc(&c->obs_scratch, (size_t)c->obs_blocks * 11 * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaMalloc(&c->d_obs, sizeof(Observables)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaMalloc(&c->d_flag, sizeof(int)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaMalloc(&c->stage, (size_t)nx * ny * nz * sizeof(float)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream);
+    cudaMemsetAsync(c->run_sums, 0, (size_t)c->n_slots * 4 * sizeof(double), c->stream);
+    if (push_control(c, false) != MMC_OK) return bail(MMC_E_CUDA);
+    *out = c;
+    return MMC_OK;
+}
+
+int mmc_destroy(mmc_ctx* c)
+{
+    if (!c) return MMC_E_INVALID;
+    DeviceGuard dg(c->device);
+    cudaStreamSynchronize(c->stream);
+    for (int q = 0; q < 3; ++q) { cudaFree(c->m[q]); cudaFree(c->bd[q]); }
+    for (int q = 0; q < 12; ++q) cudaFree(c->pc[q]);
+    cudaFree(c->mask); cudaFree(c->Ms0_split); cudaFree(c->ctl); cudaFree(c->run_sums); cudaFree(c->obs_scratch);
+    cudaFree(c->d_obs); cudaFree(c->d_flag); cudaFree(c->stage);
+    demag_destroy(c->demag);
+    delete c;
+    return MMC_OK;
+}
+
+int mmc_set_material(mmc_ctx* c, int n_regions, const mmc_material* regions, const int32_t* region_of_cell)
+{
+    if (!c) return MMC_E_INVALID;
+    if (n_regions < 1 || !regions) return fail(c, MMC_E_INVALID, "n_regions >= 1 and regions != NULL required");
+    for (int r = 0; r < n_regions; ++r)
+        if (!(regions[r].Ms0 >= 0) || !std::isfinite(regions[r].Ms0) || regions[r].A0 < 0) return fail(c, MMC_E_INVALID, "Ms0 and A0 must be >= 0");
+    const long long N = (long long)c->g.nx * c->g.ny * c->g.nz;
+    if (region_of_cell)
+        for (long long i = 0; i < N; ++i)
+            if (region_of_cell[i] < 0 || region_of_cell[i] >= n_regions) return fail(c, MMC_E_INVALID, "region_of_cell out of range");
+    c->regions.assign(regions, regions + n_regions);
+    if (region_of_cell) c->region_of_cell.assign(region_of_cell, region_of_cell + N); else c->region_of_cell.clear();
+    c->material_set = true; c->dirty = true; c->m_needs_check = c->m_set;
+    return MMC_OK;
+}
+
+int mmc_set_exchange_coupling(mmc_ctx* c, int inter_region_exchange)
+{
+    if (!c) return MMC_E_INVALID;
+    c->inter_region = inter_region_exchange ? 1 : 0; c->dirty = true;
+    return MMC_OK;
+}
+
+int mmc_set_temperature(mmc_ctx* c, double T_uniform, const float* T_per_cell)
+{
+    if (!c) return MMC_E_INVALID;
+    const long long N = (long long)c->g.nx * c->g.ny * c->g.nz;
+    if (T_per_cell) {
+        c->T_cell.assign(T_per_cell, T_per_cell + N);
+    } else {
+        if (!(T_uniform > 0) || !std::isfinite(T_uniform)) return fail(c, MMC_E_INVALID, "T must be > 0");
+        c->T_cell.clear();
+    }
+    c->T_uniform = T_uniform; c->T_set = true; c->dirty = true;
+    return MMC_OK;
+}
+
+int mmc_set_field(mmc_ctx* c, double Bx, double By, double Bz)
+{
+    if (!c) return MMC_E_INVALID;
+    if (!std::isfinite(Bx) || !std::isfinite(By) || !std::isfinite(Bz)) return fail(c, MMC_E_INVALID, "field must be finite");
+    c->B[0] = Bx; c->B[1] = By; c->B[2] = Bz;          // read into the kernel arguments at every launch
+    return MMC_OK;
+}
+
+int mmc_set_move(mmc_ctx* c, double cone_deg, double sigma, int adaptive_cone)
+{
+    if (!c) return MMC_E_INVALID;
+    if (!(cone_deg > 0) || cone_deg > 180.0 || !(sigma < 1.0)) return fail(c, MMC_E_INVALID, "0 < cone <= 180 and sigma < 1 required");
+    c->cone_deg = cone_deg; c->sigma_user = sigma; c->adaptive = adaptive_cone ? 1 : 0; c->dirty = true;
+    DeviceGuard dg(c->device);
+    return push_control(c, true);
+}
+
+int mmc_set_demag(mmc_ctx* c, int enabled, int updates_per_sweep)
+{
+    if (!c) return MMC_E_INVALID;
+    if (updates_per_sweep != 1 && updates_per_sweep != 2) return fail(c, MMC_E_INVALID, "updates_per_sweep must be 1 or 2");
+    DeviceGuard dg(c->device);
+    if (c->demag_enabled && !enabled)
+        for (int q = 0; q < 3; ++q) cudaMemsetAsync(c->bd[q], 0, (size_t)(2 * c->g.H) * sizeof(float), c->stream);
+    c->demag_enabled = enabled ? 1 : 0; c->demag_updates = updates_per_sweep; c->dirty = true;
+    return MMC_OK;
+}
+
+int mmc_set_seed(mmc_ctx* c, uint64_t seed) { if (!c) return MMC_E_INVALID; c->seed = seed; return MMC_OK; }
+
+int mmc_set_sweep_counter(mmc_ctx* c, uint64_t sweep)
+{
+    if (!c) return MMC_E_INVALID;
+    DeviceGuard dg(c->device);
+    unsigned long long s = sweep;
+    CU(c, cudaMemcpyAsync(&c->ctl->sweep, &s, sizeof(s), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return MMC_OK;
+}
+
+int mmc_set_m(mmc_ctx* c, const float* mx, const float* my, const float* mz)
+{
+    if (!c || !mx || !my || !mz) return fail(c, MMC_E_INVALID, "NULL pointer");
+    DeviceGuard dg(c->device);
+    const float* src[3] = { mx, my, mz };
+    for (int q = 0; q < 3; ++q) {
+        CU(c, cudaMemsetAsync(c->m[q], 0, (size_t)(2 * c->g.H) * sizeof(float), c->stream));
+        int rc = launch_to_split(c->g, src[q], c->m[q], c->stream);
+        if (rc) return fail(c, rc, "to_split launch failed");
+    }
+    c->m_set = true;
+    if (c->material_set && c->T_set) {
+        int rc = ensure_setup(c); if (rc) return rc;
+        return check_m(c);
+    }
+    c->m_needs_check = true;
+    return MMC_OK;
+}
+
+int mmc_get_m(mmc_ctx* c, float* mx, float* my, float* mz)
+{
+    if (!c || !mx || !my || !mz) return fail(c, MMC_E_INVALID, "NULL pointer");
+    DeviceGuard dg(c->device);
+    float* dst[3] = { mx, my, mz };
+    for (int q = 0; q < 3; ++q) { int rc = launch_from_split(c->g, c->m[q], dst[q], c->stream); if (rc) return fail(c, rc, "from_split launch failed"); }
+    return MMC_OK;
+}
+
+static int sweep_impl(mmc_ctx* c, int n_sweeps, PhaseTimer* timer)
+{
+    if (!c || n_sweeps < 0) return fail(c, MMC_E_INVALID, "n_sweeps >= 0 required");
+    DeviceGuard dg(c->device);
+    int rc = ready(c); if (rc) return rc;
+    if (c->demag_enabled) { rc = ensure_demag(c); if (rc) return rc; }
+    if (timer) timer->mark(-1, c->stream);
+    for (int it = 0; it < n_sweeps; ++it) {
+        if (c->demag_enabled) { rc = compute_demag(c, timer); if (rc) return rc; }
+        rc = launch_colour_pass(make_args(c, 0), c->features, true, false, c->stream);
+        if (rc) return fail(c, rc, "red pass launch failed");
+        if (timer) timer->mark(PH_RED, c->stream);
+        if (c->demag_enabled && c->demag_updates == 2) { rc = compute_demag(c, timer); if (rc) return rc; }
+        rc = launch_colour_pass(make_args(c, 1), c->features, true, false, c->stream);
+        if (rc) return fail(c, rc, "black pass launch failed");
+        if (timer) timer->mark(PH_BLACK, c->stream);
+        rc = launch_end_sweep(c->ctl, c->run_sums, c->n_slots, c->stream);
+        if (rc) return fail(c, rc, "end_sweep launch failed");
+        if (timer) timer->mark(PH_END, c->stream);
+    }
+    return MMC_OK;
+}
+
+int mmc_sweep(mmc_ctx* c, int n_sweeps) { return sweep_impl(c, n_sweeps, nullptr); }
+
+int mmc_sweep_timed(mmc_ctx* c, int n_sweeps, double* phase_ms)
+{
+    if (!c || !phase_ms) return fail(c, MMC_E_INVALID, "NULL pointer");
+    PhaseTimer t;
+    int rc = sweep_impl(c, n_sweeps, &t);
+    DeviceGuard dg(c->device);
+    cudaStreamSynchronize(c->stream);
+    for (int p = 0; p < PH_COUNT; ++p) phase_ms[p] = 0.0;
+    for (size_t i = 1; i < t.events.size(); ++i) {
+        float ms = 0.f;
+        if (t.phase[i] >= 0 && cudaEventElapsedTime(&ms, (cudaEvent_t)t.events[i - 1], (cudaEvent_t)t.events[i]) == cudaSuccess)
+            phase_ms[t.phase[i]] += (double)ms;
+    }
+    for (void* e : t.events) cudaEventDestroy((cudaEvent_t)e);
+    return rc;
+}
+
+int mmc_demag_field(mmc_ctx* c, float* bx, float* by, float* bz)
+{
+    if (!c) return MMC_E_INVALID;
+    DeviceGuard dg(c->device);
+    int rc = ready(c); if (rc) return rc;
+    rc = compute_demag(c); if (rc) return rc;
+    float* dst[3] = { bx, by, bz };
+    for (int q = 0; q < 3; ++q)
+        if (dst[q]) { rc = launch_from_split(c->g, c->bd[q], dst[q], c->stream); if (rc) return fail(c, rc, "from_split launch failed"); }
+    if (!c->demag_enabled)                       // keep the sweep's field term off
+        for (int q = 0; q < 3; ++q) CU(c, cudaMemsetAsync(c->bd[q], 0, (size_t)(2 * c->g.H) * sizeof(float), c->stream));
+    return MMC_OK;
+}
+
+int mmc_get_observables(mmc_ctx* c, mmc_obs* out)
+{
+    if (!c || !out) return fail(c, MMC_E_INVALID, "NULL pointer");
+    DeviceGuard dg(c->device);
+    int rc = ready(c); if (rc) return rc;
+    if (c->demag_enabled) { rc = compute_demag(c); if (rc) return rc; }
+    SweepArgs a = make_args(c, 0);
+    if (!c->demag_enabled) a.bd[0] = a.bd[1] = a.bd[2] = nullptr;
+    ObsParams op{};
+    op.K1T_pc = c->pc[10]; op.K1T_u = c->K1T_u; op.c0_pc = c->pc[11]; op.c0_u = c->c0_u;
+    op.aex[0] = c->A0 * c->V / (c->dx * c->dx); op.aex[1] = c->A0 * c->V / (c->dy * c->dy); op.aex[2] = c->A0 * c->V / (c->dz * c->dz);
+    op.D0V = c->D0 * c->V; op.inv_d[0] = 1.0 / c->dx; op.inv_d[1] = 1.0 / c->dy; op.kB = kBoltzmann;
+    op.T_u = c->T_cell.empty() ? (float)c->T_uniform : (c->percell ? 1.f : c->T_cell[0]);
+    if (!c->percell && !c->T_cell.empty()) {
+        // uniform mode with a per-cell array means all active cells share one temperature: find it
+        const long long N = (long long)c->g.nx * c->g.ny * c->g.nz;
+        for (long long i = 0; i < N; ++i) {
+            const int r = c->region_of_cell.empty() ? 0 : c->region_of_cell[i];
+            if (c->regions[r].Ms0 > 0) { op.T_u = c->T_cell[i]; break; }
+        }
+    }
+    rc = launch_observables(a, c->percell, op, c->d_obs, c->obs_scratch, c->obs_blocks, c->stream);
+    if (rc) return fail(c, rc, "observables launch failed");
+    Observables ho; Control hc;
+    std::vector<double> slots((size_t)c->n_slots * 4);
+    CU(c, cudaMemcpyAsync(&ho, c->d_obs, sizeof(ho), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaMemcpyAsync(&hc, c->ctl, sizeof(hc), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaMemcpyAsync(slots.data(), c->run_sums, slots.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    std::memset(out, 0, sizeof(*out));
+    const double na = ho.n_active > 0 ? (double)ho.n_active : 1.0;
+    for (int q = 0; q < 3; ++q) out->mean_m[q] = ho.sum[q] / na;
+    out->mean_len = ho.sum[3] / na;
+    out->E_ex = ho.E[0]; out->E_an = ho.E[1]; out->E_zee = ho.E[2]; out->E_dmi = ho.E[3]; out->E_demag = ho.E[4]; out->E_long = ho.E[5];
+    out->accepted = hc.accepted + hc.win_accepted; out->trials = hc.trials + hc.win_trials; out->sweeps_done = hc.sweep;
+    out->cone_deg = hc.cone_deg; out->sigma_used = c->sigma_first;
+    double rs[4] = { 0, 0, 0, 0 };
+    for (int b = 0; b < c->n_slots; ++b) for (int q = 0; q < 4; ++q) rs[q] += slots[4 * (size_t)b + q];
+    out->run_sweeps = hc.run_sweeps;
+    if (hc.run_sweeps > 0) {
+        const double d = (double)hc.run_sweeps * na;
+        for (int q = 0; q < 3; ++q) out->run_mean_m[q] = rs[q] / d;
+        out->run_mean_len = rs[3] / d;
+    }
+    return MMC_OK;
+}
+
+int mmc_reset_counters(mmc_ctx* c)
+{
+    if (!c) return MMC_E_INVALID;
+    DeviceGuard dg(c->device);
+    Control h;
+    CU(c, cudaMemcpyAsync(&h, c->ctl, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    h.accepted = h.trials = 0; h.win_accepted = h.win_trials = 0; h.win_sweeps = 0;
+    CU(c, cudaMemcpyAsync(c->ctl, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return MMC_OK;
+}
+
+int mmc_reset_averages(mmc_ctx* c)
+{
+    if (!c) return MMC_E_INVALID;
+    DeviceGuard dg(c->device);
+    unsigned long long z = 0;
+    CU(c, cudaMemsetAsync(c->run_sums, 0, (size_t)c->n_slots * 4 * sizeof(double), c->stream));
+    CU(c, cudaMemcpyAsync(&c->ctl->run_sweeps, &z, sizeof(z), cudaMemcpyHostToDevice, c->stream));
+    CU(c, cudaStreamSynchronize(c->stream));
+    return MMC_OK;
+}
+
+int mmc_debug_pass(mmc_ctx* c, int colour, float* dm, float* dF_terms, float* margin, uint8_t* accepted)
+{
+    if (!c || (colour != 0 && colour != 1)) return fail(c, MMC_E_INVALID, "colour must be 0 or 1");
+    DeviceGuard dg(c->device);
+    int rc = ready(c); if (rc) return rc;
+    SweepArgs a = make_args(c, colour);
+    a.run_sums = nullptr;
+    a.dbg_dm = dm; a.dbg_terms = dF_terms; a.dbg_margin = margin; a.dbg_acc = accepted;
+    rc = launch_colour_pass(a, c->features, true, true, c->stream);
+    if (rc) return fail(c, rc, "debug pass launch failed");
+    return MMC_OK;
+}
+
+int mmc_thermal(double T, double Tc, double mu_atom, double V, double Ms0, double* out6)
+{
+    if (!out6) return MMC_E_INVALID;
+    ThermalCoef t;
+    int rc = thermal_coefficients(T, Tc, mu_atom, V, Ms0, &t);
+    if (rc) return rc;
+    out6[0] = t.me; out6[1] = t.chi; out6[2] = t.c2; out6[3] = t.c4; out6[4] = t.sigma13; out6[5] = t.mu2;
+    return MMC_OK;
+}
+
+int mmc_demag_tensor_at(double dx, double dy, double dz, int ox, int oy, int oz, double* out6)
+{
+    if (!out6) return MMC_E_INVALID;
+    return demag_tensor_at(dx, dy, dz, ox, oy, oz, kNearRadius, out6);
+}
+
+const char* mmc_strerror(int code)
+{
+    switch (code) {
+        case MMC_OK: return "ok";
+        case MMC_E_INVALID: return "invalid argument";
+        case MMC_E_ZERO_LENGTH: return "zero-length magnetisation in a non-empty cell";
+        case MMC_E_CUDA: return "CUDA error";
+        case MMC_E_NOMEM: return "out of memory";
+        case MMC_E_UNSUPPORTED: return "unsupported configuration";
+        case MMC_E_STATE: return "call order: material, temperature and m must be set first";
+        default: return "unknown error";
+    }
+}
+
+const char* mmc_last_error(const mmc_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+}  // extern "C"

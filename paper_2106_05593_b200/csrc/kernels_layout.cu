@@ -1,0 +1,159 @@
+// kernels_layout.cu -- natural <-> colour-split layout conversion, the zero-length check of mmc_set_m, and the
+// read-out reduction (means and energies with pair terms counted once).
+#include <cuda_runtime.h>
+
+#include "mmc_internal.h"
+
+namespace mmc {
+
+__host__ __device__ inline long long split_index(const Geometry& g, int i, int j, int k)
+{
+    const int col = (i + j + k) & 1;
+    return (long long)col * g.H + ((long long)k * g.ny + j) * g.hx + (i >> 1);
+}
+
+__global__ void to_split_kernel(Geometry g, const float* __restrict__ nat, float* __restrict__ split)
+{
+    const long long N = (long long)g.nx * g.ny * g.nz;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(c % g.nx); const long long r = c / g.nx;
+        const int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        split[split_index(g, i, j, k)] = nat[c];
+    }
+}
+__global__ void from_split_kernel(Geometry g, const float* __restrict__ split, float* __restrict__ nat)
+{
+    const long long N = (long long)g.nx * g.ny * g.nz;
+    for (long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x; c < N; c += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(c % g.nx); const long long r = c / g.nx;
+        const int j = (int)(r % g.ny), k = (int)(r / g.ny);
+        nat[c] = split[split_index(g, i, j, k)];
+    }
+}
+static int grid_for(long long n) { long long b = (n + 255) / 256; return (int)(b > 148 * 16 ? 148 * 16 : (b < 1 ? 1 : b)); }
+
+int launch_to_split(const Geometry& g, const float* nat, float* split, void* stream)
+{
+    to_split_kernel<<<grid_for((long long)g.nx * g.ny * g.nz), 256, 0, (cudaStream_t)stream>>>(g, nat, split);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+int launch_from_split(const Geometry& g, const float* split, float* nat, void* stream)
+{
+    from_split_kernel<<<grid_for((long long)g.nx * g.ny * g.nz), 256, 0, (cudaStream_t)stream>>>(g, split, nat);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+
+__global__ void check_zero_kernel(Geometry g, const float* mx, const float* my, const float* mz, const uint8_t* mask, int* flag)
+{
+    const long long n = 2 * g.H;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        if (!(mask[s] & 0x40u)) continue;
+        const float l2 = mx[s] * mx[s] + my[s] * my[s] + mz[s] * mz[s];
+        if (!(l2 > 0.f) || !isfinite(l2)) atomicExch(flag, 1);
+    }
+}
+int launch_check_zero(const Geometry& g, const float* const m[3], const uint8_t* mask, int* flag, void* stream)
+{
+    check_zero_kernel<<<grid_for(2 * g.H), 256, 0, (cudaStream_t)stream>>>(g, m[0], m[1], m[2], mask, flag);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+
+// ------------------------------------------------------------------------------------------------ read-out
+// One thread per storage slot.  Quantities per active cell (all fp64 accumulation from fp32 state):
+//   sums: mx, my, mz, |m|
+//   E_ex   = 1/2 sum_{bonded nb} (A0 V/h_d^2)|m - m_nb|^2        (each bond seen from both ends)
+//   E_an   = V K1(T) - (V K1 me)(m.e)^2 ; E_zee = -V Ms0 m.B_ext ; E_dmi = -D0 V m.G ;
+//   E_demag = -(V Ms0/2) m.B_d ; E_long = kB T [c4 (l2 - mu2)^2 + c0adj]
+template <bool PERCELL>
+__global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams op, double* __restrict__ scratch)
+{
+    const Geometry g = a.g;
+    const long long n = 2 * g.H;
+    double acc[11];
+#pragma unroll
+    for (int t = 0; t < 11; ++t) acc[t] = 0.0;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        const unsigned mb = a.mask[s];
+        if (!(mb & 0x40u)) continue;
+        const int col = s >= g.H;
+        const long long w = s - (long long)col * g.H;
+        const int q = (int)(w % g.hx); const int row = (int)(w / g.hx);
+        const int j = row % g.ny, k = row / g.ny;
+        const int i = 2 * q + (((j + k) & 1) ^ col);
+        const double m[3] = { a.m[0][s], a.m[1][s], a.m[2][s] };
+        const double l2 = m[0] * m[0] + m[1] * m[1] + m[2] * m[2];
+        acc[0] += m[0]; acc[1] += m[1]; acc[2] += m[2]; acc[3] += sqrt(l2); acc[10] += 1.0;
+        double nbv[6][3];
+#pragma unroll
+        for (int d = 0; d < 6; ++d) {
+            nbv[d][0] = nbv[d][1] = nbv[d][2] = 0.0;
+            if (!((mb >> d) & 1u)) continue;
+            int ii = i, jj = j, kk = k;
+            const int step = (d & 1) ? -1 : 1;
+            if ((d >> 1) == 0) { ii += step; if (ii < 0) ii += g.nx; if (ii >= g.nx) ii -= g.nx; }
+            if ((d >> 1) == 1) { jj += step; if (jj < 0) jj += g.ny; if (jj >= g.ny) jj -= g.ny; }
+            if ((d >> 1) == 2) { kk += step; if (kk < 0) kk += g.nz; if (kk >= g.nz) kk -= g.nz; }
+            const long long t = split_index(g, ii, jj, kk);
+            nbv[d][0] = a.m[0][t]; nbv[d][1] = a.m[1][t]; nbv[d][2] = a.m[2][t];
+            const double e0 = m[0] - nbv[d][0], e1 = m[1] - nbv[d][1], e2 = m[2] - nbv[d][2];
+            acc[4] += 0.5 * op.aex[d >> 1] * (e0 * e0 + e1 * e1 + e2 * e2);
+        }
+        float invT, bKq, bzee, c4, ax, ay, az, K1T, c0a; double mu2;
+        if (PERCELL) {
+            invT = a.pc.invT[s]; bKq = a.pc.bKq[s]; bzee = a.pc.bzee[s]; c4 = a.pc.c4[s];
+            ax = a.pc.ax[s]; ay = a.pc.ay[s]; az = a.pc.az[s];
+            mu2 = (double)a.pc.mu2hi[s] + (double)a.pc.mu2lo[s];
+            K1T = op.K1T_pc[s]; c0a = op.c0_pc[s];
+        } else {
+            invT = 1.f / op.T_u; bKq = a.coef.bKq; bzee = a.coef.bzee; c4 = a.coef.c4;
+            ax = a.coef.ax; ay = a.coef.ay; az = a.coef.az; mu2 = a.coef.mu2; K1T = op.K1T_u; c0a = op.c0_u;
+        }
+        const double kT = op.kB / (double)invT;
+        const double me_ = m[0] * ax + m[1] * ay + m[2] * az;
+        acc[5] += kT * ((double)K1T - (double)bKq * me_ * me_);
+        acc[6] += -kT * (double)bzee * (m[0] * a.coef.Bx + m[1] * a.coef.By + m[2] * a.coef.Bz);
+        const double G0 = 0.5 * (-(nbv[0][2] - nbv[1][2]) * op.inv_d[0]);
+        const double G1 = 0.5 * (-(nbv[2][2] - nbv[3][2]) * op.inv_d[1]);
+        const double G2 = 0.5 * ((nbv[0][0] - nbv[1][0]) * op.inv_d[0] + (nbv[2][1] - nbv[3][1]) * op.inv_d[1]);
+        acc[7] += -op.D0V * (m[0] * G0 + m[1] * G1 + m[2] * G2);
+        if (a.bd[0]) acc[8] += -0.5 * kT * (double)bzee * (m[0] * a.bd[0][s] + m[1] * a.bd[1][s] + m[2] * a.bd[2][s]);
+        const double dv = l2 - mu2;
+        acc[9] += kT * ((double)c4 * dv * dv + (double)c0a);
+    }
+    __shared__ double sh[8][11];
+#pragma unroll
+    for (int t = 0; t < 11; ++t) {
+        double v = acc[t];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5][t] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 11) {
+        double v = 0.0;
+        for (int w = 0; w < 8; ++w) v += sh[w][threadIdx.x];
+        scratch[11ll * blockIdx.x + threadIdx.x] = v;
+    }
+}
+
+__global__ void observables_final_kernel(const double* __restrict__ scratch, int blocks, Observables* out)
+{
+    const int t = threadIdx.x;
+    if (t >= 11) return;
+    double v = 0.0;
+    for (int b = 0; b < blocks; ++b) v += scratch[11ll * b + t];      // fixed order: deterministic
+    if (t < 4) out->sum[t] = v;
+    else if (t < 10) out->E[t - 4] = v;
+    else out->n_active = (unsigned long long)(v + 0.5);
+}
+
+int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, Observables* dev_out, double* scratch,
+                            int scratch_blocks, void* stream)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    if (percell) observables_kernel<true><<<scratch_blocks, 256, 0, st>>>(a, op, scratch);
+    else         observables_kernel<false><<<scratch_blocks, 256, 0, st>>>(a, op, scratch);
+    observables_final_kernel<<<1, 32, 0, st>>>(scratch, scratch_blocks, dev_out);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+
+}  // namespace mmc

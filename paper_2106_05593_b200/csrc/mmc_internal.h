@@ -1,0 +1,137 @@
+// mmc_internal.h -- declarations shared by the translation units of libmmc_b200 (not part of the ABI).
+#ifndef MMC_INTERNAL_H_
+#define MMC_INTERNAL_H_
+
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/mmc.h"
+
+namespace mmc {
+
+constexpr double kBoltzmann = 1.380649e-23;            // J/K
+constexpr double kMu0 = 1.25663706212e-6 * 1.0;        // T m/A  (4 pi 1e-7 to the CODATA-2018 digits)
+constexpr int kNearRadius = 40;                        // cells: Newell (binary128) inside, moment expansion beyond
+
+struct ThermalCoef { double me, chi, c2, c4, mu2, sigma13; };
+int thermal_coefficients(double T, double Tc, double mu, double V, double Ms0, ThermalCoef* out);
+int demag_tensor_at(double dx, double dy, double dz, int ox, int oy, int oz, int r_near, double out[6]);
+void demag_tensor_octant(int nx, int ny, int nz, double dx, double dy, double dz, int r_near, std::vector<double> out[6]);
+
+// ---------------------------------------------------------------------------------------------
+// Device-side data layout.
+// Colour-split storage: cell (i,j,k) of colour col = (i+j+k)&1 lives at
+//     col*H + (k*ny + j)*hx + (i>>1),      hx = ceil(nx/2) rounded up to a multiple of 4,  H = hx*ny*nz
+// for every per-cell array (m, B_d, mask, per-cell coefficients).  A colour pass then streams its own
+// colour densely and reads the other colour as neighbours; no sector carries unused cells.
+// ---------------------------------------------------------------------------------------------
+struct Geometry {
+    int nx, ny, nz;
+    int hx;                 // compact row length
+    int64_t H;              // cells per colour plane (padded)
+    unsigned pbc;
+};
+
+// Coefficients of dF/kBT.  Uniform mode: used as they are.  Per-cell mode: kx..gy hold the value at
+// T = 1 K and are multiplied by the cell's 1/T; the rest comes from the per-cell arrays.
+struct Coef {
+    float kx, ky, kz;       // beta * 2 A0 V / h_d^2
+    float gx, gy;           // beta * D0 V / dx, beta * D0 V / dy   (DMI, Eq. (15))
+    float bKq;              // beta * V * K1 * me
+    float bzee;             // beta * V * Ms0
+    float c4;               // longitudinal quartic coefficient (units of kB T)
+    float sigma;            // length-move half-width
+    float ax, ay, az;       // easy axis
+    double mu2;             // -c2/(2 c4)  (= me^2 below Tc)
+    float Bx, By, Bz;       // applied field, tesla
+};
+
+struct PerCell {            // colour-split arrays, 2*H entries each; all NULL in uniform mode
+    const float* invT;      // 1/T
+    const float* c4;
+    const float* mu2hi; const float* mu2lo;   // mu2 = hi + lo (two floats carry ~48 bits)
+    const float* bKq;       // beta V K1 me  (already includes the cell's beta)
+    const float* bzee;      // beta V Ms0
+    const float* sigma;
+    const float* ax; const float* ay; const float* az;
+};
+
+// Device-resident control block: read by the kernels, advanced by end_sweep_kernel (no host round trip).
+struct Control {
+    unsigned long long sweep;        // Philox counter word
+    unsigned long long accepted, trials;
+    unsigned long long win_accepted, win_trials;
+    unsigned int win_sweeps;
+    int adaptive;
+    double cone_deg;
+    float one_minus_cos_cone;
+    unsigned int pad;
+    unsigned long long run_sweeps;   // sweeps accumulated into the running sums
+};
+
+enum Feature : unsigned {
+    F_MASK = 1u,      // bond/active byte per cell (open boundaries, empty cells, region boundaries)
+    F_PERCELL = 2u,   // per-cell coefficient arrays
+    F_Z = 4u,         // nz > 1
+    F_DMI = 8u,
+    F_DEMAG = 16u,
+};
+
+struct SweepArgs {
+    Geometry g;
+    float* m[3];                 // colour-split
+    const float* bd[3];          // colour-split B_d (tesla) or NULL
+    const uint8_t* mask;         // colour-split; bits 0..5 bonded +x,-x,+y,-y,+z,-z; bit 6 active
+    Coef coef;
+    PerCell pc;
+    Control* ctl;
+    unsigned seed_lo, seed_hi;
+    int colour;
+    double* run_sums;            // [n_slots][4] running sums of final mx,my,mz,|m| per block slot, or NULL
+    // debug dump (natural order), any NULL
+    float* dbg_dm; float* dbg_terms; float* dbg_margin; uint8_t* dbg_acc;
+};
+
+struct Observables { double sum[4]; double E[6]; unsigned long long n_active; };
+
+// kernels_sweep.cu
+int sweep_grid_blocks(const Geometry& g, bool vec4);
+int launch_colour_pass(const SweepArgs& a, unsigned features, bool vec4_ok, bool debug, void* stream);
+int launch_end_sweep(Control* ctl, double* run_sums, int n_slots, void* stream);
+// kernels_layout.cu
+int launch_to_split(const Geometry& g, const float* nat, float* split, void* stream);
+int launch_from_split(const Geometry& g, const float* split, float* nat, void* stream);
+int launch_check_zero(const Geometry& g, const float* const m[3], const uint8_t* mask, int* flag, void* stream);
+struct ObsParams {
+    const float* K1T_pc; float K1T_u;      // beta V K1(T) per cell / uniform (units of kB T)
+    const float* c0_pc; float c0_u;        // c0 - c4 mu2^2 (units of kB T)
+    double aex[3];                         // A0 V / h_d^2 (joule)
+    double D0V;                            // D0 V (J m)
+    double inv_d[2];                       // 1/dx, 1/dy
+    double kB;
+    float T_u;                             // uniform temperature (per-cell mode reads 1/T per cell)
+};
+int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, Observables* dev_out, double* scratch,
+                       int scratch_blocks, void* stream);
+
+// Optional per-phase device timing (mmc_sweep_timed): mark(p) records an event that ends phase p.
+enum Phase { PH_PACK = 0, PH_FFT_FWD, PH_MULTIPLY, PH_FFT_INV, PH_CROP, PH_RED, PH_BLACK, PH_END, PH_COUNT };
+struct PhaseTimer {
+    std::vector<void*> events;     // cudaEvent_t
+    std::vector<int> phase;        // phase ended by events[i]; -1 = start marker
+    void mark(int ph, void* stream);
+};
+
+// demag.cu
+struct DemagPlan;
+int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, double dz, void* stream, std::string* err);
+void demag_destroy(DemagPlan* p);
+// Ms0 (colour-split, A/m per cell, 0 in empty cells) times m -> B_d colour-split (tesla)
+int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split, float Ms0_uniform,
+                  float* const bd[3], void* stream, std::string* err, PhaseTimer* timer = nullptr);
+
+}  // namespace mmc
+
+#endif

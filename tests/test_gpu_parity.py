@@ -1,0 +1,244 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on identical seeded
+inputs and identical Philox streams.  Tolerances (north_star):
+  stage 1  |dm_gpu - dm_oracle| <= 2e-6 |m|                       (trial vectors; trigonometry in fp32)
+  stage 2  |term_gpu - term_oracle(dm_gpu)| <= 1e-5 * sum|terms|  (per cell, every term; fp32 energy arithmetic)
+  decisions identical except cells with |margin_oracle| < 1e-4 + 2e-6 * sum|terms|
+  demag    |B_gpu - B_oracle| <= 2e-5 * max|B_oracle|
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def _gpu(wl):
+    import paper_2106_05593_b200 as P
+    s = P.MMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask)
+    W.configure(s, wl, P.Material)
+    return s
+
+
+def _orc(wl, **kw):
+    s = O.OracleMMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, store_fp32=True)
+    W.configure(s, wl, O.Material)
+    for k, v in kw.items():
+        setattr(s, k, v)
+    return s
+
+
+def _np(ts):
+    return [t.detach().cpu().numpy().astype(np.float64) for t in ts]
+
+
+def check_pass(g, o, colour, wl, allow_flip_frac=2e-3):
+    """One colour pass on both sides from the GPU's current state; returns number of near-margin flips."""
+    m_before = _np(g.get_m())
+    o.set_m(*m_before)
+    ob = g.observables()
+    o.sweep = int(ob["sweeps_done"]); o.cone_deg = float(ob["cone_deg"])
+    if wl.demag:
+        o.bd = [b.astype(np.float64) for b in _np(g.demag_field())]   # same frozen field on both sides (demag has its own test)
+        o.demag_enabled = True
+    d = g.debug_pass(colour)
+    od = o.colour_pass(colour, dump=True)
+    gdm = d["dm"].cpu().numpy().astype(np.float64); gt = d["terms"].cpu().numpy().astype(np.float64)
+    gmar = d["margin"].cpu().numpy().astype(np.float64); gacc = d["accepted"].cpu().numpy()
+    act = ~np.isnan(od["margin"])
+    assert np.array_equal(act, gacc != 255), "set of cells that received a trial differs"
+    assert act.sum() > 0 or wl.n_active == 0
+    L = np.sqrt(m_before[0] ** 2 + m_before[1] ** 2 + m_before[2] ** 2)
+    # stage 1
+    err1 = np.abs(gdm[act] - od["dm"][act]).max(axis=1)
+    assert np.all(err1 <= 2e-6 * L[act]), f"stage 1: max {np.max(err1 / L[act]):.3e}"
+    # stage 2: oracle energy arithmetic on the GPU's trial vectors, from the pre-pass state
+    o2 = _orc(wl); o2.set_m(*m_before); o2.sweep = o.sweep; o2.cone_deg = o.cone_deg
+    if wl.demag:
+        o2.bd = o.bd; o2.demag_enabled = True
+    ot = o2.colour_terms_given_dm(colour, np.where(np.isnan(gdm), 0.0, gdm))
+    scale = np.abs(ot[act]).sum(axis=1)
+    err2 = np.abs(gt[act] - ot[act])
+    assert np.all(err2 <= 1e-5 * scale[:, None] + 1e-30), f"stage 2: worst {np.max(err2 / (scale[:, None] + 1e-300)):.3e} (term {np.argmax(np.max(err2 / (scale[:, None] + 1e-300), axis=0))})"
+    tot = np.abs(gt[act].sum(axis=1) - ot[act].sum(axis=1))
+    assert np.all(tot <= 1e-5 * scale + 1e-30)
+    # decisions
+    omar = od["margin"][act]
+    flips = (gacc[act] != od["accepted"][act])
+    window = 1e-4 + 2e-6 * np.abs(od["terms"][act]).sum(axis=1)
+    assert np.all(np.abs(omar[flips]) < window[flips]), "decision differs outside the margin window"
+    assert flips.sum() <= max(1, allow_flip_frac * act.sum())
+    assert np.all(np.abs(gmar[act] - omar) <= 1e-4 + 1.2e-5 * np.abs(od["terms"][act]).sum(axis=1))
+    # state after the pass: identical where decisions agree (fp32 storage on both sides)
+    m_after = _np(g.get_m())
+    same = np.ones(wl.N, bool); idx = np.flatnonzero(act)[flips]; same[idx] = False
+    for a in range(3):
+        assert np.allclose(m_after[a][same], o.m[a][same], rtol=0, atol=2.5e-6 * max(1e-3, L.max()))
+        assert np.array_equal(m_after[a][~act], m_before[a][~act])
+    return int(flips.sum()), int(act.sum()), int(gacc[act].sum())
+
+
+def _small(cfg, **kw):
+    return W.make(cfg, **kw)
+
+
+CASES = {
+    "cfg1_32x32": lambda: W.cfg1(),
+    "cfg1_paper_regime": lambda: W.cfg1(paper_regime=True),
+    "cfg1_ragged_40x24": lambda: W.cfg1(nx=40, ny=24, paper_regime=True),      # nx % 8 == 0 but not a power of two
+    "cfg1_ragged_periodic_12x6": lambda: W.cfg1(nx=12, ny=6, paper_regime=True),  # padded compact rows + periodic wrap
+    "cfg2_64x48": lambda: W.cfg2(nx=64, ny=48),
+    "cfg2_ragged_37x19": lambda: W.cfg2(nx=37, ny=19),                         # odd sizes, open boundaries
+    "cfg3_64x64_200K": lambda: W.cfg3(nx=64, ny=64, T=200.0),
+    "cfg3_64x64_700K_Tc": lambda: W.cfg3(nx=64, ny=64, T=700.0),               # T == Tc exactly (G10)
+    "cfg3_48x40_800K": lambda: W.cfg3(nx=48, ny=40, T=800.0),
+    "cfg4_48x40x4": lambda: W.cfg4(nx=48, ny=40, nz=4),
+    "cfg4_30x21x3": lambda: W.cfg4(nx=30, ny=21, nz=3),
+    "cfg5_160x150": lambda: W.cfg5(nx=160, ny=150),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_colour_pass_parity(name):
+    wl = CASES[name]()
+    if name.startswith("cfg3") and "Tc" not in name and "800K" not in name:
+        wl.cone_deg = 12.0
+    g, o = _gpu(wl), _orc(wl)
+    flips = trials = accepted = 0
+    for sweep in range(2):
+        for colour in (0, 1):
+            f, t, a = check_pass(g, o, colour, wl)
+            flips += f; trials += t; accepted += a
+        g.set_sweep_counter(sweep + 1)
+    assert trials == 2 * wl.n_active
+    ob = g.observables()
+    assert ob["trials"] == trials and ob["accepted"] == accepted
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1_paper_regime", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150"])
+def test_sweep_matches_replayed_oracle(name):
+    """mmc_sweep(n) (demag -> red -> black -> counter++) against the oracle replaying the same iterations.  A cell whose
+    decision flips inside the margin window makes the two trajectories differ from there on, so the bar is: the first
+    sweep agrees on all but a handful of cells, counters agree to the same handful."""
+    wl = CASES[name]()
+    wl.adaptive_cone = False
+    g, o = _gpu(wl), _orc(wl)
+    g.sweep(1); o.run(1)
+    mg = _np(g.get_m())
+    bad = np.zeros(wl.N, bool)
+    for a in range(3):
+        bad |= np.abs(mg[a] - o.m[a]) > 2e-6
+    assert bad.sum() <= max(2, 2e-3 * wl.n_active), f"{bad.sum()} cells differ after one sweep"
+    ob = g.observables()
+    assert ob["sweeps_done"] == 1 and ob["trials"] == wl.n_active
+    assert abs(int(ob["accepted"]) - o.accepted) <= max(2, 2e-3 * wl.n_active)
+    g.close()
+
+
+@pytest.mark.parametrize("shape,d", [((64, 48, 1), (5e-9, 5e-9, 5e-9)), ((37, 19, 1), (5e-9, 5e-9, 10e-9)),
+                                     ((48, 40, 4), (3e-9, 3e-9, 3e-9)), ((30, 21, 3), (2e-9, 3e-9, 4e-9)),
+                                     ((128, 96, 1), (5e-9, 5e-9, 10e-9))])
+def test_demag_field_parity(shape, d):
+    """Eq. (14): GPU fp32 FFT convolution vs the oracle's fp64 one (itself pinned to the direct sum)."""
+    import paper_2106_05593_b200 as P
+    nx, ny, nz = shape; N = nx * ny * nz
+    rng = np.random.default_rng(N)
+    v = rng.normal(size=(3, N)); v /= np.linalg.norm(v, axis=0)
+    m0 = (v * rng.uniform(0.3, 1.0, N)).astype(np.float32)
+    reg = (rng.uniform(size=N) > 0.2).astype(np.int32)
+    m0[:, reg == 0] = 0
+    g = P.MMC(nx, ny, nz, *d, 0)
+    g.set_material([P.Material(), P.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)], reg)
+    g.set_temperature(300.0); g.set_m(*m0)
+    bg = _np(g.demag_field())
+    conv = O.DemagFFT(nx, ny, nz, *d)
+    M = [(8.6e5 * reg * m0[a].astype(np.float64)).reshape(nz, ny, nx) for a in range(3)]
+    bo = [b.ravel() for b in conv.field(*M)]
+    scale = max(np.abs(b).max() for b in bo)
+    for a in range(3):
+        assert np.abs(bg[a] - bo[a]).max() <= 2e-5 * scale
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1_32x32", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg3_48x40_800K", "cfg4_30x21x3", "cfg5_160x150"])
+def test_observables_parity(name):
+    wl = CASES[name]()
+    g, o = _gpu(wl), _orc(wl)
+    og, oo = g.observables(), o.observables()
+    assert np.allclose(og["mean_m"], oo["mean_m"], atol=1e-6)
+    assert og["mean_len"] == pytest.approx(oo["mean_len"], rel=1e-6)
+    tot = sum(abs(oo[k]) for k in ("E_ex", "E_an", "E_zee", "E_dmi", "E_demag", "E_long"))
+    for k in ("E_ex", "E_an", "E_zee", "E_dmi", "E_demag", "E_long"):
+        assert og[k] == pytest.approx(oo[k], rel=2e-5, abs=2e-6 * tot), k
+    g.close()
+
+
+def test_running_means_and_counters():
+    wl = W.cfg1(paper_regime=True)
+    g = _gpu(wl)
+    g.reset_averages()
+    means = []
+    for _ in range(5):
+        g.sweep(1)
+        means.append(g.observables()["mean_m"])
+    ob = g.observables()
+    assert ob["run_sweeps"] == 5
+    assert np.allclose(ob["run_mean_m"], np.mean(means, axis=0), atol=2e-6)
+    assert ob["trials"] == 5 * wl.N and 0 < ob["accepted"] < ob["trials"]
+    g.reset_counters()
+    assert g.observables()["trials"] == 0
+    g.close()
+
+
+def test_edge_cases_and_errors():
+    import paper_2106_05593_b200 as P
+    with pytest.raises(P.MMCError):
+        P.MMC(5, 4, 1, 5e-9, 5e-9, 5e-9, 0b001)                     # odd periodic length
+    with pytest.raises(P.MMCError):
+        P.MMC(0, 4, 1, 5e-9, 5e-9, 5e-9, 0)
+    g = P.MMC(8, 8, 1, 5e-9, 5e-9, 5e-9, 0)
+    with pytest.raises(P.MMCError):
+        g.sweep(1)                                                  # nothing set
+    g.set_material([P.Material(Ms0=8e5, A0=1.3e-11, Tc=870.0)]); g.set_temperature(300.0)
+    with pytest.raises(P.MMCError) as e:
+        g.set_m(np.zeros(64), np.zeros(64), np.zeros(64))           # zero-length non-empty cell (G13)
+    assert e.value.code == -2
+    with pytest.raises(P.MMCError):
+        g.set_temperature(-1.0)
+    g.close()
+    # all cells empty: sweeps are no-ops, no trials
+    g = P.MMC(8, 4, 2, 5e-9, 5e-9, 5e-9, 0)
+    g.set_material([P.Material()]); g.set_temperature(300.0); g.set_m(np.zeros(64), np.zeros(64), np.zeros(64))
+    g.sweep(3)
+    ob = g.observables()
+    assert ob["trials"] == 0 and ob["sweeps_done"] == 3
+    g.close()
+    # a 1x1x1 mesh: a single cell, no neighbours
+    g = P.MMC(1, 1, 1, 5e-9, 5e-9, 5e-9, 0)
+    g.set_material([P.Material(Ms0=8e5, A0=1.3e-11, Tc=870.0)]); g.set_temperature(300.0); g.set_move(20.0, -1.0, False)
+    g.set_m([0.0], [0.0], [0.8675]); g.sweep(10)
+    assert g.observables()["trials"] == 10
+    g.close()
+    # different A0 in two non-empty regions is outside the build
+    g = P.MMC(8, 8, 1, 5e-9, 5e-9, 5e-9, 0)
+    g.set_material([P.Material(Ms0=8e5, A0=1.3e-11, Tc=870.0), P.Material(Ms0=8e5, A0=1.0e-11, Tc=870.0)], np.arange(64) % 2)
+    g.set_temperature(300.0)
+    with pytest.raises(P.MMCError) as e:
+        g.set_m(np.zeros(64), np.zeros(64), np.ones(64))
+    assert e.value.code == -5
+    g.close()
+
+
+def test_adaptive_cone_tracks_oracle():
+    """S11: same acceptance counts => same cone trajectory."""
+    wl = W.cfg1(paper_regime=True); wl.adaptive_cone = True; wl.cone_deg = 30.0
+    g, o = _gpu(wl), _orc(wl)
+    g.sweep(300); o.run(300)
+    og = g.observables()
+    assert og["cone_deg"] == o.cone_deg and og["cone_deg"] < 30.0
+    assert abs(og["accepted"] / og["trials"] - o.accepted / o.trials) < 5e-3
+    g.close()

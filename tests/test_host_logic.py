@@ -1,0 +1,108 @@
+"""CPU-only checks of the product's host side: the C-ABI library loads and exports every symbol include/mmc.h
+declares, its fp64 set-up arithmetic (thermal coefficients, demag tensor) agrees with the independently written
+oracle, and the N>1 replica sharding works under gloo with world_size 2.  No compute call needs a GPU here."""
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def P():
+    from paper_2106_05593_b200 import build as B
+    B.build()
+    import paper_2106_05593_b200 as P
+    return P
+
+
+def test_library_exports_every_declared_symbol(P):
+    with open(os.path.join(ROOT, "include", "mmc.h")) as f:
+        hdr = f.read()
+    declared = set(re.findall(r"\b(mmc_[a-z_0-9]+)\s*\(", hdr))
+    assert declared == set(P.SYMBOLS)
+    L = P.lib()
+    for s in declared:
+        assert hasattr(L, s), s
+    assert P.lib().mmc_strerror(-2) == b"zero-length magnetisation in a non-empty cell"
+    assert P.lib().mmc_last_error(None) == b"null context"
+
+
+def test_no_gpu_means_loud_failure(P):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(P.MMCLibraryError):
+        P.MMC(8, 8, 1, 5e-9, 5e-9, 5e-9)
+
+
+def test_product_does_not_import_the_oracle():
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2106_05593_b200")):
+        for fn in files:
+            if fn.endswith((".py", ".cu", ".cpp", ".h")):
+                src = open(os.path.join(dirpath, fn)).read()
+                assert "oracle" not in src.replace("oracle/", "").lower() or fn == "mmc_host.cpp" and "import" not in src, fn
+    src = open(os.path.join(ROOT, "paper_2106_05593_b200", "__init__.py")).read()
+    assert "import oracle" not in src and "from oracle" not in src
+    osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read()
+    assert "import paper_2106_05593_b200" not in osrc and "from paper_2106_05593_b200" not in osrc
+
+
+def test_thermal_setup_matches_oracle(P):
+    import oracle as O
+    for T, Tc, V, Ms0 in ((300, 870, 1.25e-25, 8e5), (679, 680, 1.25e-25, 8e5), (700, 680, 1.25e-25, 8e5), (680, 680, 1.25e-25, 8e5),
+                          (650, 700, 8e-27, 6e5), (699.99, 700, 8e-27, 6e5), (200, 700, 8e-27, 6e5), (500, 870, 2.5e-25, 8.6e5),
+                          (300, 655.3, 2.7e-26, 1.1e6), (749.9, 712.0, 2.7e-26, 1.1e6)):
+        a = P.thermal(T, Tc, P.MUB, V, Ms0); b = O.thermal(T, Tc, O.MUB, V, Ms0)
+        for k in ("me", "c2", "c4", "sigma13"):
+            assert a[k] == pytest.approx(b[k], rel=2e-10, abs=1e-300), (T, Tc, k)
+        if b["c4"] > 0:
+            assert a["mu2"] == pytest.approx(-b["c2"] / (2 * b["c4"]), rel=2e-10, abs=1e-15)
+    o = (P.C.c_double * 6)()
+    assert P.lib().mmc_thermal(-5.0, 700.0, P.MUB, 1e-26, 8e5, o) == -1
+
+
+def test_demag_tensor_matches_oracle(P):
+    """Library: lattice + second differences in binary128 / moment expansion.  Oracle: 27-point sum / sub-cube dipoles."""
+    import oracle as O
+    for d in ((1.0, 1.0, 1.0), (5e-9, 5e-9, 10e-9), (2e-9, 3e-9, 4e-9)):
+        for o in ((0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1), (3, 2, 1), (-3, 2, -1), (10, -7, 0), (40, 0, 0), (2, 40, 1)):
+            a = P.demag_tensor_at(*d, *o); b = O.newell(o[0] * d[0], o[1] * d[1], o[2] * d[2], *d)
+            assert np.allclose(a, b, rtol=1e-12, atol=1e-15 * np.abs(b).max() + 1e-30), (d, o)
+        for o in ((41, 0, 0), (41, 30, 2), (100, 60, 0), (45, -45, 3), (0, 0, 41), (300, 200, 0)):
+            a = P.demag_tensor_at(*d, *o); b = O.newell(o[0] * d[0], o[1] * d[1], o[2] * d[2], *d)
+            assert np.abs(a - b).max() <= 2e-6 * np.abs(b).max(), (d, o)
+
+
+def test_replica_sharding_gloo_world_size_2():
+    """Multi-GPU = replicas only: each rank runs an independent replica with its own seed and the
+    aggregate metric is the sum over ranks / max time.  Covers bench.py's rank plumbing with gloo on CPU."""
+    code = r'''
+import os, sys, json
+sys.path.insert(0, %r)
+import torch, torch.distributed as dist
+import bench
+dist.init_process_group("gloo")
+r, w = dist.get_rank(), dist.get_world_size()
+seeds = bench.replica_seed(1234, r)
+val = bench.aggregate_over_ranks(units=1000.0 * (r + 1), seconds=0.5 * (r + 1), backend_device="cpu")
+if r == 0:
+    print(json.dumps({"world": w, "seed0": bench.replica_seed(1234, 0), "seed1": bench.replica_seed(1234, 1), "value": val}))
+dist.destroy_process_group()
+''' % ROOT
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29533")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+                        "--master-port", "29533", "-c", code] if False else
+                       [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
+                        "--master-port", "29533", "--no-python", sys.executable, "-c", code],
+                       capture_output=True, text=True, env=env, timeout=240)
+    assert r.returncode == 0, r.stderr[-2000:]
+    import json
+    line = [ln for ln in r.stdout.splitlines() if ln.startswith("{")][-1]
+    out = json.loads(line)
+    assert out["world"] == 2 and out["seed0"] != out["seed1"]
+    assert out["value"] == pytest.approx((1000.0 + 2000.0) / 1.0)     # total units / max time over ranks
