@@ -35,7 +35,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             if f.endswith(".cu"):
                 cmd = [NVCC] + NVFLAGS + ["-c", src, "-o", obj]
             else:
-                cmd = ["g++", "-O2", "-std=gnu++17", "-fPIC", "-c", src, "-o", obj]
+                cmd = ["g++", "-O2", "-std=gnu++17", "-fPIC", "-I/usr/local/cuda/include", "-c", src, "-o", obj]
             r = subprocess.run(cmd, capture_output=True, text=True)
             log = os.path.join(OBJ, f + ".log")
             with open(log, "w") as fh:

@@ -41,7 +41,9 @@ struct mmc_ctx {
     float* bd[3] = { nullptr, nullptr, nullptr };
     uint8_t* mask = nullptr;
     float* Ms0_split = nullptr;
-    float* pc[12] = { nullptr };                  // invT,c4,mu2hi,mu2lo,bKq,bzee,sigma,ax,ay,az,K1T,c0adj
+    uint32_t* cw = nullptr;                       // per-cell mode: class << 7 | mask (colour-split)
+    float* table = nullptr; size_t table_cap = 0; // per-cell mode: kClassFloats floats per class
+    size_t n_classes = 0;
     Control* ctl = nullptr;
     double* run_sums = nullptr; int n_slots = 0;
     double* obs_scratch = nullptr; int obs_blocks = 0;
@@ -129,7 +131,7 @@ int ensure_setup(mmc_ctx* c)
     // mask (bit d: bonded neighbour in direction d; bit 6: active), Ms0
     std::vector<uint8_t> mask(S, 0);
     std::vector<float> ms0(S, 0.f);
-    bool need_mask = (g.nx % 8) != 0;
+    bool need_mask = false;
     bool ms0_uniform = true; double ms0_first = -1;
     const int nn[3] = { g.nx, g.ny, g.nz };
     for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
@@ -164,50 +166,52 @@ int ensure_setup(mmc_ctx* c)
     const double Jd[3] = { 2.0 * A0 * V / (c->dx * c->dx), 2.0 * A0 * V / (c->dy * c->dy), 2.0 * A0 * V / (c->dz * c->dz) };
     Coef cf{};
     cf.Bx = (float)c->B[0]; cf.By = (float)c->B[1]; cf.Bz = (float)c->B[2];
-    auto class_values = [&](const Cls& k, double beta, float out[12], double* mu2) {
+    // one table entry (kClassFloats floats, ClassSlot order) per class
+    auto class_values = [&](const Cls& k, double beta, float* out) {
         const mmc_material& mt = c->regions[k.region];
         double al = std::sqrt(mt.ax * mt.ax + mt.ay * mt.ay + mt.az * mt.az);
         double ex = 0, ey = 0, ez = 1;
         if (al > 0) { ex = mt.ax / al; ey = mt.ay / al; ez = mt.az / al; }
         const double sig = c->sigma_user >= 0 ? c->sigma_user : k.th.sigma13;
-        *mu2 = k.th.mu2;
-        const float hi = (float)k.th.mu2;
-        out[0] = (float)(1.0 / (double)k.T); out[1] = (float)k.th.c4; out[2] = hi; out[3] = (float)(k.th.mu2 - (double)hi);
-        out[4] = (float)(beta * V * mt.K1 * k.th.me); out[5] = (float)(beta * V * mt.Ms0); out[6] = (float)sig;
-        out[7] = (float)ex; out[8] = (float)ey; out[9] = (float)ez;
-        out[10] = (float)(beta * V * mt.K1 * k.th.me * k.th.me * k.th.me);
-        out[11] = (float)((k.th.me > 0 || k.th.mu2 == 0) ? 0.0 : -k.th.c4 * k.th.mu2 * k.th.mu2);
+        out[CS_INVT] = (float)(1.0 / (double)k.T); out[CS_C4] = (float)k.th.c4;
+        std::memcpy(&out[CS_MU2], &k.th.mu2, sizeof(double));
+        out[CS_BKQ] = (float)(beta * V * mt.K1 * k.th.me); out[CS_BZEE] = (float)(beta * V * mt.Ms0); out[CS_SIGMA] = (float)sig;
+        out[CS_AX] = (float)ex; out[CS_AY] = (float)ey; out[CS_AZ] = (float)ez;
+        out[CS_K1T] = (float)(beta * V * mt.K1 * k.th.me * k.th.me * k.th.me);
+        out[CS_C0] = (float)((k.th.me > 0 || k.th.mu2 == 0) ? 0.0 : -k.th.c4 * k.th.mu2 * k.th.mu2);
     };
+    c->n_classes = classes.size();
     if (!c->percell) {
         if (!classes.empty()) {
             const Cls& k = classes[0];
             const double beta = 1.0 / (kB * (double)k.T);
-            float v[12]; double mu2;
-            class_values(k, beta, v, &mu2);
+            float v[kClassFloats];
+            class_values(k, beta, v);
             cf.kx = (float)(beta * Jd[0]); cf.ky = (float)(beta * Jd[1]); cf.kz = (float)(beta * Jd[2]);
             cf.gx = (float)(beta * D0 * V / c->dx); cf.gy = (float)(beta * D0 * V / c->dy);
-            cf.c4 = v[1]; cf.mu2 = mu2; cf.bKq = v[4]; cf.bzee = v[5]; cf.sigma = v[6];
-            cf.ax = v[7]; cf.ay = v[8]; cf.az = v[9];
-            c->K1T_u = v[10]; c->c0_u = v[11];
-            c->sigma_first = v[6];
+            cf.c4 = v[CS_C4]; cf.mu2 = k.th.mu2; cf.bKq = v[CS_BKQ]; cf.bzee = v[CS_BZEE]; cf.sigma = v[CS_SIGMA];
+            cf.ax = v[CS_AX]; cf.ay = v[CS_AY]; cf.az = v[CS_AZ];
+            c->K1T_u = v[CS_K1T]; c->c0_u = v[CS_C0];
+            c->sigma_first = v[CS_SIGMA];
         }
     } else {
-        const double b1 = 1.0 / kB;                   // beta at T = 1 K; the kernel multiplies by the cell's 1/T
+        if (classes.size() > (size_t)kMaxClasses) return fail(c, MMC_E_UNSUPPORTED, "more than 2^25 distinct (region, T) classes");
+        const double b1 = 1.0 / kB;                   // beta at T = 1 K; the kernel multiplies by the class's 1/T
         cf.kx = (float)(b1 * Jd[0]); cf.ky = (float)(b1 * Jd[1]); cf.kz = (float)(b1 * Jd[2]);
         cf.gx = (float)(b1 * D0 * V / c->dx); cf.gy = (float)(b1 * D0 * V / c->dy);
-        std::vector<float> cv(classes.size() * 12);
-        for (size_t q = 0; q < classes.size(); ++q) { double mu2; class_values(classes[q], 1.0 / (kB * (double)classes[q].T), &cv[12 * q], &mu2); }
-        c->sigma_first = cv[6];
-        std::vector<float> arr(S);
-        for (int f = 0; f < 12; ++f) {
-            std::fill(arr.begin(), arr.end(), f == 0 ? 1.f : (f == 9 ? 1.f : 0.f));
-            for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
-                const long long cell = (long long)i + (long long)g.nx * (j + (long long)g.ny * k);
-                const int id = cls_of_cell[(size_t)cell];
-                if (id >= 0) arr[(size_t)split_index_h(g, i, j, k)] = cv[12 * (size_t)id + f];
-            }
-            rc = upload(c, &c->pc[f], arr); if (rc) return rc;
+        std::vector<float> tab(classes.size() * kClassFloats);
+        for (size_t q = 0; q < classes.size(); ++q) class_values(classes[q], 1.0 / (kB * (double)classes[q].T), &tab[kClassFloats * q]);
+        c->sigma_first = tab[CS_SIGMA];
+        if (tab.size() > c->table_cap) { cudaFree(c->table); c->table = nullptr; c->table_cap = tab.size(); }
+        rc = upload(c, &c->table, tab); if (rc) return rc;
+        std::vector<uint32_t> cw(S, 0u);
+        for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
+            const long long cell = (long long)i + (long long)g.nx * (j + (long long)g.ny * k);
+            const int id = cls_of_cell[(size_t)cell];
+            const size_t sidx = (size_t)split_index_h(g, i, j, k);
+            if (id >= 0) cw[sidx] = ((uint32_t)id << 7) | mask[sidx];
         }
+        rc = upload(c, &c->cw, cw); if (rc) return rc;
     }
     c->coef = cf;
     unsigned f = 0;
@@ -242,8 +246,7 @@ SweepArgs make_args(mmc_ctx* c, int colour)
     for (int q = 0; q < 3; ++q) { a.m[q] = c->m[q]; a.bd[q] = c->bd[q]; }
     a.mask = c->mask; a.coef = c->coef;
     a.coef.Bx = (float)c->B[0]; a.coef.By = (float)c->B[1]; a.coef.Bz = (float)c->B[2];
-    a.pc.invT = c->pc[0]; a.pc.c4 = c->pc[1]; a.pc.mu2hi = c->pc[2]; a.pc.mu2lo = c->pc[3]; a.pc.bKq = c->pc[4];
-    a.pc.bzee = c->pc[5]; a.pc.sigma = c->pc[6]; a.pc.ax = c->pc[7]; a.pc.ay = c->pc[8]; a.pc.az = c->pc[9];
+    a.cw = c->percell ? c->cw : nullptr; a.table = c->percell ? reinterpret_cast<const float4*>(c->table) : nullptr;
     a.ctl = c->ctl; a.seed_lo = (unsigned)c->seed; a.seed_hi = (unsigned)(c->seed >> 32);
     a.colour = colour; a.run_sums = c->run_sums;
     return a;
@@ -298,7 +301,7 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     if (!out) return MMC_E_INVALID;
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1 || !(dx > 0) || !(dy > 0) || !(dz > 0) || pbc_mask > 7u) return MMC_E_INVALID;
-    if ((long long)nx * ny * nz > (1ll << 31)) return MMC_E_INVALID;
+    if (2ll * ((((nx + 1) / 2) + 3) / 4 * 4) * ny * nz >= (1ll << 31)) return MMC_E_INVALID;   // kernels use 32-bit element offsets
     const int nn[3] = { nx, ny, nz };
     for (int a = 0; a < 3; ++a)
         if (((pbc_mask >> a) & 1u) && (nn[a] < 2 || (nn[a] & 1))) return MMC_E_INVALID;   // checkerboard needs even periodic lengths
@@ -320,7 +323,7 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
         cudaMemsetAsync(c->m[q], 0, S * sizeof(float), c->stream);
         cudaMemsetAsync(c->bd[q], 0, S * sizeof(float), c->stream);
     }
-    c->n_slots = sweep_grid_blocks(c->g, true);
+    c->n_slots = sweep_grid_blocks(c->g);
     c->obs_blocks = 148 * 4;
     if (cudaMalloc(&c->ctl, sizeof(Control)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->run_sums, (size_t)c->n_slots * 4 * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);
@@ -341,7 +344,7 @@ int mmc_destroy(mmc_ctx* c)
     DeviceGuard dg(c->device);
     cudaStreamSynchronize(c->stream);
     for (int q = 0; q < 3; ++q) { cudaFree(c->m[q]); cudaFree(c->bd[q]); }
-    for (int q = 0; q < 12; ++q) cudaFree(c->pc[q]);
+    cudaFree(c->cw); cudaFree(c->table);
     cudaFree(c->mask); cudaFree(c->Ms0_split); cudaFree(c->ctl); cudaFree(c->run_sums); cudaFree(c->obs_scratch);
     cudaFree(c->d_obs); cudaFree(c->d_flag); cudaFree(c->stage);
     demag_destroy(c->demag);
@@ -463,11 +466,11 @@ static int sweep_impl(mmc_ctx* c, int n_sweeps, PhaseTimer* timer)
     if (timer) timer->mark(-1, c->stream);
     for (int it = 0; it < n_sweeps; ++it) {
         if (c->demag_enabled) { rc = compute_demag(c, timer); if (rc) return rc; }
-        rc = launch_colour_pass(make_args(c, 0), c->features, true, false, c->stream);
+        rc = launch_colour_pass(make_args(c, 0), c->features, false, c->stream);
         if (rc) return fail(c, rc, "red pass launch failed");
         if (timer) timer->mark(PH_RED, c->stream);
         if (c->demag_enabled && c->demag_updates == 2) { rc = compute_demag(c, timer); if (rc) return rc; }
-        rc = launch_colour_pass(make_args(c, 1), c->features, true, false, c->stream);
+        rc = launch_colour_pass(make_args(c, 1), c->features, false, c->stream);
         if (rc) return fail(c, rc, "black pass launch failed");
         if (timer) timer->mark(PH_BLACK, c->stream);
         rc = launch_end_sweep(c->ctl, c->run_sums, c->n_slots, c->stream);
@@ -519,7 +522,7 @@ int mmc_get_observables(mmc_ctx* c, mmc_obs* out)
     SweepArgs a = make_args(c, 0);
     if (!c->demag_enabled) a.bd[0] = a.bd[1] = a.bd[2] = nullptr;
     ObsParams op{};
-    op.K1T_pc = c->pc[10]; op.K1T_u = c->K1T_u; op.c0_pc = c->pc[11]; op.c0_u = c->c0_u;
+    op.K1T_u = c->K1T_u; op.c0_u = c->c0_u;
     op.aex[0] = c->A0 * c->V / (c->dx * c->dx); op.aex[1] = c->A0 * c->V / (c->dy * c->dy); op.aex[2] = c->A0 * c->V / (c->dz * c->dz);
     op.D0V = c->D0 * c->V; op.inv_d[0] = 1.0 / c->dx; op.inv_d[1] = 1.0 / c->dy; op.kB = kBoltzmann;
     op.T_u = c->T_cell.empty() ? (float)c->T_uniform : (c->percell ? 1.f : c->T_cell[0]);
@@ -589,7 +592,7 @@ int mmc_debug_pass(mmc_ctx* c, int colour, float* dm, float* dF_terms, float* ma
     SweepArgs a = make_args(c, colour);
     a.run_sums = nullptr;
     a.dbg_dm = dm; a.dbg_terms = dF_terms; a.dbg_margin = margin; a.dbg_acc = accepted;
-    rc = launch_colour_pass(a, c->features, true, true, c->stream);
+    rc = launch_colour_pass(a, c->features, true, c->stream);
     if (rc) return fail(c, rc, "debug pass launch failed");
     return MMC_OK;
 }

@@ -100,10 +100,11 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
         }
         float invT, bKq, bzee, c4, ax, ay, az, K1T, c0a; double mu2;
         if (PERCELL) {
-            invT = a.pc.invT[s]; bKq = a.pc.bKq[s]; bzee = a.pc.bzee[s]; c4 = a.pc.c4[s];
-            ax = a.pc.ax[s]; ay = a.pc.ay[s]; az = a.pc.az[s];
-            mu2 = (double)a.pc.mu2hi[s] + (double)a.pc.mu2lo[s];
-            K1T = op.K1T_pc[s]; c0a = op.c0_pc[s];
+            const float* t = reinterpret_cast<const float*>(a.table) + (size_t)kClassFloats * (a.cw[s] >> 7);
+            invT = t[CS_INVT]; bKq = t[CS_BKQ]; bzee = t[CS_BZEE]; c4 = t[CS_C4];
+            ax = t[CS_AX]; ay = t[CS_AY]; az = t[CS_AZ];
+            mu2 = *reinterpret_cast<const double*>(t + CS_MU2);
+            K1T = t[CS_K1T]; c0a = t[CS_C0];
         } else {
             invT = 1.f / op.T_u; bKq = a.coef.bKq; bzee = a.coef.bzee; c4 = a.coef.c4;
             ax = a.coef.ax; ay = a.coef.ay; az = a.coef.az; mu2 = a.coef.mu2; K1T = op.K1T_u; c0a = op.c0_u;

@@ -1,10 +1,13 @@
 // kernels_sweep.cu -- the MMC colour pass (PAPER.md:92 steps 1-4, Eq. (5), (7), (10), (11), (14), (15)) for sm_100a.
 //
-// One thread owns four consecutive cells of the active colour in one mesh row (one float4 per SoA array of the
-// colour-split layout, see mmc_internal.h).  Neighbours are all of the other colour: the y/z neighbours are the
-// float4 at the same compact index of the adjacent rows, the x neighbours are the float4 at the same compact
-// index of the other colour's row plus one scalar.  All loads are 16-byte, fully coalesced, and every fetched
-// sector is used.  RNG: one Philox4x32-10 block per cell per sweep keyed by the natural cell index.
+// One thread owns one cell of the active colour.  A warp owns 32 consecutive compact indices of one mesh row of the
+// colour-split layout (mmc_internal.h), so every load of the warp is one fully used 128-byte line: the cell's own
+// vector and B_d, the same compact index of the other colour's row (one x neighbour), that index +-1 (the other x
+// neighbour), and the same compact index of the four adjacent rows (y and z neighbours).  A CTA is a 32 x BY x BZ
+// brick of such cells, so most neighbour lines are shared inside the CTA and come from L1.  Few live registers per
+// thread (one cell) buy the occupancy that hides the HBM latency; the instruction stream, not the byte stream, is
+// the tighter bound of this kernel.
+// RNG: one Philox4x32-10 block per cell per sweep keyed by the natural cell index (replayable on the CPU side).
 #include <cuda_runtime.h>
 
 #include "mmc_internal.h"
@@ -18,9 +21,9 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, unsigned k0, unsigned k1
 {
 #pragma unroll
     for (int r = 0; r < 10; ++r) {
-        const unsigned hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
-        const unsigned hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
-        c = make_uint4(hi1 ^ c.y ^ k0, lo1, hi0 ^ c.w ^ k1, lo0);
+        const unsigned long long p0 = (unsigned long long)0xD2511F53u * c.x;
+        const unsigned long long p1 = (unsigned long long)0xCD9E8D57u * c.z;
+        c = make_uint4((unsigned)(p1 >> 32) ^ c.y ^ k0, (unsigned)p1, (unsigned)(p0 >> 32) ^ c.w ^ k1, (unsigned)p0);
         k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
     }
     return c;
@@ -28,21 +31,51 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, unsigned k0, unsigned k1
 // 23-bit uniform strictly inside (0,1): ((x>>9) + 0.5) * 2^-23, exact in fp32.
 __device__ __forceinline__ float u01(unsigned x) { return fmaf((float)(x >> 9), 1.1920928955078125e-7f, 5.9604644775390625e-8f); }
 
-__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
-__device__ __forceinline__ float4 ld4(const float* p) { return *reinterpret_cast<const float4*>(p); }
-__device__ __forceinline__ float comp(const float4& v, int l) { return l == 0 ? v.x : l == 1 ? v.y : l == 2 ? v.z : v.w; }
+// Single-instruction approximations (MUFU), flush-to-zero: inputs here are never denormal (|m|^2 > 0 is checked at
+// set_m, u in (0,1)).  Relative error <= 2^-22 each, far inside the stage-1 parity tolerance.
+__device__ __forceinline__ float rsqrt_fast(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+// the same with one Newton step, y <- y + (y/2)(1 - x y^2): ~1 ulp, for the two normalisations that set |m + dm|
+__device__ __forceinline__ float rsqrt_1ulp(float x) { const float y = rsqrt_fast(x); return fmaf(0.5f * y, fmaf(-x * y, y, 1.f), y); }
+__device__ __forceinline__ float sqrt_fast(float x) { float y; asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float ln_fast(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y * 0.693147180559945309f; }
+
+// sin and cos of 2 pi u for u in (0,1): quadrant k = rint(4u), r = 4u - k in [-1/2, 1/2] (exact), Taylor polynomials
+// of sin(pi r/2) and cos(pi r/2) (truncation < 3e-8), quadrant fix-up by sign-bit XOR.  No branches, no slow path.
+__device__ __forceinline__ void sincos_2pi(float u, float* sn, float* cs)
+{
+    const float t = 4.f * u;
+    const float tr = t + 12582912.f;                   // 1.5 * 2^23: the low mantissa bits now hold rint(t)
+    const unsigned k = __float_as_uint(tr);
+    const float r = t - (tr - 12582912.f);
+    const float r2 = r * r;
+    float ps = 1.6044118478736e-4f;                    // (pi/2)^9 / 9!
+    ps = fmaf(ps, r2, -4.6817541353187e-3f);           // -(pi/2)^7 / 7!
+    ps = fmaf(ps, r2, 7.9692626246167e-2f);            // (pi/2)^5 / 5!
+    ps = fmaf(ps, r2, -6.4596409750625e-1f);           // -(pi/2)^3 / 3!
+    ps = fmaf(ps, r2, 1.5707963267949f);               // pi/2
+    const float s0 = ps * r;
+    float pc = 9.1926027483942e-4f;                    // (pi/2)^8 / 8!
+    pc = fmaf(pc, r2, -2.0863480763353e-2f);           // -(pi/2)^6 / 6!
+    pc = fmaf(pc, r2, 2.5366950790105e-1f);            // (pi/2)^4 / 4!
+    pc = fmaf(pc, r2, -1.2337005501362f);              // -(pi/2)^2 / 2!
+    const float c0 = fmaf(pc, r2, 1.f);
+    const bool swap = (k & 1u) != 0u;
+    const float cq = swap ? s0 : c0, sq = swap ? c0 : s0;
+    *cs = __uint_as_float(__float_as_uint(cq) ^ (((k + 1u) << 30) & 0x80000000u));   // k = 1, 2: negative
+    *sn = __uint_as_float(__float_as_uint(sq) ^ ((k << 30) & 0x80000000u));          // k = 2, 3: negative
+}
 
 struct CellCoef {
     float kx, ky, kz, gx, gy, bKq, bzee, c4, sigma, ax, ay, az;
     double mu2;
 };
 
-struct CellResult { float dm[3]; float terms[6]; float margin; bool accept; };
+struct CellResult { float dm[3]; float f, L; float terms[6]; float margin; bool accept; };
 
 // The per-cell body: trial move (O3), dF/kBT (O4), Eq. (5) in the log domain (O5).
 //   m      : current vector          S  : sum_d k_d sum_{bonded nb in d}(m_nb - m)   (beta J_d folded into k_d)
 //   selfc  : sum_d k_d n_d / 2       dzx, dzy, dxx, dyy : E-W / N-S differences of m_z, m_x, m_y for the DMI vector
-//   B      : B_ext + B_d (tesla) -- or, when SPLIT (debug), Bext and Bd kept apart for the per-term dump
+//   B      : B_ext + B_d (tesla); TERMS (debug) keeps Zeeman and demag apart for the per-term dump
 template <bool DMI, bool TERMS>
 __device__ __forceinline__ CellResult cell_update(const float m[3], const float S[3], float selfc,
                                                   float dzx, float dzy, float dxx, float dyy,
@@ -52,32 +85,35 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
     CellResult r;
     const float u_cos = u01(rnd.x), u_phi = u01(rnd.y), u_len = u01(rnd.z), u_acc = u01(rnd.w);
     const float l2 = fmaf(m[0], m[0], fmaf(m[1], m[1], m[2] * m[2]));
-    const float iL = rsqrtf(l2), L = l2 * iL;
+    const float iL = rsqrt_1ulp(l2), L = l2 * iL;
     const float n0 = m[0] * iL, n1 = m[1] * iL, n2 = m[2] * iL;
-    // tangent frame: a = axis of the smallest |m_a| (raw components, ties -> lowest index); t1 = e_a x n normalised
+    // tangent frame (O3): a = axis of the smallest |m_a| (raw components, ties -> lowest index), t1 = e_a x n / |.|,
+    // t2 = n x t1.  In the cyclic order (a,b,c) starting at that axis: t1 = (0,-n_c,n_b) it, t2 = (n_b^2+n_c^2,
+    // -n_a n_b, -n_a n_c) it with it = 1/sqrt(n_b^2+n_c^2); a cyclic relabelling keeps the handedness.
     const float a0 = fabsf(m[0]), a1 = fabsf(m[1]), a2 = fabsf(m[2]);
-    int ax = 0; float amin = a0;
-    if (a1 < amin) { ax = 1; amin = a1; }
-    if (a2 < amin) { ax = 2; }
-    float t10, t11, t12;
-    if (ax == 0)      { t10 = 0.f;  t11 = -n2;  t12 = n1; }
-    else if (ax == 1) { t10 = n2;   t11 = 0.f;  t12 = -n0; }
-    else              { t10 = -n1;  t11 = n0;   t12 = 0.f; }
-    const float it = rsqrtf(fmaf(t10, t10, fmaf(t11, t11, t12 * t12)));
-    t10 *= it; t11 *= it; t12 *= it;
-    const float t20 = n1 * t12 - n2 * t11, t21 = n2 * t10 - n0 * t12, t22 = n0 * t11 - n1 * t10;   // n x t1
+    const bool sel1 = a1 < a0;                         // axis 1 beats axis 0
+    const bool sel2 = a2 < (sel1 ? a1 : a0);           // axis 2 beats the better of 0, 1
+    const float na = sel2 ? n2 : (sel1 ? n1 : n0);
+    const float nb = sel2 ? n0 : (sel1 ? n2 : n1);
+    const float nc = sel2 ? n1 : (sel1 ? n0 : n2);
+    const float p2 = fmaf(nb, nb, nc * nc);
+    const float it = rsqrt_1ulp(p2);
     const float w = u_cos * omc;                       // 1 - cos(theta), uniform on the cap
-    const float st = sqrtf(w * (2.f - w));
+    const float st = sqrt_fast(w * (2.f - w));
     float sp, cp;
-    sincospif(2.f * u_phi, &sp, &cp);
-    const float ca = st * cp, sa = st * sp;
-    const float dn0 = fmaf(ca, t10, fmaf(sa, t20, -w * n0));
-    const float dn1 = fmaf(ca, t11, fmaf(sa, t21, -w * n1));
-    const float dn2 = fmaf(ca, t12, fmaf(sa, t22, -w * n2));
+    sincos_2pi(u_phi, &sp, &cp);
+    const float ca = st * cp * it, sa = st * sp * it;  // coefficients of the un-normalised t1, t2
+    // dn = ca (0,-nc,nb) + sa (p2, -na nb, -na nc) - w (na,nb,nc), in the (a,b,c) order
+    const float da = fmaf(sa, p2, -w * na);
+    const float db = fmaf(-ca, nc, fmaf(-sa * na, nb, -w * nb));
+    const float dc = fmaf(ca, nb, fmaf(-sa * na, nc, -w * nc));
+    const float dn0 = sel2 ? db : (sel1 ? dc : da);
+    const float dn1 = sel2 ? dc : (sel1 ? da : db);
+    const float dn2 = sel2 ? da : (sel1 ? db : dc);
     const float s = cf.sigma * fmaf(2.f, u_len, -1.f);  // f = 1 + s
     const float f = 1.f + s;
     const float dm0 = L * fmaf(f, dn0, s * n0), dm1 = L * fmaf(f, dn1, s * n1), dm2 = L * fmaf(f, dn2, s * n2);
-    r.dm[0] = dm0; r.dm[1] = dm1; r.dm[2] = dm2;
+    r.dm[0] = dm0; r.dm[1] = dm1; r.dm[2] = dm2; r.f = f; r.L = L;
     // exchange: -dm.S + selfc |dm|^2
     const float dmsq = fmaf(dm0, dm0, fmaf(dm1, dm1, dm2 * dm2));
     const float ex = fmaf(selfc, dmsq, -fmaf(dm0, S[0], fmaf(dm1, S[1], dm2 * S[2])));
@@ -97,225 +133,184 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
     // interfacial DMI: -2 beta D0 V dm.G, G = 1/2(-dzx/dx, -dzy/dy, dxx/dx + dyy/dy); gx = beta D0 V/dx
     float dmi = 0.f;
     if (DMI) dmi = fmaf(dm0, cf.gx * dzx, fmaf(dm1, cf.gy * dzy, -dm2 * fmaf(cf.gx, dxx, cf.gy * dyy)));
-    // longitudinal: dl2 c4 (2 (l2 - mu2) + dl2), dl2 = |m'|^2 - |m|^2 = l2 s (2 + s); the bracket l2 - mu2 cancels
-    // 2-3 digits below Tc, so it is formed in fp64 from the exact squares of the stored fp32 components
+    // longitudinal: dl2 c4 (2 (l2 - mu2) + dl2), dl2 = |m'|^2 - |m|^2 = l2 s (2 + s) from the length factor (O3:
+    // |m'| = f |m|; the unit vectors above are normalised to ~1 ulp so that the stored m + dm honours this to a
+    // few 1e-7).  The bracket l2 - mu2 cancels 2-3 digits below Tc, so it is formed in fp64 from the exact squares
+    // of the stored fp32 components.
     const double l2d = fma((double)m[0], (double)m[0], fma((double)m[1], (double)m[1], (double)m[2] * (double)m[2]));
     const float dev = (float)(l2d - cf.mu2);
     const float dl2 = l2 * (s * (2.f + s));
     const float lng = dl2 * cf.c4 * fmaf(2.f, dev, dl2);
     const float dF = ((ex + an) + (zee + dem)) + (dmi + lng);
     // Eq. (5): accept iff ln u < 4 ln f - dF
-    r.margin = __logf(u_acc) - 4.f * __logf(f) + dF;
+    r.margin = ln_fast(u_acc) - 4.f * ln_fast(f) + dF;
     r.accept = r.margin < 0.f;
     if (TERMS) { r.terms[0] = ex; r.terms[1] = an; r.terms[2] = zee; r.terms[3] = dmi; r.terms[4] = dem; r.terms[5] = lng; }
     return r;
 }
 
 // ------------------------------------------------------------------------------------------------ the pass
+// blockDim = (32, BY, BZ), 256 threads; grid = (ceil(hxr/32), ceil(ny/BY), ceil(nz/BZ)).
 template <unsigned F, bool DEBUG>
-__global__ void __launch_bounds__(256) colour_pass_kernel(const SweepArgs a, const int rows_first)
+__global__ void __launch_bounds__(256, DEBUG ? 1 : 3) colour_pass_kernel(const SweepArgs a)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0;
     const Geometry g = a.g;
-    const int cpr = g.hx >> 2;                       // float4 chunks per row
-    const int R = g.ny * g.nz;
-    const long long tid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    int chunk, rr;
-    if (rows_first) {                                // consecutive warps walk rows at one 128-cell x block
-        const long long gw = tid >> 5;
-        const int xb = (int)(gw / R);
-        rr = (int)(gw - (long long)xb * R);
-        chunk = xb * 32 + (threadIdx.x & 31);
-    } else {
-        rr = (int)(tid / cpr);
-        chunk = (int)(tid - (long long)rr * cpr);
-    }
-    const bool in_range = rr < R && chunk < cpr;
-    int acc_cnt = 0, tri_cnt = 0;
-    float sum0 = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
+    const int q = blockIdx.x * 32 + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = HASZ ? blockIdx.z * blockDim.z + threadIdx.z : 0;
+    const int col = a.colour;
+    const int s = ((j + k) & 1) ^ col;               // active cells of this row sit at i = 2q + s
+    const int i = 2 * q + s;
+    bool active = i < g.nx && j < g.ny && k < g.nz;
+    bool accept = false;
+    float fs0 = 0.f, fs1 = 0.f, fs2 = 0.f, fs3 = 0.f;   // the cell's final vector and length (running sums)
 
-    if (in_range) {
-        int j, k;
-        if (HASZ) { j = rr / g.nz; k = rr - j * g.nz; } else { j = rr; k = 0; }
-        const int col = a.colour;
-        const int s = ((j + k) & 1) ^ col;           // active cells of this row sit at i = 2q + s
-        const int q0 = chunk << 2;
-        const int row = k * g.ny + j;
+    const int row = k * g.ny + j;
+    // 32-bit element offsets: mmc_create guarantees 2 H < 2^31
+    const unsigned H = (unsigned)g.H;
+    const unsigned ownb = (unsigned)col * H + (unsigned)row * g.hx + q;
+    unsigned mb = 0x7fu, cls = 0u;
+    if (active) {
+        if (PERCELL) { const unsigned w = __ldg(a.cw + ownb); mb = w & 0x7fu; cls = w >> 7; }
+        else if (MASK) mb = __ldg(a.mask + ownb);
+        if ((MASK || PERCELL) && !(mb & 0x40u)) active = false;            // empty cell
+    }
+    if (active) {
         const int hxr = (g.nx + 1) >> 1;             // compact length of the real (unpadded) row
-        const long long ownb = (long long)col * g.H + (long long)row * g.hx + q0;
-        const long long othc = (long long)(1 - col) * g.H;
-        const long long othb = othc + (long long)row * g.hx + q0;
+        const unsigned othc = (unsigned)(1 - col) * H;
+        const unsigned rowb = othc + (unsigned)row * g.hx;
         // neighbour rows (wrap when periodic, else clamp: an out-of-mesh neighbour is never bonded)
         int jn = j + 1, js = j - 1;
         if (jn == g.ny) jn = (g.pbc & 2u) ? 0 : j;
         if (js < 0) js = (g.pbc & 2u) ? g.ny - 1 : j;
-        const long long nb_n = othc + (long long)(k * g.ny + jn) * g.hx + q0;
-        const long long nb_s = othc + (long long)(k * g.ny + js) * g.hx + q0;
-        long long nb_u = 0, nb_d = 0;
+        // x neighbours: s == 0: E at q, W at q-1;  s == 1: W at q, E at q+1 (wrap or clamp)
+        int qe = s ? q + 1 : q - 1;
+        if (qe < 0) qe = (g.pbc & 1u) ? hxr - 1 : 0;
+        if (qe >= hxr) qe = (g.pbc & 1u) ? 0 : q;
+        const unsigned nb_n = othc + (unsigned)(k * g.ny + jn) * g.hx + q;
+        const unsigned nb_s = othc + (unsigned)(k * g.ny + js) * g.hx + q;
+        float m[3], xa[3], xb[3], yn[3], ys[3], zu[3], zd[3], Bd[3] = { 0.f, 0.f, 0.f };
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            m[c] = a.m[c][ownb];
+            xa[c] = __ldg(a.m[c] + rowb + q);
+            xb[c] = __ldg(a.m[c] + rowb + qe);
+            yn[c] = __ldg(a.m[c] + nb_n);
+            ys[c] = __ldg(a.m[c] + nb_s);
+            if (DEMAG) Bd[c] = __ldg(a.bd[c] + ownb);
+        }
         if (HASZ) {
             int ku = k + 1, kd = k - 1;
             if (ku == g.nz) ku = (g.pbc & 4u) ? 0 : k;
             if (kd < 0) kd = (g.pbc & 4u) ? g.nz - 1 : k;
-            nb_u = othc + (long long)(ku * g.ny + j) * g.hx + q0;
-            nb_d = othc + (long long)(kd * g.ny + j) * g.hx + q0;
+            const unsigned nb_u = othc + (unsigned)(ku * g.ny + j) * g.hx + q;
+            const unsigned nb_d = othc + (unsigned)(kd * g.ny + j) * g.hx + q;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) { zu[c] = __ldg(a.m[c] + nb_u); zd[c] = __ldg(a.m[c] + nb_d); }
         }
-        // the one x neighbour outside this thread's float4 of the other colour
-        int qe = (s == 0) ? q0 - 1 : q0 + 4;
-        if (qe < 0) qe = (g.pbc & 1u) ? hxr - 1 : 0;
-        if (qe >= hxr) qe = (g.pbc & 1u) ? 0 : q0;
-        const long long exb = othc + (long long)row * g.hx + qe;
-
-        float4 own[3], ox[3], yn[3], ys[3], zu[3], zd[3], bd[3];
-        float oe[3];
+        CellCoef cf;
+        float kscale = 1.f;
+        if (PERCELL) {
+            const float4* t = a.table + 3ull * cls;
+            const float4 t0 = __ldg(t), t1 = __ldg(t + 1);
+            const float2 t2 = __ldg(reinterpret_cast<const float2*>(t + 2));
+            kscale = t0.x; cf.c4 = t0.y;
+            cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
+            cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
+        } else {
+            cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
+            cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
+        }
+        cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
+        cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
+        // bond weights (1 or 0)
+        float bE = 1.f, bW = 1.f, bN = 1.f, bS = 1.f, bU = HASZ ? 1.f : 0.f, bD = HASZ ? 1.f : 0.f;
+        if (MASK || PERCELL) {
+            bE = (mb & 1u) ? 1.f : 0.f;  bW = (mb & 2u) ? 1.f : 0.f;
+            bN = (mb & 4u) ? 1.f : 0.f;  bS = (mb & 8u) ? 1.f : 0.f;
+            bU = (mb & 16u) ? 1.f : 0.f; bD = (mb & 32u) ? 1.f : 0.f;
+        } else {
+            if (g.nx < 2) { bE = 0.f; bW = 0.f; }
+            if (g.ny < 2) { bN = 0.f; bS = 0.f; }
+        }
+        float S[3], e[3], wv[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            own[c] = ld4(a.m[c] + ownb);
-            ox[c] = ldg4(a.m[c] + othb);
-            yn[c] = ldg4(a.m[c] + nb_n);
-            ys[c] = ldg4(a.m[c] + nb_s);
-            oe[c] = __ldg(a.m[c] + exb);
-            if (HASZ) { zu[c] = ldg4(a.m[c] + nb_u); zd[c] = ldg4(a.m[c] + nb_d); }
-            if (DEMAG) bd[c] = ldg4(a.bd[c] + ownb);
+            e[c] = s ? xb[c] : xa[c]; wv[c] = s ? xa[c] : xb[c];
+            const float sx = bE * (e[c] - m[c]) + bW * (wv[c] - m[c]);
+            const float sy = bN * (yn[c] - m[c]) + bS * (ys[c] - m[c]);
+            float acc = fmaf(cf.kx, sx, cf.ky * sy);
+            if (HASZ) acc = fmaf(cf.kz, bU * (zu[c] - m[c]) + bD * (zd[c] - m[c]), acc);
+            S[c] = acc;
         }
-        unsigned mask4 = 0x7f7f7f7fu;
-        if (MASK) mask4 = __ldg(reinterpret_cast<const unsigned*>(a.mask + ownb));
-        float4 p_invT, p_c4, p_mh, p_ml, p_bKq, p_bzee, p_sig, p_ax, p_ay, p_az;
-        if (PERCELL) {
-            p_invT = ldg4(a.pc.invT + ownb); p_c4 = ldg4(a.pc.c4 + ownb);
-            p_mh = ldg4(a.pc.mu2hi + ownb);  p_ml = ldg4(a.pc.mu2lo + ownb);
-            p_bKq = ldg4(a.pc.bKq + ownb);   p_bzee = ldg4(a.pc.bzee + ownb);
-            p_sig = ldg4(a.pc.sigma + ownb);
-            p_ax = ldg4(a.pc.ax + ownb); p_ay = ldg4(a.pc.ay + ownb); p_az = ldg4(a.pc.az + ownb);
+        float selfc = 0.5f * fmaf(cf.kx, bE + bW, cf.ky * (bN + bS));
+        if (HASZ) selfc = fmaf(0.5f * cf.kz, bU + bD, selfc);
+        float dzx = 0.f, dzy = 0.f, dxx = 0.f, dyy = 0.f;
+        if (DMI) {
+            dzx = bE * e[2] - bW * wv[2];
+            dzy = bN * yn[2] - bS * ys[2];
+            dxx = bE * e[0] - bW * wv[0];
+            dyy = bN * yn[1] - bS * ys[1];
         }
         const unsigned long long sweep = a.ctl->sweep;
         const float omc = a.ctl->one_minus_cos_cone;
         const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
-        const long long nat_row = (long long)row * g.nx;
-        float outm[3][4];
-        bool any_acc = false;
-
-#pragma unroll
-        for (int l = 0; l < 4; ++l) {
-            const unsigned mb = (mask4 >> (8 * l)) & 0xffu;
-            const float m[3] = { comp(own[0], l), comp(own[1], l), comp(own[2], l) };
-            outm[0][l] = m[0]; outm[1][l] = m[1]; outm[2][l] = m[2];
-            if (MASK && !(mb & 0x40u)) continue;                         // empty or padding slot
-            const int q = q0 + l;
-            const int i = 2 * q + s;
-            // x neighbours (E = i+1, W = i-1) of the other colour
-            float e[3], wv[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                float in4_same = comp(ox[c], l);
-                if (s == 0) { e[c] = in4_same; wv[c] = (l == 0) ? oe[c] : comp(ox[c], l - 1); }
-                else        { wv[c] = in4_same; e[c] = (l == 3) ? oe[c] : comp(ox[c], l + 1); }
-            }
-            if (MASK && s == 1 && l < 3 && q == hxr - 1 && (g.pbc & 1u)) {   // ragged periodic row: E wraps to q = 0
-#pragma unroll
-                for (int c = 0; c < 3; ++c) e[c] = __ldg(a.m[c] + othc + (long long)row * g.hx);
-            }
-            CellCoef cf;
-            float kscale = 1.f;
-            if (PERCELL) {
-                kscale = comp(p_invT, l);
-                cf.bKq = comp(p_bKq, l); cf.bzee = comp(p_bzee, l); cf.c4 = comp(p_c4, l); cf.sigma = comp(p_sig, l);
-                cf.ax = comp(p_ax, l); cf.ay = comp(p_ay, l); cf.az = comp(p_az, l);
-                cf.mu2 = (double)comp(p_mh, l) + (double)comp(p_ml, l);
-            } else {
-                cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
-                cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
-            }
-            cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
-            cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
-            // bond weights (1 or 0)
-            float bE = 1.f, bW = 1.f, bN = 1.f, bS = 1.f, bU = HASZ ? 1.f : 0.f, bD = HASZ ? 1.f : 0.f;
-            if (MASK) {
-                bE = (mb & 1u) ? 1.f : 0.f;  bW = (mb & 2u) ? 1.f : 0.f;
-                bN = (mb & 4u) ? 1.f : 0.f;  bS = (mb & 8u) ? 1.f : 0.f;
-                bU = (mb & 16u) ? 1.f : 0.f; bD = (mb & 32u) ? 1.f : 0.f;
-            } else {
-                if (g.nx < 2) { bE = 0.f; bW = 0.f; }
-                if (g.ny < 2) { bN = 0.f; bS = 0.f; }
-            }
-            float S[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const float sx = bE * (e[c] - m[c]) + bW * (wv[c] - m[c]);
-                const float sy = bN * (comp(yn[c], l) - m[c]) + bS * (comp(ys[c], l) - m[c]);
-                float acc = fmaf(cf.kx, sx, cf.ky * sy);
-                if (HASZ) acc = fmaf(cf.kz, bU * (comp(zu[c], l) - m[c]) + bD * (comp(zd[c], l) - m[c]), acc);
-                S[c] = acc;
-            }
-            float selfc = 0.5f * fmaf(cf.kx, bE + bW, cf.ky * (bN + bS));
-            if (HASZ) selfc = fmaf(0.5f * cf.kz, bU + bD, selfc);
-            float dzx = 0.f, dzy = 0.f, dxx = 0.f, dyy = 0.f;
-            if (DMI) {
-                dzx = bE * e[2] - bW * wv[2];
-                dzy = bN * comp(yn[2], l) - bS * comp(ys[2], l);
-                dxx = bE * e[0] - bW * wv[0];
-                dyy = bN * comp(yn[1], l) - bS * comp(ys[1], l);
-            }
-            float Bd[3] = { 0.f, 0.f, 0.f };
-            if (DEMAG) { Bd[0] = comp(bd[0], l); Bd[1] = comp(bd[1], l); Bd[2] = comp(bd[2], l); }
-            const unsigned long long cell = (unsigned long long)(nat_row + i);
-            const uint4 rnd = philox4x32_10(make_uint4((unsigned)cell, (unsigned)(cell >> 32), (unsigned)sweep, (unsigned)(sweep >> 32)),
-                                            a.seed_lo, a.seed_hi);
-            const CellResult r = cell_update<DMI, DEBUG>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
-            tri_cnt++;
-            if (r.accept) {
-                acc_cnt++; any_acc = true;
-                outm[0][l] = m[0] + r.dm[0]; outm[1][l] = m[1] + r.dm[1]; outm[2][l] = m[2] + r.dm[2];
-            }
-            sum0 += outm[0][l]; sum1 += outm[1][l]; sum2 += outm[2][l];
-            sum3 += sqrtf(fmaf(outm[0][l], outm[0][l], fmaf(outm[1][l], outm[1][l], outm[2][l] * outm[2][l])));
-            if (DEBUG) {
-                const long long c = (long long)cell;
-                if (a.dbg_dm) { a.dbg_dm[3 * c] = r.dm[0]; a.dbg_dm[3 * c + 1] = r.dm[1]; a.dbg_dm[3 * c + 2] = r.dm[2]; }
-                if (a.dbg_terms) for (int t = 0; t < 6; ++t) a.dbg_terms[6 * c + t] = r.terms[t];
-                if (a.dbg_margin) a.dbg_margin[c] = r.margin;
-                if (a.dbg_acc) a.dbg_acc[c] = r.accept ? 1 : 0;
-            }
+        const unsigned cell = (unsigned)row * g.nx + i;                   // natural cell index (< 2^31)
+        const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
+        const CellResult r = cell_update<DMI, DEBUG>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
+        accept = r.accept;
+        fs0 = m[0]; fs1 = m[1]; fs2 = m[2]; fs3 = r.L;
+        if (accept) {
+            fs0 += r.dm[0]; fs1 += r.dm[1]; fs2 += r.dm[2]; fs3 *= r.f;     // |m'| = f |m| (O3)
+            a.m[0][ownb] = fs0; a.m[1][ownb] = fs1; a.m[2][ownb] = fs2;
         }
-        if (any_acc) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-                *reinterpret_cast<float4*>(a.m[c] + ownb) = make_float4(outm[c][0], outm[c][1], outm[c][2], outm[c][3]);
+        if (DEBUG) {
+            const size_t c = cell;
+            if (a.dbg_dm) { a.dbg_dm[3 * c] = r.dm[0]; a.dbg_dm[3 * c + 1] = r.dm[1]; a.dbg_dm[3 * c + 2] = r.dm[2]; }
+            if (a.dbg_terms) for (int t = 0; t < 6; ++t) a.dbg_terms[6 * c + t] = r.terms[t];
+            if (a.dbg_margin) a.dbg_margin[c] = r.margin;
+            if (a.dbg_acc) a.dbg_acc[c] = r.accept ? 1 : 0;
         }
     }
 
     // ---- S10: acceptance counters (exact integers) and running sums of the final vectors, per block
     __shared__ int s_cnt[8][2];
     __shared__ float s_sum[8][4];
+    const int acc_cnt = __popc(__ballot_sync(0xffffffffu, accept));
+    const int tri_cnt = __popc(__ballot_sync(0xffffffffu, active));
+    const bool want_sums = a.run_sums != nullptr;
+    if (want_sums) {
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        acc_cnt += __shfl_xor_sync(0xffffffffu, acc_cnt, o);
-        tri_cnt += __shfl_xor_sync(0xffffffffu, tri_cnt, o);
-        sum0 += __shfl_xor_sync(0xffffffffu, sum0, o);
-        sum1 += __shfl_xor_sync(0xffffffffu, sum1, o);
-        sum2 += __shfl_xor_sync(0xffffffffu, sum2, o);
-        sum3 += __shfl_xor_sync(0xffffffffu, sum3, o);
+        for (int o = 16; o > 0; o >>= 1) {
+            fs0 += __shfl_xor_sync(0xffffffffu, fs0, o);
+            fs1 += __shfl_xor_sync(0xffffffffu, fs1, o);
+            fs2 += __shfl_xor_sync(0xffffffffu, fs2, o);
+            fs3 += __shfl_xor_sync(0xffffffffu, fs3, o);
+        }
     }
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    if (lane == 0) {
+    const int tlin = threadIdx.x + 32 * (threadIdx.y + blockDim.y * threadIdx.z);
+    const int warp = tlin >> 5;
+    if (threadIdx.x == 0) {
         s_cnt[warp][0] = acc_cnt; s_cnt[warp][1] = tri_cnt;
-        s_sum[warp][0] = sum0; s_sum[warp][1] = sum1; s_sum[warp][2] = sum2; s_sum[warp][3] = sum3;
+        s_sum[warp][0] = fs0; s_sum[warp][1] = fs1; s_sum[warp][2] = fs2; s_sum[warp][3] = fs3;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        int ac = 0, tc = 0; double d0 = 0, d1 = 0, d2 = 0, d3 = 0;
-        const int nw = blockDim.x >> 5;
-        for (int w = 0; w < nw; ++w) {
+    if (tlin == 0) {
+        int ac = 0, tc = 0; float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) {
             ac += s_cnt[w][0]; tc += s_cnt[w][1];
             d0 += s_sum[w][0]; d1 += s_sum[w][1]; d2 += s_sum[w][2]; d3 += s_sum[w][3];
         }
         if (tc) {
             atomicAdd(&a.ctl->win_trials, (unsigned long long)tc);
             if (ac) atomicAdd(&a.ctl->win_accepted, (unsigned long long)ac);
-        }
-        if (a.run_sums) {                            // one slot per block: fixed summation order, no fp atomics
-            double* slot = a.run_sums + 4ll * blockIdx.x;
-            slot[0] += d0; slot[1] += d1; slot[2] += d2; slot[3] += d3;
+            if (want_sums) {                          // one slot per block: fixed summation order, no fp atomics
+                double* slot = a.run_sums + 4ll * (blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z));
+                slot[0] += (double)d0; slot[1] += (double)d1; slot[2] += (double)d2; slot[3] += (double)d3;
+            }
         }
     }
 }
@@ -348,30 +343,36 @@ int launch_end_sweep(Control* ctl, double*, int, void* stream)
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 
-int sweep_grid_blocks(const Geometry& g, bool)
+// CTA brick 32 x BY x BZ (256 threads): BZ covers up to 4 layers so that the z neighbours are lines the CTA reads anyway.
+static void brick(const Geometry& g, dim3* block, dim3* grid)
 {
-    const long long cpr = g.hx >> 2, R = (long long)g.ny * g.nz;
-    long long threads;
-    if (cpr >= 32 && cpr % 32 == 0) threads = cpr * R;
-    else threads = cpr * R;
-    return (int)((threads + 255) / 256);
+    const int bz = g.nz >= 4 ? 4 : (g.nz >= 2 ? 2 : 1);
+    const int by = 8 / bz;
+    const int hxr = (g.nx + 1) >> 1;
+    *block = dim3(32, by, bz);
+    *grid = dim3((hxr + 31) / 32, (g.ny + by - 1) / by, (g.nz + bz - 1) / bz);
+}
+
+int sweep_grid_blocks(const Geometry& g)
+{
+    dim3 b, gr; brick(g, &b, &gr);
+    return (int)(gr.x * gr.y * gr.z);
 }
 
 template <unsigned F>
 static int launch_variant(const SweepArgs& a, bool debug, cudaStream_t st)
 {
-    const long long cpr = a.g.hx >> 2;
-    const int rows_first = (cpr >= 32 && cpr % 32 == 0) ? 1 : 0;
-    const int blocks = sweep_grid_blocks(a.g, true);
-    if (debug) colour_pass_kernel<F, true><<<blocks, 256, 0, st>>>(a, rows_first);
-    else       colour_pass_kernel<F, false><<<blocks, 256, 0, st>>>(a, rows_first);
+    dim3 b, gr; brick(a.g, &b, &gr);
+    if (gr.y > 65535u || gr.z > 65535u) return MMC_E_UNSUPPORTED;
+    if (debug) colour_pass_kernel<F, true><<<gr, b, 0, st>>>(a);
+    else       colour_pass_kernel<F, false><<<gr, b, 0, st>>>(a);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 
 // Instantiated variants: the smallest instantiated superset of the requested features is used.  F_PERCELL must
-// match exactly (its arrays exist only in per-cell mode); the mask and B_d arrays always exist (B_d = 0 when the
-// demag term is off), so the other flags may be over-approximated.
-int launch_colour_pass(const SweepArgs& a, unsigned f, bool, bool debug, void* stream)
+// match exactly (its word array and table exist only in per-cell mode); the mask and B_d arrays always exist
+// (B_d = 0 when the demag term is off), so the other flags may be over-approximated.
+int launch_colour_pass(const SweepArgs& a, unsigned f, bool debug, void* stream)
 {
     cudaStream_t st = (cudaStream_t)stream;
     constexpr unsigned UALL = F_MASK | F_Z | F_DMI | F_DEMAG, PALL = UALL | F_PERCELL;

@@ -3,6 +3,7 @@
 #define MMC_INTERNAL_H_
 
 #include <stdint.h>
+#include <vector_types.h>
 
 #include <string>
 #include <vector>
@@ -48,15 +49,15 @@ struct Coef {
     float Bx, By, Bz;       // applied field, tesla
 };
 
-struct PerCell {            // colour-split arrays, 2*H entries each; all NULL in uniform mode
-    const float* invT;      // 1/T
-    const float* c4;
-    const float* mu2hi; const float* mu2lo;   // mu2 = hi + lo (two floats carry ~48 bits)
-    const float* bKq;       // beta V K1 me  (already includes the cell's beta)
-    const float* bzee;      // beta V Ms0
-    const float* sigma;
-    const float* ax; const float* ay; const float* az;
-};
+// Per-cell mode (more than one coefficient class, e.g. cfg 4: one class per distinct (region, T) pair): every cell
+// carries one 32-bit word  cw = class << 7 | mask byte  (colour-split, 2*H entries), and the coefficients of a
+// class sit in a table of kClassFloats floats per class (48 B = three 16-byte loads).  The table is a few MB for
+// the paper's granular film and stays L2-resident; the HBM cost per cell is the 4-byte word.
+constexpr int kClassFloats = 12;
+enum ClassSlot { CS_INVT = 0, CS_C4 = 1, CS_MU2 = 2 /* double in slots 2,3 */, CS_BKQ = 4, CS_BZEE = 5, CS_SIGMA = 6,
+                 CS_AX = 7, CS_AY = 8, CS_AZ = 9, CS_K1T = 10 /* beta V K1(T), read-out only */,
+                 CS_C0 = 11 /* c0 - c4 mu2^2, read-out only */ };
+constexpr unsigned kMaxClasses = 1u << 25;
 
 // Device-resident control block: read by the kernels, advanced by end_sweep_kernel (no host round trip).
 struct Control {
@@ -84,8 +85,9 @@ struct SweepArgs {
     float* m[3];                 // colour-split
     const float* bd[3];          // colour-split B_d (tesla) or NULL
     const uint8_t* mask;         // colour-split; bits 0..5 bonded +x,-x,+y,-y,+z,-z; bit 6 active
+    const uint32_t* cw;          // per-cell mode: class << 7 | mask (colour-split), else NULL
+    const float4* table;         // per-cell mode: kClassFloats floats per class, else NULL
     Coef coef;
-    PerCell pc;
     Control* ctl;
     unsigned seed_lo, seed_hi;
     int colour;
@@ -97,16 +99,16 @@ struct SweepArgs {
 struct Observables { double sum[4]; double E[6]; unsigned long long n_active; };
 
 // kernels_sweep.cu
-int sweep_grid_blocks(const Geometry& g, bool vec4);
-int launch_colour_pass(const SweepArgs& a, unsigned features, bool vec4_ok, bool debug, void* stream);
+int sweep_grid_blocks(const Geometry& g);          // CTAs of one colour pass (= number of running-sum slots)
+int launch_colour_pass(const SweepArgs& a, unsigned features, bool debug, void* stream);
 int launch_end_sweep(Control* ctl, double* run_sums, int n_slots, void* stream);
 // kernels_layout.cu
 int launch_to_split(const Geometry& g, const float* nat, float* split, void* stream);
 int launch_from_split(const Geometry& g, const float* split, float* nat, void* stream);
 int launch_check_zero(const Geometry& g, const float* const m[3], const uint8_t* mask, int* flag, void* stream);
 struct ObsParams {
-    const float* K1T_pc; float K1T_u;      // beta V K1(T) per cell / uniform (units of kB T)
-    const float* c0_pc; float c0_u;        // c0 - c4 mu2^2 (units of kB T)
+    float K1T_u;                           // beta V K1(T), uniform mode (units of kB T); per-cell mode: class table
+    float c0_u;                            // c0 - c4 mu2^2, uniform mode (units of kB T)
     double aex[3];                         // A0 V / h_d^2 (joule)
     double D0V;                            // D0 V (J m)
     double inv_d[2];                       // 1/dx, 1/dy
