@@ -45,7 +45,7 @@ struct mmc_ctx {
     float* table = nullptr; size_t table_cap = 0; // per-cell mode: kClassFloats floats per class
     size_t n_classes = 0;
     Control* ctl = nullptr;
-    double* run_sums = nullptr; int n_slots = 0;
+    unsigned long long* run_sums = nullptr;       // [4] fixed-point running sums (kSumScale)
     double* obs_scratch = nullptr; int obs_blocks = 0;
     Observables* d_obs = nullptr;
     int* d_flag = nullptr;
@@ -323,16 +323,15 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
         cudaMemsetAsync(c->m[q], 0, S * sizeof(float), c->stream);
         cudaMemsetAsync(c->bd[q], 0, S * sizeof(float), c->stream);
     }
-    c->n_slots = sweep_grid_blocks(c->g);
     c->obs_blocks = 148 * 4;
     if (cudaMalloc(&c->ctl, sizeof(Control)) != cudaSuccess) return bail(MMC_E_NOMEM);
-    if (cudaMalloc(&c->run_sums, (size_t)c->n_slots * 4 * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaMalloc(&c->run_sums, 4 * sizeof(unsigned long long)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->obs_scratch, (size_t)c->obs_blocks * 11 * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->d_obs, sizeof(Observables)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->d_flag, sizeof(int)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->stage, (size_t)nx * ny * nz * sizeof(float)) != cudaSuccess) return bail(MMC_E_NOMEM);
     cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream);
-    cudaMemsetAsync(c->run_sums, 0, (size_t)c->n_slots * 4 * sizeof(double), c->stream);
+    cudaMemsetAsync(c->run_sums, 0, 4 * sizeof(unsigned long long), c->stream);
     if (push_control(c, false) != MMC_OK) return bail(MMC_E_CUDA);
     *out = c;
     return MMC_OK;
@@ -473,7 +472,7 @@ static int sweep_impl(mmc_ctx* c, int n_sweeps, PhaseTimer* timer)
         rc = launch_colour_pass(make_args(c, 1), c->features, false, c->stream);
         if (rc) return fail(c, rc, "black pass launch failed");
         if (timer) timer->mark(PH_BLACK, c->stream);
-        rc = launch_end_sweep(c->ctl, c->run_sums, c->n_slots, c->stream);
+        rc = launch_end_sweep(c->ctl, c->stream);
         if (rc) return fail(c, rc, "end_sweep launch failed");
         if (timer) timer->mark(PH_END, c->stream);
     }
@@ -537,10 +536,10 @@ int mmc_get_observables(mmc_ctx* c, mmc_obs* out)
     rc = launch_observables(a, c->percell, op, c->d_obs, c->obs_scratch, c->obs_blocks, c->stream);
     if (rc) return fail(c, rc, "observables launch failed");
     Observables ho; Control hc;
-    std::vector<double> slots((size_t)c->n_slots * 4);
+    long long fixed[4] = { 0, 0, 0, 0 };
     CU(c, cudaMemcpyAsync(&ho, c->d_obs, sizeof(ho), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaMemcpyAsync(&hc, c->ctl, sizeof(hc), cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaMemcpyAsync(slots.data(), c->run_sums, slots.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaMemcpyAsync(fixed, c->run_sums, sizeof(fixed), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     std::memset(out, 0, sizeof(*out));
     const double na = ho.n_active > 0 ? (double)ho.n_active : 1.0;
@@ -550,7 +549,7 @@ int mmc_get_observables(mmc_ctx* c, mmc_obs* out)
     out->accepted = hc.accepted + hc.win_accepted; out->trials = hc.trials + hc.win_trials; out->sweeps_done = hc.sweep;
     out->cone_deg = hc.cone_deg; out->sigma_used = c->sigma_first;
     double rs[4] = { 0, 0, 0, 0 };
-    for (int b = 0; b < c->n_slots; ++b) for (int q = 0; q < 4; ++q) rs[q] += slots[4 * (size_t)b + q];
+    for (int q = 0; q < 4; ++q) rs[q] = (double)fixed[q] / (double)kSumScale;
     out->run_sweeps = hc.run_sweeps;
     if (hc.run_sweeps > 0) {
         const double d = (double)hc.run_sweeps * na;
@@ -578,7 +577,7 @@ int mmc_reset_averages(mmc_ctx* c)
     if (!c) return MMC_E_INVALID;
     DeviceGuard dg(c->device);
     unsigned long long z = 0;
-    CU(c, cudaMemsetAsync(c->run_sums, 0, (size_t)c->n_slots * 4 * sizeof(double), c->stream));
+    CU(c, cudaMemsetAsync(c->run_sums, 0, 4 * sizeof(unsigned long long), c->stream));
     CU(c, cudaMemcpyAsync(&c->ctl->run_sweeps, &z, sizeof(z), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     return MMC_OK;

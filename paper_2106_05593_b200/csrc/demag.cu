@@ -1,33 +1,54 @@
-// demag.cu -- demagnetising field of Eq. (14): B_d = -mu0 N (*) M by zero-padded FFT convolution.
-//   S0 pack + pad (M = Ms0 m from the colour-split state)      -> pack_kernel
-//   S1 forward real-to-complex FFT of the three components     -> cuFFT (round-1 baseline)
-//   S2 tensor multiply with the real-valued spectrum of N      -> multiply_kernel
-//   S3 inverse FFT + crop to the N physical cells              -> cuFFT + crop_kernel (writes colour-split B_d)
-// The tensor spectrum is built once at set-up in fp64 (host Newell/moment table -> device placement -> D2Z) and kept
-// in fp32 with the factor -mu0/(Px Py Pz) folded in.
+// demag.cu -- demagnetising field of Eq. (14): B_d = -mu0 N (*) M by zero-padded FFT convolution,
+// with hand-written shared-memory FFTs that never touch the padding.
+//
+//   kernel A  "rows"    S0+S1: for a tile of RJ mesh rows (all nz layers): M = Ms0 m straight from the colour-split
+//                       state (even cells = real part, odd cells = imaginary part: the colour planes ARE the even/odd
+//                       packing of the half-length real-FFT trick), FFT of length Px/2 in shared memory, untangle to
+//                       the Px/2+1 non-redundant frequencies, z-DFT across the layers in registers, store transposed:
+//                       T[c][kz][kx][j]  (j fastest, so that a column is contiguous for kernel B).
+//   kernel B  "columns" S1+S2+S3: one CTA per (kx, kz): the three components' columns (ny complex each) -> zero-pad to
+//                       Py in shared memory -> forward FFT -> real symmetric 3x3 tensor multiply in the transform's
+//                       digit-reversed order (the tensor spectrum is stored in that order) -> inverse FFT -> the ny
+//                       kept rows back in place.
+//   kernel C  "rows^-1" S3: mirror of A: inverse z-DFT in registers, re-tangle, inverse FFT of length Px/2, and the
+//                       real/imaginary parts go straight to the even/odd cells of the colour-split B_d.
+// Padded lengths are powers of two >= 2n-1 (any mesh size works).  All normalisation and -mu0 are folded into the
+// tensor spectrum, which is built once at set-up in fp64 (host Newell/moment table -> device placement -> cuFFT D2Z).
 #include <cuda_runtime.h>
 #include <cufft.h>
 
+#include <cmath>
+
+#include "fft_smem.cuh"
 #include "mmc_internal.h"
 
 namespace mmc {
 
+using fft::Plan;
+
 struct DemagPlan {
     Geometry g;
-    int Px, Py, Pz, Cx;              // padded real dims, complex x length Px/2+1
-    size_t rsize, csize;             // elements per component
-    float* rbuf = nullptr;           // 3 * rsize, zero outside the physical block (never written there)
-    float* obuf = nullptr;           // 3 * rsize, inverse-transform output
-    float2* cbuf = nullptr;          // 3 * csize
-    float* khat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };
-    cufftHandle fwd = 0, inv = 0;
-    bool have_fwd = false, have_inv = false;
+    int Px, Py, Pz, Hx, Cx;          // padded lengths, Hx = Px/2 (complex row FFT length), Cx = Hx+1 frequencies
+    int lgPz;
+    Plan px, py;                     // stage plans of the length-Hx and length-Py transforms
+    int RJ;                          // rows per CTA in kernels A and C
+    int RS;                          // shared-memory row stride (float2) in kernels A and C
+    size_t smemA, smemB;
+    int threadsA, threadsB;
+    float2* twx = nullptr;           // exp(-2 pi i k / Px), k < Px
+    float2* twy = nullptr;           // exp(-2 pi i k / Py), k < Py
+    float2* T = nullptr;             // [3][Pz][Cx][ny]
+    float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
 };
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { if (err) *err = std::string(#x) + ": " + cudaGetErrorString(e_); return MMC_E_CUDA; } } while (0)
 #define CF(x) do { cufftResult r_ = (x); if (r_ != CUFFT_SUCCESS) { if (err) *err = std::string(#x) + ": cufft error " + std::to_string((int)r_); return MMC_E_CUDA; } } while (0)
 
-// place the octant table on the padded periodic grid: offset o_d (|o_d| < N_d) at index o_d mod P_d, index N_d zero;
+static int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+static int padded_pow2(int n, int at_least) { int p = at_least; while (p < 2 * n - 1) p <<= 1; return p; }
+
+// ------------------------------------------------------------------------------------------------ set-up kernels
+// place the octant table on the padded periodic grid: offset o_d (|o_d| < N_d) at index o_d mod P_d, zero elsewhere;
 // diagonal components even, N_ab odd in coordinates a and b.
 __global__ void place_kernel(int nx, int ny, int nz, int Px, int Py, int Pz, const double* __restrict__ oct, int sx, int sy, int sz,
                              double* __restrict__ full)
@@ -37,8 +58,7 @@ __global__ void place_kernel(int nx, int ny, int nz, int Px, int Py, int Pz, con
         const int x = (int)(t % Px); const long long r = t / Px; const int y = (int)(r % Py), z = (int)(r / Py);
         int ox = x < nx ? x : x - Px, oy = y < ny ? y : y - Py, oz = z < nz ? z : z - Pz;
         double v = 0.0;
-        const bool hole = (Px > 1 && x == nx) || (Py > 1 && y == ny) || (Pz > 1 && z == nz);
-        if (!hole) {
+        if (ox > -nx && oy > -ny && oz > -nz) {
             double s = 1.0;
             if (ox < 0) { ox = -ox; s *= sx; }
             if (oy < 0) { oy = -oy; s *= sy; }
@@ -48,61 +68,304 @@ __global__ void place_kernel(int nx, int ny, int nz, int Px, int Py, int Pz, con
         full[t] = v;
     }
 }
-__global__ void real_part_kernel(const double2* __restrict__ z, float* __restrict__ out, long long n, double scale)
+// spectrum (D2Z layout [kz][ky][kx <= Px/2]) -> nhat[kz <= Pz/2][kx][p], p = position of ky in the y transform's output
+__global__ void permute_kernel(const double2* __restrict__ spec, float* __restrict__ out, int Cx, int Py, int Kz, Plan py, double scale)
 {
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x)
-        out[t] = (float)(scale * z[t].x);
+    const long long n = (long long)Kz * Cx * Py;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        const int p = (int)(t % Py); const long long r = t / Py; const int kx = (int)(r % Cx), kz = (int)(r / Cx);
+        const int ky = fft::freq_of_pos(py, p);
+        out[t] = (float)(scale * spec[((long long)kz * Py + ky) * Cx + kx].x);
+    }
+}
+__global__ void twiddle_kernel(float2* tw, int P)
+{
+    for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < P; k += gridDim.x * blockDim.x) {
+        double s, c;
+        sincospi(-2.0 * (double)k / (double)P, &s, &c);
+        tw[k] = make_float2((float)c, (float)s);
+    }
 }
 
 static int blocks_for(long long n) { long long b = (n + 255) / 256; return (int)(b > 148 * 32 ? 148 * 32 : (b < 1 ? 1 : b)); }
+
+// ------------------------------------------------------------------------------------------------ kernels A and C
+struct RowArgs {
+    Geometry g;
+    int Hx, lgHx, Cx, lgPx, RJ, lgRJ, RS;
+    Plan px;
+    const float2* twx;
+    const float* m[3]; const float* Ms0; float Ms0_u;     // kernel A input (colour-split)
+    float* bd[3];                                         // kernel C output (colour-split)
+    float2* T;                                            // [3][PZ][Cx][ny]
+};
+
+// kernel A: grid (ceil(ny/RJ), 3 components); dynamic smem = RJ * nz * RS float2
+template <int PZ>
+__global__ void __launch_bounds__(512) rows_fwd_kernel(const RowArgs a)
+{
+    extern __shared__ float2 sm[];
+    const Geometry g = a.g;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int c = blockIdx.y, j0 = blockIdx.x * a.RJ;
+    const int nrows = a.RJ * g.nz, Hx = a.Hx, hxr = (g.nx + 1) >> 1;
+    const float* __restrict__ mc = a.m[c];
+    // S0: M = Ms0 m; even cells -> real part, odd cells -> imaginary part (z[n] = x[2n] + i x[2n+1]); zero padding
+    for (int idx = tid; idx < (nrows << a.lgHx); idx += nt) {
+        const int r = idx >> a.lgHx, n = idx & (Hx - 1);
+        const int k = r >> a.lgRJ, j = j0 + (r & (a.RJ - 1));
+        float2 v = make_float2(0.f, 0.f);
+        if (j < g.ny && n < hxr) {
+            const int row = k * g.ny + j, par = (j + k) & 1;
+            const unsigned se = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx + n;
+            const unsigned so = (unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx + n;
+            v.x = (a.Ms0 ? __ldg(a.Ms0 + se) : a.Ms0_u) * __ldg(mc + se);
+            if (2 * n + 1 < g.nx) v.y = (a.Ms0 ? __ldg(a.Ms0 + so) : a.Ms0_u) * __ldg(mc + so);
+        }
+        sm[r * a.RS + fft::pad(n)] = v;
+    }
+    __syncthreads();
+    fft::fft_forward(a.px, sm, nrows, a.RS, a.twx, a.lgPx, tid, nt);
+    // untangle: Z (length Hx, digit-reversed) -> X'[k] = 2 X[k], k = 0..Hx, with X the length-Px spectrum of the real row
+    for (int idx = tid; idx < (nrows << a.lgHx); idx += nt) {
+        const int r = idx >> a.lgHx, k = idx & (Hx - 1);
+        if (2 * k > Hx) continue;
+        float2* base = sm + r * a.RS;
+        if (k == 0) {
+            const float2 z0 = base[0];
+            base[0] = make_float2(2.f * (z0.x + z0.y), 0.f);
+            base[fft::pad(Hx)] = make_float2(2.f * (z0.x - z0.y), 0.f);
+        } else {
+            const int k2 = Hx - k;
+            const int pa = fft::pad(fft::pos_of_freq(a.px, k)), pb = fft::pad(fft::pos_of_freq(a.px, k2));
+            const float2 A = base[pa], B = base[pb];                 // Z[k], Z[Hx-k]
+            const float2 S = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
+            const float2 t = fft::cmul(__ldg(a.twx + k), D);         // w^k (Z[k] - conj Z[Hx-k])
+            base[pa] = make_float2(S.x + t.y, S.y - t.x);
+            if (k2 != k) base[pb] = make_float2(S.x - t.y, -S.y - t.x);
+        }
+    }
+    __syncthreads();
+    // z-DFT across the layers (registers) and transposed store: lanes run over the RJ rows fastest
+    const int items = a.Cx << a.lgRJ;
+    for (int idx = tid; idx < items; idx += nt) {
+        const int jj = idx & (a.RJ - 1), kx = idx >> a.lgRJ, j = j0 + jj;
+        const int pp = fft::pad(kx < Hx ? fft::pos_of_freq(a.px, kx) : Hx);
+        float2 v[PZ];
+#pragma unroll
+        for (int k = 0; k < PZ; ++k) v[k] = (k < g.nz) ? sm[((k << a.lgRJ) + jj) * a.RS + pp] : make_float2(0.f, 0.f);
+        fft::dif<PZ, false>(v);
+        if (j < g.ny) {
+#pragma unroll
+            for (int kz = 0; kz < PZ; ++kz)
+                a.T[((size_t)(c * PZ + kz) * a.Cx + kx) * g.ny + j] = v[fft::bitrev<PZ>(kz)];
+        }
+    }
+}
+
+// kernel C: the mirror of kernel A
+template <int PZ>
+__global__ void __launch_bounds__(512) rows_inv_kernel(const RowArgs a)
+{
+    extern __shared__ float2 sm[];
+    const Geometry g = a.g;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int c = blockIdx.y, j0 = blockIdx.x * a.RJ;
+    const int nrows = a.RJ * g.nz, Hx = a.Hx, hxr = (g.nx + 1) >> 1;
+    const int items = a.Cx << a.lgRJ;
+    for (int idx = tid; idx < items; idx += nt) {
+        const int jj = idx & (a.RJ - 1), kx = idx >> a.lgRJ, j = j0 + jj;
+        const int pp = fft::pad(kx < Hx ? fft::pos_of_freq(a.px, kx) : Hx);
+        float2 v[PZ];
+#pragma unroll
+        for (int kz = 0; kz < PZ; ++kz)
+            v[fft::bitrev<PZ>(kz)] = (j < g.ny) ? a.T[((size_t)(c * PZ + kz) * a.Cx + kx) * g.ny + j] : make_float2(0.f, 0.f);
+        fft::dit<PZ, true>(v);
+#pragma unroll
+        for (int k = 0; k < PZ; ++k) if (k < g.nz) sm[((k << a.lgRJ) + jj) * a.RS + pp] = v[k];
+    }
+    __syncthreads();
+    // re-tangle: Y[k], k = 0..Hx  ->  Z'[k] = 2 (E[k] + i O[k]) in the digit-reversed slots of the length-Hx transform
+    for (int idx = tid; idx < (nrows << a.lgHx); idx += nt) {
+        const int r = idx >> a.lgHx, k = idx & (Hx - 1);
+        if (2 * k > Hx) continue;
+        float2* base = sm + r * a.RS;
+        if (k == 0) {
+            const float y0 = base[0].x, yh = base[fft::pad(Hx)].x;
+            base[0] = make_float2(y0 + yh, y0 - yh);
+        } else {
+            const int k2 = Hx - k;
+            const int pa = fft::pad(fft::pos_of_freq(a.px, k)), pb = fft::pad(fft::pos_of_freq(a.px, k2));
+            const float2 A = base[pa], B = base[pb];                 // Y[k], Y[Hx-k]
+            const float2 E = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
+            const float2 O = fft::cmulc(D, __ldg(a.twx + k));        // (Y[k] - conj Y[Hx-k]) conj(w^k)
+            base[pa] = make_float2(E.x - O.y, E.y + O.x);
+            if (k2 != k) base[pb] = make_float2(E.x + O.y, -E.y + O.x);
+        }
+    }
+    __syncthreads();
+    fft::fft_inverse(a.px, sm, nrows, a.RS, a.twx, a.lgPx, tid, nt);
+    // real part -> even cells, imaginary part -> odd cells of the colour-split B_d
+    for (int idx = tid; idx < (nrows << a.lgHx); idx += nt) {
+        const int r = idx >> a.lgHx, n = idx & (Hx - 1);
+        const int k = r >> a.lgRJ, j = j0 + (r & (a.RJ - 1));
+        if (j < g.ny && n < hxr) {
+            const float2 v = sm[r * a.RS + fft::pad(n)];
+            const int row = k * g.ny + j, par = (j + k) & 1;
+            a.bd[c][(unsigned)par * (unsigned)g.H + (unsigned)row * g.hx + n] = v.x;
+            if (2 * n + 1 < g.nx) a.bd[c][(unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx + n] = v.y;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ kernel B
+struct ColArgs {
+    int ny, Cx, Py, lgPy, Pz, BS;
+    Plan py;
+    const float2* twy;
+    float2* T;
+    const float* nhat[6];
+};
+
+// grid (Cx, Pz); dynamic smem = 3 * BS float2
+template <bool THREE_D>
+__global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
+{
+    extern __shared__ float2 sm[];
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int kx = blockIdx.x, kz = blockIdx.y;
+    const int Py = a.Py, ny = a.ny, BS = a.BS;
+    float2* col[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) col[c] = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+    for (int idx = tid; idx < 3 * Py; idx += nt) {
+        const int c = idx >> a.lgPy, j = idx & (Py - 1);
+        sm[c * BS + fft::pad(j)] = (j < ny) ? col[c][j] : make_float2(0.f, 0.f);
+    }
+    __syncthreads();
+    fft::fft_forward(a.py, sm, 3, BS, a.twy, a.lgPy, tid, nt);
+    // S2: B^ = K^ M^, K^ = -mu0/(2 Px Py Pz) N^ real and symmetric; planes kz and Pz-kz share |K^| (xz, yz odd in kz)
+    const int kzs = (2 * kz <= a.Pz) ? kz : a.Pz - kz;
+    const float sg = (2 * kz <= a.Pz) ? 1.f : -1.f;
+    const size_t nb = ((size_t)kzs * a.Cx + kx) * Py;
+    for (int p = tid; p < Py; p += nt) {
+        const int pp = fft::pad(p);
+        const float2 u = sm[pp], v = sm[BS + pp], w = sm[2 * BS + pp];
+        const float xx = __ldg(a.nhat[0] + nb + p), yy = __ldg(a.nhat[1] + nb + p), zz = __ldg(a.nhat[2] + nb + p), xy = __ldg(a.nhat[3] + nb + p);
+        float2 ox, oy, oz;
+        ox.x = xx * u.x + xy * v.x; ox.y = xx * u.y + xy * v.y;
+        oy.x = xy * u.x + yy * v.x; oy.y = xy * u.y + yy * v.y;
+        oz.x = zz * w.x;            oz.y = zz * w.y;
+        if (THREE_D) {
+            const float xz = sg * __ldg(a.nhat[4] + nb + p), yz = sg * __ldg(a.nhat[5] + nb + p);
+            ox.x += xz * w.x; ox.y += xz * w.y;
+            oy.x += yz * w.x; oy.y += yz * w.y;
+            oz.x += xz * u.x + yz * v.x; oz.y += xz * u.y + yz * v.y;
+        }
+        sm[pp] = ox; sm[BS + pp] = oy; sm[2 * BS + pp] = oz;
+    }
+    __syncthreads();
+    fft::fft_inverse(a.py, sm, 3, BS, a.twy, a.lgPy, tid, nt);
+    for (int idx = tid; idx < 3 * Py; idx += nt) {
+        const int c = idx >> a.lgPy, j = idx & (Py - 1);
+        if (j < ny) col[c][j] = sm[c * BS + fft::pad(j)];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ host side
+template <int PZ>
+static int launch_rows(const DemagPlan* p, const RowArgs& ra, bool inverse, cudaStream_t st)
+{
+    const dim3 grid((p->g.ny + p->RJ - 1) / p->RJ, 3);
+    if (inverse) {
+        if (p->smemA > 48 * 1024) cudaFuncSetAttribute(rows_inv_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA);
+        rows_inv_kernel<PZ><<<grid, p->threadsA, p->smemA, st>>>(ra);
+    } else {
+        if (p->smemA > 48 * 1024) cudaFuncSetAttribute(rows_fwd_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA);
+        rows_fwd_kernel<PZ><<<grid, p->threadsA, p->smemA, st>>>(ra);
+    }
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+static int launch_rows_any(const DemagPlan* p, const RowArgs& ra, bool inverse, cudaStream_t st)
+{
+    switch (p->lgPz) {
+        case 0: return launch_rows<1>(p, ra, inverse, st);
+        case 1: return launch_rows<2>(p, ra, inverse, st);
+        case 2: return launch_rows<4>(p, ra, inverse, st);
+        case 3: return launch_rows<8>(p, ra, inverse, st);
+        case 4: return launch_rows<16>(p, ra, inverse, st);
+        case 5: return launch_rows<32>(p, ra, inverse, st);
+        default: return MMC_E_UNSUPPORTED;
+    }
+}
 
 int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, double dz, void* stream, std::string* err)
 {
     cudaStream_t st = (cudaStream_t)stream;
     DemagPlan* p = new DemagPlan();
-    p->g = g;
-    p->Px = g.nx > 1 ? 2 * g.nx : 1; p->Py = g.ny > 1 ? 2 * g.ny : 1; p->Pz = g.nz > 1 ? 2 * g.nz : 1;
-    p->Cx = p->Px / 2 + 1;
-    p->rsize = (size_t)p->Px * p->Py * p->Pz;
-    p->csize = (size_t)p->Cx * p->Py * p->Pz;
     *out = p;
-    CK(cudaMalloc(&p->rbuf, 3 * p->rsize * sizeof(float)));
-    CK(cudaMalloc(&p->obuf, 3 * p->rsize * sizeof(float)));
-    CK(cudaMalloc(&p->cbuf, 3 * p->csize * sizeof(float2)));
-    CK(cudaMemsetAsync(p->rbuf, 0, 3 * p->rsize * sizeof(float), st));
-    int n3[3] = { p->Pz, p->Py, p->Px };
-    int rank = 3; int* dims = n3;
-    if (p->Pz == 1) { rank = 2; dims = n3 + 1; }
-    if (p->Pz == 1 && p->Py == 1) { rank = 1; dims = n3 + 2; }
-    CF(cufftPlanMany(&p->fwd, rank, dims, nullptr, 1, (int)p->rsize, nullptr, 1, (int)p->csize, CUFFT_R2C, 3)); p->have_fwd = true;
-    CF(cufftPlanMany(&p->inv, rank, dims, nullptr, 1, (int)p->csize, nullptr, 1, (int)p->rsize, CUFFT_C2R, 3)); p->have_inv = true;
-    CF(cufftSetStream(p->fwd, st));
-    CF(cufftSetStream(p->inv, st));
+    p->g = g;
+    p->Px = padded_pow2(g.nx, 2); p->Py = padded_pow2(g.ny, 1); p->Pz = padded_pow2(g.nz, 1);
+    p->Hx = p->Px / 2; p->Cx = p->Hx + 1; p->lgPz = ilog2(p->Pz);
+    p->px = fft::make_plan(ilog2(p->Hx)); p->py = fft::make_plan(ilog2(p->Py));
+    if (p->lgPz > 5) { if (err) *err = "demag: more than 16 layers (padded z length > 32) is not built"; return MMC_E_UNSUPPORTED; }
+    // kernels A/C: rows per CTA.  8 if that leaves room for two CTAs per SM, else 4 (32-byte store segments), less
+    // only when even that does not fit the 227 KB of one SM.
+    p->RS = fft::padded_len(p->Hx) + 1;
+    auto bytesA = [&](int rj) { return (size_t)rj * g.nz * p->RS * sizeof(float2); };
+    p->RJ = 8;
+    while (p->RJ > 4 && bytesA(p->RJ) > 100 * 1024) p->RJ >>= 1;
+    while (p->RJ > 1 && bytesA(p->RJ) > 200 * 1024) p->RJ >>= 1;
+    while (p->RJ > 1 && p->RJ / 2 >= g.ny) p->RJ >>= 1;
+    if (bytesA(p->RJ) > 220 * 1024) { if (err) *err = "demag: nz * padded nx too large for the fused row kernels"; return MMC_E_UNSUPPORTED; }
+    p->smemA = bytesA(p->RJ);
+    p->threadsA = p->smemA > 100 * 1024 ? 512 : 256;
+    p->smemB = (size_t)3 * fft::padded_len(p->Py) * sizeof(float2);
+    if (p->smemB > 220 * 1024) { if (err) *err = "demag: padded ny > 8192 is not built"; return MMC_E_UNSUPPORTED; }
+    { int t = (3 * p->Py / 16 + 31) / 32 * 32; p->threadsB = t < 32 ? 32 : (t > 256 ? 256 : t); }
+
+    const size_t nT = (size_t)3 * p->Pz * p->Cx * g.ny;
+    CK(cudaMalloc(&p->T, nT * sizeof(float2)));
+    CK(cudaMalloc(&p->twx, (size_t)p->Px * sizeof(float2)));
+    CK(cudaMalloc(&p->twy, (size_t)p->Py * sizeof(float2)));
+    twiddle_kernel<<<blocks_for(p->Px), 256, 0, st>>>(p->twx, p->Px);
+    twiddle_kernel<<<blocks_for(p->Py), 256, 0, st>>>(p->twy, p->Py);
 
     // tensor spectrum, fp64 set-up
     std::vector<double> oct[6];
     demag_tensor_octant(g.nx, g.ny, g.nz, dx, dy, dz, kNearRadius, oct);
     const size_t nO = (size_t)g.nx * g.ny * g.nz;
+    const size_t rsize = (size_t)p->Px * p->Py * p->Pz, csize = (size_t)p->Cx * p->Py * p->Pz;
+    const int Kz = p->Pz / 2 + 1;
     double *d_oct = nullptr, *d_full = nullptr; double2* d_spec = nullptr;
     CK(cudaMalloc(&d_oct, nO * sizeof(double)));
-    CK(cudaMalloc(&d_full, p->rsize * sizeof(double)));
-    CK(cudaMalloc(&d_spec, p->csize * sizeof(double2)));
+    CK(cudaMalloc(&d_full, rsize * sizeof(double)));
+    CK(cudaMalloc(&d_spec, csize * sizeof(double2)));
+    int n3[3] = { p->Pz, p->Py, p->Px };
+    int rank = 3; int* dims = n3;
+    if (p->Pz == 1) { rank = 2; dims = n3 + 1; }
+    if (p->Pz == 1 && p->Py == 1) { rank = 1; dims = n3 + 2; }
     cufftHandle pd;
     CF(cufftPlanMany(&pd, rank, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, 1));
     CF(cufftSetStream(pd, st));
     static const int SX[6] = { 1, 1, 1, -1, -1, 1 }, SY[6] = { 1, 1, 1, -1, 1, -1 }, SZ[6] = { 1, 1, 1, 1, -1, -1 };
-    const double scale = -kMu0 / (double)p->rsize;
+    const double scale = -kMu0 / (2.0 * (double)p->Px * (double)p->Py * (double)p->Pz);
     for (int q = 0; q < 6; ++q) {
         if (g.nz == 1 && q >= 4) continue;                   // N_xz = N_yz = 0 in a single layer
-        CK(cudaMalloc(&p->khat[q], p->csize * sizeof(float)));
+        const size_t nN = (size_t)Kz * p->Cx * p->Py;
+        CK(cudaMalloc(&p->nhat[q], nN * sizeof(float)));
         CK(cudaMemcpyAsync(d_oct, oct[q].data(), nO * sizeof(double), cudaMemcpyHostToDevice, st));
-        place_kernel<<<blocks_for((long long)p->rsize), 256, 0, st>>>(g.nx, g.ny, g.nz, p->Px, p->Py, p->Pz, d_oct, SX[q], SY[q], SZ[q], d_full);
+        place_kernel<<<blocks_for((long long)rsize), 256, 0, st>>>(g.nx, g.ny, g.nz, p->Px, p->Py, p->Pz, d_oct, SX[q], SY[q], SZ[q], d_full);
         CF(cufftExecD2Z(pd, d_full, (cufftDoubleComplex*)d_spec));
-        real_part_kernel<<<blocks_for((long long)p->csize), 256, 0, st>>>(d_spec, p->khat[q], (long long)p->csize, scale);
+        permute_kernel<<<blocks_for((long long)nN), 256, 0, st>>>(d_spec, p->nhat[q], p->Cx, p->Py, Kz, p->py, scale);
         CK(cudaStreamSynchronize(st));                       // oct[q] host buffer must outlive the copy
     }
     cufftDestroy(pd);
     cudaFree(d_oct); cudaFree(d_full); cudaFree(d_spec);
+    if (p->smemB > 48 * 1024) {
+        CK(cudaFuncSetAttribute(columns_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemB));
+        CK(cudaFuncSetAttribute(columns_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemB));
+    }
     CK(cudaGetLastError());
     return MMC_OK;
 }
@@ -110,89 +373,9 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
 void demag_destroy(DemagPlan* p)
 {
     if (!p) return;
-    if (p->have_fwd) cufftDestroy(p->fwd);
-    if (p->have_inv) cufftDestroy(p->inv);
-    cudaFree(p->rbuf); cudaFree(p->obuf); cudaFree(p->cbuf);
-    for (int q = 0; q < 6; ++q) cudaFree(p->khat[q]);
+    cudaFree(p->T); cudaFree(p->twx); cudaFree(p->twy);
+    for (int q = 0; q < 6; ++q) cudaFree(p->nhat[q]);
     delete p;
-}
-
-// S0: one thread per natural pair (i = 2p, 2p+1): one coalesced read from each colour array, one float2 store.
-__global__ void __launch_bounds__(256) pack_kernel(Geometry g, int Px, int Py, size_t rsize, const float* __restrict__ mx, const float* __restrict__ my,
-                            const float* __restrict__ mz, const float* __restrict__ Ms0, float Ms0_u, float* __restrict__ rbuf)
-{
-    const int hp = (g.nx + 1) >> 1;
-    const long long n = (long long)hp * g.ny * g.nz;
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
-        const int p = (int)(t % hp); const long long row = t / hp;
-        const int j = (int)(row % g.ny), k = (int)(row / g.ny);
-        const int par = (j + k) & 1;
-        const long long se = (long long)par * g.H + row * g.hx + p;          // cell i = 2p
-        const long long so = (long long)(1 - par) * g.H + row * g.hx + p;    // cell i = 2p+1
-        const float we = Ms0 ? Ms0[se] : Ms0_u;
-        const bool has_odd = 2 * p + 1 < g.nx;
-        const float wo = has_odd ? (Ms0 ? Ms0[so] : Ms0_u) : 0.f;
-        const long long dst = ((long long)k * Py + j) * Px + 2 * p;
-        const float* src[3] = { mx, my, mz };
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const float ve = we * src[c][se];
-            const float vo = has_odd ? wo * src[c][so] : 0.f;
-            float* d = rbuf + c * rsize + dst;
-            if (Px > 1) *reinterpret_cast<float2*>(d) = make_float2(ve, vo);   // Px = 2 nx is even and dst is even
-            else d[0] = ve;
-        }
-    }
-}
-
-// S2: B^ = K^ M^ with K^ = -mu0/(P) N^ real and symmetric.
-template <bool THREE_D>
-__global__ void __launch_bounds__(256) multiply_kernel(size_t csize, float2* __restrict__ c, const float* __restrict__ kxx, const float* __restrict__ kyy,
-                                const float* __restrict__ kzz, const float* __restrict__ kxy, const float* __restrict__ kxz,
-                                const float* __restrict__ kyz)
-{
-    for (size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x; t < csize; t += (size_t)gridDim.x * blockDim.x) {
-        const float2 a = c[t], b = c[csize + t], d = c[2 * csize + t];
-        const float xx = kxx[t], yy = kyy[t], zz = kzz[t], xy = kxy[t];
-        float2 ox, oy, oz;
-        ox.x = xx * a.x + xy * b.x; ox.y = xx * a.y + xy * b.y;
-        oy.x = xy * a.x + yy * b.x; oy.y = xy * a.y + yy * b.y;
-        oz.x = zz * d.x;            oz.y = zz * d.y;
-        if (THREE_D) {
-            const float xz = kxz[t], yz = kyz[t];
-            ox.x += xz * d.x; ox.y += xz * d.y;
-            oy.x += yz * d.x; oy.y += yz * d.y;
-            oz.x += xz * a.x + yz * b.x; oz.y += xz * a.y + yz * b.y;
-        }
-        c[t] = ox; c[csize + t] = oy; c[2 * csize + t] = oz;
-    }
-}
-
-// S3 (crop): natural pair -> the two colour arrays of B_d.
-__global__ void __launch_bounds__(256) crop_kernel(Geometry g, int Px, int Py, size_t rsize, const float* __restrict__ rbuf, float* __restrict__ bx,
-                            float* __restrict__ by, float* __restrict__ bz)
-{
-    const int hp = (g.nx + 1) >> 1;
-    const long long n = (long long)hp * g.ny * g.nz;
-    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
-        const int p = (int)(t % hp); const long long row = t / hp;
-        const int j = (int)(row % g.ny), k = (int)(row / g.ny);
-        const int par = (j + k) & 1;
-        const long long se = (long long)par * g.H + row * g.hx + p;
-        const long long so = (long long)(1 - par) * g.H + row * g.hx + p;
-        const bool has_odd = 2 * p + 1 < g.nx;
-        const long long srcidx = ((long long)k * Py + j) * Px + 2 * p;
-        float* dst[3] = { bx, by, bz };
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const float* s = rbuf + c * rsize + srcidx;
-            float ve, vo = 0.f;
-            if (Px > 1) { const float2 v = *reinterpret_cast<const float2*>(s); ve = v.x; vo = v.y; }
-            else ve = s[0];
-            dst[c][se] = ve;
-            if (has_odd) dst[c][so] = vo;
-        }
-    }
 }
 
 void PhaseTimer::mark(int ph, void* stream)
@@ -207,21 +390,25 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
                   void* stream, std::string* err, PhaseTimer* timer)
 {
     cudaStream_t st = (cudaStream_t)stream;
-    const Geometry& g = p->g;
-    const long long pairs = (long long)((g.nx + 1) >> 1) * g.ny * g.nz;
-    pack_kernel<<<blocks_for(pairs), 256, 0, st>>>(g, p->Px, p->Py, p->rsize, m[0], m[1], m[2], Ms0_split, Ms0_uniform, p->rbuf);
-    if (timer) timer->mark(PH_PACK, stream);
-    CF(cufftExecR2C(p->fwd, p->rbuf, (cufftComplex*)p->cbuf));
+    RowArgs ra{};
+    ra.g = p->g; ra.Hx = p->Hx; ra.lgHx = ilog2(p->Hx); ra.Cx = p->Cx; ra.lgPx = ilog2(p->Px);
+    ra.RJ = p->RJ; ra.lgRJ = ilog2(p->RJ); ra.RS = p->RS; ra.px = p->px; ra.twx = p->twx;
+    for (int c = 0; c < 3; ++c) { ra.m[c] = m[c]; ra.bd[c] = bd[c]; }
+    ra.Ms0 = Ms0_split; ra.Ms0_u = Ms0_uniform; ra.T = p->T;
+    int rc = launch_rows_any(p, ra, false, st);
+    if (rc) { if (err) *err = "rows_fwd_kernel launch failed"; return rc; }
     if (timer) timer->mark(PH_FFT_FWD, stream);
-    if (g.nz > 1)
-        multiply_kernel<true><<<blocks_for((long long)p->csize), 256, 0, st>>>(p->csize, p->cbuf, p->khat[0], p->khat[1], p->khat[2], p->khat[3], p->khat[4], p->khat[5]);
-    else
-        multiply_kernel<false><<<blocks_for((long long)p->csize), 256, 0, st>>>(p->csize, p->cbuf, p->khat[0], p->khat[1], p->khat[2], p->khat[3], nullptr, nullptr);
+    ColArgs ca{};
+    ca.ny = p->g.ny; ca.Cx = p->Cx; ca.Py = p->Py; ca.lgPy = ilog2(p->Py); ca.Pz = p->Pz; ca.BS = fft::padded_len(p->Py);
+    ca.py = p->py; ca.twy = p->twy; ca.T = p->T;
+    for (int q = 0; q < 6; ++q) ca.nhat[q] = p->nhat[q];
+    const dim3 gridB(p->Cx, p->Pz);
+    if (p->g.nz > 1) columns_kernel<true><<<gridB, p->threadsB, p->smemB, st>>>(ca);
+    else             columns_kernel<false><<<gridB, p->threadsB, p->smemB, st>>>(ca);
     if (timer) timer->mark(PH_MULTIPLY, stream);
-    CF(cufftExecC2R(p->inv, (cufftComplex*)p->cbuf, p->obuf));
+    rc = launch_rows_any(p, ra, true, st);
+    if (rc) { if (err) *err = "rows_inv_kernel launch failed"; return rc; }
     if (timer) timer->mark(PH_FFT_INV, stream);
-    crop_kernel<<<blocks_for(pairs), 256, 0, st>>>(g, p->Px, p->Py, p->rsize, p->obuf, bd[0], bd[1], bd[2]);
-    if (timer) timer->mark(PH_CROP, stream);
     CK(cudaGetLastError());
     return MMC_OK;
 }

@@ -151,26 +151,37 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
 
 // ------------------------------------------------------------------------------------------------ the pass
 // blockDim = (32, BY, BZ), 256 threads; grid = (ceil(hxr/32), ceil(ny/BY), ceil(nz/BZ)).
+// Running sums of the sweep's final vectors are kept in fixed point (kSumScale), so that they can be reduced with
+// integer warp reductions and integer atomics: exact, order-independent and therefore deterministic.
 template <unsigned F, bool DEBUG>
-__global__ void __launch_bounds__(256, DEBUG ? 1 : 3) colour_pass_kernel(const SweepArgs a)
+__global__ void __launch_bounds__(256, DEBUG ? 1 : 4) colour_pass_kernel(const SweepArgs a)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0;
-    const Geometry g = a.g;
+    __shared__ unsigned s_acc[6];                    // accepted, trials, sum mx, my, mz, |m| (fixed point, two's complement)
+    __shared__ unsigned s_arrived;
+    const int tlin = threadIdx.x + 32 * (threadIdx.y + blockDim.y * threadIdx.z);
+    if (tlin < 6) s_acc[tlin] = 0u;
+    if (tlin == 6) s_arrived = 0u;
+    __syncthreads();                                  // the only block barrier: all warps are still in step here
+
+    const int nx = a.g.nx, ny = a.g.ny, nz = a.g.nz, hx = a.g.hx;
+    const unsigned pbc = a.g.pbc;
     const int q = blockIdx.x * 32 + threadIdx.x;
     const int j = blockIdx.y * blockDim.y + threadIdx.y;
     const int k = HASZ ? blockIdx.z * blockDim.z + threadIdx.z : 0;
     const int col = a.colour;
     const int s = ((j + k) & 1) ^ col;               // active cells of this row sit at i = 2q + s
     const int i = 2 * q + s;
-    bool active = i < g.nx && j < g.ny && k < g.nz;
+    bool active = i < nx && j < ny && k < nz;
     bool accept = false;
     float fs0 = 0.f, fs1 = 0.f, fs2 = 0.f, fs3 = 0.f;   // the cell's final vector and length (running sums)
 
-    const int row = k * g.ny + j;
     // 32-bit element offsets: mmc_create guarantees 2 H < 2^31
-    const unsigned H = (unsigned)g.H;
-    const unsigned ownb = (unsigned)col * H + (unsigned)row * g.hx + q;
+    const unsigned H = (unsigned)a.g.H;
+    const int row = k * ny + j;
+    const unsigned rq = (unsigned)row * hx + q;
+    const unsigned ownb = (unsigned)col * H + rq;
     unsigned mb = 0x7fu, cls = 0u;
     if (active) {
         if (PERCELL) { const unsigned w = __ldg(a.cw + ownb); mb = w & 0x7fu; cls = w >> 7; }
@@ -178,42 +189,41 @@ __global__ void __launch_bounds__(256, DEBUG ? 1 : 3) colour_pass_kernel(const S
         if ((MASK || PERCELL) && !(mb & 0x40u)) active = false;            // empty cell
     }
     if (active) {
-        const int hxr = (g.nx + 1) >> 1;             // compact length of the real (unpadded) row
-        const unsigned othc = (unsigned)(1 - col) * H;
-        const unsigned rowb = othc + (unsigned)row * g.hx;
-        // neighbour rows (wrap when periodic, else clamp: an out-of-mesh neighbour is never bonded)
-        int jn = j + 1, js = j - 1;
-        if (jn == g.ny) jn = (g.pbc & 2u) ? 0 : j;
-        if (js < 0) js = (g.pbc & 2u) ? g.ny - 1 : j;
-        // x neighbours: s == 0: E at q, W at q-1;  s == 1: W at q, E at q+1 (wrap or clamp)
-        int qe = s ? q + 1 : q - 1;
-        if (qe < 0) qe = (g.pbc & 1u) ? hxr - 1 : 0;
-        if (qe >= hxr) qe = (g.pbc & 1u) ? 0 : q;
-        const unsigned nb_n = othc + (unsigned)(k * g.ny + jn) * g.hx + q;
-        const unsigned nb_s = othc + (unsigned)(k * g.ny + js) * g.hx + q;
+        const int hxr = (nx + 1) >> 1;               // compact length of the real (unpadded) row
+        // element deltas from this thread's slot in the other colour's plane to its six neighbours
+        // (wrap when periodic, else 0: an out-of-mesh neighbour is never bonded, any valid address will do)
+        const int dN = (j + 1 < ny) ? hx : ((pbc & 2u) ? -(ny - 1) * hx : 0);
+        const int dS = (j > 0) ? -hx : ((pbc & 2u) ? (ny - 1) * hx : 0);
+        // x: s == 0: E at q, W at q-1;  s == 1: W at q, E at q+1
+        int dX = s ? 1 : -1;
+        if (q + dX < 0) dX = (pbc & 1u) ? hxr - 1 : 0;
+        else if (q + dX >= hxr) dX = (pbc & 1u) ? -q : 0;
+        int dU = 0, dD = 0;
+        if (HASZ) {
+            const int lay = ny * hx;
+            dU = (k + 1 < nz) ? lay : ((pbc & 4u) ? -(nz - 1) * lay : 0);
+            dD = (k > 0) ? -lay : ((pbc & 4u) ? (nz - 1) * lay : 0);
+        }
+        // 32-bit offsets of the six neighbour slots (all inside [0, 2H)): one add each, one IMAD.WIDE per load
+        const unsigned othb = (unsigned)(1 - col) * H + rq;
+        const unsigned oX = othb + (unsigned)dX, oN = othb + (unsigned)dN, oS = othb + (unsigned)dS;
+        const unsigned oU = othb + (unsigned)dU, oD = othb + (unsigned)dD;
         float m[3], xa[3], xb[3], yn[3], ys[3], zu[3], zd[3], Bd[3] = { 0.f, 0.f, 0.f };
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
+            const float* __restrict__ P = a.m[c];
             m[c] = a.m[c][ownb];
-            xa[c] = __ldg(a.m[c] + rowb + q);
-            xb[c] = __ldg(a.m[c] + rowb + qe);
-            yn[c] = __ldg(a.m[c] + nb_n);
-            ys[c] = __ldg(a.m[c] + nb_s);
+            xa[c] = __ldg(P + othb);
+            xb[c] = __ldg(P + oX);
+            yn[c] = __ldg(P + oN);
+            ys[c] = __ldg(P + oS);
+            if (HASZ) { zu[c] = __ldg(P + oU); zd[c] = __ldg(P + oD); }
             if (DEMAG) Bd[c] = __ldg(a.bd[c] + ownb);
-        }
-        if (HASZ) {
-            int ku = k + 1, kd = k - 1;
-            if (ku == g.nz) ku = (g.pbc & 4u) ? 0 : k;
-            if (kd < 0) kd = (g.pbc & 4u) ? g.nz - 1 : k;
-            const unsigned nb_u = othc + (unsigned)(ku * g.ny + j) * g.hx + q;
-            const unsigned nb_d = othc + (unsigned)(kd * g.ny + j) * g.hx + q;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) { zu[c] = __ldg(a.m[c] + nb_u); zd[c] = __ldg(a.m[c] + nb_d); }
         }
         CellCoef cf;
         float kscale = 1.f;
         if (PERCELL) {
-            const float4* t = a.table + 3ull * cls;
+            const float4* t = a.table + 3u * cls;
             const float4 t0 = __ldg(t), t1 = __ldg(t + 1);
             const float2 t2 = __ldg(reinterpret_cast<const float2*>(t + 2));
             kscale = t0.x; cf.c4 = t0.y;
@@ -232,8 +242,8 @@ __global__ void __launch_bounds__(256, DEBUG ? 1 : 3) colour_pass_kernel(const S
             bN = (mb & 4u) ? 1.f : 0.f;  bS = (mb & 8u) ? 1.f : 0.f;
             bU = (mb & 16u) ? 1.f : 0.f; bD = (mb & 32u) ? 1.f : 0.f;
         } else {
-            if (g.nx < 2) { bE = 0.f; bW = 0.f; }
-            if (g.ny < 2) { bN = 0.f; bS = 0.f; }
+            if (nx < 2) { bE = 0.f; bW = 0.f; }
+            if (ny < 2) { bN = 0.f; bS = 0.f; }
         }
         float S[3], e[3], wv[3];
 #pragma unroll
@@ -257,7 +267,7 @@ __global__ void __launch_bounds__(256, DEBUG ? 1 : 3) colour_pass_kernel(const S
         const unsigned long long sweep = a.ctl->sweep;
         const float omc = a.ctl->one_minus_cos_cone;
         const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
-        const unsigned cell = (unsigned)row * g.nx + i;                   // natural cell index (< 2^31)
+        const unsigned cell = (unsigned)row * nx + i;                     // natural cell index (< 2^31)
         const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
         const CellResult r = cell_update<DMI, DEBUG>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
         accept = r.accept;
@@ -275,41 +285,37 @@ __global__ void __launch_bounds__(256, DEBUG ? 1 : 3) colour_pass_kernel(const S
         }
     }
 
-    // ---- S10: acceptance counters (exact integers) and running sums of the final vectors, per block
-    __shared__ int s_cnt[8][2];
-    __shared__ float s_sum[8][4];
-    const int acc_cnt = __popc(__ballot_sync(0xffffffffu, accept));
-    const int tri_cnt = __popc(__ballot_sync(0xffffffffu, active));
+    // ---- S10: acceptance counters and running sums.  Warp: ballot / integer REDUX.  Block: shared 64-bit atomics,
+    // the last warp to arrive flushes the block's totals with six global atomics (no second block barrier).
+    const unsigned acc_cnt = __popc(__ballot_sync(0xffffffffu, accept));
+    const unsigned tri_cnt = __popc(__ballot_sync(0xffffffffu, active));
     const bool want_sums = a.run_sums != nullptr;
+    int i0 = 0, i1 = 0, i2 = 0, i3 = 0;
     if (want_sums) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-            fs0 += __shfl_xor_sync(0xffffffffu, fs0, o);
-            fs1 += __shfl_xor_sync(0xffffffffu, fs1, o);
-            fs2 += __shfl_xor_sync(0xffffffffu, fs2, o);
-            fs3 += __shfl_xor_sync(0xffffffffu, fs3, o);
-        }
+        i0 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs0 * kSumScale));
+        i1 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs1 * kSumScale));
+        i2 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs2 * kSumScale));
+        i3 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs3 * kSumScale));
     }
-    const int tlin = threadIdx.x + 32 * (threadIdx.y + blockDim.y * threadIdx.z);
-    const int warp = tlin >> 5;
     if (threadIdx.x == 0) {
-        s_cnt[warp][0] = acc_cnt; s_cnt[warp][1] = tri_cnt;
-        s_sum[warp][0] = fs0; s_sum[warp][1] = fs1; s_sum[warp][2] = fs2; s_sum[warp][3] = fs3;
-    }
-    __syncthreads();
-    if (tlin == 0) {
-        int ac = 0, tc = 0; float d0 = 0.f, d1 = 0.f, d2 = 0.f, d3 = 0.f;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) {
-            ac += s_cnt[w][0]; tc += s_cnt[w][1];
-            d0 += s_sum[w][0]; d1 += s_sum[w][1]; d2 += s_sum[w][2]; d3 += s_sum[w][3];
+        if (tri_cnt) {
+            atomicAdd(&s_acc[0], acc_cnt);
+            atomicAdd(&s_acc[1], tri_cnt);
+            if (want_sums) {
+                atomicAdd(&s_acc[2], (unsigned)i0); atomicAdd(&s_acc[3], (unsigned)i1);
+                atomicAdd(&s_acc[4], (unsigned)i2); atomicAdd(&s_acc[5], (unsigned)i3);
+            }
         }
-        if (tc) {
-            atomicAdd(&a.ctl->win_trials, (unsigned long long)tc);
-            if (ac) atomicAdd(&a.ctl->win_accepted, (unsigned long long)ac);
-            if (want_sums) {                          // one slot per block: fixed summation order, no fp atomics
-                double* slot = a.run_sums + 4ll * (blockIdx.x + (long long)gridDim.x * (blockIdx.y + (long long)gridDim.y * blockIdx.z));
-                slot[0] += (double)d0; slot[1] += (double)d1; slot[2] += (double)d2; slot[3] += (double)d3;
+        __threadfence_block();
+        if (atomicAdd(&s_arrived, 1u) == 7u) {         // 8 warps per block
+            __threadfence_block();
+            const unsigned tc = atomicAdd(&s_acc[1], 0u);
+            if (tc) {
+                atomicAdd(&a.ctl->win_trials, (unsigned long long)tc);
+                const unsigned ac = atomicAdd(&s_acc[0], 0u);
+                if (ac) atomicAdd(&a.ctl->win_accepted, (unsigned long long)ac);
+                if (want_sums)                         // sign-extend the block's 32-bit fixed-point sums
+                    for (int t = 0; t < 4; ++t) atomicAdd(&a.run_sums[t], (unsigned long long)(long long)(int)atomicAdd(&s_acc[2 + t], 0u));
             }
         }
     }
@@ -337,7 +343,7 @@ __global__ void end_sweep_kernel(Control* ctl)
     }
 }
 
-int launch_end_sweep(Control* ctl, double*, int, void* stream)
+int launch_end_sweep(Control* ctl, void* stream)
 {
     end_sweep_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(ctl);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
@@ -351,12 +357,6 @@ static void brick(const Geometry& g, dim3* block, dim3* grid)
     const int hxr = (g.nx + 1) >> 1;
     *block = dim3(32, by, bz);
     *grid = dim3((hxr + 31) / 32, (g.ny + by - 1) / by, (g.nz + bz - 1) / bz);
-}
-
-int sweep_grid_blocks(const Geometry& g)
-{
-    dim3 b, gr; brick(g, &b, &gr);
-    return (int)(gr.x * gr.y * gr.z);
 }
 
 template <unsigned F>

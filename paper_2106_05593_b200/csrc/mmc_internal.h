@@ -58,6 +58,7 @@ enum ClassSlot { CS_INVT = 0, CS_C4 = 1, CS_MU2 = 2 /* double in slots 2,3 */, C
                  CS_AX = 7, CS_AY = 8, CS_AZ = 9, CS_K1T = 10 /* beta V K1(T), read-out only */,
                  CS_C0 = 11 /* c0 - c4 mu2^2, read-out only */ };
 constexpr unsigned kMaxClasses = 1u << 25;
+constexpr float kSumScale = 4194304.f;              // 2^22: fixed-point scale of the running sums (a 256-cell block sum fits int32 for |m| < 2)
 
 // Device-resident control block: read by the kernels, advanced by end_sweep_kernel (no host round trip).
 struct Control {
@@ -91,7 +92,7 @@ struct SweepArgs {
     Control* ctl;
     unsigned seed_lo, seed_hi;
     int colour;
-    double* run_sums;            // [n_slots][4] running sums of final mx,my,mz,|m| per block slot, or NULL
+    unsigned long long* run_sums; // [4] running sums of the sweeps' final mx,my,mz,|m| in fixed point (two's complement, kSumScale), or NULL
     // debug dump (natural order), any NULL
     float* dbg_dm; float* dbg_terms; float* dbg_margin; uint8_t* dbg_acc;
 };
@@ -99,9 +100,8 @@ struct SweepArgs {
 struct Observables { double sum[4]; double E[6]; unsigned long long n_active; };
 
 // kernels_sweep.cu
-int sweep_grid_blocks(const Geometry& g);          // CTAs of one colour pass (= number of running-sum slots)
 int launch_colour_pass(const SweepArgs& a, unsigned features, bool debug, void* stream);
-int launch_end_sweep(Control* ctl, double* run_sums, int n_slots, void* stream);
+int launch_end_sweep(Control* ctl, void* stream);
 // kernels_layout.cu
 int launch_to_split(const Geometry& g, const float* nat, float* split, void* stream);
 int launch_from_split(const Geometry& g, const float* split, float* nat, void* stream);
