@@ -19,6 +19,7 @@
 
 #include <cmath>
 
+#include "fft_reg.cuh"
 #include "fft_smem.cuh"
 #include "mmc_internal.h"
 
@@ -37,6 +38,9 @@ struct DemagPlan {
     int threadsA, threadsB;
     float2* twx = nullptr;           // exp(-2 pi i k / Px), k < Px
     float2* twy = nullptr;           // exp(-2 pi i k / Py), k < Py
+    bool fastB = false;              // columns: register-resident transform (fft_reg.cuh), Py in 2^8 .. 2^12
+    float2* twB1 = nullptr;          // its twiddle tables, 15 * Py/16 entries each
+    float2* twB2 = nullptr;
     float2* T = nullptr;             // [3][Pz][Cx][ny]
     float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
 };
@@ -69,12 +73,14 @@ __global__ void place_kernel(int nx, int ny, int nz, int Px, int Py, int Pz, con
     }
 }
 // spectrum (D2Z layout [kz][ky][kx <= Px/2]) -> nhat[kz <= Pz/2][kx][p], p = position of ky in the y transform's output
-__global__ void permute_kernel(const double2* __restrict__ spec, float* __restrict__ out, int Cx, int Py, int Kz, Plan py, double scale)
+__global__ void permute_kernel(const double2* __restrict__ spec, float* __restrict__ out, int Cx, int Py, int Kz, Plan py, double scale,
+                               int fast_lg)
 {
     const long long n = (long long)Kz * Cx * Py;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
         const int p = (int)(t % Py); const long long r = t / Py; const int kx = (int)(r % Cx), kz = (int)(r / Cx);
-        const int ky = fft::freq_of_pos(py, p);
+        // fast path: slot e of thread tid sits at p = e * (Py/16) + tid
+        const int ky = fast_lg ? fftr::freq_of_slot(fast_lg, p % (Py >> 4), p / (Py >> 4)) : fft::freq_of_pos(py, p);
         out[t] = (float)(scale * spec[((long long)kz * Py + ky) * Cx + kx].x);
     }
 }
@@ -272,6 +278,109 @@ __global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
     }
 }
 
+// kernel B, register-resident variant (fft_reg.cuh) for Py = 2^LGN, 8 <= LGN <= 12: T = Py/16 threads per (kx, kz)
+// column set, G column sets (adjacent kx) per CTA.  Each thread keeps its 16 points of all three components in
+// registers from the forward transform through the tensor multiply into the inverse transform; shared memory only
+// carries the two exchanges of each transform.  HALF (2 ny == Py): the zero half of the input and the discarded half
+// of the output are pruned at compile time.  grid (ceil(Cx/G), Pz), block (T, G).
+struct ColFastArgs {
+    int ny, Cx, Pz;
+    const float2* tw1; const float2* tw2;
+    float2* T;
+    const float* nhat[6];
+};
+
+template <int LGN, bool HALF>
+__global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G, fftr::Shape<LGN>::T >= 256 ? 2 : 3)
+columns_fast_kernel(const ColFastArgs a)
+{
+    using S = fftr::Shape<LGN>;
+    constexpr int N = S::N, T = S::T;
+    extern __shared__ float2 sm[];
+    float2* s1 = sm + threadIdx.y * S::SMEM;
+    float2* s2 = s1 + S::S1;
+    const int tid = threadIdx.x;
+    const int kxr = blockIdx.x * S::G + threadIdx.y, kz = blockIdx.y;
+    const bool live = kxr < a.Cx;                      // idle groups still walk through the barriers
+    const int kx = live ? kxr : a.Cx - 1;
+    const int ny = a.ny;
+    float2 v[3][16];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) {
+            const int j = tid + n1 * T;
+            if (HALF) v[c][n1] = (n1 < 8) ? col[j] : make_float2(0.f, 0.f);
+            else v[c][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
+        }
+        fftr::forward<LGN, HALF>(v[c], s1, s2, a.tw1, a.tw2, tid);
+    }
+    // S2: B^ = K^ M^ (see columns_kernel); slot e of thread tid reads the permuted spectrum at e*T + tid
+    {
+        const int kzs = (2 * kz <= a.Pz) ? kz : a.Pz - kz;
+        const float sg = (2 * kz <= a.Pz) ? 1.f : -1.f;
+        const size_t nb = ((size_t)kzs * a.Cx + kx) * N + tid;
+        const bool three_d = a.nhat[4] != nullptr;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float2 u = v[0][e], w1 = v[1][e], w = v[2][e];
+            const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T),
+                        zz = __ldg(a.nhat[2] + nb + e * T), xy = __ldg(a.nhat[3] + nb + e * T);
+            float2 ox, oy, oz;
+            ox.x = fmaf(xx, u.x, xy * w1.x); ox.y = fmaf(xx, u.y, xy * w1.y);
+            oy.x = fmaf(xy, u.x, yy * w1.x); oy.y = fmaf(xy, u.y, yy * w1.y);
+            oz.x = zz * w.x;                 oz.y = zz * w.y;
+            if (three_d) {
+                const float xz = sg * __ldg(a.nhat[4] + nb + e * T), yz = sg * __ldg(a.nhat[5] + nb + e * T);
+                ox.x = fmaf(xz, w.x, ox.x); ox.y = fmaf(xz, w.y, ox.y);
+                oy.x = fmaf(yz, w.x, oy.x); oy.y = fmaf(yz, w.y, oy.y);
+                oz.x = fmaf(xz, u.x, fmaf(yz, w1.x, oz.x)); oz.y = fmaf(xz, u.y, fmaf(yz, w1.y, oz.y));
+            }
+            v[0][e] = ox; v[1][e] = oy; v[2][e] = oz;
+        }
+    }
+    __syncthreads();                                   // every thread is done reading exchange buffer 2
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        fftr::inverse<LGN>(v[c], s1, s2, a.tw1, a.tw2, tid);
+        float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+#pragma unroll
+        for (int n1 = 0; n1 < (HALF ? 8 : 16); ++n1) {
+            const int j = tid + n1 * T;
+            if (live && (HALF || j < ny)) col[j] = v[c][n1];
+        }
+    }
+}
+
+template <int LGN>
+static int launch_columns_fast(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
+{
+    using S = fftr::Shape<LGN>;
+    const dim3 grid((p->Cx + S::G - 1) / S::G, p->Pz), block(S::T, S::G);
+    const size_t smem = (size_t)S::G * S::SMEM * sizeof(float2);
+    const bool half = 2 * p->g.ny == p->Py;
+    if (half) {
+        if (smem > 48 * 1024) cudaFuncSetAttribute(columns_fast_kernel<LGN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        columns_fast_kernel<LGN, true><<<grid, block, smem, st>>>(ca);
+    } else {
+        if (smem > 48 * 1024) cudaFuncSetAttribute(columns_fast_kernel<LGN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        columns_fast_kernel<LGN, false><<<grid, block, smem, st>>>(ca);
+    }
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+static int launch_columns_fast_any(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
+{
+    switch (ilog2(p->Py)) {
+        case 8: return launch_columns_fast<8>(p, ca, st);
+        case 9: return launch_columns_fast<9>(p, ca, st);
+        case 10: return launch_columns_fast<10>(p, ca, st);
+        case 11: return launch_columns_fast<11>(p, ca, st);
+        case 12: return launch_columns_fast<12>(p, ca, st);
+        default: return MMC_E_UNSUPPORTED;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ host side
 template <int PZ>
 static int launch_rows(const DemagPlan* p, const RowArgs& ra, bool inverse, cudaStream_t st)
@@ -324,6 +433,16 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     if (p->smemB > 220 * 1024) { if (err) *err = "demag: padded ny > 8192 is not built"; return MMC_E_UNSUPPORTED; }
     { int t = (3 * p->Py / 16 + 31) / 32 * 32; p->threadsB = t < 32 ? 32 : (t > 256 ? 256 : t); }
 
+    {
+        const int lgPy = ilog2(p->Py);
+        p->fastB = lgPy >= fftr::kMinLg && lgPy <= fftr::kMaxLg;
+        if (p->fastB) {
+            const size_t ntw = (size_t)15 * (p->Py / 16);
+            CK(cudaMalloc(&p->twB1, ntw * sizeof(float2)));
+            CK(cudaMalloc(&p->twB2, ntw * sizeof(float2)));
+            fftr::twiddle_tables_kernel<<<blocks_for((long long)ntw), 256, 0, st>>>(p->twB1, p->twB2, lgPy);
+        }
+    }
     const size_t nT = (size_t)3 * p->Pz * p->Cx * g.ny;
     CK(cudaMalloc(&p->T, nT * sizeof(float2)));
     CK(cudaMalloc(&p->twx, (size_t)p->Px * sizeof(float2)));
@@ -357,7 +476,7 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
         CK(cudaMemcpyAsync(d_oct, oct[q].data(), nO * sizeof(double), cudaMemcpyHostToDevice, st));
         place_kernel<<<blocks_for((long long)rsize), 256, 0, st>>>(g.nx, g.ny, g.nz, p->Px, p->Py, p->Pz, d_oct, SX[q], SY[q], SZ[q], d_full);
         CF(cufftExecD2Z(pd, d_full, (cufftDoubleComplex*)d_spec));
-        permute_kernel<<<blocks_for((long long)nN), 256, 0, st>>>(d_spec, p->nhat[q], p->Cx, p->Py, Kz, p->py, scale);
+        permute_kernel<<<blocks_for((long long)nN), 256, 0, st>>>(d_spec, p->nhat[q], p->Cx, p->Py, Kz, p->py, scale, p->fastB ? ilog2(p->Py) : 0);
         CK(cudaStreamSynchronize(st));                       // oct[q] host buffer must outlive the copy
     }
     cufftDestroy(pd);
@@ -373,7 +492,7 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
 void demag_destroy(DemagPlan* p)
 {
     if (!p) return;
-    cudaFree(p->T); cudaFree(p->twx); cudaFree(p->twy);
+    cudaFree(p->T); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2);
     for (int q = 0; q < 6; ++q) cudaFree(p->nhat[q]);
     delete p;
 }
@@ -402,9 +521,17 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
     ca.ny = p->g.ny; ca.Cx = p->Cx; ca.Py = p->Py; ca.lgPy = ilog2(p->Py); ca.Pz = p->Pz; ca.BS = fft::padded_len(p->Py);
     ca.py = p->py; ca.twy = p->twy; ca.T = p->T;
     for (int q = 0; q < 6; ++q) ca.nhat[q] = p->nhat[q];
-    const dim3 gridB(p->Cx, p->Pz);
-    if (p->g.nz > 1) columns_kernel<true><<<gridB, p->threadsB, p->smemB, st>>>(ca);
-    else             columns_kernel<false><<<gridB, p->threadsB, p->smemB, st>>>(ca);
+    if (p->fastB) {
+        ColFastArgs fa{};
+        fa.ny = p->g.ny; fa.Cx = p->Cx; fa.Pz = p->Pz; fa.tw1 = p->twB1; fa.tw2 = p->twB2; fa.T = p->T;
+        for (int q = 0; q < 6; ++q) fa.nhat[q] = p->nhat[q];
+        rc = launch_columns_fast_any(p, fa, st);
+        if (rc) { if (err) *err = "columns_fast_kernel launch failed"; return rc; }
+    } else {
+        const dim3 gridB(p->Cx, p->Pz);
+        if (p->g.nz > 1) columns_kernel<true><<<gridB, p->threadsB, p->smemB, st>>>(ca);
+        else             columns_kernel<false><<<gridB, p->threadsB, p->smemB, st>>>(ca);
+    }
     if (timer) timer->mark(PH_MULTIPLY, stream);
     rc = launch_rows_any(p, ra, true, st);
     if (rc) { if (err) *err = "rows_inv_kernel launch failed"; return rc; }

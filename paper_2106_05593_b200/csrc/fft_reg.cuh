@@ -1,0 +1,171 @@
+// fft_reg.cuh -- register-resident power-of-two complex FFTs for the demag convolution (demag.cu), lengths 2^8 .. 2^12.
+//
+// Every thread keeps 16 points of one transform in registers; a transform of length N = 16 * 16 * R3 (R3 = N/256 in
+// {1, 2, 4, 8, 16}) is two radix-16 steps and one radix-R3 step with two exchanges through shared memory in between.
+// All lengths, strides and radices are template parameters, so every shared-memory and table access is
+// "per-thread base + immediate" and the butterflies are straight-line code.  T = N/16 threads work on one transform.
+//
+// Forward (decimation in frequency), thread `tid` of the transform:
+//   in   v[n1] = x[tid + n1*T]                                  (HALF: x[n] = 0 for n >= N/2 is folded at compile time)
+//   1    radix-16 over n1, twiddle w_N^(tid*q1)                 -> s1[q1*(T+1) + tid]
+//   2    thread = (u = tid>>4, q1 = tid&15): radix-16 over t1 of s1[q1*(T+1) + t1*R3 + u], twiddle w_T^(u*q2)
+//                                                               -> s2[u*272 + 17*q1 + q2]
+//   3    pairs p = tid + i*T (i < 16/R3), p = 16*q1 + q2: radix-R3 over u of s2[u*272 + p + (p>>4)]
+//   out  v[i*R3 + q3] = X[q1 + 16*q2 + 256*q3]
+// The output order is whatever falls out (freq_of_slot below); the convolution multiplies in that order (the tensor
+// spectrum is stored permuted), and the inverse transform is the exact mirror, so no reordering pass exists.
+// The paddings (T+1, 17, 272) make every exchange access hit distinct bank pairs within a half-warp.
+#ifndef MMC_FFT_REG_CUH_
+#define MMC_FFT_REG_CUH_
+
+#include "fft_smem.cuh"
+
+namespace mmc {
+namespace fftr {
+
+constexpr int kMinLg = 8, kMaxLg = 12;
+
+template <int LGN>
+struct Shape {
+    static constexpr int N = 1 << LGN, T = N / 16, R3 = N / 256, NI = 16 / R3;
+    static constexpr int U = 272;                                  // row stride of exchange buffer 2
+    static constexpr int S1 = 16 * (T + 1);                        // float2 elements of exchange buffer 1
+    static constexpr int S2 = R3 > 1 ? R3 * U : 0;                 // ... and 2
+    static constexpr int SMEM = S1 + S2;                           // per transform group
+    static constexpr int G = T >= 128 ? 1 : 128 / T;               // transforms side by side in one CTA
+};
+
+// frequency held by register slot e of thread tid after forward<LGN>
+__host__ __device__ inline int freq_of_slot(int lgN, int tid, int e)
+{
+    const int N = 1 << lgN, T = N / 16, R3 = N / 256;
+    if (R3 == 1) return tid + 16 * e;
+    const int i = e / R3, q3 = e % R3, p = tid + i * T;
+    return (p >> 4) + 16 * (p & 15) + 256 * q3;
+}
+
+#ifdef __CUDACC__
+
+// tw1[(q-1)*T + t] = exp(-2 pi i t q / N), tw2[(q-1)*T + t] = exp(-2 pi i (t>>4) q / T), q = 1..15
+__global__ void twiddle_tables_kernel(float2* tw1, float2* tw2, int lgN)
+{
+    const int N = 1 << lgN, T = N / 16;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < 15 * T; idx += gridDim.x * blockDim.x) {
+        const int q = idx / T + 1, t = idx % T;
+        double s, c;
+        sincospi(-2.0 * (double)(t * q) / (double)N, &s, &c);
+        tw1[idx] = make_float2((float)c, (float)s);
+        sincospi(-2.0 * (double)((t >> 4) * q) / (double)T, &s, &c);
+        tw2[idx] = make_float2((float)c, (float)s);
+    }
+}
+
+template <int LGN, bool HALF>
+__device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
+                                        const float2* __restrict__ tw1, const float2* __restrict__ tw2, int tid)
+{
+    using S = Shape<LGN>;
+    constexpr int T = S::T, R3 = S::R3;
+    if (HALF) {                                   // first butterfly level with a zero upper half
+#pragma unroll
+        for (int k = 0; k < 8; ++k) v[k + 8] = fft::mul_root<16, false>(v[k], k);
+        fft::dif<8, false>(v); fft::dif<8, false>(v + 8);
+    } else {
+        fft::dif<16, false>(v);
+    }
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        float2 y = v[fft::bitrev<16>(q)];
+        if (q > 0) y = fft::cmul(y, __ldg(tw1 + (q - 1) * T + tid));
+        s1[q * (T + 1) + tid] = y;
+    }
+    __syncthreads();
+    const int u = tid >> 4, q1 = tid & 15;
+    {
+        const float2* r1 = s1 + q1 * (T + 1) + u;
+#pragma unroll
+        for (int t1 = 0; t1 < 16; ++t1) v[t1] = r1[t1 * R3];
+    }
+    fft::dif<16, false>(v);
+    if constexpr (R3 > 1) {
+        float2* w2 = s2 + u * S::U + 17 * q1;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            float2 y = v[fft::bitrev<16>(q)];
+            if (q > 0) y = fft::cmul(y, __ldg(tw2 + (q - 1) * T + tid));
+            w2[q] = y;
+        }
+        __syncthreads();
+        const float2* r2 = s2 + tid + (tid >> 4);
+#pragma unroll
+        for (int i = 0; i < S::NI; ++i) {
+            float2 x[R3];
+#pragma unroll
+            for (int uu = 0; uu < R3; ++uu) x[uu] = r2[uu * S::U + i * (T + R3)];
+            fft::dif<R3, false>(x);
+#pragma unroll
+            for (int q = 0; q < R3; ++q) v[i * R3 + q] = x[fft::bitrev<R3>(q)];
+        }
+    } else {
+        float2 x[16];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x[q] = v[fft::bitrev<16>(q)];
+#pragma unroll
+        for (int q = 0; q < 16; ++q) v[q] = x[q];
+    }
+}
+
+// the mirror: v[e] = Y[freq_of_slot(tid, e)] on entry, v[n1] = N * y[tid + n1*T] on exit
+template <int LGN>
+__device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
+                                        const float2* __restrict__ tw1, const float2* __restrict__ tw2, int tid)
+{
+    using S = Shape<LGN>;
+    constexpr int T = S::T, R3 = S::R3;
+    const int u = tid >> 4, q1 = tid & 15;
+    float2 x16[16];
+    if constexpr (R3 > 1) {
+        float2* w2 = s2 + tid + (tid >> 4);
+#pragma unroll
+        for (int i = 0; i < S::NI; ++i) {
+            float2 x[R3];
+#pragma unroll
+            for (int q = 0; q < R3; ++q) x[fft::bitrev<R3>(q)] = v[i * R3 + q];
+            fft::dit<R3, true>(x);
+#pragma unroll
+            for (int uu = 0; uu < R3; ++uu) w2[uu * S::U + i * (T + R3)] = x[uu];
+        }
+        __syncthreads();
+        const float2* r2 = s2 + u * S::U + 17 * q1;
+#pragma unroll
+        for (int q = 0; q < 16; ++q) {
+            float2 y = r2[q];
+            if (q > 0) y = fft::cmulc(y, __ldg(tw2 + (q - 1) * T + tid));
+            x16[fft::bitrev<16>(q)] = y;
+        }
+    } else {
+#pragma unroll
+        for (int q = 0; q < 16; ++q) x16[fft::bitrev<16>(q)] = v[q];
+    }
+    fft::dit<16, true>(x16);
+    {
+        float2* w1 = s1 + q1 * (T + 1) + u;
+#pragma unroll
+        for (int t1 = 0; t1 < 16; ++t1) w1[t1 * R3] = x16[t1];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int q = 0; q < 16; ++q) {
+        float2 y = s1[q * (T + 1) + tid];
+        if (q > 0) y = fft::cmulc(y, __ldg(tw1 + (q - 1) * T + tid));
+        v[fft::bitrev<16>(q)] = y;
+    }
+    fft::dit<16, true>(v);
+}
+
+#endif  // __CUDACC__
+
+}  // namespace fftr
+}  // namespace mmc
+
+#endif

@@ -155,7 +155,14 @@ def test_sweep_matches_replayed_oracle(name):
 
 @pytest.mark.parametrize("shape,d", [((64, 48, 1), (5e-9, 5e-9, 5e-9)), ((37, 19, 1), (5e-9, 5e-9, 10e-9)),
                                      ((48, 40, 4), (3e-9, 3e-9, 3e-9)), ((30, 21, 3), (2e-9, 3e-9, 4e-9)),
-                                     ((128, 96, 1), (5e-9, 5e-9, 10e-9))])
+                                     ((128, 96, 1), (5e-9, 5e-9, 10e-9)),
+                                     # column transforms of length 2^8 .. 2^12 (register-resident kernels), with the
+                                     # padding exactly half (pruned variant) and ragged, one and several layers
+                                     ((128, 128, 1), (5e-9, 5e-9, 5e-9)), ((100, 200, 1), (5e-9, 4e-9, 3e-9)),
+                                     ((64, 256, 2), (3e-9, 3e-9, 3e-9)), ((72, 512, 1), (2e-9, 2e-9, 2e-9)),
+                                     ((40, 600, 1), (5e-9, 5e-9, 10e-9)), ((48, 1024, 2), (3e-9, 3e-9, 3e-9)),
+                                     ((20, 700, 3), (3e-9, 3e-9, 3e-9)),
+                                     ((32, 2048, 1), (5e-9, 5e-9, 10e-9)), ((36, 1100, 1), (5e-9, 5e-9, 5e-9))])
 def test_demag_field_parity(shape, d):
     """Eq. (14): GPU fp32 FFT convolution vs the oracle's fp64 one (itself pinned to the direct sum)."""
     import paper_2106_05593_b200 as P
