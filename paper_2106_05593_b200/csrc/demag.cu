@@ -41,6 +41,10 @@ struct DemagPlan {
     bool fastB = false;              // columns: register-resident transform (fft_reg.cuh), Py in 2^8 .. 2^12
     float2* twB1 = nullptr;          // its twiddle tables, 15 * Py/16 entries each
     float2* twB2 = nullptr;
+    bool fastA = false;              // rows: register-resident transform, Hx in 2^8 .. 2^11, Pz in {1, 4, 8, 16}, fits shared memory
+    float2* twA1 = nullptr;
+    float2* twA2 = nullptr;
+    float2* twu = nullptr;           // (un)tangling roots in slot order, Hx entries
     float2* T = nullptr;             // [3][Pz][Cx][ny]
     float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
 };
@@ -90,6 +94,18 @@ __global__ void twiddle_kernel(float2* tw, int P)
         double s, c;
         sincospi(-2.0 * (double)k / (double)P, &s, &c);
         tw[k] = make_float2((float)c, (float)s);
+    }
+}
+
+// twu[e*T + t] = exp(-2 pi i k / (2 Hx)), k = frequency in register slot e of thread t (fft_reg.cuh), Hx = 2^lgH
+__global__ void slot_roots_kernel(float2* twu, int lgH)
+{
+    const int Hx = 1 << lgH, T = Hx / 16;
+    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < Hx; idx += gridDim.x * blockDim.x) {
+        const int k = fftr::freq_of_slot(lgH, idx % T, idx / T);
+        double s, c;
+        sincospi(-(double)k / (double)Hx, &s, &c);
+        twu[idx] = make_float2((float)c, (float)s);
     }
 }
 
@@ -278,6 +294,228 @@ __global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
     }
 }
 
+// ------------------------------------------------------------------------------------------------ kernels A and C, register-resident
+// Same work as rows_fwd_kernel / rows_inv_kernel with the length-Hx transform of fft_reg.cuh (Hx = 2^LGH, 8 <= LGH <= 11).
+// block (RJ = 4, T = Hx/16): threadIdx.x = row of the tile (fastest, so that the four rows' values of one frequency are
+// one 32-byte sector of the transposed array T[c][kz][kx][j]), threadIdx.y = thread of the row's transform.
+// Shared memory: nat[nz][4][NS] (spectra in natural order, padded index k + (k>>4), for the mirror-frequency access of
+// the real-transform (un)tangling and for the z-DFT across layers) + one pair of exchange buffers per row.  Row strides
+// are = 4 (mod 16) elements, so that the four rows of a half-warp sit in different bank groups.
+// grid (ceil(ny/4), 3 components).
+constexpr int kRJ = 4;
+template <int LGH> struct RowShape {
+    using S = fftr::Shape<LGH>;
+    static constexpr int Hx = S::N, T = S::T;
+    static constexpr int NS = Hx + Hx / 16 + 4;          // nat row stride; pad(Hx) = Hx + Hx/16 is its last used element
+    static constexpr int ES = S::SMEM + 4;               // exchange row stride
+    static constexpr int CP = Hx + Hx / 16;              // pad(k) + pad(Hx - k) (+1 when k & 15 != 0)
+};
+struct RowFastArgs {
+    Geometry g;
+    int Cx;
+    const float2* tw1; const float2* tw2;                 // fft_reg tables of the length-Hx transform
+    const float2* twu;                                    // exp(-2 pi i k / Px) at k = freq_of_slot(t, e), stored at [e*T + t]
+    const float* m[3]; const float* Ms0; float Ms0_u;
+    float* bd[3];
+    float2* T;
+};
+
+template <int LGH, int PZ>
+__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_fwd_fast_kernel(const RowFastArgs a)
+{
+    using R = RowShape<LGH>;
+    constexpr int T = R::T, Hx = R::Hx;
+    extern __shared__ float2 sm[];
+    const Geometry g = a.g;
+    const int nz = g.nz, ny = g.ny;
+    const int jj = threadIdx.x, t = threadIdx.y;
+    const int c = blockIdx.y, j = blockIdx.x * kRJ + jj;
+    const bool valid = j < ny;
+    const int hxr = (g.nx + 1) >> 1;
+    float2* nat = sm + jj * R::NS;                                  // + k * kRJ * NS per layer
+    float2* s1 = sm + nz * kRJ * R::NS + jj * R::ES;
+    float2* s2 = s1 + R::S::S1;
+    const int pb = fftr::pbase<LGH>(t);
+    const float* __restrict__ mc = a.m[c];
+    for (int k = 0; k < nz; ++k) {
+        // S0: M = Ms0 m; even cells -> real part, odd cells -> imaginary part; only n < Hx/2 can be non-zero
+        float2 v[16];
+        const int row = k * ny + (valid ? j : 0), par = ((valid ? j : 0) + k) & 1;
+        const unsigned be = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx;
+        const unsigned bo = (unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx;
+#pragma unroll
+        for (int n1 = 0; n1 < 8; ++n1) {
+            const int n = t + n1 * T;
+            float2 x = make_float2(0.f, 0.f);
+            if (valid && n < hxr) {
+                x.x = (a.Ms0 ? __ldg(a.Ms0 + be + n) : a.Ms0_u) * __ldg(mc + be + n);
+                if (2 * n + 1 < g.nx) x.y = (a.Ms0 ? __ldg(a.Ms0 + bo + n) : a.Ms0_u) * __ldg(mc + bo + n);
+            }
+            v[n1] = x;
+        }
+#pragma unroll
+        for (int n1 = 8; n1 < 16; ++n1) v[n1] = make_float2(0.f, 0.f);
+        fftr::forward<LGH, true>(v, s1, s2, a.tw1, a.tw2, t);
+        float2* nk = nat + k * kRJ * R::NS + pb;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) nk[fftr::pconst<LGH>(e)] = v[e];
+    }
+    __syncthreads();
+    // untangle (X' = 2 X of the real row, from Z[k] and Z[Hx-k]), z-DFT across the layers, transposed store
+    const int kb = fftr::kbase<LGH>(t);
+    float2* __restrict__ out = a.T + (size_t)c * PZ * a.Cx * ny + (valid ? j : 0);
+    const size_t plane = (size_t)a.Cx * ny;
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const int kx = kb + fftr::kconst<LGH>(e);
+        const int pa = pb + fftr::pconst<LGH>(e);
+        const int pm = (kx == 0) ? pa : R::CP - pa - (fftr::lo_nonzero<LGH>(t, e) ? 1 : 0);
+        const float2 w = __ldg(a.twu + e * T + t);
+        float2 x[PZ];
+#pragma unroll
+        for (int k = 0; k < PZ; ++k) {
+            x[k] = make_float2(0.f, 0.f);
+            if (k < nz) {
+                const float2 A = nat[k * kRJ * R::NS + pa], B = nat[k * kRJ * R::NS + pm];
+                const float2 Sm = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
+                const float2 tt = fft::cmul(w, D);
+                x[k] = make_float2(Sm.x + tt.y, Sm.y - tt.x);
+            }
+        }
+        fft::dif<PZ, false>(x);
+        if (valid) {
+#pragma unroll
+            for (int kz = 0; kz < PZ; ++kz) out[kz * plane + (size_t)kx * ny] = x[fft::bitrev<PZ>(kz)];
+        }
+    }
+    if (t == 0) {                                                    // the Nyquist column kx = Hx: X'[Hx] = 2 (Re Z[0] - Im Z[0])
+        float2 x[PZ];
+#pragma unroll
+        for (int k = 0; k < PZ; ++k) {
+            x[k] = make_float2(0.f, 0.f);
+            if (k < nz) { const float2 z0 = nat[k * kRJ * R::NS]; x[k].x = 2.f * (z0.x - z0.y); }
+        }
+        fft::dif<PZ, false>(x);
+        if (valid) {
+#pragma unroll
+            for (int kz = 0; kz < PZ; ++kz) out[kz * plane + (size_t)Hx * ny] = x[fft::bitrev<PZ>(kz)];
+        }
+    }
+}
+
+template <int LGH, int PZ>
+__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_inv_fast_kernel(const RowFastArgs a)
+{
+    using R = RowShape<LGH>;
+    constexpr int T = R::T, Hx = R::Hx;
+    extern __shared__ float2 sm[];
+    const Geometry g = a.g;
+    const int nz = g.nz, ny = g.ny;
+    const int jj = threadIdx.x, t = threadIdx.y;
+    const int c = blockIdx.y, j = blockIdx.x * kRJ + jj;
+    const bool valid = j < ny;
+    const int hxr = (g.nx + 1) >> 1;
+    float2* nat = sm + jj * R::NS;
+    float2* s1 = sm + nz * kRJ * R::NS + jj * R::ES;
+    float2* s2 = s1 + R::S::S1;
+    const int pb = fftr::pbase<LGH>(t), kb = fftr::kbase<LGH>(t);
+    const float2* __restrict__ in = a.T + (size_t)c * PZ * a.Cx * ny + (valid ? j : 0);
+    const size_t plane = (size_t)a.Cx * ny;
+    // inverse z-DFT of every frequency this thread owns, all layers into nat
+#pragma unroll
+    for (int e = 0; e < 16; ++e) {
+        const int kx = kb + fftr::kconst<LGH>(e);
+        float2 x[PZ];
+#pragma unroll
+        for (int kz = 0; kz < PZ; ++kz) x[fft::bitrev<PZ>(kz)] = valid ? in[kz * plane + (size_t)kx * ny] : make_float2(0.f, 0.f);
+        fft::dit<PZ, true>(x);
+#pragma unroll
+        for (int k = 0; k < PZ; ++k) if (k < nz) nat[k * kRJ * R::NS + pb + fftr::pconst<LGH>(e)] = x[k];
+    }
+    if (t == 0) {
+        float2 x[PZ];
+#pragma unroll
+        for (int kz = 0; kz < PZ; ++kz) x[fft::bitrev<PZ>(kz)] = valid ? in[kz * plane + (size_t)Hx * ny] : make_float2(0.f, 0.f);
+        fft::dit<PZ, true>(x);
+#pragma unroll
+        for (int k = 0; k < PZ; ++k) if (k < nz) nat[k * kRJ * R::NS + R::CP] = x[k];
+    }
+    __syncthreads();
+    float* __restrict__ bc = a.bd[c];
+    for (int k = 0; k < nz; ++k) {
+        // re-tangle: Y[k], Y[Hx-k] -> Z'[k] = 2 (E[k] + i O[k]) in this thread's slots
+        float2 v[16];
+        const float2* nk = nat + k * kRJ * R::NS;
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const int pa = pb + fftr::pconst<LGH>(e);
+            const int pm = R::CP - pa - (fftr::lo_nonzero<LGH>(t, e) ? 1 : 0);
+            const float2 A = nk[pa], B = nk[pm];
+            const float2 w = __ldg(a.twu + e * T + t);
+            const float2 E = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
+            const float2 O = fft::cmulc(D, w);
+            v[e] = make_float2(E.x - O.y, E.y + O.x);
+            if (e == 0 && t == 0) v[e] = make_float2(A.x + B.x, A.x - B.x);     // k = 0: Y[0] and Y[Hx] are real
+        }
+        fftr::inverse<LGH>(v, s1, s2, a.tw1, a.tw2, t);
+        // real part -> even cells, imaginary part -> odd cells of the colour-split B_d
+        const int row = k * ny + (valid ? j : 0), par = ((valid ? j : 0) + k) & 1;
+        const unsigned be = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx;
+        const unsigned bo = (unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx;
+#pragma unroll
+        for (int n1 = 0; n1 < 8; ++n1) {
+            const int n = t + n1 * T;
+            if (valid && n < hxr) {
+                bc[be + n] = v[n1].x;
+                if (2 * n + 1 < g.nx) bc[bo + n] = v[n1].y;
+            }
+        }
+    }
+}
+
+template <int LGH, int PZ>
+static int launch_rows_fast(const DemagPlan* p, const RowFastArgs& ra, bool inverse, cudaStream_t st)
+{
+    using R = RowShape<LGH>;
+    const dim3 grid((p->g.ny + kRJ - 1) / kRJ, 3), block(kRJ, R::T);
+    const size_t smem = ((size_t)p->g.nz * kRJ * R::NS + (size_t)kRJ * R::ES) * sizeof(float2);
+    if (inverse) {
+        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_inv_fast_kernel<LGH, PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        rows_inv_fast_kernel<LGH, PZ><<<grid, block, smem, st>>>(ra);
+    } else {
+        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_fwd_fast_kernel<LGH, PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        rows_fwd_fast_kernel<LGH, PZ><<<grid, block, smem, st>>>(ra);
+    }
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+template <int LGH>
+static int launch_rows_fast_pz(const DemagPlan* p, const RowFastArgs& ra, bool inverse, cudaStream_t st)
+{
+    switch (p->Pz) {
+        case 1: return launch_rows_fast<LGH, 1>(p, ra, inverse, st);
+        case 4: return launch_rows_fast<LGH, 4>(p, ra, inverse, st);
+        case 8: return launch_rows_fast<LGH, 8>(p, ra, inverse, st);
+        case 16: return launch_rows_fast<LGH, 16>(p, ra, inverse, st);
+        default: return MMC_E_UNSUPPORTED;
+    }
+}
+static size_t rows_fast_smem(int lgH, int nz)
+{
+    const int Hx = 1 << lgH, T = Hx / 16, R3 = Hx / 256;
+    const size_t NS = Hx + Hx / 16 + 4, ES = 16 * (T + 1) + (R3 > 1 ? R3 * 272 : 0) + 4;
+    return ((size_t)nz * kRJ * NS + (size_t)kRJ * ES) * sizeof(float2);
+}
+static int launch_rows_fast_any(const DemagPlan* p, const RowFastArgs& ra, bool inverse, cudaStream_t st)
+{
+    switch (ilog2(p->Hx)) {
+        case 8: return launch_rows_fast_pz<8>(p, ra, inverse, st);
+        case 9: return launch_rows_fast_pz<9>(p, ra, inverse, st);
+        case 10: return launch_rows_fast_pz<10>(p, ra, inverse, st);
+        case 11: return launch_rows_fast_pz<11>(p, ra, inverse, st);
+        default: return MMC_E_UNSUPPORTED;
+    }
+}
+
 // kernel B, register-resident variant (fft_reg.cuh) for Py = 2^LGN, 8 <= LGN <= 12: T = Py/16 threads per (kx, kz)
 // column set, G column sets (adjacent kx) per CTA.  Each thread keeps its 16 points of all three components in
 // registers from the forward transform through the tensor multiply into the inverse transform; shared memory only
@@ -426,7 +664,20 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     while (p->RJ > 4 && bytesA(p->RJ) > 100 * 1024) p->RJ >>= 1;
     while (p->RJ > 1 && bytesA(p->RJ) > 200 * 1024) p->RJ >>= 1;
     while (p->RJ > 1 && p->RJ / 2 >= g.ny) p->RJ >>= 1;
-    if (bytesA(p->RJ) > 220 * 1024) { if (err) *err = "demag: nz * padded nx too large for the fused row kernels"; return MMC_E_UNSUPPORTED; }
+    {
+        const int lgH = ilog2(p->Hx);
+        p->fastA = lgH >= 8 && lgH <= 11 && (p->Pz == 1 || p->Pz == 4 || p->Pz == 8 || p->Pz == 16) &&
+                   rows_fast_smem(lgH, g.nz) <= 227 * 1024;
+        if (p->fastA) {
+            const size_t ntw = (size_t)15 * (p->Hx / 16);
+            CK(cudaMalloc(&p->twA1, ntw * sizeof(float2)));
+            CK(cudaMalloc(&p->twA2, ntw * sizeof(float2)));
+            CK(cudaMalloc(&p->twu, (size_t)p->Hx * sizeof(float2)));
+            fftr::twiddle_tables_kernel<<<blocks_for((long long)ntw), 256, 0, st>>>(p->twA1, p->twA2, lgH);
+            slot_roots_kernel<<<blocks_for(p->Hx), 256, 0, st>>>(p->twu, lgH);
+        }
+    }
+    if (!p->fastA && bytesA(p->RJ) > 220 * 1024) { if (err) *err = "demag: nz * padded nx too large for the fused row kernels"; return MMC_E_UNSUPPORTED; }
     p->smemA = bytesA(p->RJ);
     p->threadsA = p->smemA > 100 * 1024 ? 512 : 256;
     p->smemB = (size_t)3 * fft::padded_len(p->Py) * sizeof(float2);
@@ -493,6 +744,7 @@ void demag_destroy(DemagPlan* p)
 {
     if (!p) return;
     cudaFree(p->T); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2);
+    cudaFree(p->twA1); cudaFree(p->twA2); cudaFree(p->twu);
     for (int q = 0; q < 6; ++q) cudaFree(p->nhat[q]);
     delete p;
 }
@@ -514,7 +766,11 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
     ra.RJ = p->RJ; ra.lgRJ = ilog2(p->RJ); ra.RS = p->RS; ra.px = p->px; ra.twx = p->twx;
     for (int c = 0; c < 3; ++c) { ra.m[c] = m[c]; ra.bd[c] = bd[c]; }
     ra.Ms0 = Ms0_split; ra.Ms0_u = Ms0_uniform; ra.T = p->T;
-    int rc = launch_rows_any(p, ra, false, st);
+    RowFastArgs rf{};
+    rf.g = p->g; rf.Cx = p->Cx; rf.tw1 = p->twA1; rf.tw2 = p->twA2; rf.twu = p->twu;
+    for (int c = 0; c < 3; ++c) { rf.m[c] = m[c]; rf.bd[c] = bd[c]; }
+    rf.Ms0 = Ms0_split; rf.Ms0_u = Ms0_uniform; rf.T = p->T;
+    int rc = p->fastA ? launch_rows_fast_any(p, rf, false, st) : launch_rows_any(p, ra, false, st);
     if (rc) { if (err) *err = "rows_fwd_kernel launch failed"; return rc; }
     if (timer) timer->mark(PH_FFT_FWD, stream);
     ColArgs ca{};
@@ -533,7 +789,7 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
         else             columns_kernel<false><<<gridB, p->threadsB, p->smemB, st>>>(ca);
     }
     if (timer) timer->mark(PH_MULTIPLY, stream);
-    rc = launch_rows_any(p, ra, true, st);
+    rc = p->fastA ? launch_rows_fast_any(p, rf, true, st) : launch_rows_any(p, ra, true, st);
     if (rc) { if (err) *err = "rows_inv_kernel launch failed"; return rc; }
     if (timer) timer->mark(PH_FFT_INV, stream);
     CK(cudaGetLastError());

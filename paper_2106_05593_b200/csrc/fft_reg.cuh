@@ -112,6 +112,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
         for (int q = 0; q < 16; ++q) x[q] = v[fft::bitrev<16>(q)];
 #pragma unroll
         for (int q = 0; q < 16; ++q) v[q] = x[q];
+        __syncthreads();                          // buffer 1 was read last: the next transform may overwrite it
     }
 }
 
@@ -161,6 +162,25 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
         v[fft::bitrev<16>(q)] = y;
     }
     fft::dit<16, true>(v);
+    if constexpr (R3 == 1) __syncthreads();       // as in forward
+}
+
+// Slot bookkeeping for kernels that need to know which frequency a register holds (demag.cu rows kernels):
+// freq_of_slot(tid, e) = kbase(tid) + kconst(e); its padded natural-order index k + (k >> 4) = pbase(tid) + pconst(e).
+template <int LGN> __device__ __forceinline__ int kbase(int tid) { return Shape<LGN>::R3 == 1 ? tid : (tid >> 4) + 16 * (tid & 15); }
+template <int LGN> __device__ __forceinline__ int pbase(int tid) { return Shape<LGN>::R3 == 1 ? tid : (tid >> 4) + 17 * (tid & 15); }
+template <int LGN> __host__ __device__ constexpr int kconst(int e)
+{
+    return Shape<LGN>::R3 == 1 ? 16 * e : (e / Shape<LGN>::R3) * Shape<LGN>::R3 + 256 * (e % Shape<LGN>::R3);
+}
+template <int LGN> __host__ __device__ constexpr int pconst(int e)
+{
+    return Shape<LGN>::R3 == 1 ? 17 * e : (e / Shape<LGN>::R3) * Shape<LGN>::R3 + 272 * (e % Shape<LGN>::R3);
+}
+// low nibble of the frequency is non-zero (decides the padded index of the mirror frequency N - k)
+template <int LGN> __device__ __forceinline__ bool lo_nonzero(int tid, int e)
+{
+    return Shape<LGN>::R3 == 1 ? tid > 0 : (e / Shape<LGN>::R3 > 0 || tid >= 16);
 }
 
 #endif  // __CUDACC__

@@ -162,7 +162,16 @@ def test_sweep_matches_replayed_oracle(name):
                                      ((64, 256, 2), (3e-9, 3e-9, 3e-9)), ((72, 512, 1), (2e-9, 2e-9, 2e-9)),
                                      ((40, 600, 1), (5e-9, 5e-9, 10e-9)), ((48, 1024, 2), (3e-9, 3e-9, 3e-9)),
                                      ((20, 700, 3), (3e-9, 3e-9, 3e-9)),
-                                     ((32, 2048, 1), (5e-9, 5e-9, 10e-9)), ((36, 1100, 1), (5e-9, 5e-9, 5e-9))])
+                                     ((32, 2048, 1), (5e-9, 5e-9, 10e-9)), ((36, 1100, 1), (5e-9, 5e-9, 5e-9)),
+                                     # row transforms of length 2^8 .. 2^11 (register-resident kernels): 1, 2, 3, 4, 5 layers
+                                     # (padded z length 1, 4, 8, 8, 16), ragged row tiles, odd nx
+                                     ((200, 40, 1), (5e-9, 5e-9, 5e-9)), ((256, 22, 4), (3e-9, 3e-9, 3e-9)),
+                                     ((301, 18, 3), (2e-9, 3e-9, 4e-9)), ((512, 16, 2), (3e-9, 3e-9, 3e-9)),
+                                     ((1024, 10, 1), (5e-9, 5e-9, 10e-9)), ((700, 9, 4), (3e-9, 3e-9, 3e-9)),
+                                     ((520, 6, 5), (3e-9, 3e-9, 3e-9)), ((2048, 7, 1), (5e-9, 5e-9, 10e-9)),
+                                     ((1500, 5, 2), (3e-9, 3e-9, 3e-9)),
+                                     # both fast paths together
+                                     ((256, 256, 1), (5e-9, 5e-9, 5e-9)), ((512, 128, 4), (3e-9, 3e-9, 3e-9))])
 def test_demag_field_parity(shape, d):
     """Eq. (14): GPU fp32 FFT convolution vs the oracle's fp64 one (itself pinned to the direct sum)."""
     import paper_2106_05593_b200 as P
