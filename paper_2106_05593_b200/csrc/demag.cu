@@ -39,12 +39,9 @@ struct DemagPlan {
     float2* twx = nullptr;           // exp(-2 pi i k / Px), k < Px
     float2* twy = nullptr;           // exp(-2 pi i k / Py), k < Py
     bool fastB = false;              // columns: register-resident transform (fft_reg.cuh), Py in 2^8 .. 2^12
-    float2* twB1 = nullptr;          // its twiddle tables, 15 * Py/16 entries each
+    float2* twB1 = nullptr;          // its twiddle tables (fftr::Twiddles), 15 * Py/16 entries each
     float2* twB2 = nullptr;
     bool fastA = false;              // rows: register-resident transform, Hx in 2^8 .. 2^11, Pz in {1, 4, 8, 16}, fits shared memory
-    float2* twA1 = nullptr;
-    float2* twA2 = nullptr;
-    float2* twu = nullptr;           // (un)tangling roots in slot order, Hx entries
     float2* T = nullptr;             // [3][Pz][Cx][ny]
     float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
 };
@@ -94,18 +91,6 @@ __global__ void twiddle_kernel(float2* tw, int P)
         double s, c;
         sincospi(-2.0 * (double)k / (double)P, &s, &c);
         tw[k] = make_float2((float)c, (float)s);
-    }
-}
-
-// twu[e*T + t] = exp(-2 pi i k / (2 Hx)), k = frequency in register slot e of thread t (fft_reg.cuh), Hx = 2^lgH
-__global__ void slot_roots_kernel(float2* twu, int lgH)
-{
-    const int Hx = 1 << lgH, T = Hx / 16;
-    for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < Hx; idx += gridDim.x * blockDim.x) {
-        const int k = fftr::freq_of_slot(lgH, idx % T, idx / T);
-        double s, c;
-        sincospi(-(double)k / (double)Hx, &s, &c);
-        twu[idx] = make_float2((float)c, (float)s);
     }
 }
 
@@ -313,8 +298,7 @@ template <int LGH> struct RowShape {
 struct RowFastArgs {
     Geometry g;
     int Cx;
-    const float2* tw1; const float2* tw2;                 // fft_reg tables of the length-Hx transform
-    const float2* twu;                                    // exp(-2 pi i k / Px) at k = freq_of_slot(t, e), stored at [e*T + t]
+    float2 cu[16];                                        // exp(-2 pi i kconst(e) / Px): slot part of the (un)tangling root
     const float* m[3]; const float* Ms0; float Ms0_u;
     float* bd[3];
     float2* T;
@@ -336,26 +320,34 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_fwd_fast_kerne
     float2* s1 = sm + nz * kRJ * R::NS + jj * R::ES;
     float2* s2 = s1 + R::S::S1;
     const int pb = fftr::pbase<LGH>(t);
+    const fftr::Twiddles tw{ fftr::root(t, Hx), fftr::root(t >> 4, T), nullptr, nullptr };
     const float* __restrict__ mc = a.m[c];
-    for (int k = 0; k < nz; ++k) {
-        // S0: M = Ms0 m; even cells -> real part, odd cells -> imaginary part; only n < Hx/2 can be non-zero
-        float2 v[16];
+    // S0: M = Ms0 m; even cells -> real part, odd cells -> imaginary part; only n < Hx/2 can be non-zero.
+    // The next layer's cells are requested before the current layer is transformed.
+    float2 raw[8], rws[8];                         // m and Ms0 as loaded; multiplied when consumed
+    auto fetch = [&](int k) {
         const int row = k * ny + (valid ? j : 0), par = ((valid ? j : 0) + k) & 1;
         const unsigned be = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx;
         const unsigned bo = (unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx;
 #pragma unroll
         for (int n1 = 0; n1 < 8; ++n1) {
             const int n = t + n1 * T;
-            float2 x = make_float2(0.f, 0.f);
+            float2 x = make_float2(0.f, 0.f), ms = make_float2(a.Ms0_u, a.Ms0_u);
             if (valid && n < hxr) {
-                x.x = (a.Ms0 ? __ldg(a.Ms0 + be + n) : a.Ms0_u) * __ldg(mc + be + n);
-                if (2 * n + 1 < g.nx) x.y = (a.Ms0 ? __ldg(a.Ms0 + bo + n) : a.Ms0_u) * __ldg(mc + bo + n);
+                x.x = __ldg(mc + be + n);
+                if (a.Ms0) ms.x = __ldg(a.Ms0 + be + n);
+                if (2 * n + 1 < g.nx) { x.y = __ldg(mc + bo + n); if (a.Ms0) ms.y = __ldg(a.Ms0 + bo + n); }
             }
-            v[n1] = x;
+            raw[n1] = x; rws[n1] = ms;
         }
+    };
+    fetch(0);
+    for (int k = 0; k < nz; ++k) {
+        float2 v[16];
 #pragma unroll
-        for (int n1 = 8; n1 < 16; ++n1) v[n1] = make_float2(0.f, 0.f);
-        fftr::forward<LGH, true>(v, s1, s2, a.tw1, a.tw2, t);
+        for (int n1 = 0; n1 < 8; ++n1) { v[n1] = make_float2(raw[n1].x * rws[n1].x, raw[n1].y * rws[n1].y); v[n1 + 8] = make_float2(0.f, 0.f); }
+        if (k + 1 < nz) fetch(k + 1);
+        fftr::forward<LGH, true, false>(v, s1, s2, tw, t);
         float2* nk = nat + k * kRJ * R::NS + pb;
 #pragma unroll
         for (int e = 0; e < 16; ++e) nk[fftr::pconst<LGH>(e)] = v[e];
@@ -363,6 +355,7 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_fwd_fast_kerne
     __syncthreads();
     // untangle (X' = 2 X of the real row, from Z[k] and Z[Hx-k]), z-DFT across the layers, transposed store
     const int kb = fftr::kbase<LGH>(t);
+    const float2 wub = fftr::root(kb, 2 * Hx);
     float2* __restrict__ out = a.T + (size_t)c * PZ * a.Cx * ny + (valid ? j : 0);
     const size_t plane = (size_t)a.Cx * ny;
 #pragma unroll
@@ -370,7 +363,7 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_fwd_fast_kerne
         const int kx = kb + fftr::kconst<LGH>(e);
         const int pa = pb + fftr::pconst<LGH>(e);
         const int pm = (kx == 0) ? pa : R::CP - pa - (fftr::lo_nonzero<LGH>(t, e) ? 1 : 0);
-        const float2 w = __ldg(a.twu + e * T + t);
+        const float2 w = fft::cmul(wub, a.cu[e]);
         float2 x[PZ];
 #pragma unroll
         for (int k = 0; k < PZ; ++k) {
@@ -419,6 +412,8 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_inv_fast_kerne
     float2* s1 = sm + nz * kRJ * R::NS + jj * R::ES;
     float2* s2 = s1 + R::S::S1;
     const int pb = fftr::pbase<LGH>(t), kb = fftr::kbase<LGH>(t);
+    const fftr::Twiddles tw{ fftr::root(t, Hx), fftr::root(t >> 4, T), nullptr, nullptr };
+    const float2 wub = fftr::root(kb, 2 * Hx);
     const float2* __restrict__ in = a.T + (size_t)c * PZ * a.Cx * ny + (valid ? j : 0);
     const size_t plane = (size_t)a.Cx * ny;
     // inverse z-DFT of every frequency this thread owns, all layers into nat
@@ -451,13 +446,13 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_inv_fast_kerne
             const int pa = pb + fftr::pconst<LGH>(e);
             const int pm = R::CP - pa - (fftr::lo_nonzero<LGH>(t, e) ? 1 : 0);
             const float2 A = nk[pa], B = nk[pm];
-            const float2 w = __ldg(a.twu + e * T + t);
+            const float2 w = fft::cmul(wub, a.cu[e]);
             const float2 E = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
             const float2 O = fft::cmulc(D, w);
             v[e] = make_float2(E.x - O.y, E.y + O.x);
             if (e == 0 && t == 0) v[e] = make_float2(A.x + B.x, A.x - B.x);     // k = 0: Y[0] and Y[Hx] are real
         }
-        fftr::inverse<LGH>(v, s1, s2, a.tw1, a.tw2, t);
+        fftr::inverse<LGH, false>(v, s1, s2, tw, t);
         // real part -> even cells, imaginary part -> odd cells of the colour-split B_d
         const int row = k * ny + (valid ? j : 0), par = ((valid ? j : 0) + k) & 1;
         const unsigned be = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx;
@@ -523,7 +518,7 @@ static int launch_rows_fast_any(const DemagPlan* p, const RowFastArgs& ra, bool 
 // of the output are pruned at compile time.  grid (ceil(Cx/G), Pz), block (T, G).
 struct ColFastArgs {
     int ny, Cx, Pz;
-    const float2* tw1; const float2* tw2;
+    const float2* tw1; const float2* tw2;      // fft_reg.cuh twiddle tables of the length-Py transform
     float2* T;
     const float* nhat[6];
 };
@@ -542,17 +537,42 @@ columns_fast_kernel(const ColFastArgs a)
     const bool live = kxr < a.Cx;                      // idle groups still walk through the barriers
     const int kx = live ? kxr : a.Cx - 1;
     const int ny = a.ny;
+    const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), a.tw1, a.tw2 };
     float2 v[3][16];
+    // all three components' columns are requested at once, and the tensor spectrum this thread will need after the
+    // forward transforms is pulled into L2 meanwhile (no registers held)
+    if (HALF) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < 8; ++n1) v[c][n1] = col[tid + n1 * T];
+        }
+    }
+    {
+        const int kzs = (2 * kz <= a.Pz) ? kz : a.Pz - kz;
+        const size_t nb = ((size_t)kzs * a.Cx + kx) * N + tid;
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            if (a.nhat[q] == nullptr) continue;
+#pragma unroll
+            for (int e = 0; e < 16; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
+        }
+    }
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        const float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+        if (HALF) {
 #pragma unroll
-        for (int n1 = 0; n1 < 16; ++n1) {
-            const int j = tid + n1 * T;
-            if (HALF) v[c][n1] = (n1 < 8) ? col[j] : make_float2(0.f, 0.f);
-            else v[c][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
+            for (int n1 = 8; n1 < 16; ++n1) v[c][n1] = make_float2(0.f, 0.f);
+        } else {
+            const float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const int j = tid + n1 * T;
+                v[c][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
+            }
         }
-        fftr::forward<LGN, HALF>(v[c], s1, s2, a.tw1, a.tw2, tid);
+        fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
     }
     // S2: B^ = K^ M^ (see columns_kernel); slot e of thread tid reads the permuted spectrum at e*T + tid
     {
@@ -581,7 +601,7 @@ columns_fast_kernel(const ColFastArgs a)
     __syncthreads();                                   // every thread is done reading exchange buffer 2
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        fftr::inverse<LGN>(v[c], s1, s2, a.tw1, a.tw2, tid);
+        fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
         float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
         for (int n1 = 0; n1 < (HALF ? 8 : 16); ++n1) {
@@ -668,14 +688,6 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
         const int lgH = ilog2(p->Hx);
         p->fastA = lgH >= 8 && lgH <= 11 && (p->Pz == 1 || p->Pz == 4 || p->Pz == 8 || p->Pz == 16) &&
                    rows_fast_smem(lgH, g.nz) <= 227 * 1024;
-        if (p->fastA) {
-            const size_t ntw = (size_t)15 * (p->Hx / 16);
-            CK(cudaMalloc(&p->twA1, ntw * sizeof(float2)));
-            CK(cudaMalloc(&p->twA2, ntw * sizeof(float2)));
-            CK(cudaMalloc(&p->twu, (size_t)p->Hx * sizeof(float2)));
-            fftr::twiddle_tables_kernel<<<blocks_for((long long)ntw), 256, 0, st>>>(p->twA1, p->twA2, lgH);
-            slot_roots_kernel<<<blocks_for(p->Hx), 256, 0, st>>>(p->twu, lgH);
-        }
     }
     if (!p->fastA && bytesA(p->RJ) > 220 * 1024) { if (err) *err = "demag: nz * padded nx too large for the fused row kernels"; return MMC_E_UNSUPPORTED; }
     p->smemA = bytesA(p->RJ);
@@ -743,8 +755,7 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
 void demag_destroy(DemagPlan* p)
 {
     if (!p) return;
-    cudaFree(p->T); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2);
-    cudaFree(p->twA1); cudaFree(p->twA2); cudaFree(p->twu);
+    cudaFree(p->T); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2); 
     for (int q = 0; q < 6; ++q) cudaFree(p->nhat[q]);
     delete p;
 }
@@ -767,7 +778,14 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
     for (int c = 0; c < 3; ++c) { ra.m[c] = m[c]; ra.bd[c] = bd[c]; }
     ra.Ms0 = Ms0_split; ra.Ms0_u = Ms0_uniform; ra.T = p->T;
     RowFastArgs rf{};
-    rf.g = p->g; rf.Cx = p->Cx; rf.tw1 = p->twA1; rf.tw2 = p->twA2; rf.twu = p->twu;
+    rf.g = p->g; rf.Cx = p->Cx;
+    if (p->fastA) {
+        const int lgH = ilog2(p->Hx);
+        for (int e = 0; e < 16; ++e) {                      // kconst(e) of fft_reg.cuh = freq_of_slot(thread 0, e)
+            const double ang = -2.0 * M_PI * (double)fftr::freq_of_slot(lgH, 0, e) / (double)p->Px;
+            rf.cu[e] = make_float2((float)std::cos(ang), (float)std::sin(ang));
+        }
+    }
     for (int c = 0; c < 3; ++c) { rf.m[c] = m[c]; rf.bd[c] = bd[c]; }
     rf.Ms0 = Ms0_split; rf.Ms0_u = Ms0_uniform; rf.T = p->T;
     int rc = p->fastA ? launch_rows_fast_any(p, rf, false, st) : launch_rows_any(p, ra, false, st);

@@ -2,8 +2,9 @@
 //
 // Every thread keeps 16 points of one transform in registers; a transform of length N = 16 * 16 * R3 (R3 = N/256 in
 // {1, 2, 4, 8, 16}) is two radix-16 steps and one radix-R3 step with two exchanges through shared memory in between.
-// All lengths, strides and radices are template parameters, so every shared-memory and table access is
-// "per-thread base + immediate" and the butterflies are straight-line code.  T = N/16 threads work on one transform.
+// All lengths, strides and radices are template parameters, so every shared-memory access is "per-thread base +
+// immediate" and the butterflies are straight-line code; the twiddles of a thread are the powers of one root per
+// stage (w_N^tid, w_T^(tid>>4)), formed in registers, so no twiddle table is read.  T = N/16 threads work on one transform.
 //
 // Forward (decimation in frequency), thread `tid` of the transform:
 //   in   v[n1] = x[tid + n1*T]                                  (HALF: x[n] = 0 for n >= N/2 is folded at compile time)
@@ -46,23 +47,60 @@ __host__ __device__ inline int freq_of_slot(int lgN, int tid, int e)
 
 #ifdef __CUDACC__
 
-// tw1[(q-1)*T + t] = exp(-2 pi i t q / N), tw2[(q-1)*T + t] = exp(-2 pi i (t>>4) q / T), q = 1..15
-__global__ void twiddle_tables_kernel(float2* tw1, float2* tw2, int lgN)
+// exp(-2 pi i num / den), |num/den| <= 1: sincospif is exact in its range reduction and ~1 ulp
+__device__ __forceinline__ float2 root(int num, int den)
+{
+    float sn, cs;
+    sincospif(-2.f * (float)num / (float)den, &sn, &cs);      // num/den is exact for den a power of two, num < 2^24
+    return make_float2(cs, sn);
+}
+// pw[q-1] = w^q, q = 1..15, by a product tree of depth <= 4 (a few ulp): the stage twiddles of a thread are the
+// powers of ONE root (w_N^tid, w_T^u), so no twiddle table is read anywhere
+__device__ __forceinline__ void powers15(float2 w, float2 (&pw)[15])
+{
+    pw[0] = w;
+    pw[1] = fft::cmul(w, w);
+    pw[2] = fft::cmul(pw[1], w);
+    pw[3] = fft::cmul(pw[1], pw[1]);
+#pragma unroll
+    for (int q = 0; q < 3; ++q) pw[4 + q] = fft::cmul(pw[3], pw[q]);
+    pw[7] = fft::cmul(pw[3], pw[3]);
+#pragma unroll
+    for (int q = 0; q < 7; ++q) pw[8 + q] = fft::cmul(pw[7], pw[q]);
+}
+
+// Stage twiddles of one thread, either way:
+//   computed: the powers of w1 = w_N^tid and w2 = w_T^(tid>>4) (kernels whose L1 is taken by shared memory)
+//   table:    t1[(q-1)*T + tid] = w_N^(tid q), t2[(q-1)*T + tid] = w_T^((tid>>4) q), q = 1..15, L1-resident
+struct Twiddles { float2 w1, w2; const float2* t1; const float2* t2; };
+
+__global__ void twiddle_tables_kernel(float2* t1, float2* t2, int lgN)
 {
     const int N = 1 << lgN, T = N / 16;
     for (int idx = blockIdx.x * blockDim.x + threadIdx.x; idx < 15 * T; idx += gridDim.x * blockDim.x) {
         const int q = idx / T + 1, t = idx % T;
         double s, c;
         sincospi(-2.0 * (double)(t * q) / (double)N, &s, &c);
-        tw1[idx] = make_float2((float)c, (float)s);
+        t1[idx] = make_float2((float)c, (float)s);
         sincospi(-2.0 * (double)((t >> 4) * q) / (double)T, &s, &c);
-        tw2[idx] = make_float2((float)c, (float)s);
+        t2[idx] = make_float2((float)c, (float)s);
     }
 }
 
-template <int LGN, bool HALF>
+template <int T, bool TABLE>
+__device__ __forceinline__ void stage_twiddles(float2 w, const float2* __restrict__ tab, int tid, float2 (&pw)[15])
+{
+    if (TABLE) {
+#pragma unroll
+        for (int q = 0; q < 15; ++q) pw[q] = __ldg(tab + q * T + tid);
+    } else {
+        powers15(w, pw);
+    }
+}
+
+template <int LGN, bool HALF, bool TABLE>
 __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
-                                        const float2* __restrict__ tw1, const float2* __restrict__ tw2, int tid)
+                                        const Twiddles& tw, int tid)
 {
     using S = Shape<LGN>;
     constexpr int T = S::T, R3 = S::R3;
@@ -73,11 +111,15 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
     } else {
         fft::dif<16, false>(v);
     }
+    {
+        float2 pw[15];
+        stage_twiddles<T, TABLE>(tw.w1, tw.t1, tid, pw);
 #pragma unroll
-    for (int q = 0; q < 16; ++q) {
-        float2 y = v[fft::bitrev<16>(q)];
-        if (q > 0) y = fft::cmul(y, __ldg(tw1 + (q - 1) * T + tid));
-        s1[q * (T + 1) + tid] = y;
+        for (int q = 0; q < 16; ++q) {
+            float2 y = v[fft::bitrev<16>(q)];
+            if (q > 0) y = fft::cmul(y, pw[q - 1]);
+            s1[q * (T + 1) + tid] = y;
+        }
     }
     __syncthreads();
     const int u = tid >> 4, q1 = tid & 15;
@@ -88,12 +130,14 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
     }
     fft::dif<16, false>(v);
     if constexpr (R3 > 1) {
-        float2* w2 = s2 + u * S::U + 17 * q1;
+        float2* d2 = s2 + u * S::U + 17 * q1;
+        float2 pw[15];
+        stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw);
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             float2 y = v[fft::bitrev<16>(q)];
-            if (q > 0) y = fft::cmul(y, __ldg(tw2 + (q - 1) * T + tid));
-            w2[q] = y;
+            if (q > 0) y = fft::cmul(y, pw[q - 1]);
+            d2[q] = y;
         }
         __syncthreads();
         const float2* r2 = s2 + tid + (tid >> 4);
@@ -117,16 +161,16 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
 }
 
 // the mirror: v[e] = Y[freq_of_slot(tid, e)] on entry, v[n1] = N * y[tid + n1*T] on exit
-template <int LGN>
+template <int LGN, bool TABLE>
 __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
-                                        const float2* __restrict__ tw1, const float2* __restrict__ tw2, int tid)
+                                        const Twiddles& tw, int tid)
 {
     using S = Shape<LGN>;
     constexpr int T = S::T, R3 = S::R3;
     const int u = tid >> 4, q1 = tid & 15;
     float2 x16[16];
     if constexpr (R3 > 1) {
-        float2* w2 = s2 + tid + (tid >> 4);
+        float2* d2 = s2 + tid + (tid >> 4);
 #pragma unroll
         for (int i = 0; i < S::NI; ++i) {
             float2 x[R3];
@@ -134,14 +178,16 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
             for (int q = 0; q < R3; ++q) x[fft::bitrev<R3>(q)] = v[i * R3 + q];
             fft::dit<R3, true>(x);
 #pragma unroll
-            for (int uu = 0; uu < R3; ++uu) w2[uu * S::U + i * (T + R3)] = x[uu];
+            for (int uu = 0; uu < R3; ++uu) d2[uu * S::U + i * (T + R3)] = x[uu];
         }
+        float2 pw[15];
+        stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw);
         __syncthreads();
         const float2* r2 = s2 + u * S::U + 17 * q1;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             float2 y = r2[q];
-            if (q > 0) y = fft::cmulc(y, __ldg(tw2 + (q - 1) * T + tid));
+            if (q > 0) y = fft::cmulc(y, pw[q - 1]);
             x16[fft::bitrev<16>(q)] = y;
         }
     } else {
@@ -150,16 +196,20 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
     }
     fft::dit<16, true>(x16);
     {
-        float2* w1 = s1 + q1 * (T + 1) + u;
+        float2* d1 = s1 + q1 * (T + 1) + u;
 #pragma unroll
-        for (int t1 = 0; t1 < 16; ++t1) w1[t1 * R3] = x16[t1];
+        for (int t1 = 0; t1 < 16; ++t1) d1[t1 * R3] = x16[t1];
     }
-    __syncthreads();
+    {
+        float2 pw[15];
+        stage_twiddles<T, TABLE>(tw.w1, tw.t1, tid, pw);
+        __syncthreads();
 #pragma unroll
-    for (int q = 0; q < 16; ++q) {
-        float2 y = s1[q * (T + 1) + tid];
-        if (q > 0) y = fft::cmulc(y, __ldg(tw1 + (q - 1) * T + tid));
-        v[fft::bitrev<16>(q)] = y;
+        for (int q = 0; q < 16; ++q) {
+            float2 y = s1[q * (T + 1) + tid];
+            if (q > 0) y = fft::cmulc(y, pw[q - 1]);
+            v[fft::bitrev<16>(q)] = y;
+        }
     }
     fft::dit<16, true>(v);
     if constexpr (R3 == 1) __syncthreads();       // as in forward
