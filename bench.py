@@ -27,9 +27,56 @@ if ROOT not in sys.path:
 
 METRIC = "cell_updates_per_sec"
 UNIT = "cell updates/s"
-# algorithmic (compulsory) bytes per cell update of the colour pass: own m read 12 + write 12,
-# B_d 12 (demag configs), mask 1 (cfg 4, 5), per-cell coefficients 28 (cfg 4)
-ALGO_BYTES_PER_UPDATE = {1: 24, 2: 36, 3: 36, 4: 65, 5: 37}
+# Algorithmic (compulsory) bytes, DESIGN.md section 6.
+# Colour pass, per cell update: own m read 12 + write 12, B_d 12 (demag configs), + 1 mask byte (open boundaries, empty
+# cells) or + 4 (the class word = coefficient class << 7 | mask, cfg 4; SURVEY's alternative to 28 B of per-cell
+# coefficients).  Units per launch = non-empty cells of one colour.
+def layout_flags(wl):
+    """(per-cell classes?, mask byte?, per-cell Ms0 array?) as libmmc_b200 decides them for this workload."""
+    nonempty = [r for r in wl.regions if r["Ms0"] > 0]
+    percell = wl.T_per_cell is not None or len(nonempty) > 1
+    open_bc = any(n > 1 and not (wl.pbc_mask >> a) & 1 for a, n in enumerate((wl.nx, wl.ny, wl.nz)))
+    mask = open_bc or wl.n_active < wl.N or (len(nonempty) > 1 and not wl.inter_region_exchange)
+    ms0_per_cell = wl.n_active < wl.N or len({r["Ms0"] for r in nonempty}) > 1
+    return percell, mask, ms0_per_cell
+
+
+def pass_bytes_per_update(wl):
+    percell, mask, _ = layout_flags(wl)
+    return 24 + (12 if wl.demag else 0) + (4 if percell else (1 if mask else 0))
+
+
+def _pow2_at_least(n, start):
+    p = start
+    while p < 2 * n - 1:
+        p *= 2
+    return p
+
+
+def demag_kernel_bytes(wl, ms0_per_cell):
+    """Algorithmic bytes per launch of the three demag kernels (units per launch = the N mesh cells of one convolution).
+    T = the transposed half-spectrum array [3][Pz][Px/2+1][ny] complex64 that the rows kernels write/read and the columns
+    kernel transforms in place (only the ny kept rows are ever stored); tensor = 4 (one layer) or 6 real arrays over
+    [Pz/2+1][Px/2+1][Py]."""
+    Px, Py = _pow2_at_least(wl.nx, 2), _pow2_at_least(wl.ny, 1)
+    Pz = _pow2_at_least(wl.nz, 1)
+    Cx = Px // 2 + 1
+    T = 3 * Pz * Cx * wl.ny * 8
+    tensor = (4 if wl.nz == 1 else 6) * (Pz // 2 + 1) * Cx * Py * 4
+    state = 3 * wl.N * 4
+    # algorithmic flops (5 n log2 n per complex transform of length n, + the 3x3 real-symmetric multiply)
+    import math
+    fl_rows = 3 * wl.ny * wl.nz * 5 * (Px // 2) * math.log2(Px // 2)
+    fl_cols = 3 * Pz * Cx * 2 * 5 * Py * math.log2(Py) + Pz * Cx * Py * (20 if wl.nz == 1 else 36)
+    return {"rows_fwd": {"bytes": state + (wl.N * 4 if ms0_per_cell else 0) + T, "flops": fl_rows},
+            "columns": {"bytes": 2 * T + tensor, "flops": fl_cols},
+            "rows_inv": {"bytes": T + state, "flops": fl_rows}}
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/), cfg 4
+NCU_TRAFFIC_CFG4 = {   # profiles/r1d_summary.md
+    "colour_pass_kernel": 113.5e6, "demag_rows_fwd_kernel": 199.4e6, "demag_columns_kernel": 780.3e6, "demag_rows_inv_kernel": 237.0e6,
+}
 
 
 def replica_seed(base_seed: int, rank: int) -> int:
@@ -129,7 +176,11 @@ def time_oracle(cfg: int, steps: int, warmup: int):
     W.configure(o, wl, O.Material)
     if wl.demag:
         o.demag_field()                       # tensor set-up outside the timed region (as on the GPU side)
+    t0 = time.perf_counter()
     o.run(max(1, warmup))
+    per = (time.perf_counter() - t0) / max(1, warmup)
+    if steps is None:                         # cpu_baseline leg: about 10 s of CPU work
+        steps = int(min(400, max(2, round(10.0 / max(per, 1e-3)))))
     t0 = time.perf_counter()
     o.run(steps)
     dt = time.perf_counter() - t0
@@ -195,22 +246,18 @@ def run_ours(args):
     value = aggregate_over_ranks(units, ms * 1e-3)
     ob = g.observables()
 
-    # e2e through the C ABI with host buffers: pinned H2D of the step's m, one iteration, D2H of m + observables
+    # e2e through the C ABI with HOST buffers (mmc_set_m_host / mmc_get_m_host do the copies on the ctx stream): pinned
+    # H2D of the step's m, one iteration, D2H of m and of the read-out struct
     nE = max(3, min(K, 20))
     host_in = [torch.from_numpy(np.ascontiguousarray(wl.m0[a])).pin_memory() for a in range(3)]
     host_out = [torch.empty(wl.N, dtype=torch.float32).pin_memory() for _ in range(3)]
-    dbuf = [torch.empty(wl.N, dtype=torch.float32, device=dev) for _ in range(3)]
     L = P.lib()
     obs = P.Obs()
 
     def e2e_step():
-        for a in range(3):
-            dbuf[a].copy_(host_in[a], non_blocking=True)
-        g._ck(L.mmc_set_m(g._h, dbuf[0].data_ptr(), dbuf[1].data_ptr(), dbuf[2].data_ptr()))
+        g._ck(L.mmc_set_m_host(g._h, host_in[0].data_ptr(), host_in[1].data_ptr(), host_in[2].data_ptr()))
         g._ck(L.mmc_sweep(g._h, 1))
-        g._ck(L.mmc_get_m(g._h, dbuf[0].data_ptr(), dbuf[1].data_ptr(), dbuf[2].data_ptr()))
-        for a in range(3):
-            host_out[a].copy_(dbuf[a], non_blocking=True)
+        g._ck(L.mmc_get_m_host(g._h, host_out[0].data_ptr(), host_out[1].data_ptr(), host_out[2].data_ptr()))
         g._ck(L.mmc_get_observables(g._h, P.C.byref(obs)))      # synchronises; D2H of the read-out struct
 
     e2e_step(); barrier()
@@ -225,33 +272,58 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = _peaks()
         step_ms = sum(phases.values()) / K
-        # dominant kernel among OUR kernels (the two cuFFT legs are library code in this round): the colour pass
-        own = {k: v for k, v in phases.items() if k not in ("fft_fwd", "fft_inv")}
+        percell, mask, ms0_pc = layout_flags(wl)
+        # per-launch time, algorithmic bytes and flops of every kernel of the step (CUDA events on the ctx stream)
+        kern = {}
         pass_ms = (phases["red"] + phases["black"]) / (2 * K)
-        algo_bytes = ALGO_BYTES_PER_UPDATE[cfg] * (wl.n_active / 2.0)
-        achieved = algo_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
+        bpu = pass_bytes_per_update(wl)
+        kern["colour_pass_kernel"] = {"launch_ms": pass_ms, "launches_per_step": 2, "bytes": bpu * wl.n_active / 2.0,
+                                      "units_per_launch": wl.n_active / 2.0, "bytes_per_unit": bpu}
+        if wl.demag:
+            db = demag_kernel_bytes(wl, ms0_pc)
+            for name, ph in (("rows_fwd", "rows_fwd"), ("columns", "columns"), ("rows_inv", "rows_inv")):
+                kern["demag_" + name + "_kernel"] = {"launch_ms": phases[ph] / K, "launches_per_step": 1, "bytes": db[name]["bytes"],
+                                                    "flops": db[name]["flops"], "units_per_launch": wl.N,
+                                                    "bytes_per_unit": db[name]["bytes"] / wl.N}
+        for k, d in kern.items():
+            t = d["launch_ms"] * 1e-3
+            d["achieved_GBs"] = d["bytes"] / t / 1e9 if t > 0 else 0.0
+            d["frac_of_hbm_peak"] = d["achieved_GBs"] / peak
+            d["share_of_step"] = d["launch_ms"] * d["launches_per_step"] / step_ms if step_ms > 0 else None
+            if "flops" in d:
+                d["achieved_TFLOPs"] = d["flops"] / t / 1e12 if t > 0 else 0.0
+            d["ncu_traffic_bytes"] = NCU_TRAFFIC_CFG4.get(k) if (cfg == 4 and not args.small) else None
+        dom = max(kern, key=lambda k: kern[k]["launch_ms"])          # the dominant kernel = longest single launch
+        dk = kern[dom]
+        demag_ms = sum(phases[k] for k in ("pack", "rows_fwd", "columns", "rows_inv", "crop")) / K
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": f"{wl.name} {wl.nx}x{wl.ny}x{wl.nz} ({wl.n_active} non-empty cells)", "cfg": cfg,
-                       "step": "1 MMC iteration = demag FFT convolution + red + black colour pass + bookkeeping",
-                       "l2": "working set (state + coefficients + FFT buffers) exceeds the 126 MB L2" if wl.N >= 2 ** 22 else
-                             "working set fits L2 (small config); every iteration still streams the FFT buffers",
+                       "step": "1 MMC iteration = demag FFT convolution (rows, columns + tensor multiply, inverse rows) + red + "
+                               "black colour pass + bookkeeping",
+                       "l2": "inputs larger than L2: state + B_d + class words + FFT work array + tensor spectrum = "
+                             f"{(kern.get('demag_columns_kernel', {'bytes': 0})['bytes'] + 7 * 4 * wl.N) / 1e6:.0f} MB streamed per step "
+                             "(L2 = 126 MB)" if wl.N >= 2 ** 22 else
+                             "working set fits L2 (small config, a parity case rather than a bench line)",
                        "parallelism": "replicas" if world > 1 else "single GPU", "cone_deg": wl.cone_deg,
                        "acceptance": ob["accepted"] / max(1, ob["trials"])},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nE},
             "gpu_launches": (6 if wl.demag else 3) * K,
             "phases_ms_per_step": {k: v / K for k, v in phases.items()},
-            "sweep_only_updates_per_sec": wl.n_active / ((phases["red"] + phases["black"]) / K * 1e-3) if pass_ms > 0 else None,
-            "demag_convolutions_per_sec": (K / (sum(phases[k] for k in ("pack", "fft_fwd", "multiply", "fft_inv", "crop")) * 1e-3)) if wl.demag else None,
-            "roofline": {"kernel": "colour_pass_kernel (one colour pass)", "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
-                         "algorithmic_bytes_per_update": ALGO_BYTES_PER_UPDATE[cfg], "updates_per_launch": wl.n_active / 2.0,
-                         "launch_ms": pass_ms, "share_of_step": (phases["red"] + phases["black"]) / K / step_ms if step_ms > 0 else None},
+            "sweep_only_updates_per_sec": wl.n_active / (2 * pass_ms * 1e-3) if pass_ms > 0 else None,
+            "demag_convolutions_per_sec": (1e3 / demag_ms) if (wl.demag and demag_ms > 0) else None,
+            "roofline": {"kernel": dom, "bound": "hbm", "achieved": dk["achieved_GBs"], "peak": peak, "unit": "GB/s",
+                         "frac": dk["frac_of_hbm_peak"], "traffic": dk["ncu_traffic_bytes"], "peak_source": peak_src,
+                         "algorithmic_bytes_per_unit": dk["bytes_per_unit"], "units_per_launch": dk["units_per_launch"],
+                         "launch_ms": dk["launch_ms"], "share_of_step": dk["share_of_step"],
+                         "note": "FFT kernels are co-limited by the FP32 pipes: see kernels[*].achieved_TFLOPs against "
+                                 "148 SM x 128 lanes x 1.965 GHz = 37.2 T FP32 instr/s (74.4 TFLOP/s if every one were an FMA)"},
+            "kernels": kern,
         }
         if not args.no_cpu_baseline and world == 1:
-            v, dt, cores, sample = time_oracle(cfg, 2, 1)
+            v, dt, cores, sample = time_oracle(cfg, None, 1)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
         print(json.dumps(line))
     g.close()
@@ -263,8 +335,8 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
-    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=400)
+    ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5],
                     help="BASELINE.json config (default 4: the largest fully magnetic mesh, 1024x1024x4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])

@@ -94,11 +94,19 @@ int mmc_set_sweep_counter(mmc_ctx* ctx, uint64_t sweep);
 /* device pointers, N floats each, natural cell order.  Fails with MMC_E_ZERO_LENGTH if a non-empty cell is 0. */
 int mmc_set_m(mmc_ctx* ctx, const float* mx, const float* my, const float* mz);
 int mmc_get_m(mmc_ctx* ctx, float* mx, float* my, float* mz);
+/* The same with HOST pointers (N floats each; pinned memory makes the copies asynchronous): the library does the
+ * host<->device copies on the ctx stream.  mmc_set_m_host returns after the zero-length check (synchronises);
+ * mmc_get_m_host only enqueues: the buffers are valid after the next synchronising call (mmc_get_observables) or a
+ * stream synchronise by the caller.  This is the end-to-end path of a caller whose state lives on the host. */
+int mmc_set_m_host(mmc_ctx* ctx, const float* mx, const float* my, const float* mz);
+int mmc_get_m_host(mmc_ctx* ctx, float* mx, float* my, float* mz);
 /* n iterations, asynchronous on the ctx stream. */
 int mmc_sweep(mmc_ctx* ctx, int n_sweeps);
 /* Same as mmc_sweep, but brackets every phase of every iteration with CUDA events on the ctx stream, synchronises, and
- * returns the summed device time per phase in milliseconds: phase_ms[8] (host) = pack+pad, forward FFT, tensor multiply,
- * inverse FFT, crop, red pass, black pass, end-of-sweep bookkeeping. */
+ * returns the summed device time per phase in milliseconds: phase_ms[8] (host) = [0] unused (pack+pad is fused into
+ * the rows kernel), [1] rows kernel (S0 + x transform + z-DFT), [2] columns kernel (y transform, tensor multiply S2,
+ * inverse y transform), [3] inverse rows kernel (S3, writes B_d), [4] unused (crop is fused), [5] red pass, [6] black
+ * pass, [7] end-of-sweep bookkeeping. */
 int mmc_sweep_timed(mmc_ctx* ctx, int n_sweeps, double* phase_ms);
 /* One demag convolution of the current state; bx/by/bz device float[N] (natural order) receive B_d = mu0 H_d
  * in tesla; any of them may be NULL (then the field is only computed).  Works with demag disabled too. */

@@ -20,7 +20,7 @@ MUB = 9.2740100783e-24
 SYMBOLS = [
     "mmc_create", "mmc_destroy", "mmc_set_material", "mmc_set_exchange_coupling", "mmc_set_temperature",
     "mmc_set_field", "mmc_set_move", "mmc_set_demag", "mmc_set_seed", "mmc_set_sweep_counter", "mmc_set_m",
-    "mmc_get_m", "mmc_sweep", "mmc_sweep_timed", "mmc_demag_field", "mmc_get_observables", "mmc_reset_counters", "mmc_reset_averages",
+    "mmc_get_m", "mmc_set_m_host", "mmc_get_m_host", "mmc_sweep", "mmc_sweep_timed", "mmc_demag_field", "mmc_get_observables", "mmc_reset_counters", "mmc_reset_averages",
     "mmc_debug_pass", "mmc_thermal", "mmc_demag_tensor_at", "mmc_strerror", "mmc_last_error",
 ]
 
@@ -80,6 +80,8 @@ def lib():
     L.mmc_set_sweep_counter.argtypes = [vp, u64]
     L.mmc_set_m.argtypes = [vp, vp, vp, vp]
     L.mmc_get_m.argtypes = [vp, vp, vp, vp]
+    L.mmc_set_m_host.argtypes = [vp, vp, vp, vp]
+    L.mmc_get_m_host.argtypes = [vp, vp, vp, vp]
     L.mmc_sweep.argtypes = [vp, i32]
     L.mmc_sweep_timed.argtypes = [vp, i32, C.POINTER(dbl)]
     L.mmc_demag_field.argtypes = [vp, vp, vp, vp]
@@ -196,6 +198,21 @@ class MMC:
     def set_m_device_ptrs(self, px, py, pz):
         self._ck(lib().mmc_set_m(self._h, px, py, pz))
 
+    def set_m_host(self, mx, my, mz):
+        """mmc_set_m_host: host tensors / arrays (float32, N each; pinned tensors copy asynchronously)."""
+        self._ck(lib().mmc_set_m_host(self._h, *[self._host_ptr(a) for a in (mx, my, mz)]))
+
+    def get_m_host(self, mx, my, mz):
+        """mmc_get_m_host: enqueue the copy of m into the given host buffers (valid after a synchronising call)."""
+        self._ck(lib().mmc_get_m_host(self._h, *[self._host_ptr(a) for a in (mx, my, mz)]))
+
+    def _host_ptr(self, a):
+        if hasattr(a, "data_ptr"):
+            assert (not a.is_cuda) and a.dtype == self._torch.float32 and a.is_contiguous() and a.numel() == self.N
+            return a.data_ptr()
+        assert a.dtype == np.float32 and a.flags["C_CONTIGUOUS"] and a.size == self.N
+        return a.ctypes.data
+
     # -- work -----------------------------------------------------------------------------------
     def get_m(self):
         torch = self._torch
@@ -208,7 +225,7 @@ class MMC:
 
     run = sweep
 
-    PHASES = ("pack", "fft_fwd", "multiply", "fft_inv", "crop", "red", "black", "end_sweep")
+    PHASES = ("pack", "rows_fwd", "columns", "rows_inv", "crop", "red", "black", "end_sweep")
 
     def sweep_timed(self, n_sweeps=1):
         """mmc_sweep_timed: dict phase -> summed device milliseconds over the n iterations (synchronises)."""

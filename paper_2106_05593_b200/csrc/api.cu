@@ -447,6 +447,41 @@ int mmc_set_m(mmc_ctx* c, const float* mx, const float* my, const float* mz)
     return MMC_OK;
 }
 
+int mmc_set_m_host(mmc_ctx* c, const float* mx, const float* my, const float* mz)
+{
+    if (!c || !mx || !my || !mz) return fail(c, MMC_E_INVALID, "NULL pointer");
+    DeviceGuard dg(c->device);
+    const size_t N = (size_t)c->g.nx * c->g.ny * c->g.nz;
+    const float* src[3] = { mx, my, mz };
+    for (int q = 0; q < 3; ++q) {                      // one staging buffer, reused in stream order
+        CU(c, cudaMemcpyAsync(c->stage, src[q], N * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+        CU(c, cudaMemsetAsync(c->m[q], 0, (size_t)(2 * c->g.H) * sizeof(float), c->stream));
+        int rc = launch_to_split(c->g, c->stage, c->m[q], c->stream);
+        if (rc) return fail(c, rc, "to_split launch failed");
+    }
+    c->m_set = true;
+    if (c->material_set && c->T_set) {
+        int rc = ensure_setup(c); if (rc) return rc;
+        return check_m(c);
+    }
+    c->m_needs_check = true;
+    return MMC_OK;
+}
+
+int mmc_get_m_host(mmc_ctx* c, float* mx, float* my, float* mz)
+{
+    if (!c || !mx || !my || !mz) return fail(c, MMC_E_INVALID, "NULL pointer");
+    DeviceGuard dg(c->device);
+    const size_t N = (size_t)c->g.nx * c->g.ny * c->g.nz;
+    float* dst[3] = { mx, my, mz };
+    for (int q = 0; q < 3; ++q) {
+        int rc = launch_from_split(c->g, c->m[q], c->stage, c->stream);
+        if (rc) return fail(c, rc, "from_split launch failed");
+        CU(c, cudaMemcpyAsync(dst[q], c->stage, N * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    }
+    return MMC_OK;
+}
+
 int mmc_get_m(mmc_ctx* c, float* mx, float* my, float* mz)
 {
     if (!c || !mx || !my || !mz) return fail(c, MMC_E_INVALID, "NULL pointer");

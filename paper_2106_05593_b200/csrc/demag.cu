@@ -1,17 +1,19 @@
 // demag.cu -- demagnetising field of Eq. (14): B_d = -mu0 N (*) M by zero-padded FFT convolution,
-// with hand-written shared-memory FFTs that never touch the padding.
+// with hand-written FFTs that never touch the padding.
 //
-//   kernel A  "rows"    S0+S1: for a tile of RJ mesh rows (all nz layers): M = Ms0 m straight from the colour-split
+//   kernel A  "rows"    S0+S1: for a tile of 4 mesh rows (all nz layers): M = Ms0 m straight from the colour-split
 //                       state (even cells = real part, odd cells = imaginary part: the colour planes ARE the even/odd
-//                       packing of the half-length real-FFT trick), FFT of length Px/2 in shared memory, untangle to
-//                       the Px/2+1 non-redundant frequencies, z-DFT across the layers in registers, store transposed:
+//                       packing of the half-length real-FFT trick), FFT of length Px/2, untangle to the Px/2+1
+//                       non-redundant frequencies, z-DFT across the layers in registers, store transposed:
 //                       T[c][kz][kx][j]  (j fastest, so that a column is contiguous for kernel B).
-//   kernel B  "columns" S1+S2+S3: one CTA per (kx, kz): the three components' columns (ny complex each) -> zero-pad to
-//                       Py in shared memory -> forward FFT -> real symmetric 3x3 tensor multiply in the transform's
-//                       digit-reversed order (the tensor spectrum is stored in that order) -> inverse FFT -> the ny
-//                       kept rows back in place.
+//   kernel B  "columns" S1+S2+S3: one CTA per (kx, kz): the three components' columns (ny complex each, the zero
+//                       padding to Py only implied) -> forward FFT -> real symmetric 3x3 tensor multiply in the
+//                       transform's own output order (the tensor spectrum is stored in that order) -> inverse FFT ->
+//                       the ny kept rows back in place.
 //   kernel C  "rows^-1" S3: mirror of A: inverse z-DFT in registers, re-tangle, inverse FFT of length Px/2, and the
 //                       real/imaginary parts go straight to the even/odd cells of the colour-split B_d.
+// Each kernel exists twice: the register-resident variant (fft_reg.cuh: 16 points per thread, compile-time lengths
+// 2^8 .. 2^12, the one the paper-sized meshes use) and the generic shared-memory variant (fft_smem.cuh) for other lengths.
 // Padded lengths are powers of two >= 2n-1 (any mesh size works).  All normalisation and -mu0 are folded into the
 // tensor spectrum, which is built once at set-up in fp64 (host Newell/moment table -> device placement -> cuFFT D2Z).
 #include <cuda_runtime.h>

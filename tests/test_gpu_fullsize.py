@@ -1,0 +1,172 @@
+"""Parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (production kernels through
+mmc_sweep / mmc_demag_field, not the debug pass), plus the equilibrium 3-sigma checks of north_star.
+
+  demag   sampled outputs the oracle computes one by one: B_d(r_i) = -mu0 sum_j N(r_i - r_j) M_j (Eq. (14),
+          PAPER.md:120) as a direct sum over the oracle's own tensor table, at cells spread over the mesh
+          (corners, edges, centre, random); bar 2e-5 max|B| as in test_gpu_parity.
+  sweep   one whole iteration of mmc_sweep on the full mesh against the oracle's red + black passes on the same
+          state and Philox stream, each side with its own demag field; bar as in
+          test_sweep_matches_replayed_oracle: all cells equal to 2e-6 except a 2e-3 fraction (near-margin decisions
+          and their black neighbours).
+  equilibrium  8 seeds on each side, blocked means after discarding the first half, Welch test at 3 sigma.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+MU0 = 4e-7 * np.pi
+
+
+def _np(ts):
+    return [t.detach().cpu().numpy().astype(np.float64) for t in ts]
+
+
+def _gpu(wl):
+    import paper_2106_05593_b200 as P
+    s = P.MMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask)
+    W.configure(s, wl, P.Material)
+    return s
+
+
+def _orc(wl):
+    s = O.OracleMMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, store_fp32=True)
+    W.configure(s, wl, O.Material)
+    return s
+
+
+_CONV = {}
+
+
+def _conv(cfg, wl):
+    """The oracle's fp64 FFT convolution object (tensor table + spectrum) of a config, built once per session."""
+    if cfg not in _CONV:
+        _CONV[cfg] = O.DemagFFT(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz)
+    return _CONV[cfg]
+
+
+def _ms0_of_cell(wl):
+    ms = np.array([r["Ms0"] for r in wl.regions], dtype=np.float64)
+    if wl.region_of_cell is None:
+        return np.full(wl.N, ms[0])
+    return ms[wl.region_of_cell]
+
+
+def _direct_sample(tab, M, i, j, k):
+    """Eq. (14) at one cell: the octant table holds N(|ox|,|oy|,|oz|); diagonal components are even in every coordinate,
+    N_ab (a != b) is odd in coordinates a and b."""
+    _, nz, ny, nx = tab.shape
+    ox = i - np.arange(nx); oy = j - np.arange(ny); oz = k - np.arange(nz)
+    ax, ay, az = np.abs(ox), np.abs(oy), np.abs(oz)
+    sx, sy, sz = np.sign(ox), np.sign(oy), np.sign(oz)
+    sub = [tab[q][np.ix_(az, ay, ax)] for q in range(6)]
+    SX = sx[None, None, :]; SY = sy[None, :, None]; SZ = sz[:, None, None]
+    xx, yy, zz = sub[0], sub[1], sub[2]
+    xy = sub[3] * SX * SY; xz = sub[4] * SX * SZ; yz = sub[5] * SY * SZ
+    Mx, My, Mz = M
+    hx = -(xx * Mx + xy * My + xz * Mz).sum()
+    hy = -(xy * Mx + yy * My + yz * Mz).sum()
+    hz = -(xz * Mx + yz * My + zz * Mz).sum()
+    return MU0 * np.array([hx, hy, hz])
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_demag_sampled(cfg):
+    wl = W.make(cfg)
+    g = _gpu(wl)
+    bg = _np(g.demag_field())
+    g.close()
+    nx, ny, nz = wl.nx, wl.ny, wl.nz
+    tab = _conv(cfg, wl).tab
+    ms0 = _ms0_of_cell(wl)
+    M = [(ms0 * wl.m0[a].astype(np.float64)).reshape(nz, ny, nx) for a in range(3)]
+    rng = np.random.default_rng(1000 + cfg)
+    pts = [(0, 0, 0), (nx - 1, ny - 1, nz - 1), (nx - 1, 0, 0), (0, ny - 1, nz - 1), (nx // 2, ny // 2, nz // 2),
+           (nx // 2 - 1, 0, 0), (1, ny // 2, nz - 1), (nx - 2, ny - 3, 0)]
+    pts += [(int(rng.integers(nx)), int(rng.integers(ny)), int(rng.integers(nz))) for _ in range(16)]
+    worst = scale = 0.0                       # scale = max |B| over the oracle's own samples (corners and edges included)
+    for (i, j, k) in pts:
+        bo = _direct_sample(tab, M, i, j, k)
+        c = i + nx * (j + ny * k)
+        worst = max(worst, max(abs(bg[a][c] - bo[a]) for a in range(3)))
+        scale = max(scale, np.abs(bo).max())
+    assert worst <= 2e-5 * scale, f"cfg{cfg}: worst sampled |B_gpu - B_direct| = {worst:.3e} T vs scale {scale:.3e} T"
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 4, 5])
+def test_full_size_sweep(cfg):
+    wl = W.make(cfg)
+    wl.adaptive_cone = False
+    g, o = _gpu(wl), _orc(wl)
+    if wl.demag:
+        o._demag = _conv(cfg, wl)             # the oracle's own field (numpy.fft on the padded grid), nothing from the GPU
+    g.sweep(1)
+    o.run(1)
+    mg = _np(g.get_m())
+    bad = np.zeros(wl.N, bool)
+    for a in range(3):
+        bad |= np.abs(mg[a] - o.m[a]) > 2e-6
+    assert bad.sum() <= max(2, 2e-3 * wl.n_active), f"cfg{cfg}: {bad.sum()} of {wl.n_active} cells differ after one sweep"
+    ob = g.observables()
+    assert ob["sweeps_done"] == 1 and ob["trials"] == wl.n_active
+    assert abs(int(ob["accepted"]) - o.accepted) <= max(2, 2e-3 * wl.n_active)
+    # empty cells are never touched
+    if wl.n_active < wl.N:
+        empty = _ms0_of_cell(wl) == 0
+        for a in range(3):
+            assert np.array_equal(mg[a][empty], wl.m0[a][empty].astype(np.float64))
+    g.close()
+
+
+# ------------------------------------------------------------------------------------------------ equilibrium, 3 sigma
+def _series_gpu(wl, seed, n_sweeps):
+    wl.seed = seed
+    g = _gpu(wl)
+    g.sweep(n_sweeps // 2)
+    g.reset_averages(); g.reset_counters()
+    g.sweep(n_sweeps - n_sweeps // 2)
+    ob = g.observables()
+    g.close()
+    return np.array([ob["run_mean_len"], ob["run_mean_m"][2], ob["accepted"] / ob["trials"]])
+
+
+def _series_oracle(wl, seed, n_sweeps):
+    wl.seed = seed
+    o = _orc(wl)
+    o.run(n_sweeps // 2)
+    acc0, tri0 = o.accepted, o.trials
+    s_len = s_mz = 0.0
+    n2 = n_sweeps - n_sweeps // 2
+    act = _ms0_of_cell(wl) > 0
+    for _ in range(n2):
+        o.run(1)
+        s_len += np.sqrt(o.m[0] ** 2 + o.m[1] ** 2 + o.m[2] ** 2)[act].mean()
+        s_mz += o.m[2][act].mean()
+    return np.array([s_len / n2, s_mz / n2, (o.accepted - acc0) / (o.trials - tri0)])
+
+
+EQ_CASES = {
+    # exchange + uniaxial anisotropy, paper regime (acceptance ~ 0.5), far below Tc
+    "cfg1_paper_regime_32x32": (lambda: W.cfg1(paper_regime=True), 4000),
+    # chiral film just below Tc (650 K of Tc 700 K): exchange + DMI + anisotropy + Zeeman + demag + wide length distribution
+    "cfg3_32x32_650K": (lambda: W.cfg3(nx=32, ny=32, T=650.0), 3000),
+    # granular film: per-cell classes, grain boundaries, hot spot above Tc, 3 layers, demag
+    "cfg4_24x24x3": (lambda: W.cfg4(nx=24, ny=24, nz=3), 2000),
+}
+
+
+@pytest.mark.parametrize("name", list(EQ_CASES))
+def test_equilibrium_observables_within_3_sigma(name):
+    """north_star: equilibrium observables within 3 sigma.  8 independent Philox keys per side (different keys on the
+    two sides, so this is a statistical comparison, not a replay); per-run means of <|m|>, <m_z> and the acceptance
+    rate over the second half of the run; Welch statistic |mean_g - mean_o| <= 3 sqrt(var_g/8 + var_o/8)."""
+    make, n_sweeps = EQ_CASES[name]
+    G = np.array([_series_gpu(make(), 7000 + s, n_sweeps) for s in range(8)])
+    Oo = np.array([_series_oracle(make(), 9000 + s, n_sweeps) for s in range(8)])
+    for q, label in enumerate(("mean |m|", "mean m_z", "acceptance")):
+        mg, mo = G[:, q].mean(), Oo[:, q].mean()
+        se = np.sqrt(G[:, q].var(ddof=1) / 8 + Oo[:, q].var(ddof=1) / 8)
+        assert abs(mg - mo) <= 3.0 * se + 1e-7, f"{name}: {label}: gpu {mg:.6f} vs oracle {mo:.6f}, 3 sigma = {3 * se:.2e}"
