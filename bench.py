@@ -68,13 +68,19 @@ def demag_kernel_bytes(wl, ms0_per_cell):
     import math
     fl_rows = 3 * wl.ny * wl.nz * 5 * (Px // 2) * math.log2(Px // 2)
     fl_cols = 3 * Pz * Cx * 2 * 5 * Py * math.log2(Py) + Pz * Cx * Py * (20 if wl.nz == 1 else 36)
-    return {"rows_fwd": {"bytes": state + (wl.N * 4 if ms0_per_cell else 0) + T, "flops": fl_rows},
-            "columns": {"bytes": 2 * T + tensor, "flops": fl_cols},
-            "rows_inv": {"bytes": T + state, "flops": fl_rows}}
+    # several layers: the rows kernels work per layer on U = [3][nz][Cx][ny] (the z-DFT is fused into the columns kernel's
+    # load, its inverse is the z_inverse pass T -> U); one layer: U = T, no z pass
+    U = 3 * wl.nz * Cx * wl.ny * 8
+    out = {"rows_fwd": {"bytes": state + (wl.N * 4 if ms0_per_cell else 0) + U, "flops": fl_rows},
+           "columns": {"bytes": U + T + tensor, "flops": fl_cols},
+           "rows_inv": {"bytes": U + state, "flops": fl_rows}}
+    if wl.nz > 1:
+        out["z_inverse"] = {"bytes": T + U, "flops": 3 * Cx * wl.ny * 5 * Pz * math.log2(Pz)}
+    return out
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/), cfg 4
-NCU_TRAFFIC_CFG4 = {   # profiles/r1d_summary.md
+NCU_TRAFFIC_CFG4 = {   # profiles/r1d_summary.md (stale keys are ignored)
     "colour_pass_kernel": 113.5e6, "demag_rows_fwd_kernel": 199.4e6, "demag_columns_kernel": 780.3e6, "demag_rows_inv_kernel": 237.0e6,
 }
 
@@ -281,7 +287,9 @@ def run_ours(args):
                                       "units_per_launch": wl.n_active / 2.0, "bytes_per_unit": bpu}
         if wl.demag:
             db = demag_kernel_bytes(wl, ms0_pc)
-            for name, ph in (("rows_fwd", "rows_fwd"), ("columns", "columns"), ("rows_inv", "rows_inv")):
+            for name, ph in (("rows_fwd", "rows_fwd"), ("columns", "columns"), ("z_inverse", "z_inverse"), ("rows_inv", "rows_inv")):
+                if name not in db:
+                    continue
                 kern["demag_" + name + "_kernel"] = {"launch_ms": phases[ph] / K, "launches_per_step": 1, "bytes": db[name]["bytes"],
                                                     "flops": db[name]["flops"], "units_per_launch": wl.N,
                                                     "bytes_per_unit": db[name]["bytes"] / wl.N}
@@ -295,7 +303,7 @@ def run_ours(args):
             d["ncu_traffic_bytes"] = NCU_TRAFFIC_CFG4.get(k) if (cfg == 4 and not args.small) else None
         dom = max(kern, key=lambda k: kern[k]["launch_ms"])          # the dominant kernel = longest single launch
         dk = kern[dom]
-        demag_ms = sum(phases[k] for k in ("pack", "rows_fwd", "columns", "rows_inv", "crop")) / K
+        demag_ms = sum(phases[k] for k in ("pack", "rows_fwd", "columns", "rows_inv", "z_inverse")) / K
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -310,7 +318,7 @@ def run_ours(args):
                        "acceptance": ob["accepted"] / max(1, ob["trials"])},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nE},
-            "gpu_launches": (6 if wl.demag else 3) * K,
+            "gpu_launches": ((7 if wl.nz > 1 else 6) if wl.demag else 3) * K,
             "phases_ms_per_step": {k: v / K for k, v in phases.items()},
             "sweep_only_updates_per_sec": wl.n_active / (2 * pass_ms * 1e-3) if pass_ms > 0 else None,
             "demag_convolutions_per_sec": (1e3 / demag_ms) if (wl.demag and demag_ms > 0) else None,

@@ -105,7 +105,8 @@ int mmc_sweep(mmc_ctx* ctx, int n_sweeps);
 /* Same as mmc_sweep, but brackets every phase of every iteration with CUDA events on the ctx stream, synchronises, and
  * returns the summed device time per phase in milliseconds: phase_ms[8] (host) = [0] unused (pack+pad is fused into
  * the rows kernel), [1] rows kernel (S0 + x transform + z-DFT), [2] columns kernel (y transform, tensor multiply S2,
- * inverse y transform), [3] inverse rows kernel (S3, writes B_d), [4] unused (crop is fused), [5] red pass, [6] black
+ * inverse y transform), [3] inverse rows kernel (S3, writes B_d), [4] inverse z-DFT pass (several layers only; it runs
+ * between [2] and [3]), [5] red pass, [6] black
  * pass, [7] end-of-sweep bookkeeping. */
 int mmc_sweep_timed(mmc_ctx* ctx, int n_sweeps, double* phase_ms);
 /* One demag convolution of the current state; bx/by/bz device float[N] (natural order) receive B_d = mu0 H_d

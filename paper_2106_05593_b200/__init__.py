@@ -225,7 +225,7 @@ class MMC:
 
     run = sweep
 
-    PHASES = ("pack", "rows_fwd", "columns", "rows_inv", "crop", "red", "black", "end_sweep")
+    PHASES = ("pack", "rows_fwd", "columns", "rows_inv", "z_inverse", "red", "black", "end_sweep")
 
     def sweep_timed(self, n_sweeps=1):
         """mmc_sweep_timed: dict phase -> summed device milliseconds over the n iterations (synchronises)."""

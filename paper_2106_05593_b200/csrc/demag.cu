@@ -12,13 +12,17 @@
 //                       the ny kept rows back in place.
 //   kernel C  "rows^-1" S3: mirror of A: inverse z-DFT in registers, re-tangle, inverse FFT of length Px/2, and the
 //                       real/imaginary parts go straight to the even/odd cells of the colour-split B_d.
-// Each kernel exists twice: the register-resident variant (fft_reg.cuh: 16 points per thread, compile-time lengths
-// 2^8 .. 2^12, the one the paper-sized meshes use) and the generic shared-memory variant (fft_smem.cuh) for other lengths.
+// Each kernel exists twice: the generic shared-memory variant described above (fft_smem.cuh, any length) and the
+// register-resident variant (fft_reg.cuh: 16 points per thread, compile-time lengths 2^8 .. 2^12) that the paper-sized
+// meshes use.  In the latter the rows kernels work layer by layer (several CTAs per SM instead of one holding all layers):
+// the forward z-DFT is fused into the columns kernel's load (CTA (kx, kz) sums its plane from the nz layers, which the
+// Pz CTAs of one kx read together and find in L2), the inverse z-DFT is a streaming pass of its own (z_inverse_kernel).
 // Padded lengths are powers of two >= 2n-1 (any mesh size works).  All normalisation and -mu0 are folded into the
 // tensor spectrum, which is built once at set-up in fp64 (host Newell/moment table -> device placement -> cuFFT D2Z).
 #include <cuda_runtime.h>
 #include <cufft.h>
 
+#include <algorithm>
 #include <cmath>
 
 #include "fft_reg.cuh"
@@ -43,8 +47,9 @@ struct DemagPlan {
     bool fastB = false;              // columns: register-resident transform (fft_reg.cuh), Py in 2^8 .. 2^12
     float2* twB1 = nullptr;          // its twiddle tables (fftr::Twiddles), 15 * Py/16 entries each
     float2* twB2 = nullptr;
-    bool fastA = false;              // rows: register-resident transform, Hx in 2^8 .. 2^11, Pz in {1, 4, 8, 16}, fits shared memory
+    bool fastA = false;              // rows: register-resident per-layer kernels (Hx in 2^8 .. 2^11); needs fastB (z-DFT outside the rows kernels)
     float2* T = nullptr;             // [3][Pz][Cx][ny]
+    float2* U = nullptr;             // fastA with nz > 1: [3][nz][Cx][ny], the layers before the z-DFT and after its inverse
     float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
 };
 
@@ -282,20 +287,21 @@ __global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
 }
 
 // ------------------------------------------------------------------------------------------------ kernels A and C, register-resident
-// Same work as rows_fwd_kernel / rows_inv_kernel with the length-Hx transform of fft_reg.cuh (Hx = 2^LGH, 8 <= LGH <= 11).
+// The x direction with the length-Hx transform of fft_reg.cuh (Hx = 2^LGH, 8 <= LGH <= 11), one (component, layer) per
+// CTA: the z-DFT lives in the columns kernel (cluster), so these kernels have no coupling between layers and
+// T[c][k][kx][j] holds nz planes per component.
 // block (RJ = 4, T = Hx/16): threadIdx.x = row of the tile (fastest, so that the four rows' values of one frequency are
-// one 32-byte sector of the transposed array T[c][kz][kx][j]), threadIdx.y = thread of the row's transform.
-// Shared memory: nat[nz][4][NS] (spectra in natural order, padded index k + (k>>4), for the mirror-frequency access of
-// the real-transform (un)tangling and for the z-DFT across layers) + one pair of exchange buffers per row.  Row strides
-// are = 4 (mod 16) elements, so that the four rows of a half-warp sit in different bank groups.
-// grid (ceil(ny/4), 3 components).
+// one 32-byte sector of the transposed array), threadIdx.y = thread of the row's transform.
+// Shared memory per row: the two exchange buffers, which the natural-order spectrum (padded index k + (k>>4), needed for
+// the mirror-frequency access of the real-transform (un)tangling) reuses between barriers.  Row strides are = 4 (mod 16)
+// elements, so that the four rows of a half-warp sit in different bank groups.
+// grid (ceil(ny/4), 3 components * nz layers).
 constexpr int kRJ = 4;
 template <int LGH> struct RowShape {
     using S = fftr::Shape<LGH>;
     static constexpr int Hx = S::N, T = S::T;
-    static constexpr int NS = Hx + Hx / 16 + 4;          // nat row stride; pad(Hx) = Hx + Hx/16 is its last used element
-    static constexpr int ES = S::SMEM + 4;               // exchange row stride
-    static constexpr int CP = Hx + Hx / 16;              // pad(k) + pad(Hx - k) (+1 when k & 15 != 0)
+    static constexpr int CP = Hx + Hx / 16;              // pad(k) + pad(Hx - k) (+1 when k & 15 != 0); = pad(Hx)
+    static constexpr int ES = (S::SMEM > CP ? S::SMEM : CP) + 4;   // row stride
 };
 struct RowFastArgs {
     Geometry g;
@@ -306,8 +312,8 @@ struct RowFastArgs {
     float2* T;
 };
 
-template <int LGH, int PZ>
-__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_fwd_fast_kernel(const RowFastArgs a)
+template <int LGH>
+__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, RowShape<LGH>::T > 64 ? 1 : 2) rows_fwd_fast_kernel(const RowFastArgs a)
 {
     using R = RowShape<LGH>;
     constexpr int T = R::T, Hx = R::Hx;
@@ -315,22 +321,22 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_fwd_fast_kerne
     const Geometry g = a.g;
     const int nz = g.nz, ny = g.ny;
     const int jj = threadIdx.x, t = threadIdx.y;
-    const int c = blockIdx.y, j = blockIdx.x * kRJ + jj;
+    const int c = blockIdx.y / nz, k = blockIdx.y - c * nz, j = blockIdx.x * kRJ + jj;
     const bool valid = j < ny;
     const int hxr = (g.nx + 1) >> 1;
-    float2* nat = sm + jj * R::NS;                                  // + k * kRJ * NS per layer
-    float2* s1 = sm + nz * kRJ * R::NS + jj * R::ES;
+    float2* s1 = sm + jj * R::ES;
     float2* s2 = s1 + R::S::S1;
-    const int pb = fftr::pbase<LGH>(t);
+    float2* nat = s1;
+    const int pb = fftr::pbase<LGH>(t), kb = fftr::kbase<LGH>(t);
     const fftr::Twiddles tw{ fftr::root(t, Hx), fftr::root(t >> 4, T), nullptr, nullptr };
     const float* __restrict__ mc = a.m[c];
-    // S0: M = Ms0 m; even cells -> real part, odd cells -> imaginary part; only n < Hx/2 can be non-zero.
-    // The next layer's cells are requested before the current layer is transformed.
-    float2 raw[8], rws[8];                         // m and Ms0 as loaded; multiplied when consumed
-    auto fetch = [&](int k) {
+    // S0: M = Ms0 m; even cells -> real part, odd cells -> imaginary part; only n < Hx/2 can be non-zero
+    float2 v[16];
+    {
         const int row = k * ny + (valid ? j : 0), par = ((valid ? j : 0) + k) & 1;
         const unsigned be = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx;
         const unsigned bo = (unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx;
+        float2 raw[8], rws[8];
 #pragma unroll
         for (int n1 = 0; n1 < 8; ++n1) {
             const int n = t + n1 * T;
@@ -342,64 +348,33 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_fwd_fast_kerne
             }
             raw[n1] = x; rws[n1] = ms;
         }
-    };
-    fetch(0);
-    for (int k = 0; k < nz; ++k) {
-        float2 v[16];
 #pragma unroll
         for (int n1 = 0; n1 < 8; ++n1) { v[n1] = make_float2(raw[n1].x * rws[n1].x, raw[n1].y * rws[n1].y); v[n1 + 8] = make_float2(0.f, 0.f); }
-        if (k + 1 < nz) fetch(k + 1);
-        fftr::forward<LGH, true, false>(v, s1, s2, tw, t);
-        float2* nk = nat + k * kRJ * R::NS + pb;
-#pragma unroll
-        for (int e = 0; e < 16; ++e) nk[fftr::pconst<LGH>(e)] = v[e];
     }
+    fftr::forward<LGH, true, false>(v, s1, s2, tw, t);
+    if (R::S::R3 > 1) __syncthreads();                               // exchange buffer 2 is read (R3 == 1: forward ends with a barrier)
+#pragma unroll
+    for (int e = 0; e < 16; ++e) nat[pb + fftr::pconst<LGH>(e)] = v[e];
     __syncthreads();
-    // untangle (X' = 2 X of the real row, from Z[k] and Z[Hx-k]), z-DFT across the layers, transposed store
-    const int kb = fftr::kbase<LGH>(t);
+    // untangle (X' = 2 X of the real row, from Z[k] and Z[Hx-k]) and transposed store
     const float2 wub = fftr::root(kb, 2 * Hx);
-    float2* __restrict__ out = a.T + (size_t)c * PZ * a.Cx * ny + (valid ? j : 0);
-    const size_t plane = (size_t)a.Cx * ny;
+    float2* __restrict__ out = a.T + ((size_t)blockIdx.y * a.Cx) * ny + (valid ? j : 0);
 #pragma unroll
     for (int e = 0; e < 16; ++e) {
         const int kx = kb + fftr::kconst<LGH>(e);
         const int pa = pb + fftr::pconst<LGH>(e);
         const int pm = (kx == 0) ? pa : R::CP - pa - (fftr::lo_nonzero<LGH>(t, e) ? 1 : 0);
         const float2 w = fft::cmul(wub, a.cu[e]);
-        float2 x[PZ];
-#pragma unroll
-        for (int k = 0; k < PZ; ++k) {
-            x[k] = make_float2(0.f, 0.f);
-            if (k < nz) {
-                const float2 A = nat[k * kRJ * R::NS + pa], B = nat[k * kRJ * R::NS + pm];
-                const float2 Sm = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
-                const float2 tt = fft::cmul(w, D);
-                x[k] = make_float2(Sm.x + tt.y, Sm.y - tt.x);
-            }
-        }
-        fft::dif<PZ, false>(x);
-        if (valid) {
-#pragma unroll
-            for (int kz = 0; kz < PZ; ++kz) out[kz * plane + (size_t)kx * ny] = x[fft::bitrev<PZ>(kz)];
-        }
-    }
-    if (t == 0) {                                                    // the Nyquist column kx = Hx: X'[Hx] = 2 (Re Z[0] - Im Z[0])
-        float2 x[PZ];
-#pragma unroll
-        for (int k = 0; k < PZ; ++k) {
-            x[k] = make_float2(0.f, 0.f);
-            if (k < nz) { const float2 z0 = nat[k * kRJ * R::NS]; x[k].x = 2.f * (z0.x - z0.y); }
-        }
-        fft::dif<PZ, false>(x);
-        if (valid) {
-#pragma unroll
-            for (int kz = 0; kz < PZ; ++kz) out[kz * plane + (size_t)Hx * ny] = x[fft::bitrev<PZ>(kz)];
-        }
+        const float2 A = v[e], B = nat[pm];
+        const float2 Sm = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
+        const float2 tt = fft::cmul(w, D);
+        if (valid) out[(size_t)kx * ny] = make_float2(Sm.x + tt.y, Sm.y - tt.x);
+        if (e == 0 && t == 0 && valid) out[(size_t)Hx * ny] = make_float2(2.f * (A.x - A.y), 0.f);   // Nyquist column
     }
 }
 
-template <int LGH, int PZ>
-__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_inv_fast_kernel(const RowFastArgs a)
+template <int LGH>
+__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, RowShape<LGH>::T > 64 ? 1 : 2) rows_inv_fast_kernel(const RowFastArgs a)
 {
     using R = RowShape<LGH>;
     constexpr int T = R::T, Hx = R::Hx;
@@ -407,108 +382,75 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, 1) rows_inv_fast_kerne
     const Geometry g = a.g;
     const int nz = g.nz, ny = g.ny;
     const int jj = threadIdx.x, t = threadIdx.y;
-    const int c = blockIdx.y, j = blockIdx.x * kRJ + jj;
+    const int c = blockIdx.y / nz, k = blockIdx.y - c * nz, j = blockIdx.x * kRJ + jj;
     const bool valid = j < ny;
     const int hxr = (g.nx + 1) >> 1;
-    float2* nat = sm + jj * R::NS;
-    float2* s1 = sm + nz * kRJ * R::NS + jj * R::ES;
+    float2* s1 = sm + jj * R::ES;
     float2* s2 = s1 + R::S::S1;
+    float2* nat = s1;
     const int pb = fftr::pbase<LGH>(t), kb = fftr::kbase<LGH>(t);
     const fftr::Twiddles tw{ fftr::root(t, Hx), fftr::root(t >> 4, T), nullptr, nullptr };
     const float2 wub = fftr::root(kb, 2 * Hx);
-    const float2* __restrict__ in = a.T + (size_t)c * PZ * a.Cx * ny + (valid ? j : 0);
-    const size_t plane = (size_t)a.Cx * ny;
-    // inverse z-DFT of every frequency this thread owns, all layers into nat
+    const float2* __restrict__ in = a.T + ((size_t)blockIdx.y * a.Cx) * ny + (valid ? j : 0);
+    float2 v[16];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) v[e] = valid ? in[(size_t)(kb + fftr::kconst<LGH>(e)) * ny] : make_float2(0.f, 0.f);
+    float2 yh = make_float2(0.f, 0.f);
+    if (t == 0 && valid) yh = in[(size_t)Hx * ny];
+#pragma unroll
+    for (int e = 0; e < 16; ++e) nat[pb + fftr::pconst<LGH>(e)] = v[e];
+    __syncthreads();
+    // re-tangle: Y[k], Y[Hx-k] -> Z'[k] = 2 (E[k] + i O[k]) in this thread's slots
 #pragma unroll
     for (int e = 0; e < 16; ++e) {
-        const int kx = kb + fftr::kconst<LGH>(e);
-        float2 x[PZ];
-#pragma unroll
-        for (int kz = 0; kz < PZ; ++kz) x[fft::bitrev<PZ>(kz)] = valid ? in[kz * plane + (size_t)kx * ny] : make_float2(0.f, 0.f);
-        fft::dit<PZ, true>(x);
-#pragma unroll
-        for (int k = 0; k < PZ; ++k) if (k < nz) nat[k * kRJ * R::NS + pb + fftr::pconst<LGH>(e)] = x[k];
+        const int pa = pb + fftr::pconst<LGH>(e);
+        const int pm = R::CP - pa - (fftr::lo_nonzero<LGH>(t, e) ? 1 : 0);
+        const bool first = (e == 0 && t == 0);                     // k = 0: the mirror is the Nyquist value; both are real
+        const float2 A = v[e], B = first ? yh : nat[first ? pa : pm];
+        const float2 w = fft::cmul(wub, a.cu[e]);
+        const float2 E = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
+        const float2 O = fft::cmulc(D, w);
+        v[e] = first ? make_float2(A.x + B.x, A.x - B.x) : make_float2(E.x - O.y, E.y + O.x);
     }
-    if (t == 0) {
-        float2 x[PZ];
-#pragma unroll
-        for (int kz = 0; kz < PZ; ++kz) x[fft::bitrev<PZ>(kz)] = valid ? in[kz * plane + (size_t)Hx * ny] : make_float2(0.f, 0.f);
-        fft::dit<PZ, true>(x);
-#pragma unroll
-        for (int k = 0; k < PZ; ++k) if (k < nz) nat[k * kRJ * R::NS + R::CP] = x[k];
-    }
-    __syncthreads();
+    __syncthreads();                                                 // the natural-order array is read: exchanges may reuse it
+    fftr::inverse<LGH, false>(v, s1, s2, tw, t);
+    // real part -> even cells, imaginary part -> odd cells of the colour-split B_d
     float* __restrict__ bc = a.bd[c];
-    for (int k = 0; k < nz; ++k) {
-        // re-tangle: Y[k], Y[Hx-k] -> Z'[k] = 2 (E[k] + i O[k]) in this thread's slots
-        float2 v[16];
-        const float2* nk = nat + k * kRJ * R::NS;
+    const int row = k * ny + (valid ? j : 0), par = ((valid ? j : 0) + k) & 1;
+    const unsigned be = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx;
+    const unsigned bo = (unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx;
 #pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const int pa = pb + fftr::pconst<LGH>(e);
-            const int pm = R::CP - pa - (fftr::lo_nonzero<LGH>(t, e) ? 1 : 0);
-            const float2 A = nk[pa], B = nk[pm];
-            const float2 w = fft::cmul(wub, a.cu[e]);
-            const float2 E = make_float2(A.x + B.x, A.y - B.y), D = make_float2(A.x - B.x, A.y + B.y);
-            const float2 O = fft::cmulc(D, w);
-            v[e] = make_float2(E.x - O.y, E.y + O.x);
-            if (e == 0 && t == 0) v[e] = make_float2(A.x + B.x, A.x - B.x);     // k = 0: Y[0] and Y[Hx] are real
-        }
-        fftr::inverse<LGH, false>(v, s1, s2, tw, t);
-        // real part -> even cells, imaginary part -> odd cells of the colour-split B_d
-        const int row = k * ny + (valid ? j : 0), par = ((valid ? j : 0) + k) & 1;
-        const unsigned be = (unsigned)par * (unsigned)g.H + (unsigned)row * g.hx;
-        const unsigned bo = (unsigned)(1 - par) * (unsigned)g.H + (unsigned)row * g.hx;
-#pragma unroll
-        for (int n1 = 0; n1 < 8; ++n1) {
-            const int n = t + n1 * T;
-            if (valid && n < hxr) {
-                bc[be + n] = v[n1].x;
-                if (2 * n + 1 < g.nx) bc[bo + n] = v[n1].y;
-            }
+    for (int n1 = 0; n1 < 8; ++n1) {
+        const int n = t + n1 * T;
+        if (valid && n < hxr) {
+            bc[be + n] = v[n1].x;
+            if (2 * n + 1 < g.nx) bc[bo + n] = v[n1].y;
         }
     }
 }
 
-template <int LGH, int PZ>
+template <int LGH>
 static int launch_rows_fast(const DemagPlan* p, const RowFastArgs& ra, bool inverse, cudaStream_t st)
 {
     using R = RowShape<LGH>;
-    const dim3 grid((p->g.ny + kRJ - 1) / kRJ, 3), block(kRJ, R::T);
-    const size_t smem = ((size_t)p->g.nz * kRJ * R::NS + (size_t)kRJ * R::ES) * sizeof(float2);
+    const dim3 grid((p->g.ny + kRJ - 1) / kRJ, 3 * p->g.nz), block(kRJ, R::T);
+    const size_t smem = (size_t)kRJ * R::ES * sizeof(float2);
     if (inverse) {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_inv_fast_kernel<LGH, PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        rows_inv_fast_kernel<LGH, PZ><<<grid, block, smem, st>>>(ra);
+        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_inv_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        rows_inv_fast_kernel<LGH><<<grid, block, smem, st>>>(ra);
     } else {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_fwd_fast_kernel<LGH, PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        rows_fwd_fast_kernel<LGH, PZ><<<grid, block, smem, st>>>(ra);
+        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_fwd_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        rows_fwd_fast_kernel<LGH><<<grid, block, smem, st>>>(ra);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
-}
-template <int LGH>
-static int launch_rows_fast_pz(const DemagPlan* p, const RowFastArgs& ra, bool inverse, cudaStream_t st)
-{
-    switch (p->Pz) {
-        case 1: return launch_rows_fast<LGH, 1>(p, ra, inverse, st);
-        case 4: return launch_rows_fast<LGH, 4>(p, ra, inverse, st);
-        case 8: return launch_rows_fast<LGH, 8>(p, ra, inverse, st);
-        case 16: return launch_rows_fast<LGH, 16>(p, ra, inverse, st);
-        default: return MMC_E_UNSUPPORTED;
-    }
-}
-static size_t rows_fast_smem(int lgH, int nz)
-{
-    const int Hx = 1 << lgH, T = Hx / 16, R3 = Hx / 256;
-    const size_t NS = Hx + Hx / 16 + 4, ES = 16 * (T + 1) + (R3 > 1 ? R3 * 272 : 0) + 4;
-    return ((size_t)nz * kRJ * NS + (size_t)kRJ * ES) * sizeof(float2);
 }
 static int launch_rows_fast_any(const DemagPlan* p, const RowFastArgs& ra, bool inverse, cudaStream_t st)
 {
     switch (ilog2(p->Hx)) {
-        case 8: return launch_rows_fast_pz<8>(p, ra, inverse, st);
-        case 9: return launch_rows_fast_pz<9>(p, ra, inverse, st);
-        case 10: return launch_rows_fast_pz<10>(p, ra, inverse, st);
-        case 11: return launch_rows_fast_pz<11>(p, ra, inverse, st);
+        case 8: return launch_rows_fast<8>(p, ra, inverse, st);
+        case 9: return launch_rows_fast<9>(p, ra, inverse, st);
+        case 10: return launch_rows_fast<10>(p, ra, inverse, st);
+        case 11: return launch_rows_fast<11>(p, ra, inverse, st);
         default: return MMC_E_UNSUPPORTED;
     }
 }
@@ -520,8 +462,10 @@ static int launch_rows_fast_any(const DemagPlan* p, const RowFastArgs& ra, bool 
 // of the output are pruned at compile time.  grid (ceil(Cx/G), Pz), block (T, G).
 struct ColFastArgs {
     int ny, Cx, Pz;
+    int nz;                                    // > 0: forward z-DFT fused into the load: Tin holds nz layers per component
     const float2* tw1; const float2* tw2;      // fft_reg.cuh twiddle tables of the length-Py transform
-    float2* T;
+    const float2* Tin;                         // [3][nz or Pz][Cx][ny]
+    float2* Tout;                              // [3][Pz][Cx][ny] (== Tin when nz == 0: in place)
     const float* nhat[6];
 };
 
@@ -530,12 +474,16 @@ __global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G, fft
 columns_fast_kernel(const ColFastArgs a)
 {
     using S = fftr::Shape<LGN>;
-    constexpr int N = S::N, T = S::T;
+    constexpr int N = S::N, T = S::T, NL = HALF ? 8 : 16;
     extern __shared__ float2 sm[];
     float2* s1 = sm + threadIdx.y * S::SMEM;
     float2* s2 = s1 + S::S1;
     const int tid = threadIdx.x;
-    const int kxr = blockIdx.x * S::G + threadIdx.y, kz = blockIdx.y;
+    // with the fused z-DFT the Pz CTAs of one kx read the same layers: kz is the fastest block index so that they run
+    // together and all but the first find them in L2
+    const bool zf = a.nz > 0;
+    const int kz = zf ? blockIdx.x : blockIdx.y;
+    const int kxr = (zf ? blockIdx.y : blockIdx.x) * S::G + threadIdx.y;
     const bool live = kxr < a.Cx;                      // idle groups still walk through the barriers
     const int kx = live ? kxr : a.Cx - 1;
     const int ny = a.ny;
@@ -543,10 +491,39 @@ columns_fast_kernel(const ColFastArgs a)
     float2 v[3][16];
     // all three components' columns are requested at once, and the tensor spectrum this thread will need after the
     // forward transforms is pulled into L2 meanwhile (no registers held)
-    if (HALF) {
+    if (zf) {
+        // S1, z direction: plane kz of the length-Pz DFT over the nz layers, X[kz] = sum_k w^(k kz) x[k], w = exp(-2 pi i / Pz)
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
-            const float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+            const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz) * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < NL; ++n1) {
+                const int j = tid + n1 * T;
+                v[c][n1] = (HALF || j < ny) ? col[j] : make_float2(0.f, 0.f);
+            }
+        }
+        const float2 wz = fftr::root(kz, a.Pz);
+        float2 wk = wz;
+        for (int k = 1; k < a.nz; ++k) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + k) * a.Cx + kx) * ny;
+#pragma unroll
+                for (int n1 = 0; n1 < NL; ++n1) {
+                    const int j = tid + n1 * T;
+                    if (HALF || j < ny) {
+                        const float2 x = col[j];
+                        v[c][n1].x = fmaf(wk.x, x.x, fmaf(-wk.y, x.y, v[c][n1].x));
+                        v[c][n1].y = fmaf(wk.x, x.y, fmaf(wk.y, x.x, v[c][n1].y));
+                    }
+                }
+            }
+            wk = fft::cmul(wk, wz);
+        }
+    } else if (HALF) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float2* __restrict__ col = a.Tin + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
             for (int n1 = 0; n1 < 8; ++n1) v[c][n1] = col[tid + n1 * T];
         }
@@ -566,8 +543,8 @@ columns_fast_kernel(const ColFastArgs a)
         if (HALF) {
 #pragma unroll
             for (int n1 = 8; n1 < 16; ++n1) v[c][n1] = make_float2(0.f, 0.f);
-        } else {
-            const float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+        } else if (!zf) {
+            const float2* __restrict__ col = a.Tin + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
                 const int j = tid + n1 * T;
@@ -604,30 +581,63 @@ columns_fast_kernel(const ColFastArgs a)
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
-        float2* __restrict__ col = a.T + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+        float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
-        for (int n1 = 0; n1 < (HALF ? 8 : 16); ++n1) {
+        for (int n1 = 0; n1 < NL; ++n1) {
             const int j = tid + n1 * T;
             if (live && (HALF || j < ny)) col[j] = v[c][n1];
         }
     }
 }
 
+// S3, z direction, for the per-layer rows kernels: inverse length-Pz DFT across the planes of every (component, kx, j),
+// the nz kept layers written to `out` [3][nz][Cx][ny].  A plain streaming pass (reads 8 Pz, writes 8 nz bytes per point).
+template <int PZ>
+__global__ void __launch_bounds__(256) z_inverse_kernel(const float2* __restrict__ in, float2* __restrict__ out, size_t plane, int nz)
+{
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            float2 x[PZ];
+#pragma unroll
+            for (int kz = 0; kz < PZ; ++kz) x[fft::bitrev<PZ>(kz)] = __ldcs(in + (size_t)(c * PZ + kz) * plane + i);
+            fft::dit<PZ, true>(x);
+#pragma unroll
+            for (int k = 0; k < PZ; ++k) if (k < nz) out[(size_t)(c * nz + k) * plane + i] = x[k];
+        }
+    }
+}
+static int launch_z_inverse(const DemagPlan* p, const float2* in, float2* out, cudaStream_t st)
+{
+    const size_t plane = (size_t)p->Cx * p->g.ny;
+    const int blocks = (int)std::min<size_t>((plane + 255) / 256, (size_t)148 * 16);
+    switch (p->Pz) {
+        case 4: z_inverse_kernel<4><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
+        case 8: z_inverse_kernel<8><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
+        case 16: z_inverse_kernel<16><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
+        case 32: z_inverse_kernel<32><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
+        default: return MMC_E_UNSUPPORTED;
+    }
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+
+template <int LGN, bool HALF>
+static int launch_columns_fast_h(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
+{
+    using S = fftr::Shape<LGN>;
+    const size_t smem = (size_t)S::G * S::SMEM * sizeof(float2);
+    auto kern = columns_fast_kernel<LGN, HALF>;
+    if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+    const unsigned nbx = (p->Cx + S::G - 1) / S::G;
+    const dim3 grid = ca.nz > 0 ? dim3(p->Pz, nbx) : dim3(nbx, p->Pz), block(S::T, S::G);
+    if (grid.y > 65535u) return MMC_E_UNSUPPORTED;
+    kern<<<grid, block, smem, st>>>(ca);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
 template <int LGN>
 static int launch_columns_fast(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
 {
-    using S = fftr::Shape<LGN>;
-    const dim3 grid((p->Cx + S::G - 1) / S::G, p->Pz), block(S::T, S::G);
-    const size_t smem = (size_t)S::G * S::SMEM * sizeof(float2);
-    const bool half = 2 * p->g.ny == p->Py;
-    if (half) {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(columns_fast_kernel<LGN, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        columns_fast_kernel<LGN, true><<<grid, block, smem, st>>>(ca);
-    } else {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(columns_fast_kernel<LGN, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        columns_fast_kernel<LGN, false><<<grid, block, smem, st>>>(ca);
-    }
-    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+    return 2 * p->g.ny == p->Py ? launch_columns_fast_h<LGN, true>(p, ca, st) : launch_columns_fast_h<LGN, false>(p, ca, st);
 }
 static int launch_columns_fast_any(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
 {
@@ -688,8 +698,9 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     while (p->RJ > 1 && p->RJ / 2 >= g.ny) p->RJ >>= 1;
     {
         const int lgH = ilog2(p->Hx);
-        p->fastA = lgH >= 8 && lgH <= 11 && (p->Pz == 1 || p->Pz == 4 || p->Pz == 8 || p->Pz == 16) &&
-                   rows_fast_smem(lgH, g.nz) <= 227 * 1024;
+        const int lgPy = ilog2(p->Py);
+        // per-layer rows kernels need the columns kernel to do the forward z-DFT
+        p->fastA = lgH >= 8 && lgH <= 11 && lgPy >= fftr::kMinLg && lgPy <= fftr::kMaxLg;
     }
     if (!p->fastA && bytesA(p->RJ) > 220 * 1024) { if (err) *err = "demag: nz * padded nx too large for the fused row kernels"; return MMC_E_UNSUPPORTED; }
     p->smemA = bytesA(p->RJ);
@@ -710,6 +721,7 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     }
     const size_t nT = (size_t)3 * p->Pz * p->Cx * g.ny;
     CK(cudaMalloc(&p->T, nT * sizeof(float2)));
+    if (p->fastA && g.nz > 1) CK(cudaMalloc(&p->U, (size_t)3 * g.nz * p->Cx * g.ny * sizeof(float2)));
     CK(cudaMalloc(&p->twx, (size_t)p->Px * sizeof(float2)));
     CK(cudaMalloc(&p->twy, (size_t)p->Py * sizeof(float2)));
     twiddle_kernel<<<blocks_for(p->Px), 256, 0, st>>>(p->twx, p->Px);
@@ -757,7 +769,7 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
 void demag_destroy(DemagPlan* p)
 {
     if (!p) return;
-    cudaFree(p->T); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2); 
+    cudaFree(p->T); cudaFree(p->U); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2); 
     for (int q = 0; q < 6; ++q) cudaFree(p->nhat[q]);
     delete p;
 }
@@ -789,7 +801,7 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
         }
     }
     for (int c = 0; c < 3; ++c) { rf.m[c] = m[c]; rf.bd[c] = bd[c]; }
-    rf.Ms0 = Ms0_split; rf.Ms0_u = Ms0_uniform; rf.T = p->T;
+    rf.Ms0 = Ms0_split; rf.Ms0_u = Ms0_uniform; rf.T = p->U ? p->U : p->T;
     int rc = p->fastA ? launch_rows_fast_any(p, rf, false, st) : launch_rows_any(p, ra, false, st);
     if (rc) { if (err) *err = "rows_fwd_kernel launch failed"; return rc; }
     if (timer) timer->mark(PH_FFT_FWD, stream);
@@ -799,16 +811,23 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
     for (int q = 0; q < 6; ++q) ca.nhat[q] = p->nhat[q];
     if (p->fastB) {
         ColFastArgs fa{};
-        fa.ny = p->g.ny; fa.Cx = p->Cx; fa.Pz = p->Pz; fa.tw1 = p->twB1; fa.tw2 = p->twB2; fa.T = p->T;
+        fa.ny = p->g.ny; fa.Cx = p->Cx; fa.Pz = p->Pz; fa.nz = p->U ? p->g.nz : 0; fa.tw1 = p->twB1; fa.tw2 = p->twB2;
+        fa.Tin = p->U ? p->U : p->T; fa.Tout = p->T;
         for (int q = 0; q < 6; ++q) fa.nhat[q] = p->nhat[q];
         rc = launch_columns_fast_any(p, fa, st);
         if (rc) { if (err) *err = "columns_fast_kernel launch failed"; return rc; }
+        if (timer) timer->mark(PH_MULTIPLY, stream);
+        if (p->U) {
+            rc = launch_z_inverse(p, p->T, p->U, st);
+            if (rc) { if (err) *err = "z_inverse_kernel launch failed"; return rc; }
+            if (timer) timer->mark(PH_CROP, stream);
+        }
     } else {
         const dim3 gridB(p->Cx, p->Pz);
         if (p->g.nz > 1) columns_kernel<true><<<gridB, p->threadsB, p->smemB, st>>>(ca);
         else             columns_kernel<false><<<gridB, p->threadsB, p->smemB, st>>>(ca);
+        if (timer) timer->mark(PH_MULTIPLY, stream);
     }
-    if (timer) timer->mark(PH_MULTIPLY, stream);
     rc = p->fastA ? launch_rows_fast_any(p, rf, true, st) : launch_rows_any(p, ra, true, st);
     if (rc) { if (err) *err = "rows_inv_kernel launch failed"; return rc; }
     if (timer) timer->mark(PH_FFT_INV, stream);

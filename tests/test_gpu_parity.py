@@ -170,8 +170,14 @@ def test_sweep_matches_replayed_oracle(name):
                                      ((1024, 10, 1), (5e-9, 5e-9, 10e-9)), ((700, 9, 4), (3e-9, 3e-9, 3e-9)),
                                      ((520, 6, 5), (3e-9, 3e-9, 3e-9)), ((2048, 7, 1), (5e-9, 5e-9, 10e-9)),
                                      ((1500, 5, 2), (3e-9, 3e-9, 3e-9)),
-                                     # both fast paths together
-                                     ((256, 256, 1), (5e-9, 5e-9, 5e-9)), ((512, 128, 4), (3e-9, 3e-9, 3e-9))])
+                                     # register-resident rows AND columns kernels, z-DFT over a thread-block cluster of the
+                                     # columns kernel (2, 3, 4 layers: clusters of 4, 8, 8 CTAs; ragged chunks) or none (1 layer)
+                                     ((256, 256, 1), (5e-9, 5e-9, 5e-9)), ((512, 128, 4), (3e-9, 3e-9, 3e-9)),
+                                     ((200, 70, 1), (5e-9, 5e-9, 5e-9)), ((256, 66, 4), (3e-9, 3e-9, 3e-9)),
+                                     ((301, 67, 3), (2e-9, 3e-9, 4e-9)), ((512, 72, 2), (3e-9, 3e-9, 3e-9)),
+                                     ((1024, 65, 1), (5e-9, 5e-9, 10e-9)), ((700, 69, 4), (3e-9, 3e-9, 3e-9)),
+                                     ((2048, 66, 1), (5e-9, 5e-9, 10e-9)), ((1500, 65, 2), (3e-9, 3e-9, 3e-9)),
+                                     ((130, 300, 3), (3e-9, 3e-9, 3e-9))])
 def test_demag_field_parity(shape, d):
     """Eq. (14): GPU fp32 FFT convolution vs the oracle's fp64 one (itself pinned to the direct sum)."""
     import paper_2106_05593_b200 as P
