@@ -590,20 +590,34 @@ columns_fast_kernel(const ColFastArgs a)
     }
 }
 
-// S3, z direction, for the per-layer rows kernels: inverse length-Pz DFT across the planes of every (component, kx, j),
-// the nz kept layers written to `out` [3][nz][Cx][ny].  A plain streaming pass (reads 8 Pz, writes 8 nz bytes per point).
-template <int PZ>
-__global__ void __launch_bounds__(256) z_inverse_kernel(const float2* __restrict__ in, float2* __restrict__ out, size_t plane, int nz)
+// S3, z direction, for the per-layer rows kernels: inverse length-Pz DFT (Pz = 2 NZ - 1, a direct sum) across the planes of
+// every (component, kx, j), the NZ kept layers written to `out` [3][NZ][Cx][ny].  A plain streaming pass (reads 8 Pz,
+// writes 8 NZ bytes per point).
+constexpr int kMaxFastLayers = 8;
+template <int NZ>
+__global__ void __launch_bounds__(256) z_inverse_kernel(const float2* __restrict__ in, float2* __restrict__ out, size_t plane)
 {
+    constexpr int PZ = 2 * NZ - 1;
+    __shared__ float2 w[PZ];                               // exp(+2 pi i q / Pz)
+    if (threadIdx.x < PZ) { const float2 r = fftr::root(threadIdx.x, PZ); w[threadIdx.x] = make_float2(r.x, -r.y); }
+    __syncthreads();
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             float2 x[PZ];
 #pragma unroll
-            for (int kz = 0; kz < PZ; ++kz) x[fft::bitrev<PZ>(kz)] = __ldcs(in + (size_t)(c * PZ + kz) * plane + i);
-            fft::dit<PZ, true>(x);
+            for (int kz = 0; kz < PZ; ++kz) x[kz] = __ldcs(in + (size_t)(c * PZ + kz) * plane + i);
 #pragma unroll
-            for (int k = 0; k < PZ; ++k) if (k < nz) out[(size_t)(c * nz + k) * plane + i] = x[k];
+            for (int k = 0; k < NZ; ++k) {
+                float2 acc = x[0];
+#pragma unroll
+                for (int kz = 1; kz < PZ; ++kz) {
+                    const float2 t = w[(k * kz) % PZ];
+                    acc.x = fmaf(t.x, x[kz].x, fmaf(-t.y, x[kz].y, acc.x));
+                    acc.y = fmaf(t.x, x[kz].y, fmaf(t.y, x[kz].x, acc.y));
+                }
+                out[(size_t)(c * NZ + k) * plane + i] = acc;
+            }
         }
     }
 }
@@ -611,11 +625,14 @@ static int launch_z_inverse(const DemagPlan* p, const float2* in, float2* out, c
 {
     const size_t plane = (size_t)p->Cx * p->g.ny;
     const int blocks = (int)std::min<size_t>((plane + 255) / 256, (size_t)148 * 16);
-    switch (p->Pz) {
-        case 4: z_inverse_kernel<4><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
-        case 8: z_inverse_kernel<8><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
-        case 16: z_inverse_kernel<16><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
-        case 32: z_inverse_kernel<32><<<blocks, 256, 0, st>>>(in, out, plane, p->g.nz); break;
+    switch (p->g.nz) {
+        case 2: z_inverse_kernel<2><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 3: z_inverse_kernel<3><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 4: z_inverse_kernel<4><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 5: z_inverse_kernel<5><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 6: z_inverse_kernel<6><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 7: z_inverse_kernel<7><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 8: z_inverse_kernel<8><<<blocks, 256, 0, st>>>(in, out, plane); break;
         default: return MMC_E_UNSUPPORTED;
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
@@ -685,7 +702,17 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     *out = p;
     p->g = g;
     p->Px = padded_pow2(g.nx, 2); p->Py = padded_pow2(g.ny, 1); p->Pz = padded_pow2(g.nz, 1);
-    p->Hx = p->Px / 2; p->Cx = p->Hx + 1; p->lgPz = ilog2(p->Pz);
+    p->Hx = p->Px / 2; p->Cx = p->Hx + 1;
+    {
+        // register-resident path: per-layer rows kernels, z-DFT outside them (fused into the columns kernel's load, and
+        // the z_inverse pass).  Its z length is the SHORTEST that makes the cyclic convolution linear, Pz = 2 nz - 1
+        // (7 planes instead of 8 for four layers, 5 instead of 8 for three): the z-DFT is a direct sum there, so any
+        // length will do, and every plane saved is a whole set of column transforms saved.
+        const int lgH = ilog2(p->Hx), lgPy = ilog2(p->Py);
+        p->fastA = lgH >= 8 && lgH <= 11 && lgPy >= fftr::kMinLg && lgPy <= fftr::kMaxLg && g.nz <= kMaxFastLayers;
+        if (p->fastA && g.nz > 1) p->Pz = 2 * g.nz - 1;
+    }
+    p->lgPz = ilog2(p->Pz);
     p->px = fft::make_plan(ilog2(p->Hx)); p->py = fft::make_plan(ilog2(p->Py));
     if (p->lgPz > 5) { if (err) *err = "demag: more than 16 layers (padded z length > 32) is not built"; return MMC_E_UNSUPPORTED; }
     // kernels A/C: rows per CTA.  8 if that leaves room for two CTAs per SM, else 4 (32-byte store segments), less
@@ -696,12 +723,6 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     while (p->RJ > 4 && bytesA(p->RJ) > 100 * 1024) p->RJ >>= 1;
     while (p->RJ > 1 && bytesA(p->RJ) > 200 * 1024) p->RJ >>= 1;
     while (p->RJ > 1 && p->RJ / 2 >= g.ny) p->RJ >>= 1;
-    {
-        const int lgH = ilog2(p->Hx);
-        const int lgPy = ilog2(p->Py);
-        // per-layer rows kernels need the columns kernel to do the forward z-DFT
-        p->fastA = lgH >= 8 && lgH <= 11 && lgPy >= fftr::kMinLg && lgPy <= fftr::kMaxLg;
-    }
     if (!p->fastA && bytesA(p->RJ) > 220 * 1024) { if (err) *err = "demag: nz * padded nx too large for the fused row kernels"; return MMC_E_UNSUPPORTED; }
     p->smemA = bytesA(p->RJ);
     p->threadsA = p->smemA > 100 * 1024 ? 512 : 256;
