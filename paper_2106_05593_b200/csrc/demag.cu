@@ -296,12 +296,15 @@ __global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
 // the mirror-frequency access of the real-transform (un)tangling) reuses between barriers.  Row strides are = 4 (mod 16)
 // elements, so that the four rows of a half-warp sit in different bank groups.
 // grid (ceil(ny/4), 3 components * nz layers).
-constexpr int kRJ = 4;
+#ifndef MMC_ROWS_RJ11
+#define MMC_ROWS_RJ11 4
+#endif
 template <int LGH> struct RowShape {
     using S = fftr::Shape<LGH>;
     static constexpr int Hx = S::N, T = S::T;
+    static constexpr int RJ = LGH >= 11 ? MMC_ROWS_RJ11 : 4;   // mesh rows per CTA
     static constexpr int CP = Hx + Hx / 16;              // pad(k) + pad(Hx - k) (+1 when k & 15 != 0); = pad(Hx)
-    static constexpr int ES = (S::SMEM > CP ? S::SMEM : CP) + 4;   // row stride
+    static constexpr int ES = (S::SMEM > CP ? S::SMEM : CP) + 16 / RJ;   // row stride: RJ rows of a half-warp in different bank groups
 };
 struct RowFastArgs {
     Geometry g;
@@ -313,7 +316,7 @@ struct RowFastArgs {
 };
 
 template <int LGH>
-__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, RowShape<LGH>::T > 64 ? 1 : 2) rows_fwd_fast_kernel(const RowFastArgs a)
+__global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape<LGH>::RJ * RowShape<LGH>::T > 256 ? 1 : 2) rows_fwd_fast_kernel(const RowFastArgs a)
 {
     using R = RowShape<LGH>;
     constexpr int T = R::T, Hx = R::Hx;
@@ -321,7 +324,7 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, RowShape<LGH>::T > 64 
     const Geometry g = a.g;
     const int nz = g.nz, ny = g.ny;
     const int jj = threadIdx.x, t = threadIdx.y;
-    const int c = blockIdx.y / nz, k = blockIdx.y - c * nz, j = blockIdx.x * kRJ + jj;
+    const int c = blockIdx.y / nz, k = blockIdx.y - c * nz, j = blockIdx.x * R::RJ + jj;
     const bool valid = j < ny;
     const int hxr = (g.nx + 1) >> 1;
     float2* s1 = sm + jj * R::ES;
@@ -374,7 +377,7 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, RowShape<LGH>::T > 64 
 }
 
 template <int LGH>
-__global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, RowShape<LGH>::T > 64 ? 1 : 2) rows_inv_fast_kernel(const RowFastArgs a)
+__global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape<LGH>::RJ * RowShape<LGH>::T > 256 ? 1 : 2) rows_inv_fast_kernel(const RowFastArgs a)
 {
     using R = RowShape<LGH>;
     constexpr int T = R::T, Hx = R::Hx;
@@ -382,7 +385,7 @@ __global__ void __launch_bounds__(kRJ * RowShape<LGH>::T, RowShape<LGH>::T > 64 
     const Geometry g = a.g;
     const int nz = g.nz, ny = g.ny;
     const int jj = threadIdx.x, t = threadIdx.y;
-    const int c = blockIdx.y / nz, k = blockIdx.y - c * nz, j = blockIdx.x * kRJ + jj;
+    const int c = blockIdx.y / nz, k = blockIdx.y - c * nz, j = blockIdx.x * R::RJ + jj;
     const bool valid = j < ny;
     const int hxr = (g.nx + 1) >> 1;
     float2* s1 = sm + jj * R::ES;
@@ -433,8 +436,8 @@ template <int LGH>
 static int launch_rows_fast(const DemagPlan* p, const RowFastArgs& ra, bool inverse, cudaStream_t st)
 {
     using R = RowShape<LGH>;
-    const dim3 grid((p->g.ny + kRJ - 1) / kRJ, 3 * p->g.nz), block(kRJ, R::T);
-    const size_t smem = (size_t)kRJ * R::ES * sizeof(float2);
+    const dim3 grid((p->g.ny + R::RJ - 1) / R::RJ, 3 * p->g.nz), block(R::RJ, R::T);
+    const size_t smem = (size_t)R::RJ * R::ES * sizeof(float2);
     if (inverse) {
         if (smem > 48 * 1024) cudaFuncSetAttribute(rows_inv_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         rows_inv_fast_kernel<LGH><<<grid, block, smem, st>>>(ra);

@@ -150,11 +150,17 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
 }
 
 // ------------------------------------------------------------------------------------------------ the pass
-// blockDim = (32, BY, BZ), 256 threads; grid = (ceil(hxr/32), ceil(ny/BY), ceil(nz/BZ)).
+// blockDim = (32, BY, BZ), kPassThreads = 512 threads (measured on cfg 4 / cfg 5: 128 threads 110 / 100 us per pass,
+// 256: 69 / 59, 512: 65 / 52, 1024: 68 / 55: the larger brick shares more neighbour rows through L1);
+// grid = (ceil(hxr/32), ceil(ny/BY), ceil(nz/BZ)).
 // Running sums of the sweep's final vectors are kept in fixed point (kSumScale), so that they can be reduced with
 // integer warp reductions and integer atomics: exact, order-independent and therefore deterministic.
+#ifndef MMC_PASS_THREADS
+#define MMC_PASS_THREADS 512
+#endif
+constexpr int kPassThreads = MMC_PASS_THREADS;      // CTA = 32 x BY x BZ brick of this many cells
 template <unsigned F, bool DEBUG>
-__global__ void __launch_bounds__(256, DEBUG ? 1 : 4) colour_pass_kernel(const SweepArgs a)
+__global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads) colour_pass_kernel(const SweepArgs a)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0;
@@ -307,7 +313,7 @@ __global__ void __launch_bounds__(256, DEBUG ? 1 : 4) colour_pass_kernel(const S
             }
         }
         __threadfence_block();
-        if (atomicAdd(&s_arrived, 1u) == 7u) {         // 8 warps per block
+        if (atomicAdd(&s_arrived, 1u) == (unsigned)(kPassThreads / 32 - 1)) {   // last warp of the block
             __threadfence_block();
             const unsigned tc = atomicAdd(&s_acc[1], 0u);
             if (tc) {
@@ -349,11 +355,11 @@ int launch_end_sweep(Control* ctl, void* stream)
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 
-// CTA brick 32 x BY x BZ (256 threads): BZ covers up to 4 layers so that the z neighbours are lines the CTA reads anyway.
+// CTA brick 32 x BY x BZ (kPassThreads threads): BZ covers up to 4 layers so that the z neighbours are lines the CTA reads anyway.
 static void brick(const Geometry& g, dim3* block, dim3* grid)
 {
     const int bz = g.nz >= 4 ? 4 : (g.nz >= 2 ? 2 : 1);
-    const int by = 8 / bz;
+    const int by = kPassThreads / 32 / bz;
     const int hxr = (g.nx + 1) >> 1;
     *block = dim3(32, by, bz);
     *grid = dim3((hxr + 31) / 32, (g.ny + by - 1) / by, (g.nz + bz - 1) / bz);
