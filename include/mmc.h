@@ -115,6 +115,21 @@ int mmc_demag_field(mmc_ctx* ctx, float* bx, float* by, float* bz);
 int mmc_get_observables(mmc_ctx* ctx, mmc_obs* host_out);      /* synchronises */
 int mmc_reset_counters(mmc_ctx* ctx);                          /* accepted/trials := 0 */
 int mmc_reset_averages(mmc_ctx* ctx);                          /* run_mean_* := 0 */
+/* Chunked convergence of one field step: iterations run in chunks of chunk_sweeps (the paper uses 2000);
+ * every chunk's ensemble average of m (mean over the non-empty cells of the state after each iteration, averaged over
+ * the chunk) is projected on the unit vector along (ux, uy, uz) -- the applied field direction --; after at least
+ * min_chunks (>= 2) chunks the step is accepted when the last two chunk averages differ by at most `threshold` (the
+ * paper's "0.01 normalized change": read as an absolute change of <M_par>/Ms0), or given up after max_chunks.
+ * The field itself is set with mmc_set_field before the call.  Synchronises once per chunk; uses (and resets) the
+ * running averages.  SURVEY 8(f) row 1. */
+typedef struct {
+    int      chunks_done, converged;
+    double   mean_par_last, mean_par_prev;       /* last two chunk averages along the direction */
+    double   mean_m[3], mean_len;                /* last chunk's averages */
+    uint64_t sweeps;                             /* iterations spent in this call */
+} mmc_relax_result;
+int mmc_relax(mmc_ctx* ctx, double ux, double uy, double uz, int chunk_sweeps, int min_chunks, int max_chunks,
+              double threshold, mmc_relax_result* host_out);
 /* One colour pass (colour 0 or 1) at the current sweep counter with a per-cell dump, natural cell order, device
  * pointers, any may be NULL: dm float[3N] (cell-major: dm[3c+a]), dF_terms float[6N] (ex, an, zee, dmi, demag,
  * long in units of kB T), margin float[N] (= ln u - 4 ln f + dF; accept <=> margin < 0), accepted uint8[N].

@@ -392,6 +392,33 @@ class OracleMMC:
         for _ in range(n_sweeps):
             self.sweep_once()
 
+    def relax(self, direction, chunk_sweeps=2000, min_chunks=2, max_chunks=50, threshold=0.01):
+        """Chunked convergence of one field step: "a chunk with a fixed number of iterations (2000) is
+        defined, with an ensemble average magnetization value computed for each chunk ... executed for at least 2 chunks
+        ... if their respective final average magnetization values along the applied field direction are close enough
+        within an acceptance threshold (0.01 normalized change ...) the computation accepts the last chunk average".
+        Reading: the chunk average is the mean over non-empty cells of the state after each iteration,
+        averaged over the chunk's iterations; "normalized change" = absolute change of <M_par>/Ms0."""
+        u = np.asarray(direction, dtype=np.float64); u = u / np.linalg.norm(u)
+        self._setup()
+        act = np.asarray(self.coef["Ms0"]) > 0
+        prev = 0.0; res = None
+        for n in range(1, max_chunks + 1):
+            acc = np.zeros(3); acc_len = 0.0
+            for _ in range(chunk_sweeps):
+                self.sweep_once()
+                acc += np.array([self.m[a][act].mean() for a in range(3)])
+                acc_len += np.sqrt(self.m[0] ** 2 + self.m[1] ** 2 + self.m[2] ** 2)[act].mean()
+            mean = acc / chunk_sweeps
+            par = float(mean @ u)
+            res = dict(chunks_done=n, converged=False, mean_par_last=par, mean_par_prev=prev, mean_m=mean,
+                       mean_len=acc_len / chunk_sweeps, sweeps=n * chunk_sweeps)
+            if n >= min_chunks and abs(par - prev) <= threshold:
+                res["converged"] = True
+                break
+            prev = par
+        return res
+
     def colour_terms_given_dm(self, colour, dm):
         """O4 for every active cell of `colour` with caller-supplied trial vectors dm[N,3] -> terms[N,6] (NaN elsewhere)."""
         p = self._problem()

@@ -20,7 +20,7 @@ MUB = 9.2740100783e-24
 SYMBOLS = [
     "mmc_create", "mmc_destroy", "mmc_set_material", "mmc_set_exchange_coupling", "mmc_set_temperature",
     "mmc_set_field", "mmc_set_move", "mmc_set_demag", "mmc_set_seed", "mmc_set_sweep_counter", "mmc_set_m",
-    "mmc_get_m", "mmc_set_m_host", "mmc_get_m_host", "mmc_sweep", "mmc_sweep_timed", "mmc_demag_field", "mmc_get_observables", "mmc_reset_counters", "mmc_reset_averages",
+    "mmc_get_m", "mmc_set_m_host", "mmc_get_m_host", "mmc_sweep", "mmc_sweep_timed", "mmc_demag_field", "mmc_get_observables", "mmc_reset_counters", "mmc_reset_averages", "mmc_relax",
     "mmc_debug_pass", "mmc_thermal", "mmc_demag_tensor_at", "mmc_strerror", "mmc_last_error",
 ]
 
@@ -51,6 +51,12 @@ class Obs(C.Structure):
                 ("accepted", C.c_uint64), ("trials", C.c_uint64), ("sweeps_done", C.c_uint64),
                 ("cone_deg", C.c_double), ("sigma_used", C.c_double),
                 ("run_mean_m", C.c_double * 3), ("run_mean_len", C.c_double), ("run_sweeps", C.c_uint64)]
+
+
+class RelaxResult(C.Structure):
+    """mmc_relax_result."""
+    _fields_ = [("chunks_done", C.c_int), ("converged", C.c_int), ("mean_par_last", C.c_double), ("mean_par_prev", C.c_double),
+                ("mean_m", C.c_double * 3), ("mean_len", C.c_double), ("sweeps", C.c_uint64)]
 
 
 _lib = None
@@ -88,6 +94,7 @@ def lib():
     L.mmc_get_observables.argtypes = [vp, C.POINTER(Obs)]
     L.mmc_reset_counters.argtypes = [vp]
     L.mmc_reset_averages.argtypes = [vp]
+    L.mmc_relax.argtypes = [vp, dbl, dbl, dbl, i32, i32, i32, dbl, C.POINTER(RelaxResult)]
     L.mmc_debug_pass.argtypes = [vp, i32, vp, vp, vp, vp]
     L.mmc_thermal.argtypes = [dbl] * 5 + [C.POINTER(dbl)]
     L.mmc_demag_tensor_at.argtypes = [dbl, dbl, dbl, i32, i32, i32, C.POINTER(dbl)]
@@ -249,6 +256,14 @@ class MMC:
                                         "trials", "sweeps_done", "cone_deg", "sigma_used", "run_mean_len", "run_sweeps")}
         d["mean_m"] = np.array(list(o.mean_m)); d["run_mean_m"] = np.array(list(o.run_mean_m))
         return d
+
+    def relax(self, direction, chunk_sweeps=2000, min_chunks=2, max_chunks=50, threshold=0.01):
+        """mmc_relax: chunked convergence of one field step; returns a dict of mmc_relax_result."""
+        r = RelaxResult()
+        self._ck(lib().mmc_relax(self._h, float(direction[0]), float(direction[1]), float(direction[2]), int(chunk_sweeps),
+                                 int(min_chunks), int(max_chunks), float(threshold), C.byref(r)))
+        return dict(chunks_done=r.chunks_done, converged=bool(r.converged), mean_par_last=r.mean_par_last,
+                    mean_par_prev=r.mean_par_prev, mean_m=np.array(list(r.mean_m)), mean_len=r.mean_len, sweeps=r.sweeps)
 
     def reset_counters(self):
         self._ck(lib().mmc_reset_counters(self._h))

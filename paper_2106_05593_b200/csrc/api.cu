@@ -618,6 +618,31 @@ int mmc_reset_averages(mmc_ctx* c)
     return MMC_OK;
 }
 
+int mmc_relax(mmc_ctx* c, double ux, double uy, double uz, int chunk_sweeps, int min_chunks, int max_chunks, double threshold,
+              mmc_relax_result* out)
+{
+    if (!c || !out) return fail(c, MMC_E_INVALID, "NULL pointer");
+    const double un = std::sqrt(ux * ux + uy * uy + uz * uz);
+    if (!(un > 0) || chunk_sweeps < 1 || min_chunks < 2 || max_chunks < min_chunks || !(threshold >= 0))
+        return fail(c, MMC_E_INVALID, "direction != 0, chunk_sweeps >= 1, 2 <= min_chunks <= max_chunks, threshold >= 0 required");
+    std::memset(out, 0, sizeof(*out));
+    double prev = 0.0;
+    for (int n = 1; n <= max_chunks; ++n) {
+        int rc = mmc_reset_averages(c); if (rc) return rc;
+        rc = mmc_sweep(c, chunk_sweeps); if (rc) return rc;
+        mmc_obs ob;
+        rc = mmc_get_observables(c, &ob); if (rc) return rc;
+        const double par = (ob.run_mean_m[0] * ux + ob.run_mean_m[1] * uy + ob.run_mean_m[2] * uz) / un;
+        out->chunks_done = n; out->sweeps += (uint64_t)chunk_sweeps;
+        out->mean_par_prev = prev; out->mean_par_last = par;
+        for (int q = 0; q < 3; ++q) out->mean_m[q] = ob.run_mean_m[q];
+        out->mean_len = ob.run_mean_len;
+        if (n >= min_chunks && std::fabs(par - prev) <= threshold) { out->converged = 1; break; }
+        prev = par;
+    }
+    return MMC_OK;
+}
+
 int mmc_debug_pass(mmc_ctx* c, int colour, float* dm, float* dF_terms, float* margin, uint8_t* accepted)
 {
     if (!c || (colour != 0 && colour != 1)) return fail(c, MMC_E_INVALID, "colour must be 0 or 1");

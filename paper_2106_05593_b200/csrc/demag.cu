@@ -472,8 +472,11 @@ struct ColFastArgs {
     const float* nhat[6];
 };
 
+#ifndef MMC_COLS_MINB
+#define MMC_COLS_MINB 3
+#endif
 template <int LGN, bool HALF>
-__global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G, fftr::Shape<LGN>::T >= 256 ? 2 : 3)
+__global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G, fftr::Shape<LGN>::T >= 256 ? 2 : MMC_COLS_MINB)
 columns_fast_kernel(const ColFastArgs a)
 {
     using S = fftr::Shape<LGN>;

@@ -121,6 +121,8 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
             s1[q * (T + 1) + tid] = y;
         }
     }
+    float2 pw2[15];                               // requested before the barrier: the registers of v are free here
+    if constexpr (R3 > 1) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw2);
     __syncthreads();
     const int u = tid >> 4, q1 = tid & 15;
     {
@@ -131,8 +133,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
     fft::dif<16, false>(v);
     if constexpr (R3 > 1) {
         float2* d2 = s2 + u * S::U + 17 * q1;
-        float2 pw[15];
-        stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw);
+        float2 (&pw)[15] = pw2;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             float2 y = v[fft::bitrev<16>(q)];

@@ -278,3 +278,29 @@ def test_adaptive_cone_tracks_oracle():
     assert og["cone_deg"] == o.cone_deg and og["cone_deg"] < 30.0
     assert abs(og["accepted"] / og["trials"] - o.accepted / o.trials) < 5e-3
     g.close()
+
+
+def test_relax_chunked_convergence():
+    """mmc_relax against the oracle's driver of the same protocol on a small film:
+    the same number of chunks, chunk averages within the trajectory noise of near-margin flips; and, exactly, against the
+    library's own running averages of a second context driven by hand (integer fixed-point sums: bit-identical)."""
+    wl = W.cfg2(nx=24, ny=20)
+    wl.adaptive_cone = False
+    g, o = _gpu(wl), _orc(wl)
+    rg = g.relax((1.0, 0.0, 0.0), chunk_sweeps=20, min_chunks=2, max_chunks=5, threshold=5e-3)
+    ro = o.relax((1.0, 0.0, 0.0), chunk_sweeps=20, min_chunks=2, max_chunks=5, threshold=5e-3)
+    assert rg["chunks_done"] == ro["chunks_done"] and rg["converged"] == ro["converged"] and rg["sweeps"] == ro["sweeps"]
+    assert abs(rg["mean_par_last"] - ro["mean_par_last"]) < 2e-4 and abs(rg["mean_len"] - ro["mean_len"]) < 2e-5
+    h = _gpu(wl)
+    for _ in range(rg["chunks_done"]):
+        h.reset_averages(); h.sweep(20)
+    ob = h.observables()
+    assert np.array_equal(ob["run_mean_m"], rg["mean_m"]) and ob["run_mean_len"] == rg["mean_len"]
+    # protocol edges: zero threshold never accepts; invalid arguments are refused
+    r0 = g.relax((1.0, 0.0, 0.0), chunk_sweeps=3, min_chunks=2, max_chunks=3, threshold=0.0)
+    assert (not r0["converged"]) and r0["chunks_done"] == 3 and r0["sweeps"] == 9
+    import paper_2106_05593_b200 as P
+    for bad in (dict(direction=(0, 0, 0)), dict(direction=(1, 0, 0), min_chunks=1), dict(direction=(1, 0, 0), chunk_sweeps=0)):
+        with pytest.raises(P.MMCError):
+            g.relax(**bad)
+    g.close(); h.close()

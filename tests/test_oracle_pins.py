@@ -424,3 +424,46 @@ def test_compound_move_joint_length_and_angle():
     assert ml == pytest.approx(mean_len_q, rel=8e-3)
     assert mc == pytest.approx(mean_cos_q, abs=4e-3)
     assert mz == pytest.approx(mean_mz_q, rel=1.5e-2)
+
+
+# ------------------------------------------------------------------------------------------------ chunked convergence
+def _relax_case(seed=4242):
+    import workloads as W
+    wl = W.cfg2(nx=12, ny=10)
+    wl.demag = False; wl.adaptive_cone = False; wl.seed = seed
+    o = O.OracleMMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, store_fp32=True)
+    W.configure(o, wl, O.Material)
+    return wl, o
+
+
+def test_relax_driver_follows_the_papers_protocol():
+    """The driver of PAPER.md:135 pinned against its own definition written out by hand: chunk averages = plain means of
+    the per-iteration cell means of a replayed run; at least two chunks; stops at the first chunk >= 2 whose average
+    along the field differs from the previous one by <= threshold; never more than max_chunks."""
+    wl, o = _relax_case()
+    r = o.relax((1.0, 0.0, 0.0), chunk_sweeps=7, min_chunks=2, max_chunks=6, threshold=1e-4)
+    # replay by hand with the same Philox stream
+    wl2, o2 = _relax_case()
+    per_sweep = []
+    for _ in range(r["sweeps"]):
+        o2.run(1)
+        per_sweep.append(o2.m[0].mean())
+    chunks = np.array(per_sweep).reshape(-1, 7).mean(axis=1)
+    assert r["chunks_done"] == len(chunks) and 2 <= r["chunks_done"] <= 6
+    assert abs(r["mean_par_last"] - chunks[-1]) < 1e-15 and abs(r["mean_par_prev"] - chunks[-2]) < 1e-15
+    d = np.abs(np.diff(chunks))
+    if r["converged"]:
+        assert d[-1] <= 1e-4 and np.all(d[:-1] > 1e-4)          # the first acceptable pair stops the step
+    else:
+        assert r["chunks_done"] == 6 and np.all(d > 1e-4)
+    # a huge threshold accepts after exactly min_chunks, a zero threshold never accepts
+    _, o3 = _relax_case()
+    r3 = o3.relax((1.0, 0.0, 0.0), chunk_sweeps=3, min_chunks=3, max_chunks=9, threshold=10.0)
+    assert r3["converged"] and r3["chunks_done"] == 3 and r3["sweeps"] == 9
+    _, o4 = _relax_case()
+    r4 = o4.relax((1.0, 0.0, 0.0), chunk_sweeps=2, min_chunks=2, max_chunks=4, threshold=0.0)
+    assert (not r4["converged"]) and r4["chunks_done"] == 4
+    # the direction is normalised: (2, 0, 0) and (1, 0, 0) give the same projection
+    _, o5 = _relax_case()
+    r5 = o5.relax((2.0, 0.0, 0.0), chunk_sweeps=7, min_chunks=2, max_chunks=6, threshold=1e-4)
+    assert r5["chunks_done"] == r["chunks_done"] and abs(r5["mean_par_last"] - r["mean_par_last"]) < 1e-15
