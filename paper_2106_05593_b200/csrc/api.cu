@@ -220,6 +220,7 @@ int ensure_setup(mmc_ctx* c)
     if (g.nz > 1) f |= F_Z;
     if (D0 != 0.0) f |= F_DMI;
     if (c->demag_enabled) f |= F_DEMAG;
+    if (n_active == (unsigned long long)N) f |= F_DENSE;
     c->features = f;
     c->dirty = false;
     return MMC_OK;

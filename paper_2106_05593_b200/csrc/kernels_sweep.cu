@@ -163,7 +163,7 @@ template <unsigned F, bool DEBUG>
 __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads) colour_pass_kernel(const SweepArgs a)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
-                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0;
+                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
     __shared__ unsigned s_acc[6];                    // accepted, trials, sum mx, my, mz, |m| (fixed point, two's complement)
     __shared__ unsigned s_arrived;
     const int tlin = threadIdx.x + 32 * (threadIdx.y + blockDim.y * threadIdx.z);
@@ -192,7 +192,8 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
     if (active) {
         if (PERCELL) { const unsigned w = __ldg(a.cw + ownb); mb = w & 0x7fu; cls = w >> 7; }
         else if (MASK) mb = __ldg(a.mask + ownb);
-        if ((MASK || PERCELL) && !(mb & 0x40u)) active = false;            // empty cell
+        // DENSE (no empty cell in the mesh): the vector loads below do not have to wait for this word to arrive
+        if (!DENSE && (MASK || PERCELL) && !(mb & 0x40u)) active = false;   // empty cell
     }
     if (active) {
         const int hxr = (nx + 1) >> 1;               // compact length of the real (unpadded) row
@@ -382,15 +383,23 @@ int launch_colour_pass(const SweepArgs& a, unsigned f, bool debug, void* stream)
 {
     cudaStream_t st = (cudaStream_t)stream;
     constexpr unsigned UALL = F_MASK | F_Z | F_DMI | F_DEMAG, PALL = UALL | F_PERCELL;
+    const bool dense = (f & F_DENSE) != 0;             // only ever a promise, never over-approximated
+    f &= ~F_DENSE;
     if (f & F_PERCELL) {
         if (debug) return launch_variant<PALL>(a, true, st);
-        if (!(f & F_DMI)) return launch_variant<F_MASK | F_PERCELL | F_Z | F_DEMAG>(a, false, st);          // cfg 4
+        if (!(f & F_DMI)) {                                                                                  // cfg 4
+            if (dense) return launch_variant<F_MASK | F_PERCELL | F_Z | F_DEMAG | F_DENSE>(a, false, st);
+            return launch_variant<F_MASK | F_PERCELL | F_Z | F_DEMAG>(a, false, st);
+        }
         return launch_variant<PALL>(a, false, st);
     }
     if (debug) return launch_variant<UALL>(a, true, st);
     if (f == 0u) return launch_variant<0u>(a, false, st);                                                   // cfg 1
     if ((f & ~(F_DEMAG)) == 0u) return launch_variant<F_DEMAG>(a, false, st);
-    if ((f & ~(F_MASK | F_DEMAG)) == 0u) return launch_variant<F_MASK | F_DEMAG>(a, false, st);             // cfg 2, 5
+    if ((f & ~(F_MASK | F_DEMAG)) == 0u) {                                                                  // cfg 2 (dense), 5
+        if (dense) return launch_variant<F_MASK | F_DEMAG | F_DENSE>(a, false, st);
+        return launch_variant<F_MASK | F_DEMAG>(a, false, st);
+    }
     if ((f & ~(F_DMI | F_DEMAG)) == 0u) return launch_variant<F_DMI | F_DEMAG>(a, false, st);               // cfg 3
     if ((f & ~(F_MASK | F_Z | F_DEMAG)) == 0u) return launch_variant<F_MASK | F_Z | F_DEMAG>(a, false, st);
     return launch_variant<UALL>(a, false, st);

@@ -79,6 +79,7 @@ enum Feature : unsigned {
     F_Z = 4u,         // nz > 1
     F_DMI = 8u,
     F_DEMAG = 16u,
+    F_DENSE = 32u,    // no empty cell: every in-mesh cell is active, so no load has to wait for the mask / class word
 };
 
 struct SweepArgs {
