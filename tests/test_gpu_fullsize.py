@@ -9,6 +9,8 @@ mmc_sweep / mmc_demag_field, not the debug pass), plus the equilibrium 3-sigma c
           test_sweep_matches_replayed_oracle: all cells equal to 2e-6 except a 2e-3 fraction (near-margin decisions
           and their black neighbours).
   equilibrium  8 seeds on each side, blocked means after discarding the first half, Welch test at 3 sigma.
+  paper       the length distribution of the CUDA path itself against the exact chain means derived from Eq. (7)
+              (tests/golden/length_means.txt), five temperatures below, at and above Tc, two sigma.
 """
 import numpy as np
 import pytest
@@ -170,3 +172,45 @@ def test_equilibrium_observables_within_3_sigma(name):
         mg, mo = G[:, q].mean(), Oo[:, q].mean()
         se = np.sqrt(G[:, q].var(ddof=1) / 8 + Oo[:, q].var(ddof=1) / 8)
         assert abs(mg - mo) <= 3.0 * se + 1e-7, f"{name}: {label}: gpu {mg:.6f} vs oracle {mo:.6f}, 3 sigma = {3 * se:.2e}"
+
+
+# ------------------------------------------------------------------------------------------------ the CUDA path against the paper's distribution
+def _golden_rows():
+    import os
+    rows = []
+    with open(os.path.join(os.path.dirname(__file__), "golden", "length_means.txt")) as f:
+        for ln in f:
+            if ln.strip() and not ln.startswith("#"):
+                rows.append([float(x) for x in ln.split()])
+    return rows
+
+
+@pytest.mark.parametrize("sigma_col", [(0.03, 2), (0.05, 3)], ids=["sigma0.03", "sigma0.05"])
+@pytest.mark.parametrize("row", _golden_rows(), ids=lambda r: f"T{int(r[0])}")
+def test_gpu_length_distribution_matches_eq7_chain(row, sigma_col):
+    """PAPER.md:108 / Eq. (7) on the CUDA path itself, against values that come from the paper and not from the oracle:
+    1 048 576 decoupled cells (A0 = 0, no anisotropy, no field, no demag: an ensemble of single-cell chains) at the
+    paper's Fig. 1 parameters (Tc 680 K, V = (5 nm)^3, Ms0 8e5 A/m, mu_B), 20 000 iterations of burn-in from a spread of
+    lengths and 20 000 of averaging (the length walk near Tc decorrelates over thousands of iterations).  The running
+    mean of |m| must hit the exact stationary mean of the literal (m_B/m_A)^4 chain (tests/golden/length_means.txt,
+    SURVEY 8(c) G1; T = 680 K is the T = Tc limit of G10) to 5e-4 relative (measured: 3e-5 .. 1.3e-4) -- which tells
+    sigma = 0.03 from 0.05 (1.6e-3 .. 3e-3 apart) and the chain from the Eq. (7) quadrature mean (2.4e-3 .. 8e-3 below it,
+    the bias linear in sigma of reading G1)."""
+    import paper_2106_05593_b200 as P
+    sigma, col = sigma_col
+    T, m7, ref = row[0], row[1], row[col]
+    n = 1024
+    rng = np.random.default_rng(int(T))
+    v = rng.normal(size=(3, n * n)); v /= np.linalg.norm(v, axis=0)
+    m0 = (row[2] * rng.uniform(0.3, 1.7, n * n) * v).astype(np.float32)
+    g = P.MMC(n, n, 1, 5e-9, 5e-9, 5e-9, 0b011)
+    g.set_material([P.Material(Ms0=8e5, A0=0.0, K1=0.0, Tc=680.0)])
+    g.set_temperature(T); g.set_field(0.0, 0.0, 0.0); g.set_move(60.0, sigma, False); g.set_demag(False)
+    g.set_seed(680000 + int(T)); g.set_m(*m0)
+    g.sweep(20000)
+    g.reset_averages()
+    g.sweep(20000)
+    ob = g.observables()
+    g.close()
+    assert ob["run_mean_len"] == pytest.approx(ref, rel=5e-4)
+    assert ob["run_mean_len"] > m7 * (1.0 + 1.5e-3)
