@@ -214,3 +214,29 @@ def test_gpu_length_distribution_matches_eq7_chain(row, sigma_col):
     g.close()
     assert ob["run_mean_len"] == pytest.approx(ref, rel=5e-4)
     assert ob["run_mean_len"] > m7 * (1.0 + 1.5e-3)
+
+
+def test_gpu_angular_distribution_is_langevin():
+    """Transverse part of the distribution (Eq. (6), :114) on the CUDA path against the closed form: decoupled
+    cells of fixed length (sigma = 0: the move is a pure cone rotation) in a field along z sample exp(xi cos(theta)) uniformly in
+    solid angle (reading G6), so <cos(theta)> = coth(xi) - 1/xi with xi = V Ms0 |m| B / kB T."""
+    import paper_2106_05593_b200 as P
+    kB = 1.380649e-23
+    T, V, Ms0, L = 300.0, (5e-9) ** 3, 8e5, 0.9
+    for xi in (0.5, 3.0, 12.0):
+        B = xi * kB * T / (V * Ms0 * L)
+        n = 512
+        rng = np.random.default_rng(int(10 * xi))
+        v = rng.normal(size=(3, n * n)); v /= np.linalg.norm(v, axis=0)
+        m0 = (L * v).astype(np.float32)
+        g = P.MMC(n, n, 1, 5e-9, 5e-9, 5e-9, 0b011)
+        g.set_material([P.Material(Ms0=Ms0, A0=0.0, K1=0.0, Tc=680.0)])
+        g.set_temperature(T); g.set_field(0.0, 0.0, B); g.set_move(50.0, 0.0, False); g.set_demag(False)
+        g.set_seed(int(1000 * xi)); g.set_m(*m0)
+        g.sweep(1500); g.reset_averages(); g.sweep(3000)
+        ob = g.observables()
+        g.close()
+        assert ob["run_mean_len"] == pytest.approx(L, rel=2e-6)                 # rotations keep the length
+        expect = 1.0 / np.tanh(xi) - 1.0 / xi
+        assert ob["run_mean_m"][2] / L == pytest.approx(expect, abs=3e-4), f"xi = {xi}"
+        assert abs(ob["run_mean_m"][0]) < 3e-4 and abs(ob["run_mean_m"][1]) < 3e-4
