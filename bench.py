@@ -334,6 +334,12 @@ def run_ours(args):
                          "launch_ms": dk["launch_ms"], "share_of_step": dk["share_of_step"],
                          "note": "FFT kernels are co-limited by the FP32 pipes: see kernels[*].achieved_TFLOPs against "
                                  "148 SM x 128 lanes x 1.965 GHz = 37.2 T FP32 instr/s (74.4 TFLOP/s if every one were an FMA)"},
+            # the same kernel against the plain-ALU peak (no tensor cores: nothing here is a contraction): algorithmic flops
+            # (5 n log2 n per complex transform + the tensor multiply) over 148 SM x 128 FP32 lanes x 2 (FMA) x 1.965 GHz
+            "roofline_alu": ({"kernel": dom, "bound": "alu", "achieved": dk["achieved_TFLOPs"], "peak": 74.4, "unit": "TFLOP/s",
+                              "frac": dk["achieved_TFLOPs"] / 74.4,
+                              "peak_source": "derived: 148 SM x 128 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts and clocks)"}
+                             if "achieved_TFLOPs" in dk else None),
             "kernels": kern,
         }
         if not args.no_cpu_baseline and world == 1:

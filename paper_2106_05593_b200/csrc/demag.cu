@@ -376,8 +376,11 @@ __global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape
     }
 }
 
+#ifndef MMC_ROWS_INV_MINB
+#define MMC_ROWS_INV_MINB 2
+#endif
 template <int LGH>
-__global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape<LGH>::RJ * RowShape<LGH>::T > 256 ? 1 : 2) rows_inv_fast_kernel(const RowFastArgs a)
+__global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape<LGH>::RJ * RowShape<LGH>::T > 256 ? 1 : MMC_ROWS_INV_MINB) rows_inv_fast_kernel(const RowFastArgs a)
 {
     using R = RowShape<LGH>;
     constexpr int T = R::T, Hx = R::Hx;
