@@ -115,6 +115,13 @@ int mmc_demag_field(mmc_ctx* ctx, float* bx, float* by, float* bz);
 int mmc_get_observables(mmc_ctx* ctx, mmc_obs* host_out);      /* synchronises */
 int mmc_reset_counters(mmc_ctx* ctx);                          /* accepted/trials := 0 */
 int mmc_reset_averages(mmc_ctx* ctx);                          /* run_mean_* := 0 */
+/* Histograms of the current state over the non-empty cells, the paper's verification read-outs (PAPER.md:108 length
+ * distribution, PAPER.md:114 angular deviation from the mean direction).  kind 0: x = |m|; kind 1: x =
+ * polar angle in radians between m and the mean direction (sum of m over the non-empty cells).  nbins (1..4096) equal bins
+ * over [lo, hi), bin = floor((x - lo) nbins / (hi - lo)) evaluated in fp64 from the fp32 state; counts: host uint64[nbins];
+ * under_over: host uint64[2] (x < lo or NaN, x >= hi), may be NULL.  The paper's solid-angle weighting of the angular
+ * histogram is a division by the bin's sin(theta) d(theta) on the caller's side.  Synchronises. */
+int mmc_histogram(mmc_ctx* ctx, int kind, int nbins, double lo, double hi, uint64_t* counts, uint64_t* under_over);
 /* Chunked convergence of one field step: iterations run in chunks of chunk_sweeps (the paper uses 2000);
  * every chunk's ensemble average of m (mean over the non-empty cells of the state after each iteration, averaged over
  * the chunk) is projected on the unit vector along (ux, uy, uz) -- the applied field direction --; after at least

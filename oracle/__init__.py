@@ -392,6 +392,26 @@ class OracleMMC:
         for _ in range(n_sweeps):
             self.sweep_once()
 
+    def histogram(self, kind, nbins, lo, hi):
+        """The paper's verification read-outs over the non-empty cells: kind "length": x = |m|; kind "angle":
+        x = polar angle between m and the mean direction, "for each micromagnetic magnetization configuration the mean
+        direction is obtained, and for each vector ... the polar angle theta to this mean direction is found".
+        Equal bins over [lo, hi): bin = floor((x - lo) nbins / (hi - lo)); returns (counts, under, over)."""
+        self._setup()
+        act = np.asarray(self.coef["Ms0"]) > 0
+        m = np.stack([np.asarray(self.m[a], dtype=np.float64)[act] for a in range(3)])
+        L = np.sqrt(m[0] * m[0] + m[1] * m[1] + m[2] * m[2])
+        if kind == "length":
+            x = L
+        else:
+            d = m.sum(axis=1); d = d / np.linalg.norm(d)
+            x = np.arccos(np.clip((m[0] * d[0] + m[1] * d[1] + m[2] * d[2]) / L, -1.0, 1.0))
+        t = (x - lo) * (nbins / (hi - lo))
+        under = int(np.count_nonzero(~(t >= 0.0))); over = int(np.count_nonzero(t >= nbins))
+        ok = (t >= 0.0) & (t < nbins)
+        counts = np.bincount(t[ok].astype(np.int64), minlength=nbins).astype(np.uint64)
+        return counts, under, over
+
     def relax(self, direction, chunk_sweeps=2000, min_chunks=2, max_chunks=50, threshold=0.01):
         """Chunked convergence of one field step: "a chunk with a fixed number of iterations (2000) is
         defined, with an ensemble average magnetization value computed for each chunk ... executed for at least 2 chunks

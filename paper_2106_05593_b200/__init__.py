@@ -20,7 +20,7 @@ MUB = 9.2740100783e-24
 SYMBOLS = [
     "mmc_create", "mmc_destroy", "mmc_set_material", "mmc_set_exchange_coupling", "mmc_set_temperature",
     "mmc_set_field", "mmc_set_move", "mmc_set_demag", "mmc_set_seed", "mmc_set_sweep_counter", "mmc_set_m",
-    "mmc_get_m", "mmc_set_m_host", "mmc_get_m_host", "mmc_sweep", "mmc_sweep_timed", "mmc_demag_field", "mmc_get_observables", "mmc_reset_counters", "mmc_reset_averages", "mmc_relax",
+    "mmc_get_m", "mmc_set_m_host", "mmc_get_m_host", "mmc_sweep", "mmc_sweep_timed", "mmc_demag_field", "mmc_get_observables", "mmc_reset_counters", "mmc_reset_averages", "mmc_relax", "mmc_histogram",
     "mmc_debug_pass", "mmc_thermal", "mmc_demag_tensor_at", "mmc_strerror", "mmc_last_error",
 ]
 
@@ -94,6 +94,7 @@ def lib():
     L.mmc_get_observables.argtypes = [vp, C.POINTER(Obs)]
     L.mmc_reset_counters.argtypes = [vp]
     L.mmc_reset_averages.argtypes = [vp]
+    L.mmc_histogram.argtypes = [vp, i32, i32, dbl, dbl, vp, vp]
     L.mmc_relax.argtypes = [vp, dbl, dbl, dbl, i32, i32, i32, dbl, C.POINTER(RelaxResult)]
     L.mmc_debug_pass.argtypes = [vp, i32, vp, vp, vp, vp]
     L.mmc_thermal.argtypes = [dbl] * 5 + [C.POINTER(dbl)]
@@ -256,6 +257,14 @@ class MMC:
                                         "trials", "sweeps_done", "cone_deg", "sigma_used", "run_mean_len", "run_sweeps")}
         d["mean_m"] = np.array(list(o.mean_m)); d["run_mean_m"] = np.array(list(o.run_mean_m))
         return d
+
+    def histogram(self, kind, nbins, lo, hi):
+        """mmc_histogram: kind "length" (|m|, PAPER.md:108) or "angle" (polar angle to the mean direction, PAPER.md:114);
+        returns (counts uint64[nbins], under, over)."""
+        k = {"length": 0, "angle": 1}[kind]
+        counts = np.zeros(int(nbins), dtype=np.uint64); uo = np.zeros(2, dtype=np.uint64)
+        self._ck(lib().mmc_histogram(self._h, k, int(nbins), float(lo), float(hi), counts.ctypes.data, uo.ctypes.data))
+        return counts, int(uo[0]), int(uo[1])
 
     def relax(self, direction, chunk_sweeps=2000, min_chunks=2, max_chunks=50, threshold=0.01):
         """mmc_relax: chunked convergence of one field step; returns a dict of mmc_relax_result."""

@@ -619,6 +619,35 @@ int mmc_reset_averages(mmc_ctx* c)
     return MMC_OK;
 }
 
+int mmc_histogram(mmc_ctx* c, int kind, int nbins, double lo, double hi, uint64_t* counts, uint64_t* under_over)
+{
+    if (!c || !counts) return fail(c, MMC_E_INVALID, "NULL pointer");
+    if ((kind != 0 && kind != 1) || nbins < 1 || nbins > 4096 || !(hi > lo) || !std::isfinite(lo) || !std::isfinite(hi))
+        return fail(c, MMC_E_INVALID, "kind 0 or 1, 1 <= nbins <= 4096 and finite lo < hi required");
+    DeviceGuard dg(c->device);
+    int rc = ready(c); if (rc) return rc;
+    double dir[3] = { 0.0, 0.0, 1.0 };
+    if (kind == 1) {
+        mmc_obs ob;
+        rc = mmc_get_observables(c, &ob); if (rc) return rc;
+        const double n = std::sqrt(ob.mean_m[0] * ob.mean_m[0] + ob.mean_m[1] * ob.mean_m[1] + ob.mean_m[2] * ob.mean_m[2]);
+        if (!(n > 0)) return fail(c, MMC_E_INVALID, "the mean magnetisation vanishes: no mean direction");
+        for (int q = 0; q < 3; ++q) dir[q] = ob.mean_m[q] / n;
+    }
+    unsigned long long* d = nullptr;
+    CU(c, cudaMalloc(&d, (size_t)(nbins + 2) * sizeof(unsigned long long)));
+    rc = launch_histogram(c->g, c->m, c->mask, kind, dir, nbins, lo, hi, d, c->stream);
+    std::vector<unsigned long long> h((size_t)nbins + 2);
+    cudaError_t e = rc ? cudaErrorUnknown : cudaMemcpyAsync(h.data(), d, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    cudaFree(d);
+    if (rc) return fail(c, rc, "histogram launch failed");
+    if (e != cudaSuccess) return fail(c, MMC_E_CUDA, std::string("histogram: ") + cudaGetErrorString(e));
+    for (int b = 0; b < nbins; ++b) counts[b] = h[(size_t)b];
+    if (under_over) { under_over[0] = h[(size_t)nbins]; under_over[1] = h[(size_t)nbins + 1]; }
+    return MMC_OK;
+}
+
 int mmc_relax(mmc_ctx* c, double ux, double uy, double uz, int chunk_sweeps, int min_chunks, int max_chunks, double threshold,
               mmc_relax_result* out)
 {

@@ -2,6 +2,8 @@
 // read-out reduction (means and energies with pair terms counted once).
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "mmc_internal.h"
 
 namespace mmc {
@@ -145,6 +147,53 @@ __global__ void observables_final_kernel(const double* __restrict__ scratch, int
     if (t < 4) out->sum[t] = v;
     else if (t < 10) out->E[t - 4] = v;
     else out->n_active = (unsigned long long)(v + 0.5);
+}
+
+// Histograms of the current state over the non-empty cells.  kind 0: x = |m|; kind 1: x = polar angle
+// (radians) between m and the direction (dx, dy, dz).  Everything in fp64 from the fp32 state, bin = floor((x - lo) * scale),
+// scale = nbins / (hi - lo); out-of-range values go to under/over.  Shared-memory counters per CTA, 64-bit global atomics:
+// exact integers, order-independent.
+__global__ void __launch_bounds__(256) histogram_kernel(Geometry g, const float* __restrict__ mx, const float* __restrict__ my,
+                                                        const float* __restrict__ mz, const uint8_t* __restrict__ mask, int kind,
+                                                        double dx, double dy, double dz, int nbins, double lo, double scale,
+                                                        unsigned long long* __restrict__ counts /* nbins + 2 */)
+{
+    extern __shared__ unsigned int h[];
+    for (int b = threadIdx.x; b < nbins + 2; b += blockDim.x) h[b] = 0u;
+    __syncthreads();
+    const long long n = 2 * g.H;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+        if (!(mask[s] & 0x40u)) continue;
+        const double a = mx[s], b = my[s], c = mz[s];
+        const double len = sqrt(a * a + b * b + c * c);
+        double x = len;
+        if (kind == 1) {
+            double cs = (a * dx + b * dy + c * dz) / len;
+            cs = cs > 1.0 ? 1.0 : (cs < -1.0 ? -1.0 : cs);
+            x = acos(cs);
+        }
+        const double t = (x - lo) * scale;
+        int bin;
+        if (!(t >= 0.0)) bin = nbins;                    // under (also NaN)
+        else if (t >= (double)nbins) bin = nbins + 1;    // over
+        else bin = (int)t;
+        atomicAdd(&h[bin], 1u);
+    }
+    __syncthreads();
+    for (int b = threadIdx.x; b < nbins + 2; b += blockDim.x)
+        if (h[b]) atomicAdd(&counts[b], (unsigned long long)h[b]);
+}
+
+int launch_histogram(const Geometry& g, const float* const m[3], const uint8_t* mask, int kind, const double dir[3], int nbins,
+                     double lo, double hi, unsigned long long* dev_counts, void* stream)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    if (cudaMemsetAsync(dev_counts, 0, (size_t)(nbins + 2) * sizeof(unsigned long long), st) != cudaSuccess) return MMC_E_CUDA;
+    const long long n = 2 * g.H;
+    const int blocks = (int)std::min<long long>((n + 255) / 256, 148 * 8);
+    histogram_kernel<<<blocks, 256, (size_t)(nbins + 2) * sizeof(unsigned int), st>>>(g, m[0], m[1], m[2], mask, kind, dir[0], dir[1], dir[2],
+                                                                                    nbins, lo, (double)nbins / (hi - lo), dev_counts);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 
 int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, Observables* dev_out, double* scratch,

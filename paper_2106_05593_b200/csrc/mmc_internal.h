@@ -119,6 +119,9 @@ struct ObsParams {
 int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, Observables* dev_out, double* scratch,
                        int scratch_blocks, void* stream);
 
+int launch_histogram(const Geometry& g, const float* const m[3], const uint8_t* mask, int kind, const double dir[3], int nbins,
+                     double lo, double hi, unsigned long long* dev_counts, void* stream);
+
 // Optional per-phase device timing (mmc_sweep_timed): mark(p) records an event that ends phase p.
 enum Phase { PH_PACK = 0, PH_FFT_FWD, PH_MULTIPLY, PH_FFT_INV, PH_CROP, PH_RED, PH_BLACK, PH_END, PH_COUNT };
 struct PhaseTimer {

@@ -467,3 +467,44 @@ def test_relax_driver_follows_the_papers_protocol():
     _, o5 = _relax_case()
     r5 = o5.relax((2.0, 0.0, 0.0), chunk_sweeps=7, min_chunks=2, max_chunks=6, threshold=1e-4)
     assert r5["chunks_done"] == r["chunks_done"] and abs(r5["mean_par_last"] - r["mean_par_last"]) < 1e-15
+
+
+# ------------------------------------------------------------------------------------------------ histograms
+def test_histograms_against_numpy_and_closed_forms():
+    """The oracle's length / angle histograms pinned against numpy.histogram (a library routine with its own edge logic) on
+    states without values on bin edges, against hand-placed vectors with known angles to the mean direction, and against
+    the totals."""
+    import workloads as W
+    wl = W.cfg5(nx=160, ny=150)                      # empty cells present
+    o = O.OracleMMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, store_fp32=True)
+    W.configure(o, wl, O.Material)
+    rng = np.random.default_rng(5)
+    v = rng.normal(size=(3, wl.N)); v /= np.linalg.norm(v, axis=0)
+    v[2] = np.abs(v[2]) + 0.3                        # a clear mean direction
+    o.set_m(*(rng.uniform(0.2, 0.9, wl.N) * v).astype(np.float32))
+    ms = np.array([r["Ms0"] for r in wl.regions])[wl.region_of_cell] > 0
+    m = np.stack([np.asarray(o.m[a], dtype=np.float64)[ms] for a in range(3)])
+    L = np.linalg.norm(m, axis=0)
+    c, u, ov = o.histogram("length", 100, 0.25, 0.8)
+    ref, _ = np.histogram(L, bins=100, range=(0.25, 0.8))
+    assert np.array_equal(c.astype(np.int64), ref - np.bincount([99], minlength=100) * np.count_nonzero(L == 0.8))
+    assert u == np.count_nonzero(L < 0.25) and ov == np.count_nonzero(L >= 0.8) and c.sum() + u + ov == ms.sum() > 1000
+    d = m.sum(axis=1); d /= np.linalg.norm(d)
+    th = np.arccos(np.clip(m.T @ d / L, -1, 1))
+    c2, u2, ov2 = o.histogram("angle", 100, th.min(), th.max() * (1 + 1e-12))       # the paper's range: min .. max theta
+    ref2, _ = np.histogram(th, bins=100, range=(th.min(), th.max() * (1 + 1e-12)))
+    assert np.array_equal(c2.astype(np.int64), ref2) and u2 == 0 and ov2 == 0
+    # hand-placed: 3 vectors at polar angle 30 deg around z with azimuths 0, 120, 240 deg (mean direction = z exactly by
+    # symmetry) and one along z: angles 30, 30, 30, 0 degrees
+    o2 = O.OracleMMC(2, 2, 1, 5e-9, 5e-9, 5e-9, 0, store_fp32=False)
+    o2.set_material([O.Material(Ms0=8e5, A0=1e-11, Tc=800.0)], None); o2.set_temperature(300.0, None)
+    s, cth = np.sin(np.pi / 6), np.cos(np.pi / 6)
+    az = np.array([0.0, 2 * np.pi / 3, 4 * np.pi / 3])
+    o2.set_m(np.append(0.5 * s * np.cos(az), 0.0), np.append(0.5 * s * np.sin(az), 0.0), np.append(0.5 * cth * np.ones(3), 0.7))
+    c3, u3, ov3 = o2.histogram("angle", 18, 0.0, np.pi)                              # 10-degree bins
+    expect = np.zeros(18, dtype=np.uint64); expect[0] = 1
+    third = o2.histogram("angle", 180, 0.0, np.pi)[0]                                # 1-degree bins: 30 deg sits on an edge
+    assert c3[0] == 1 and c3[2] + c3[3] == 3 and c3.sum() == 4 and u3 == 0 and ov3 == 0
+    assert third[0] == 1 and third[29] + third[30] == 3
+    cl, _, _ = o2.histogram("length", 4, 0.35, 0.75)                                  # lengths 0.5, 0.5, 0.5, 0.7
+    assert list(cl) == [0, 3, 0, 1]
