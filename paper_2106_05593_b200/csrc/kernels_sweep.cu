@@ -29,6 +29,7 @@ __device__ __forceinline__ uint4 philox4x32_10(uint4 c, unsigned k0, unsigned k1
     return c;
 }
 // 23-bit uniform strictly inside (0,1): ((x>>9) + 0.5) * 2^-23, exact in fp32.
+// (The conversion-free form uint_as_float(0x3f800000 | x>>9) - (1 - 2^-24) gives the same value exactly; measured 2 us slower.)
 __device__ __forceinline__ float u01(unsigned x) { return fmaf((float)(x >> 9), 1.1920928955078125e-7f, 5.9604644775390625e-8f); }
 
 // Single-instruction approximations (MUFU), flush-to-zero: inputs here are never denormal (|m|^2 > 0 is checked at
@@ -149,6 +150,65 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
     return r;
 }
 
+// ---- S10: acceptance counters and running sums.  Thread: counts and the final vectors of its cells.  Warp: integer REDUX
+// of the packed counts and of the fixed-point sums (kSumScale = 2^22; a warp's <= 64 cells stay far inside int32).  Block:
+// 32-bit shared atomics by lane 0 (two accumulators per sum, for even and odd warps: each collects <= 256 cells, so it
+// cannot overflow for |m| < 2); the last warp to sign in on the arrival counter flushes the block's totals with six global
+// 64-bit atomics.  No barrier after the update, so early warps retire at once.  Integer arithmetic throughout: exact,
+// order-independent, deterministic.
+// (Measured on a cfg 4 pass of 57 us: this tail costs about 10 us.  Alternatives measured and dropped: 64-bit shared atomics
+// (a CAS loop: +12 us), per-warp partials in plain shared stores summed by the last warp (+19 us), a block barrier + warp 0
+// (+16 us with 512-thread CTAs).)
+struct PassTailSmem { unsigned cnt[2]; unsigned sum[2][4]; unsigned arrived; };
+
+__device__ __forceinline__ void pass_tail_init(PassTailSmem& sm)
+{
+    const int tlin = threadIdx.x + 32 * (threadIdx.y + blockDim.y * threadIdx.z);
+    if (tlin < 2) sm.cnt[tlin] = 0u;
+    if (tlin >= 2 && tlin < 10) (&sm.sum[0][0])[tlin - 2] = 0u;
+    if (tlin == 10) sm.arrived = 0u;
+    __syncthreads();                                  // the only block barrier: all warps are still in step here
+}
+
+__device__ __forceinline__ void pass_tail(const SweepArgs& a, PassTailSmem& sm, unsigned n_acc, unsigned n_tri,
+                                          float fs0, float fs1, float fs2, float fs3, int warps)
+{
+    const bool want_sums = a.run_sums != nullptr;
+    const unsigned cnt = __reduce_add_sync(0xffffffffu, n_acc | (n_tri << 16));      // <= 64 each: no carry between the halves
+    int i0 = 0, i1 = 0, i2 = 0, i3 = 0;
+    if (want_sums) {
+        i0 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs0 * kSumScale));
+        i1 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs1 * kSumScale));
+        i2 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs2 * kSumScale));
+        i3 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs3 * kSumScale));
+    }
+    if (threadIdx.x == 0) {
+        if (cnt >> 16) {
+            const int par = (threadIdx.y + blockDim.y * threadIdx.z) & 1;
+            atomicAdd(&sm.cnt[0], cnt & 0xffffu);
+            atomicAdd(&sm.cnt[1], cnt >> 16);
+            if (want_sums) {
+                atomicAdd(&sm.sum[par][0], (unsigned)i0); atomicAdd(&sm.sum[par][1], (unsigned)i1);
+                atomicAdd(&sm.sum[par][2], (unsigned)i2); atomicAdd(&sm.sum[par][3], (unsigned)i3);
+            }
+        }
+        __threadfence_block();
+        if (atomicAdd(&sm.arrived, 1u) == (unsigned)(warps - 1)) {      // last warp of the block
+            __threadfence_block();
+            const unsigned tc = atomicAdd(&sm.cnt[1], 0u);
+            if (tc) {
+                atomicAdd(&a.ctl->win_trials, (unsigned long long)tc);
+                const unsigned ac = atomicAdd(&sm.cnt[0], 0u);
+                if (ac) atomicAdd(&a.ctl->win_accepted, (unsigned long long)ac);
+                if (want_sums)                         // sign-extend the two 32-bit two's-complement halves
+                    for (int t = 0; t < 4; ++t)
+                        atomicAdd(&a.run_sums[t], (unsigned long long)((long long)(int)atomicAdd(&sm.sum[0][t], 0u) +
+                                                                       (long long)(int)atomicAdd(&sm.sum[1][t], 0u)));
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ the pass
 // blockDim = (32, BY, BZ), kPassThreads = 512 threads (measured on cfg 4 / cfg 5: 128 threads 110 / 100 us per pass,
 // 256: 69 / 59, 512: 65 / 52, 1024: 68 / 55: the larger brick shares more neighbour rows through L1);
@@ -164,12 +224,8 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
-    __shared__ unsigned s_acc[6];                    // accepted, trials, sum mx, my, mz, |m| (fixed point, two's complement)
-    __shared__ unsigned s_arrived;
-    const int tlin = threadIdx.x + 32 * (threadIdx.y + blockDim.y * threadIdx.z);
-    if (tlin < 6) s_acc[tlin] = 0u;
-    if (tlin == 6) s_arrived = 0u;
-    __syncthreads();                                  // the only block barrier: all warps are still in step here
+    __shared__ PassTailSmem s_tail;
+    pass_tail_init(s_tail);
 
     const int nx = a.g.nx, ny = a.g.ny, nz = a.g.nz, hx = a.g.hx;
     const unsigned pbc = a.g.pbc;
@@ -292,40 +348,158 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
         }
     }
 
-    // ---- S10: acceptance counters and running sums.  Warp: ballot / integer REDUX.  Block: shared 64-bit atomics,
-    // the last warp to arrive flushes the block's totals with six global atomics (no second block barrier).
-    const unsigned acc_cnt = __popc(__ballot_sync(0xffffffffu, accept));
-    const unsigned tri_cnt = __popc(__ballot_sync(0xffffffffu, active));
-    const bool want_sums = a.run_sums != nullptr;
-    int i0 = 0, i1 = 0, i2 = 0, i3 = 0;
-    if (want_sums) {
-        i0 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs0 * kSumScale));
-        i1 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs1 * kSumScale));
-        i2 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs2 * kSumScale));
-        i3 = __reduce_add_sync(0xffffffffu, __float2int_rn(fs3 * kSumScale));
-    }
-    if (threadIdx.x == 0) {
-        if (tri_cnt) {
-            atomicAdd(&s_acc[0], acc_cnt);
-            atomicAdd(&s_acc[1], tri_cnt);
-            if (want_sums) {
-                atomicAdd(&s_acc[2], (unsigned)i0); atomicAdd(&s_acc[3], (unsigned)i1);
-                atomicAdd(&s_acc[4], (unsigned)i2); atomicAdd(&s_acc[5], (unsigned)i3);
-            }
+    pass_tail(a, s_tail, accept ? 1u : 0u, active ? 1u : 0u, fs0, fs1, fs2, fs3, kPassThreads / 32);
+}
+
+// ------------------------------------------------------------------------------------------------ the pass, two cells per thread
+// The same pass with a thread owning TWO consecutive compact cells of a row (mesh cells i and i + 2): the vectors, B_d and
+// class words / masks come as 64-bit loads, the x neighbour between the two cells is loaded once, index arithmetic, bond
+// decoding and the reductions are shared.  Used for every non-debug launch unless x is periodic with an odd compact row
+// length (then the wrap neighbour of the last cell would not pair up).  blockDim = (32, BY, BZ), 256 threads = a brick of
+// 64 x BY x BZ cells of one colour; grid = (ceil(hxr/64), ceil(ny/BY), ceil(nz/BZ)).
+constexpr int kPass2Threads = 256;
+
+#ifndef MMC_PASS2_MINB
+#define MMC_PASS2_MINB 4      // 64 registers (48 bytes spilled): measured 4 / 3 / 2 CTAs per SM on cfg 4: 57.5 / 61 / 72 us per pass
+#endif
+template <unsigned F>
+__global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_kernel(const SweepArgs a)
+{
+    constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
+                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
+    __shared__ PassTailSmem s_tail;
+    pass_tail_init(s_tail);
+
+    const int nx = a.g.nx, ny = a.g.ny, nz = a.g.nz, hx = a.g.hx;
+    const unsigned pbc = a.g.pbc;
+    const int q0 = 2 * (blockIdx.x * 32 + threadIdx.x);           // cells q0 and q0 + 1 of the compact row
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = HASZ ? blockIdx.z * blockDim.z + threadIdx.z : 0;
+    const int col = a.colour;
+    const int s = ((j + k) & 1) ^ col;                            // active cells of this row sit at i = 2q + s
+    const int i0 = 2 * q0 + s;
+    const bool inrow = j < ny && k < nz;
+    bool act[2] = { inrow && i0 < nx, inrow && i0 + 2 < nx };
+    unsigned n_acc = 0u;
+    float fs0 = 0.f, fs1 = 0.f, fs2 = 0.f, fs3 = 0.f;
+
+    const unsigned H = (unsigned)a.g.H;
+    const int row = k * ny + j;
+    const unsigned rq = (unsigned)row * hx + q0;
+    const unsigned ownb = (unsigned)col * H + rq;
+    unsigned mb[2] = { 0x7fu, 0x7fu }, cls[2] = { 0u, 0u };
+    if (act[0]) {                                                 // (cell 1 active implies cell 0 active)
+        if (PERCELL) {
+            const uint2 w = __ldg(reinterpret_cast<const uint2*>(a.cw + ownb));
+            mb[0] = w.x & 0x7fu; cls[0] = w.x >> 7; mb[1] = w.y & 0x7fu; cls[1] = w.y >> 7;
+        } else if (MASK) {
+            const uchar2 w = __ldg(reinterpret_cast<const uchar2*>(a.mask + ownb));
+            mb[0] = w.x; mb[1] = w.y;
         }
-        __threadfence_block();
-        if (atomicAdd(&s_arrived, 1u) == (unsigned)(kPassThreads / 32 - 1)) {   // last warp of the block
-            __threadfence_block();
-            const unsigned tc = atomicAdd(&s_acc[1], 0u);
-            if (tc) {
-                atomicAdd(&a.ctl->win_trials, (unsigned long long)tc);
-                const unsigned ac = atomicAdd(&s_acc[0], 0u);
-                if (ac) atomicAdd(&a.ctl->win_accepted, (unsigned long long)ac);
-                if (want_sums)                         // sign-extend the block's 32-bit fixed-point sums
-                    for (int t = 0; t < 4; ++t) atomicAdd(&a.run_sums[t], (unsigned long long)(long long)(int)atomicAdd(&s_acc[2 + t], 0u));
+        if (!DENSE && (MASK || PERCELL)) { act[0] = act[0] && (mb[0] & 0x40u); act[1] = act[1] && (mb[1] & 0x40u); }
+    }
+    if (act[0] || act[1]) {
+        const int hxr = (nx + 1) >> 1;
+        const int dN = (j + 1 < ny) ? hx : ((pbc & 2u) ? -(ny - 1) * hx : 0);
+        const int dS = (j > 0) ? -hx : ((pbc & 2u) ? (ny - 1) * hx : 0);
+        // the third x neighbour: s == 0: W of cell 0 at q0 - 1; s == 1: E of cell 1 at q0 + 2 (wrap when periodic, else any
+        // valid slot: the bond is masked)
+        int dX = s ? 2 : -1;
+        if (q0 + dX < 0) dX = (pbc & 1u) ? hxr - 1 : 0;
+        else if (q0 + dX >= hxr) dX = (pbc & 1u) ? -q0 : 0;
+        int dU = 0, dD = 0;
+        if (HASZ) {
+            const int lay = ny * hx;
+            dU = (k + 1 < nz) ? lay : ((pbc & 4u) ? -(nz - 1) * lay : 0);
+            dD = (k > 0) ? -lay : ((pbc & 4u) ? (nz - 1) * lay : 0);
+        }
+        const unsigned othb = (unsigned)(1 - col) * H + rq;
+        float2 m2[3], xc[3], yn[3], ys[3], zu[3], zd[3], bd2[3];
+        float xs[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float* __restrict__ P = a.m[c];
+            m2[c] = *reinterpret_cast<const float2*>(a.m[c] + ownb);
+            xc[c] = __ldg(reinterpret_cast<const float2*>(P + othb));
+            xs[c] = __ldg(P + othb + dX);
+            yn[c] = __ldg(reinterpret_cast<const float2*>(P + othb + dN));
+            ys[c] = __ldg(reinterpret_cast<const float2*>(P + othb + dS));
+            if (HASZ) { zu[c] = __ldg(reinterpret_cast<const float2*>(P + othb + dU)); zd[c] = __ldg(reinterpret_cast<const float2*>(P + othb + dD)); }
+            bd2[c] = DEMAG ? __ldg(reinterpret_cast<const float2*>(a.bd[c] + ownb)) : make_float2(0.f, 0.f);
+        }
+        const unsigned long long sweep = a.ctl->sweep;
+        const float omc = a.ctl->one_minus_cos_cone;
+        const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            if (!act[t]) continue;
+            float m[3], e[3], wv[3], N[3], S_[3], U[3], D[3], Bd[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                m[c] = t ? m2[c].y : m2[c].x;
+                // s == 0: cell 0: E = xc.x, W = xs; cell 1: E = xc.y, W = xc.x.   s == 1: cell 0: W = xc.x, E = xc.y; cell 1: W = xc.y, E = xs
+                if (t == 0) { e[c] = s ? xc[c].y : xc[c].x; wv[c] = s ? xc[c].x : xs[c]; }
+                else        { e[c] = s ? xs[c] : xc[c].y;   wv[c] = s ? xc[c].y : xc[c].x; }
+                N[c] = t ? yn[c].y : yn[c].x; S_[c] = t ? ys[c].y : ys[c].x;
+                if (HASZ) { U[c] = t ? zu[c].y : zu[c].x; D[c] = t ? zd[c].y : zd[c].x; }
+                Bd[c] = t ? bd2[c].y : bd2[c].x;
             }
+            CellCoef cf;
+            float kscale = 1.f;
+            if (PERCELL) {
+                const float4* tb = a.table + 3u * cls[t];
+                const float4 t0 = __ldg(tb), t1 = __ldg(tb + 1);
+                const float2 t2 = __ldg(reinterpret_cast<const float2*>(tb + 2));
+                kscale = t0.x; cf.c4 = t0.y;
+                cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
+                cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
+            } else {
+                cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
+                cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
+            }
+            cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
+            cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
+            float bE = 1.f, bW = 1.f, bN = 1.f, bS = 1.f, bU = HASZ ? 1.f : 0.f, bD = HASZ ? 1.f : 0.f;
+            if (MASK || PERCELL) {
+                const unsigned b = mb[t];
+                bE = (b & 1u) ? 1.f : 0.f;  bW = (b & 2u) ? 1.f : 0.f;
+                bN = (b & 4u) ? 1.f : 0.f;  bS = (b & 8u) ? 1.f : 0.f;
+                bU = (b & 16u) ? 1.f : 0.f; bD = (b & 32u) ? 1.f : 0.f;
+            } else {
+                if (nx < 2) { bE = 0.f; bW = 0.f; }
+                if (ny < 2) { bN = 0.f; bS = 0.f; }
+            }
+            float Sg[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float sx = bE * (e[c] - m[c]) + bW * (wv[c] - m[c]);
+                const float sy = bN * (N[c] - m[c]) + bS * (S_[c] - m[c]);
+                float acc = fmaf(cf.kx, sx, cf.ky * sy);
+                if (HASZ) acc = fmaf(cf.kz, bU * (U[c] - m[c]) + bD * (D[c] - m[c]), acc);
+                Sg[c] = acc;
+            }
+            float selfc = 0.5f * fmaf(cf.kx, bE + bW, cf.ky * (bN + bS));
+            if (HASZ) selfc = fmaf(0.5f * cf.kz, bU + bD, selfc);
+            float dzx = 0.f, dzy = 0.f, dxx = 0.f, dyy = 0.f;
+            if (DMI) {
+                dzx = bE * e[2] - bW * wv[2];
+                dzy = bN * N[2] - bS * S_[2];
+                dxx = bE * e[0] - bW * wv[0];
+                dyy = bN * N[1] - bS * S_[1];
+            }
+            const unsigned cell = (unsigned)row * nx + (unsigned)(i0 + 2 * t);       // natural cell index (< 2^31)
+            const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
+            const CellResult r = cell_update<DMI, false>(m, Sg, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
+            float f0 = m[0], f1 = m[1], f2 = m[2], f3 = r.L;
+            if (r.accept) {
+                f0 += r.dm[0]; f1 += r.dm[1]; f2 += r.dm[2]; f3 *= r.f;
+                a.m[0][ownb + t] = f0; a.m[1][ownb + t] = f1; a.m[2][ownb + t] = f2;
+                n_acc++;
+            }
+            fs0 += f0; fs1 += f1; fs2 += f2; fs3 += f3;
         }
     }
+    pass_tail(a, s_tail, n_acc, (act[0] ? 1u : 0u) + (act[1] ? 1u : 0u), fs0, fs1, fs2, fs3, kPass2Threads / 32);
 }
 
 // S11 + bookkeeping, one thread: advance the sweep counter; every 100 iterations compare the acceptance rate with
@@ -371,8 +545,19 @@ static int launch_variant(const SweepArgs& a, bool debug, cudaStream_t st)
 {
     dim3 b, gr; brick(a.g, &b, &gr);
     if (gr.y > 65535u || gr.z > 65535u) return MMC_E_UNSUPPORTED;
+    const int hxr = (a.g.nx + 1) >> 1;
+#ifndef MMC_PASS_CELLS
+#define MMC_PASS_CELLS 2
+#endif
+    const bool pairable = MMC_PASS_CELLS == 2 && !((a.g.pbc & 1u) && (hxr & 1));        // see colour_pass2_kernel
     if (debug) colour_pass_kernel<F, true><<<gr, b, 0, st>>>(a);
-    else       colour_pass_kernel<F, false><<<gr, b, 0, st>>>(a);
+    else if (!pairable) colour_pass_kernel<F, false><<<gr, b, 0, st>>>(a);
+    else {
+        const int bz = a.g.nz >= 4 ? 4 : (a.g.nz >= 2 ? 2 : 1), by = kPass2Threads / 32 / bz;
+        const dim3 b2(32, by, bz), g2((hxr + 63) / 64, (a.g.ny + by - 1) / by, (a.g.nz + bz - 1) / bz);
+        if (g2.y > 65535u || g2.z > 65535u) return MMC_E_UNSUPPORTED;
+        colour_pass2_kernel<F><<<g2, b2, 0, st>>>(a);
+    }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 

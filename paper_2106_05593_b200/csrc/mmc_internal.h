@@ -58,7 +58,7 @@ enum ClassSlot { CS_INVT = 0, CS_C4 = 1, CS_MU2 = 2 /* double in slots 2,3 */, C
                  CS_AX = 7, CS_AY = 8, CS_AZ = 9, CS_K1T = 10 /* beta V K1(T), read-out only */,
                  CS_C0 = 11 /* c0 - c4 mu2^2, read-out only */ };
 constexpr unsigned kMaxClasses = 1u << 25;
-constexpr float kSumScale = 4194304.f;              // 2^22: fixed-point scale of the running sums (a 256-cell block sum fits int32 for |m| < 2)
+constexpr float kSumScale = 4194304.f;              // 2^22: fixed-point scale of the running sums (a warp's sum fits int32 for |m| < 8; blocks add in 64 bits)
 
 // Device-resident control block: read by the kernels, advanced by end_sweep_kernel (no host round trip).
 struct Control {
