@@ -54,6 +54,7 @@ class _Problem(C.Structure):
         ("A0", C.c_double), ("D0", C.c_double), ("Bext", C.c_double * 3),
         ("bdx", C.c_void_p), ("bdy", C.c_void_p), ("bdz", C.c_void_p),
         ("one_minus_cos_cone", C.c_double), ("seed", C.c_uint64),
+        ("K1cT", C.c_void_p), ("K2cT", C.c_void_p), ("cub", C.c_void_p),
     ]
 
 
@@ -205,6 +206,19 @@ class Material:
     Ms0: float = 0.0; A0: float = 0.0; K1: float = 0.0
     ax: float = 0.0; ay: float = 0.0; az: float = 1.0
     D0: float = 0.0; Tc: float = 1.0; mu_atom: float = MUB
+    # cubic anisotropy, Eq. (12): 4th and 6th order constants (J/m^3) and two of the cubic axes (the third is their cross
+    # product; orthonormalised by Gram-Schmidt)
+    K1c: float = 0.0; K2c: float = 0.0
+    c1x: float = 1.0; c1y: float = 0.0; c1z: float = 0.0
+    c2x: float = 0.0; c2y: float = 1.0; c2z: float = 0.0
+
+
+def cubic_axes(r):
+    """The three orthonormal cubic axes of a region record as 9 numbers: e1 = c1/|c1|, e2 = the part of c2 orthogonal
+    to e1, normalised, e3 = e1 x e2."""
+    e1 = np.array([r.c1x, r.c1y, r.c1z], dtype=np.float64); e1 /= np.linalg.norm(e1)
+    e2 = np.array([r.c2x, r.c2y, r.c2z], dtype=np.float64); e2 -= (e2 @ e1) * e1; e2 /= np.linalg.norm(e2)
+    return np.concatenate([e1, e2, np.cross(e1, e2)])
 
 
 class OracleMMC:
@@ -233,6 +247,7 @@ class OracleMMC:
         self.demag_updates = 1
         self.demag_r_near = 32
         self._demag = None
+        self.has_cubic = False
         self.seed = 0
         self.sweep = 0
         self.accepted = 0; self.trials = 0
@@ -315,6 +330,17 @@ class OracleMMC:
             cls["me"][q] = th["me"]
         for k in names:
             arr[k] = np.ascontiguousarray(cls[k][inv])
+        # cubic anisotropy (Eq. (12); K(T) = K me^(l(l+1)/2), l = 4 and 6)
+        self.has_cubic = any(r.Ms0 > 0 and (r.K1c != 0 or r.K2c != 0) for r in self.regions)
+        if self.has_cubic:
+            k1 = np.zeros(uniq.size); k2 = np.zeros(uniq.size); ax9 = np.zeros((uniq.size, 9))
+            for q in range(uniq.size):
+                r = self.regions[reg[first[q]]]
+                ax9[q] = cubic_axes(r)
+                if r.Ms0 > 0:
+                    k1[q] = r.K1c * cls["me"][q] ** 10; k2[q] = r.K2c * cls["me"][q] ** 21
+            arr["K1cT"] = np.ascontiguousarray(k1[inv]); arr["K2cT"] = np.ascontiguousarray(k2[inv])
+            arr["cub"] = np.ascontiguousarray(ax9[inv])
         self.coef = arr
         self._dirty = False
 
@@ -336,6 +362,10 @@ class OracleMMC:
             p.bdx = p.bdy = p.bdz = None
         p.one_minus_cos_cone = 2.0 * np.sin(0.5 * np.deg2rad(self.cone_deg)) ** 2
         p.seed = self.seed
+        if self.has_cubic:
+            p.K1cT, p.K2cT, p.cub = (self.coef[k].ctypes.data for k in ("K1cT", "K2cT", "cub"))
+        else:
+            p.K1cT = p.K2cT = p.cub = None
         return p
 
     # -- demag ----------------------------------------------------------------------------

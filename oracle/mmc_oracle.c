@@ -154,7 +154,22 @@ typedef struct {
     const double *bdx, *bdy, *bdz;/* N each, frozen B_d = mu0 H_d (tesla); NULL = no demag */
     double one_minus_cos_cone;    /* 1 - cos(theta_c) */
     uint64_t seed;
+    /* cubic anisotropy, Eq. (12): NULL = none */
+    const double *K1cT, *K2cT;    /* N, K1c me^10 and K2c me^21 (me^(l(l+1)/2), l = 4, 6), 0 for T >= Tc */
+    const double *cub;            /* 9N: the three orthonormal cubic axes of the cell, cub[9c + 3a + q] */
 } orc_problem;
+
+/* Eq. (12): alpha^2 beta^2 + alpha^2 gamma^2 + beta^2 gamma^2 and alpha^2 beta^2 gamma^2 of the DIRECTION of v          */
+/* ("direction cosines of the magnetization vector") with respect to the cell's cubic axes.                */
+static void orc_cubic_invariants(const double *ax9, const double v[3], double *c1, double *c2)
+{
+    double L = sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
+    double a = (v[0] * ax9[0] + v[1] * ax9[1] + v[2] * ax9[2]) / L;
+    double b = (v[0] * ax9[3] + v[1] * ax9[4] + v[2] * ax9[5]) / L;
+    double g = (v[0] * ax9[6] + v[1] * ax9[7] + v[2] * ax9[8]) / L;
+    *c1 = a * a * b * b + a * a * g * g + b * b * g * g;
+    *c2 = a * a * b * b * g * g;
+}
 
 static inline int64_t orc_idx(const orc_problem *p, int i, int j, int k)
 {
@@ -270,6 +285,14 @@ void orc_cell_dF(const orc_problem *p, const double *mx, const double *my, const
     double dme = dm[0] * e[0] + dm[1] * e[1] + dm[2] * e[2];
     double sme = (2 * m[0] + dm[0]) * e[0] + (2 * m[1] + dm[1]) * e[1] + (2 * m[2] + dm[2]) * e[2];
     terms[1] = -beta * V * p->Kq[c] * dme * sme;
+    /* cubic anisotropy, Eq. (12), both terms times V: the plain difference of the energy of the trial and the current direction */
+    if (p->cub) {
+        double mp[3] = { m[0] + dm[0], m[1] + dm[1], m[2] + dm[2] };
+        double a1, a2, b1, b2;
+        orc_cubic_invariants(p->cub + 9 * c, m, &a1, &a2);
+        orc_cubic_invariants(p->cub + 9 * c, mp, &b1, &b2);
+        terms[1] += beta * V * (p->K1cT[c] * (b1 - a1) + p->K2cT[c] * (b2 - a2));
+    }
     /* Zeeman */
     double bvm = beta * V * p->Ms0[c];
     terms[2] = -bvm * (dm[0] * p->Bext[0] + dm[1] * p->Bext[1] + dm[2] * p->Bext[2]);
@@ -398,6 +421,11 @@ void orc_observables(const orc_problem *p, const double *mx, const double *my, c
         Edmi += -p->D0 * V * (m[0] * G[0] + m[1] * G[1] + m[2] * G[2]);
         double me_ = m[0] * p->ax[c] + m[1] * p->ay[c] + m[2] * p->az[c];
         Ean += V * (p->K1T[c] - p->Kq[c] * me_ * me_);
+        if (p->cub) {
+            double c1, c2;
+            orc_cubic_invariants(p->cub + 9 * c, m, &c1, &c2);
+            Ean += V * (p->K1cT[c] * c1 + p->K2cT[c] * c2);
+        }
         Ezee += -V * p->Ms0[c] * (m[0] * p->Bext[0] + m[1] * p->Bext[1] + m[2] * p->Bext[2]);
         if (p->bdx) Edem += -0.5 * V * p->Ms0[c] * (m[0] * p->bdx[c] + m[1] * p->bdy[c] + m[2] * p->bdz[c]);
         Elong += (1.0 / p->beta[c]) * (p->c4[c] * l2 * l2 + p->c2[c] * l2 + p->c0[c]);

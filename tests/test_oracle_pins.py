@@ -168,7 +168,8 @@ def test_local_dF_equals_global_dE_bruteforce(shape, pbc):
     nx, ny, nz = shape; N = nx * ny * nz
     rng = np.random.default_rng(11 + N + pbc)
     mats = [O.Material(), O.Material(Ms0=8e5, A0=1.3e-11, K1=5e5, ax=0.3, ay=-0.2, az=0.9, D0=2.5e-3, Tc=870.0),
-            O.Material(Ms0=6e5, A0=1.3e-11, K1=-2e5, ax=1.0, ay=0.0, az=0.0, D0=2.5e-3, Tc=500.0)]
+            O.Material(Ms0=6e5, A0=1.3e-11, K1=-2e5, ax=1.0, ay=0.0, az=0.0, D0=2.5e-3, Tc=500.0,
+                       K1c=4.8e4, K2c=-1e4, c1x=1.0, c1y=0.4, c1z=-0.2, c2x=0.1, c2y=1.0, c2z=0.3)]    # + cubic, Eq. (12)
     reg = rng.integers(0, 3, N).astype(np.int32); reg[0] = 1
     Tcell = rng.uniform(250, 650, N).astype(np.float32)
     for inter in (1, 0):
@@ -508,3 +509,85 @@ def test_histograms_against_numpy_and_closed_forms():
     assert third[0] == 1 and third[29] + third[30] == 3
     cl, _, _ = o2.histogram("length", 4, 0.35, 0.75)                                  # lengths 0.5, 0.5, 0.5, 0.7
     assert list(cl) == [0, 3, 0, 1]
+
+
+# ------------------------------------------------------------------------------------------------ cubic anisotropy, Eq. (12)
+def _cubic_cell(K1c, K2c, axes=((1, 0, 0), (0, 1, 0)), T=300.0, Tc=1044.0):
+    s = O.OracleMMC(2, 2, 1, 5e-9, 5e-9, 5e-9, 0, store_fp32=False)
+    (a, b) = axes
+    s.set_material([O.Material(Ms0=1.71e6, A0=0.0, Tc=Tc, K1c=K1c, K2c=K2c, c1x=a[0], c1y=a[1], c1z=a[2], c2x=b[0], c2y=b[1], c2z=b[2])], None)
+    s.set_temperature(T, None)
+    return s
+
+
+def test_cubic_anisotropy_textbook_values_symmetry_and_scaling():
+    """Eq. (12) against what the mathematics fixes: the textbook energies of the principal directions
+    (<100>: 0, <110>: K1/4, <111>: K1/3 + K2/27), invariance under the cubic group and under a common rotation of axes and
+    vector, independence of |m| ("direction cosines"), the me^10 / me^21 temperature scaling of PAPER.md:143, and
+    local dF == difference of the read-out energy."""
+    V = (5e-9) ** 3
+    me = O.me_of_T(300.0, 1044.0)
+    for K1c, K2c in ((4.8e4, 0.0), (0.0, -1e4), (4.8e4, -1e4)):
+        s = _cubic_cell(K1c, K2c)
+        def E(v):
+            s.set_m(*[np.full(4, x, dtype=np.float64) for x in v]); return s.observables()["E_an"] / 4
+        k1, k2 = K1c * me ** 10, K2c * me ** 21
+        assert E((0.7, 0, 0)) == pytest.approx(0.0, abs=1e-40)
+        assert E((0.5, 0.5, 0)) == pytest.approx(V * k1 / 4, rel=1e-12)
+        assert E((0.3, 0.3, 0.3)) == pytest.approx(V * (k1 / 3 + k2 / 27), rel=1e-12)
+        v = np.array([0.31, -0.52, 0.77])
+        e0 = E(v)
+        assert E(2.5 * v) == pytest.approx(e0, rel=1e-12)                         # direction only
+        for perm in ((1, 0, 2), (2, 1, 0), (1, 2, 0)):
+            for sg in ((1, 1, 1), (-1, 1, 1), (1, -1, -1)):
+                assert E(np.array(sg) * v[list(perm)]) == pytest.approx(e0, rel=1e-12)
+    # common rotation of the axes and the vector
+    rng = np.random.default_rng(3)
+    Q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+    s0 = _cubic_cell(4.8e4, -1e4); s1 = _cubic_cell(4.8e4, -1e4, axes=(Q[:, 0], Q[:, 1] + 0.3 * Q[:, 0]))   # Gram-Schmidt removes the 0.3
+    v = np.array([0.31, -0.52, 0.77]); w = Q @ v * np.linalg.det(np.column_stack([Q[:, 0], Q[:, 1], np.cross(Q[:, 0], Q[:, 1])]))
+    s0.set_m(*[np.full(4, x) for x in v]); s1.set_m(*[np.full(4, x) for x in (Q @ v)])
+    assert s1.observables()["E_an"] == pytest.approx(s0.observables()["E_an"], rel=1e-12)
+    # temperature scaling (PAPER.md:143): K1 ~ me^10, K2 ~ me^21; zero at and above Tc
+    for K1c, K2c, power in ((4.8e4, 0.0, 10), (0.0, -1e4, 21)):
+        Es = []
+        for T in (300.0, 800.0):
+            s = _cubic_cell(K1c, K2c, T=T); s.set_m(*[np.full(4, x) for x in (0.3, 0.3, 0.3)]); Es.append(s.observables()["E_an"])
+        assert Es[1] / Es[0] == pytest.approx((O.me_of_T(800.0, 1044.0) / me) ** power, rel=1e-10)
+    s = _cubic_cell(4.8e4, -1e4, T=1044.0); s.set_m(*[np.full(4, x) for x in (0.3, 0.3, 0.3)])
+    assert s.observables()["E_an"] == 0.0
+    # local dF = difference of the read-out, in units of kB T
+    s = _cubic_cell(4.8e4, -1e4)
+    m0 = np.array([0.5, 0.2, -0.4]); s.set_m(*[np.full(4, x) for x in m0])
+    dm = np.array([-0.1, 0.25, 0.05])
+    eb = s.observables()["E_an"]; t = s.cell_dF(1, 0, 0, dm)
+    s.m[0][1] += dm[0]; s.m[1][1] += dm[1]; s.m[2][1] += dm[2]
+    assert t[1] * KB * 300.0 == pytest.approx(s.observables()["E_an"] - eb, rel=1e-10)
+
+
+def test_cubic_anisotropy_single_cell_distribution():
+    """Fixed-length cells with cubic anisotropy only sample exp(-V K1(T) c1(n) / kT) uniformly in solid angle (Eq. (6),
+    reading G6): <c1> against a plain quadrature over the sphere; K1 > 0 favours <100>, so <c1> lies below the isotropic 1/5."""
+    T, Tc, L = 300.0, 1044.0, 0.9
+    V = (8e-9) ** 3
+    s = O.OracleMMC(24, 24, 1, 8e-9, 8e-9, 8e-9, 0b011, store_fp32=False)
+    s.set_material([O.Material(Ms0=1.71e6, A0=0.0, Tc=Tc, K1c=2.0e5, K2c=0.0)], None)
+    s.set_temperature(T, None); s.set_move(40.0, 0.0, False); s.set_seed(12)
+    rng = np.random.default_rng(8)
+    v = rng.normal(size=(3, 576)); v /= np.linalg.norm(v, axis=0)
+    s.set_m(*(L * v))
+    s.run(300)
+    acc = 0.0; n = 0
+    for _ in range(120):
+        s.run(5)
+        a, b, g = (s.m[q] / L for q in range(3))
+        acc += (a * a * b * b + a * a * g * g + b * b * g * g).mean(); n += 1
+    kappa = V * 2.0e5 * O.me_of_T(T, Tc) ** 10 / (KB * T)
+    th = np.linspace(0, np.pi, 1201); ph = np.linspace(0, 2 * np.pi, 2401)
+    TH, PH = np.meshgrid(th, ph, indexing="ij")
+    x, y, z = np.sin(TH) * np.cos(PH), np.sin(TH) * np.sin(PH), np.cos(TH)
+    c1 = x * x * y * y + x * x * z * z + y * y * z * z
+    w = np.exp(-kappa * c1) * np.sin(TH)
+    expect = np.trapezoid(np.trapezoid(c1 * w, ph, axis=1), th) / np.trapezoid(np.trapezoid(w, ph, axis=1), th)
+    assert kappa > 1.0 and expect < 0.19
+    assert acc / n == pytest.approx(expect, rel=2e-2)
