@@ -59,7 +59,7 @@ def demag_kernel_bytes(wl, ms0_per_cell):
     kernel transforms in place (only the ny kept rows are ever stored); tensor = 4 (one layer) or 6 real arrays over
     [Pz/2+1][Px/2+1][Py]."""
     Px, Py = _pow2_at_least(wl.nx, 2), _pow2_at_least(wl.ny, 1)
-    Pz = 2 * wl.nz - 1 if 1 < wl.nz <= 8 else _pow2_at_least(wl.nz, 1)   # register-resident path: shortest linear length
+    Pz = 2 * wl.nz - 1 if 1 < wl.nz <= 16 else _pow2_at_least(wl.nz, 1)   # register-resident path: shortest linear length
     Cx = Px // 2 + 1
     T = 3 * Pz * Cx * wl.ny * 8
     tensor = (4 if wl.nz == 1 else 6) * (Pz // 2 + 1) * Cx * Py * 4
@@ -161,7 +161,8 @@ def _peaks():
 def _workload(cfg: int, small: bool):
     import workloads as W
     if small:
-        kw = {1: {}, 2: dict(nx=64, ny=64), 3: dict(nx=64, ny=64), 4: dict(nx=64, ny=64, nz=4), 5: dict(nx=140, ny=140)}[cfg]
+        kw = {1: {}, 2: dict(nx=64, ny=64), 3: dict(nx=64, ny=64), 4: dict(nx=64, ny=64, nz=4), 5: dict(nx=140, ny=140),
+              6: dict(nx=64, ny=64, nz=4)}[cfg]
         return W.make(cfg, **kw)
     return W.make(cfg)
 
@@ -170,7 +171,8 @@ def _workload(cfg: int, small: bool):
 def oracle_sample(cfg: int):
     """Bounded sample of config `cfg` for the CPU legs: same recipe, reduced mesh."""
     import workloads as W
-    kw = {1: {}, 2: {}, 3: dict(nx=256, ny=256), 4: dict(nx=256, ny=256, nz=4), 5: dict(nx=560, ny=560)}[cfg]
+    kw = {1: {}, 2: {}, 3: dict(nx=256, ny=256), 4: dict(nx=256, ny=256, nz=4), 5: dict(nx=560, ny=560),
+          6: dict(nx=128, ny=128, nz=10)}[cfg]
     return W.make(cfg, **kw), kw
 
 
@@ -357,7 +359,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5],
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5, 6],
                     help="BASELINE.json config (default 4: the largest fully magnetic mesh, 1024x1024x4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--small", action="store_true", help="reduced mesh (debugging only; not a bench number)")

@@ -50,12 +50,20 @@ typedef struct mmc_ctx mmc_ctx;   /* opaque, owned by the library */
  * A0: exchange stiffness at T=0 (A(T) = A0 me^2); K1 + unit axis (ax,ay,az): uniaxial
  * anisotropy constant at T=0 (K1(T) = K1 me^3, Eq. (11)); D0: interfacial DMI at T=0
  * (D(T) = D0 me^2, Eq. (15)); Tc: Curie temperature; mu_atom: atomic moment in J/T
- * (Eq. (8)).  A0 and D0 must be equal in all non-empty regions (MMC_E_UNSUPPORTED). */
-typedef struct { double Ms0, A0, K1, ax, ay, az, D0, Tc, mu_atom; } mmc_material;
+ * (Eq. (8)).  A0 and D0 must be equal in all non-empty regions (MMC_E_UNSUPPORTED).
+ * Cubic anisotropy, Eq. (12): K1c, K2c = 4th / 6th order constants at T = 0 in J/m^3,
+ * F = V K1c(T) [a^2 b^2 + a^2 g^2 + b^2 g^2] + V K2c(T) a^2 b^2 g^2 with a, b, g the direction cosines of m with respect
+ * to the cubic axes and K(T) = K me^(l(l+1)/2), l = 4 and 6; zero at and above Tc.  (c1x,c1y,c1z) and
+ * (c2x,c2y,c2z) give two of the axes (orthonormalised by Gram-Schmidt; the third is their cross product); they are
+ * ignored when K1c = K2c = 0 and must not be parallel otherwise. */
+typedef struct {
+    double Ms0, A0, K1, ax, ay, az, D0, Tc, mu_atom;
+    double K1c, K2c, c1x, c1y, c1z, c2x, c2y, c2z;
+} mmc_material;
 
 /* Read-out (PAPER.md:100 acceptance rate; PAPER.md:135 average magnetisation; Appendix B energies).
  * Means are over non-empty cells.  Energies in joule with pair terms counted once:
- * E_ex = sum_bonds (A0 V/h^2)|m_i-m_j|^2, E_an = sum V[K1(T) - K1 me (m.e)^2], E_zee = -V sum Ms0 m.B_ext,
+ * E_ex = sum_bonds (A0 V/h^2)|m_i-m_j|^2, E_an = sum V[K1(T) - K1 me (m.e)^2] + the cubic energy of Eq. (12), E_zee = -V sum Ms0 m.B_ext,
  * E_dmi = -D0 V sum m.G, E_demag = -(V/2) sum Ms0 m.B_d (B_d of the current state), E_long = sum kB T F_l. */
 typedef struct {
     double   mean_m[3], mean_len;

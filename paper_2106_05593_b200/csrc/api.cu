@@ -179,6 +179,21 @@ int ensure_setup(mmc_ctx* c)
         out[CS_AX] = (float)ex; out[CS_AY] = (float)ey; out[CS_AZ] = (float)ez;
         out[CS_K1T] = (float)(beta * V * mt.K1 * k.th.me * k.th.me * k.th.me);
         out[CS_C0] = (float)((k.th.me > 0 || k.th.mu2 == 0) ? 0.0 : -k.th.c4 * k.th.mu2 * k.th.mu2);
+        // cubic anisotropy: K(T) = K me^(l(l+1)/2), l = 4, 6; axes by Gram-Schmidt, e3 = e1 x e2
+        out[CS_BK1C] = (float)(beta * V * mt.K1c * std::pow(k.th.me, 10.0));
+        out[CS_BK2C] = (float)(beta * V * mt.K2c * std::pow(k.th.me, 21.0));
+        double e1[3] = { mt.c1x, mt.c1y, mt.c1z }, e2[3] = { mt.c2x, mt.c2y, mt.c2z };
+        double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
+        if (!(n1 > 0)) { e1[0] = 1; e1[1] = e1[2] = 0; n1 = 1; }
+        for (int q = 0; q < 3; ++q) e1[q] /= n1;
+        const double pr = e2[0] * e1[0] + e2[1] * e1[1] + e2[2] * e1[2];
+        for (int q = 0; q < 3; ++q) e2[q] -= pr * e1[q];
+        double n2 = std::sqrt(e2[0] * e2[0] + e2[1] * e2[1] + e2[2] * e2[2]);
+        if (!(n2 > 1e-12)) { const int a = std::fabs(e1[0]) < 0.9 ? 0 : 1; e2[0] = e2[1] = e2[2] = 0; e2[a] = 1;   // unused axes: any frame
+            const double p2 = e1[a]; for (int q = 0; q < 3; ++q) e2[q] -= p2 * e1[q]; n2 = std::sqrt(e2[0] * e2[0] + e2[1] * e2[1] + e2[2] * e2[2]); }
+        for (int q = 0; q < 3; ++q) e2[q] /= n2;
+        const double e3[3] = { e1[1] * e2[2] - e1[2] * e2[1], e1[2] * e2[0] - e1[0] * e2[2], e1[0] * e2[1] - e1[1] * e2[0] };
+        for (int q = 0; q < 3; ++q) { out[CS_CUB + q] = (float)e1[q]; out[CS_CUB + 3 + q] = (float)e2[q]; out[CS_CUB + 6 + q] = (float)e3[q]; }
     };
     c->n_classes = classes.size();
     if (!c->percell) {
@@ -191,6 +206,8 @@ int ensure_setup(mmc_ctx* c)
             cf.gx = (float)(beta * D0 * V / c->dx); cf.gy = (float)(beta * D0 * V / c->dy);
             cf.c4 = v[CS_C4]; cf.mu2 = k.th.mu2; cf.bKq = v[CS_BKQ]; cf.bzee = v[CS_BZEE]; cf.sigma = v[CS_SIGMA];
             cf.ax = v[CS_AX]; cf.ay = v[CS_AY]; cf.az = v[CS_AZ];
+            cf.bK1c = v[CS_BK1C]; cf.bK2c = v[CS_BK2C];
+            for (int q = 0; q < 9; ++q) cf.cub[q] = v[CS_CUB + q];
             c->K1T_u = v[CS_K1T]; c->c0_u = v[CS_C0];
             c->sigma_first = v[CS_SIGMA];
         }
@@ -221,6 +238,8 @@ int ensure_setup(mmc_ctx* c)
     if (D0 != 0.0) f |= F_DMI;
     if (c->demag_enabled) f |= F_DEMAG;
     if (n_active == (unsigned long long)N) f |= F_DENSE;
+    for (const auto& r : c->regions)
+        if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0)) f |= F_CUBIC;
     c->features = f;
     c->dirty = false;
     return MMC_OK;
@@ -313,7 +332,7 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     c->g.H = (int64_t)c->g.hx * ny * nz;
     c->dx = dx; c->dy = dy; c->dz = dz; c->V = dx * dy * dz;
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
-    c->regions.push_back(mmc_material{ 0, 0, 0, 0, 0, 1, 0, 1, 9.2740100783e-24 });
+    c->regions.push_back(mmc_material{ 0, 0, 0, 0, 0, 1, 0, 1, 9.2740100783e-24, 0, 0, 1, 0, 0, 0, 1, 0 });
     DeviceGuard dg(device);
     auto bail = [&](int code) { mmc_destroy(c); return code; };
     if (!dg.ok) return bail(MMC_E_CUDA);
@@ -358,6 +377,13 @@ int mmc_set_material(mmc_ctx* c, int n_regions, const mmc_material* regions, con
     if (n_regions < 1 || !regions) return fail(c, MMC_E_INVALID, "n_regions >= 1 and regions != NULL required");
     for (int r = 0; r < n_regions; ++r)
         if (!(regions[r].Ms0 >= 0) || !std::isfinite(regions[r].Ms0) || regions[r].A0 < 0) return fail(c, MMC_E_INVALID, "Ms0 and A0 must be >= 0");
+    for (int r = 0; r < n_regions; ++r) {
+        const mmc_material& mt = regions[r];
+        if (mt.K1c == 0.0 && mt.K2c == 0.0) continue;
+        const double cx = mt.c1y * mt.c2z - mt.c1z * mt.c2y, cy = mt.c1z * mt.c2x - mt.c1x * mt.c2z, cz = mt.c1x * mt.c2y - mt.c1y * mt.c2x;
+        const double n1 = mt.c1x * mt.c1x + mt.c1y * mt.c1y + mt.c1z * mt.c1z, n2 = mt.c2x * mt.c2x + mt.c2y * mt.c2y + mt.c2z * mt.c2z;
+        if (!(cx * cx + cy * cy + cz * cz > 1e-12 * n1 * n2)) return fail(c, MMC_E_INVALID, "cubic axes c1, c2 must not be parallel or zero");
+    }
     const long long N = (long long)c->g.nx * c->g.ny * c->g.nz;
     if (region_of_cell)
         for (long long i = 0; i < N; ++i)

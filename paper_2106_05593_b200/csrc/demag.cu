@@ -602,7 +602,7 @@ columns_fast_kernel(const ColFastArgs a)
 // S3, z direction, for the per-layer rows kernels: inverse length-Pz DFT (Pz = 2 NZ - 1, a direct sum) across the planes of
 // every (component, kx, j), the NZ kept layers written to `out` [3][NZ][Cx][ny].  A plain streaming pass (reads 8 Pz,
 // writes 8 NZ bytes per point).
-constexpr int kMaxFastLayers = 8;
+constexpr int kMaxFastLayers = 16;
 template <int NZ>
 __global__ void __launch_bounds__(256) z_inverse_kernel(const float2* __restrict__ in, float2* __restrict__ out, size_t plane)
 {
@@ -642,6 +642,14 @@ static int launch_z_inverse(const DemagPlan* p, const float2* in, float2* out, c
         case 6: z_inverse_kernel<6><<<blocks, 256, 0, st>>>(in, out, plane); break;
         case 7: z_inverse_kernel<7><<<blocks, 256, 0, st>>>(in, out, plane); break;
         case 8: z_inverse_kernel<8><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 9: z_inverse_kernel<9><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 10: z_inverse_kernel<10><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 11: z_inverse_kernel<11><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 12: z_inverse_kernel<12><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 13: z_inverse_kernel<13><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 14: z_inverse_kernel<14><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 15: z_inverse_kernel<15><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 16: z_inverse_kernel<16><<<blocks, 256, 0, st>>>(in, out, plane); break;
         default: return MMC_E_UNSUPPORTED;
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;

@@ -114,6 +114,19 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
         const double kT = op.kB / (double)invT;
         const double me_ = m[0] * ax + m[1] * ay + m[2] * az;
         acc[5] += kT * ((double)K1T - (double)bKq * me_ * me_);
+        {   // cubic anisotropy, Eq. (12): direction cosines with respect to the class's cubic axes
+            const float* cb; float bK1c, bK2c;
+            if (PERCELL) { const float* t = reinterpret_cast<const float*>(a.table) + (size_t)kClassFloats * (a.cw[s] >> 7);
+                           cb = t + CS_CUB; bK1c = t[CS_BK1C]; bK2c = t[CS_BK2C]; }
+            else { cb = a.coef.cub; bK1c = a.coef.bK1c; bK2c = a.coef.bK2c; }
+            if (bK1c != 0.f || bK2c != 0.f) {
+                const double il = 1.0 / sqrt(l2);
+                const double al = (m[0] * cb[0] + m[1] * cb[1] + m[2] * cb[2]) * il, be = (m[0] * cb[3] + m[1] * cb[4] + m[2] * cb[5]) * il,
+                             ga = (m[0] * cb[6] + m[1] * cb[7] + m[2] * cb[8]) * il;
+                const double A = al * al, B = be * be, G = ga * ga;
+                acc[5] += kT * ((double)bK1c * (A * B + A * G + B * G) + (double)bK2c * A * B * G);
+            }
+        }
         acc[6] += -kT * (double)bzee * (m[0] * a.coef.Bx + m[1] * a.coef.By + m[2] * a.coef.Bz);
         const double G0 = 0.5 * (-(nbv[0][2] - nbv[1][2]) * op.inv_d[0]);
         const double G1 = 0.5 * (-(nbv[2][2] - nbv[3][2]) * op.inv_d[1]);

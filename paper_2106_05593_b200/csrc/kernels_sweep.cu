@@ -69,7 +69,17 @@ __device__ __forceinline__ void sincos_2pi(float u, float* sn, float* cs)
 struct CellCoef {
     float kx, ky, kz, gx, gy, bKq, bzee, c4, sigma, ax, ay, az;
     double mu2;
+    float bK1c, bK2c, cub[9];          // cubic anisotropy (only read when CUBIC)
 };
+
+// class table slots CS_BK1C .. CS_CUB + 8 (floats 12 .. 22 of a class)
+__device__ __forceinline__ void load_cubic(const float4* t, CellCoef& cf)
+{
+    const float4 t3 = __ldg(t + 3), t4 = __ldg(t + 4), t5 = __ldg(t + 5);
+    cf.bK1c = t3.x; cf.bK2c = t3.y; cf.cub[0] = t3.z; cf.cub[1] = t3.w;
+    cf.cub[2] = t4.x; cf.cub[3] = t4.y; cf.cub[4] = t4.z; cf.cub[5] = t4.w;
+    cf.cub[6] = t5.x; cf.cub[7] = t5.y; cf.cub[8] = t5.z;
+}
 
 struct CellResult { float dm[3]; float f, L; float terms[6]; float margin; bool accept; };
 
@@ -77,7 +87,7 @@ struct CellResult { float dm[3]; float f, L; float terms[6]; float margin; bool 
 //   m      : current vector          S  : sum_d k_d sum_{bonded nb in d}(m_nb - m)   (beta J_d folded into k_d)
 //   selfc  : sum_d k_d n_d / 2       dzx, dzy, dxx, dyy : E-W / N-S differences of m_z, m_x, m_y for the DMI vector
 //   B      : B_ext + B_d (tesla); TERMS (debug) keeps Zeeman and demag apart for the per-term dump
-template <bool DMI, bool TERMS>
+template <bool DMI, bool TERMS, bool CUBIC>
 __device__ __forceinline__ CellResult cell_update(const float m[3], const float S[3], float selfc,
                                                   float dzx, float dzy, float dxx, float dyy,
                                                   const float Bext[3], const float Bd[3],
@@ -121,7 +131,23 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
     // uniaxial anisotropy: -beta V Kq (dm.e)((2m+dm).e)
     const float dme = fmaf(dm0, cf.ax, fmaf(dm1, cf.ay, dm2 * cf.az));
     const float sme = fmaf(fmaf(2.f, m[0], dm0), cf.ax, fmaf(fmaf(2.f, m[1], dm1), cf.ay, fmaf(2.f, m[2], dm2) * cf.az));
-    const float an = -cf.bKq * dme * sme;
+    float an = -cf.bKq * dme * sme;
+    if (CUBIC) {
+        // Eq. (12) for the directions n and n' = n + dn (the trial vector is L f (n + dn)): squares of the direction cosines
+        // A, B, G and their changes dA = d(alpha)(2 alpha + d(alpha)), ...; both invariants as differences without cancellation
+        const float al = fmaf(n0, cf.cub[0], fmaf(n1, cf.cub[1], n2 * cf.cub[2]));
+        const float be = fmaf(n0, cf.cub[3], fmaf(n1, cf.cub[4], n2 * cf.cub[5]));
+        const float ga = fmaf(n0, cf.cub[6], fmaf(n1, cf.cub[7], n2 * cf.cub[8]));
+        const float dal = fmaf(dn0, cf.cub[0], fmaf(dn1, cf.cub[1], dn2 * cf.cub[2]));
+        const float dbe = fmaf(dn0, cf.cub[3], fmaf(dn1, cf.cub[4], dn2 * cf.cub[5]));
+        const float dga = fmaf(dn0, cf.cub[6], fmaf(dn1, cf.cub[7], dn2 * cf.cub[8]));
+        const float A = al * al, B = be * be, G = ga * ga;
+        const float dA = dal * fmaf(2.f, al, dal), dB = dbe * fmaf(2.f, be, dbe), dG = dga * fmaf(2.f, ga, dga);
+        const float Ap = A + dA, Bp = B + dB;
+        const float d1 = fmaf(A, dB, fmaf(Bp, dA, fmaf(A, dG, fmaf(G + dG, dA, fmaf(B, dG, (G + dG) * dB)))));
+        const float d2 = fmaf(dA * B, G, Ap * fmaf(dB, G, Bp * dG));
+        an = fmaf(cf.bK1c, d1, fmaf(cf.bK2c, d2, an));
+    }
     // Zeeman + demag: -beta V Ms0 dm.(B_ext + B_d)
     float zee, dem;
     if (TERMS) {
@@ -223,7 +249,7 @@ template <unsigned F, bool DEBUG>
 __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads) colour_pass_kernel(const SweepArgs a)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
-                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
+                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0, CUBIC = (F & F_CUBIC) != 0;
     __shared__ PassTailSmem s_tail;
     pass_tail_init(s_tail);
 
@@ -286,15 +312,17 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
         CellCoef cf;
         float kscale = 1.f;
         if (PERCELL) {
-            const float4* t = a.table + 3u * cls;
+            const float4* t = a.table + (kClassFloats / 4) * cls;
             const float4 t0 = __ldg(t), t1 = __ldg(t + 1);
             const float2 t2 = __ldg(reinterpret_cast<const float2*>(t + 2));
             kscale = t0.x; cf.c4 = t0.y;
             cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
             cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
+            if (CUBIC) load_cubic(t, cf);
         } else {
             cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
             cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
+            if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; }
         }
         cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
         cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
@@ -332,7 +360,7 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
         const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
         const unsigned cell = (unsigned)row * nx + i;                     // natural cell index (< 2^31)
         const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
-        const CellResult r = cell_update<DMI, DEBUG>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
+        const CellResult r = cell_update<DMI, DEBUG, CUBIC>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
         accept = r.accept;
         fs0 = m[0]; fs1 = m[1]; fs2 = m[2]; fs3 = r.L;
         if (accept) {
@@ -366,7 +394,7 @@ template <unsigned F>
 __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_kernel(const SweepArgs a)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
-                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
+                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0, CUBIC = (F & F_CUBIC) != 0;
     __shared__ PassTailSmem s_tail;
     pass_tail_init(s_tail);
 
@@ -447,15 +475,17 @@ __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_ke
             CellCoef cf;
             float kscale = 1.f;
             if (PERCELL) {
-                const float4* tb = a.table + 3u * cls[t];
+                const float4* tb = a.table + (kClassFloats / 4) * cls[t];
                 const float4 t0 = __ldg(tb), t1 = __ldg(tb + 1);
                 const float2 t2 = __ldg(reinterpret_cast<const float2*>(tb + 2));
                 kscale = t0.x; cf.c4 = t0.y;
                 cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
                 cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
+                if (CUBIC) load_cubic(tb, cf);
             } else {
                 cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
                 cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
+                if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; }
             }
             cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
             cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
@@ -489,7 +519,7 @@ __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_ke
             }
             const unsigned cell = (unsigned)row * nx + (unsigned)(i0 + 2 * t);       // natural cell index (< 2^31)
             const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
-            const CellResult r = cell_update<DMI, false>(m, Sg, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
+            const CellResult r = cell_update<DMI, false, CUBIC>(m, Sg, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
             float f0 = m[0], f1 = m[1], f2 = m[2], f3 = r.L;
             if (r.accept) {
                 f0 += r.dm[0]; f1 += r.dm[1]; f2 += r.dm[2]; f3 *= r.f;
@@ -570,6 +600,10 @@ int launch_colour_pass(const SweepArgs& a, unsigned f, bool debug, void* stream)
     constexpr unsigned UALL = F_MASK | F_Z | F_DMI | F_DEMAG, PALL = UALL | F_PERCELL;
     const bool dense = (f & F_DENSE) != 0;             // only ever a promise, never over-approximated
     f &= ~F_DENSE;
+    if (f & F_CUBIC) {                                 // cubic anisotropy: the all-features variants
+        if (f & F_PERCELL) return launch_variant<PALL | F_CUBIC>(a, debug, st);
+        return launch_variant<UALL | F_CUBIC>(a, debug, st);
+    }
     if (f & F_PERCELL) {
         if (debug) return launch_variant<PALL>(a, true, st);
         if (!(f & F_DMI)) {                                                                                  // cfg 4

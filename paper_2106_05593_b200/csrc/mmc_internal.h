@@ -47,16 +47,19 @@ struct Coef {
     float ax, ay, az;       // easy axis
     double mu2;             // -c2/(2 c4)  (= me^2 below Tc)
     float Bx, By, Bz;       // applied field, tesla
+    float bK1c, bK2c;       // beta V K1c me^10, beta V K2c me^21  (cubic anisotropy, Eq. (12))
+    float cub[9];           // the three orthonormal cubic axes
 };
 
 // Per-cell mode (more than one coefficient class, e.g. cfg 4: one class per distinct (region, T) pair): every cell
 // carries one 32-bit word  cw = class << 7 | mask byte  (colour-split, 2*H entries), and the coefficients of a
-// class sit in a table of kClassFloats floats per class (48 B = three 16-byte loads).  The table is a few MB for
+// class sit in a table of kClassFloats floats per class (96 B; the passes read the first 40 B, 96 B with cubic anisotropy).  The table is a few MB for
 // the paper's granular film and stays L2-resident; the HBM cost per cell is the 4-byte word.
-constexpr int kClassFloats = 12;
+constexpr int kClassFloats = 24;      // six 16-byte loads; the last three only with cubic anisotropy
 enum ClassSlot { CS_INVT = 0, CS_C4 = 1, CS_MU2 = 2 /* double in slots 2,3 */, CS_BKQ = 4, CS_BZEE = 5, CS_SIGMA = 6,
                  CS_AX = 7, CS_AY = 8, CS_AZ = 9, CS_K1T = 10 /* beta V K1(T), read-out only */,
-                 CS_C0 = 11 /* c0 - c4 mu2^2, read-out only */ };
+                 CS_C0 = 11 /* c0 - c4 mu2^2, read-out only */,
+                 CS_BK1C = 12, CS_BK2C = 13, CS_CUB = 14 /* 9 floats */ };
 constexpr unsigned kMaxClasses = 1u << 25;
 constexpr float kSumScale = 4194304.f;              // 2^22: fixed-point scale of the running sums (a warp's sum fits int32 for |m| < 8; blocks add in 64 bits)
 
@@ -79,7 +82,8 @@ enum Feature : unsigned {
     F_Z = 4u,         // nz > 1
     F_DMI = 8u,
     F_DEMAG = 16u,
-    F_DENSE = 32u,    // no empty cell: every in-mesh cell is active, so no load has to wait for the mask / class word
+    F_DENSE = 32u,
+    F_CUBIC = 64u,    // cubic anisotropy, Eq. (12)    // no empty cell: every in-mesh cell is active, so no load has to wait for the mask / class word
 };
 
 struct SweepArgs {

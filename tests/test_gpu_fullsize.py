@@ -157,6 +157,8 @@ EQ_CASES = {
     "cfg3_32x32_650K": (lambda: W.cfg3(nx=32, ny=32, T=650.0), 3000),
     # granular film: per-cell classes, grain boundaries, hot spot above Tc, 3 layers, demag
     "cfg4_24x24x3": (lambda: W.cfg4(nx=24, ny=24, nz=3), 2000),
+    # granular Fe film: cubic anisotropy (Eq. (12)) with random axes per grain, periodic in the plane, demag
+    "fe_film_cubic_24x24x3": (lambda: W.fe_film(nx=24, ny=24, nz=3), 2000),
 }
 
 

@@ -112,6 +112,9 @@ CASES = {
     "cfg4_48x40x4": lambda: W.cfg4(nx=48, ny=40, nz=4),
     "cfg4_30x21x3": lambda: W.cfg4(nx=30, ny=21, nz=3),
     "cfg5_160x150": lambda: W.cfg5(nx=160, ny=150),
+    # cubic anisotropy (Eq. (12), K1c + K2c, random cubic axes per grain), periodic in the plane, phase-separated grains
+    "fe_film_cubic_48x40x3": lambda: W.fe_film(nx=48, ny=40, nz=3),
+    "fe_film_cubic_36x22x10": lambda: W.fe_film(nx=36, ny=22, nz=10),
 }
 
 
@@ -133,7 +136,8 @@ def test_colour_pass_parity(name):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["cfg1_paper_regime", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150"])
+@pytest.mark.parametrize("name", ["cfg1_paper_regime", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150",
+                                  "fe_film_cubic_48x40x3"])
 def test_sweep_matches_replayed_oracle(name):
     """mmc_sweep(n) (demag -> red -> black -> counter++) against the oracle replaying the same iterations.  A cell whose
     decision flips inside the margin window makes the two trajectories differ from there on, so the bar is: the first
@@ -177,7 +181,8 @@ def test_sweep_matches_replayed_oracle(name):
                                      ((301, 67, 3), (2e-9, 3e-9, 4e-9)), ((512, 72, 2), (3e-9, 3e-9, 3e-9)),
                                      ((1024, 65, 1), (5e-9, 5e-9, 10e-9)), ((700, 69, 4), (3e-9, 3e-9, 3e-9)),
                                      ((2048, 66, 1), (5e-9, 5e-9, 10e-9)), ((1500, 65, 2), (3e-9, 3e-9, 3e-9)),
-                                     ((130, 300, 3), (3e-9, 3e-9, 3e-9))])
+                                     ((130, 300, 3), (3e-9, 3e-9, 3e-9)), ((132, 70, 10), (2e-9, 2e-9, 2e-9)),
+                                     ((256, 65, 16), (2e-9, 2e-9, 2e-9))])
 def test_demag_field_parity(shape, d):
     """Eq. (14): GPU fp32 FFT convolution vs the oracle's fp64 one (itself pinned to the direct sum)."""
     import paper_2106_05593_b200 as P
@@ -200,7 +205,8 @@ def test_demag_field_parity(shape, d):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["cfg1_32x32", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg3_48x40_800K", "cfg4_30x21x3", "cfg5_160x150"])
+@pytest.mark.parametrize("name", ["cfg1_32x32", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg3_48x40_800K", "cfg4_30x21x3", "cfg5_160x150",
+                                  "fe_film_cubic_48x40x3"])
 def test_observables_parity(name):
     wl = CASES[name]()
     g, o = _gpu(wl), _orc(wl)

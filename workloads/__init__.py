@@ -53,8 +53,12 @@ class Workload:
         return int((ms[self.region_of_cell] > 0).sum())
 
 
-def _mat(Ms0=0.0, A0=0.0, K1=0.0, axis=(0.0, 0.0, 1.0), D0=0.0, Tc=1.0, mu_atom=MUB):
-    return dict(Ms0=Ms0, A0=A0, K1=K1, ax=axis[0], ay=axis[1], az=axis[2], D0=D0, Tc=Tc, mu_atom=mu_atom)
+def _mat(Ms0=0.0, A0=0.0, K1=0.0, axis=(0.0, 0.0, 1.0), D0=0.0, Tc=1.0, mu_atom=MUB, K1c=0.0, K2c=0.0,
+         c1=(1.0, 0.0, 0.0), c2=(0.0, 1.0, 0.0)):
+    d = dict(Ms0=Ms0, A0=A0, K1=K1, ax=axis[0], ay=axis[1], az=axis[2], D0=D0, Tc=Tc, mu_atom=mu_atom)
+    if K1c != 0.0 or K2c != 0.0:                     # cubic anisotropy, Eq. (12): two of the cubic axes
+        d.update(K1c=K1c, K2c=K2c, c1x=c1[0], c1y=c1[1], c1z=c1[2], c2x=c2[0], c2y=c2[1], c2z=c2[2])
+    return d
 
 
 def _random_unit(rng, n):
@@ -174,6 +178,36 @@ def cfg5(nx=2048, ny=2048):
 
 
 CONFIGS = {1: cfg1, 2: cfg2, 3: cfg3, 4: cfg4, 5: cfg5}
+
+
+def fe_film(nx=400, ny=400, nz=10):
+    """The paper's granular Fe film with cubic anisotropy (Fig. 5; SURVEY 8(f) row 3's workload): 2 nm cubic
+    cells, periodic in the plane (exchange; the demag convolution is open-boundary as everywhere), Ms0 1.71e6, A0 2.1e-11,
+    K1c 4.8e4, K2c -1e4 (4th / 6th order), Tc 1044, T 300 K; 3-D Voronoi grains with 10 nm mean seed spacing and phase
+    separation (no exchange between grains); field along +x.  Filler the paper leaves open: each grain's cubic axes are a
+    random rotation (seeded); start saturated along +x at |m0| = 0.97 (~me(300 K))."""
+    from scipy.spatial import cKDTree
+    rng = np.random.Generator(np.random.PCG64(BASE_SEED + 6))
+    h = 2.0
+    n_seeds = max(2, int(round(nx * ny * nz * h ** 3 / 10.0 ** 3)))
+    seeds = rng.uniform(0.0, 1.0, (n_seeds, 3)) * np.array([nx * h, ny * h, nz * h])
+    k, j, i = np.meshgrid(np.arange(nz), np.arange(ny), np.arange(nx), indexing="ij")
+    pts = np.stack([(i.ravel() + 0.5) * h, (j.ravel() + 0.5) * h, (k.ravel() + 0.5) * h], axis=1)
+    _, grain = cKDTree(seeds).query(pts, workers=-1)
+    grain = grain.astype(np.int32)
+    regions = []
+    for g in range(n_seeds):
+        q, _ = np.linalg.qr(rng.normal(size=(3, 3)))
+        regions.append(_mat(1.71e6, 2.1e-11, 0.0, (0.0, 0.0, 1.0), 0.0, 1044.0, K1c=4.8e4, K2c=-1.0e4,
+                            c1=tuple(q[:, 0]), c2=tuple(q[:, 1])))
+    N = nx * ny * nz
+    m0 = np.zeros((3, N), dtype=np.float32); m0[0] = 0.97
+    sched = [("B", (1e-3 * b, 0.0, 0.0), 2000) for b in range(-200, 201, 10)]
+    return Workload("fe_film_cubic", nx, ny, nz, 2e-9, 2e-9, 2e-9, 0b011, regions, grain, 0, 300.0, None,
+                    (0.05, 0.0, 0.0), 30.0, -1.0, True, True, BASE_SEED + 6, m0, sched)
+
+
+CONFIGS[6] = fe_film
 
 
 def make(cfg: int, **kw) -> Workload:
