@@ -85,6 +85,10 @@ def lib():
         L.orc_newell.argtypes = [C.c_double] * 6 + [dp]
         L.orc_demag_tensor.argtypes = [C.c_int] * 3 + [C.c_double] * 3 + [C.c_int, dp]
         L.orc_demag_direct.argtypes = [C.c_int] * 3 + [dp] * 7
+        L.orc_exact_demag_dF.restype = C.c_double
+        L.orc_exact_demag_dF.argtypes = [C.POINTER(_Problem)] + [dp] * 4 + [C.c_int64, dp]
+        L.orc_serial_exact_sweep.restype = C.c_int64
+        L.orc_serial_exact_sweep.argtypes = [C.POINTER(_Problem)] + [dp] * 7 + [C.c_uint64, C.c_int, C.POINTER(C.c_int64)]
         _lib = L
     return _lib
 
@@ -421,6 +425,34 @@ class OracleMMC:
     def run(self, n_sweeps):
         for _ in range(n_sweeps):
             self.sweep_once()
+
+    def exact_demag_dF(self, cell, dm, b=None):
+        """beta dE_demag of the single-cell move dm with the exact field of the current state (+ self term)."""
+        p = self._problem()
+        if self._demag is None:
+            self._demag = DemagFFT(self.nx, self.ny, self.nz, self.dx, self.dy, self.dz, self.demag_r_near)
+        tab = np.ascontiguousarray(self._demag.tab)
+        b = [np.ascontiguousarray(x, dtype=np.float64) for x in (self.demag_field() if b is None else b)]
+        dm = np.ascontiguousarray(dm, dtype=np.float64)
+        return lib().orc_exact_demag_dF(C.byref(p), _dp(tab), _dp(b[0]), _dp(b[1]), _dp(b[2]), int(cell), _dp(dm))
+
+    def run_serial_exact(self, n_sweeps):
+        """Validation mode (Appendix B): serial MMC, cells one after the other, with the
+        exact demag energy change (current field + self term) and the field updated after every accepted move.  The
+        oracle's parallel mode is the paper's approximation of this; Appendix B claims no statistical difference."""
+        p = self._problem()
+        if self._demag is None:
+            self._demag = DemagFFT(self.nx, self.ny, self.nz, self.dx, self.dy, self.dz, self.demag_r_near)
+        tab = np.ascontiguousarray(self._demag.tab)
+        b = [np.ascontiguousarray(x, dtype=np.float64) for x in self.demag_field()]
+        for _ in range(n_sweeps):
+            tri = C.c_int64()
+            acc = lib().orc_serial_exact_sweep(C.byref(p), _dp(self.m[0]), _dp(self.m[1]), _dp(self.m[2]), _dp(tab),
+                                               _dp(b[0]), _dp(b[1]), _dp(b[2]), self.sweep, int(self.store_fp32), C.byref(tri))
+            self.accepted += acc; self.trials += tri.value
+            self.sweep += 1
+        self.bd = b
+        return b
 
     def histogram(self, kind, nbins, lo, hi):
         """The paper's verification read-outs over the non-empty cells: kind "length": x = |m|; kind "angle":

@@ -580,6 +580,72 @@ void orc_demag_direct(int nx, int ny, int nz, const double *tab,
     }
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* Serial MMC with the EXACT demagnetising energy change ("a serial MMC algorithm ... the           */
+/* demagnetizing field updated after every accepted move", Appendix B / PAPER.md:218).         */
+/* Validation mode of the oracle only: cells are visited one after the other in lexicographic order; for a move   */
+/* dM = Ms0 dm of cell c the total demag energy E_d = (mu0 V/2) sum_ij M_i N_ij M_j changes by                    */
+/*     dE_d = -V dM . B_d(c) + (mu0 V/2) dM . N(0) . dM        (field term with the CURRENT field + self term),   */
+/* and after an accepted move the field of every cell is updated, B_d(i) -= mu0 N(r_i - r_c) dM.                   */
+/* tab = octant tensor table of orc_demag_tensor; bx,by,bz = B_d of the state on entry, kept current.              */
+/* All other energy terms, the trial move, the random numbers and Eq. (5) are those of orc_visit.                  */
+/* ------------------------------------------------------------------------------------------ */
+/* beta * dE_d of the move dm of cell c with the current field b (tesla) and the self term; see above */
+double orc_exact_demag_dF(const orc_problem *p, const double *tab, const double *bx, const double *by, const double *bz,
+                          int64_t c, const double dm[3])
+{
+    const int64_t P = (int64_t)p->nx * p->ny * p->nz;
+    const double V = p->dx * p->dy * p->dz;
+    double dM[3] = { p->Ms0[c] * dm[0], p->Ms0[c] * dm[1], p->Ms0[c] * dm[2] };
+    double field = -V * (dM[0] * bx[c] + dM[1] * by[c] + dM[2] * bz[c]);
+    double self = 0.5 * ORC_MU0 * V * (tab[0] * dM[0] * dM[0] + tab[P] * dM[1] * dM[1] + tab[2 * P] * dM[2] * dM[2]);   /* N(0) is diagonal */
+    return p->beta[c] * (field + self);
+}
+
+int64_t orc_serial_exact_sweep(const orc_problem *p, double *mx, double *my, double *mz, const double *tab,
+                               double *bx, double *by, double *bz, uint64_t sweep, int store_fp32, int64_t *trials_out)
+{
+    const int nx = p->nx, ny = p->ny, nz = p->nz;
+    const int64_t P = (int64_t)nx * ny * nz;
+    orc_problem q = *p;
+    q.bdx = bx; q.bdy = by; q.bdz = bz;
+    int64_t accepted = 0, trials = 0;
+    for (int k = 0; k < nz; ++k) for (int j = 0; j < ny; ++j) for (int i = 0; i < nx; ++i) {
+        int64_t c = orc_idx(p, i, j, k);
+        if (!p->active[c]) continue;
+        trials++;
+        double u[4];
+        orc_cell_uniforms(p->seed, sweep, (uint64_t)c, u);
+        double m[3] = { mx[c], my[c], mz[c] };
+        double dm[3], f, terms[6];
+        orc_trial(m, u, p->one_minus_cos_cone, p->sigma[c], dm, &f);
+        orc_cell_dF(&q, mx, my, mz, i, j, k, dm, terms);
+        terms[4] = orc_exact_demag_dF(p, tab, bx, by, bz, c, dm);
+        double dM[3];
+        double dF = terms[0] + terms[1] + terms[2] + terms[3] + terms[4] + terms[5];
+        if (!(log(u[3]) - 4.0 * log(f) + dF < 0.0)) continue;
+        accepted++;
+        double a = m[0] + dm[0], b = m[1] + dm[1], d = m[2] + dm[2];
+        if (store_fp32) { a = (double)(float)a; b = (double)(float)b; d = (double)(float)d; }
+        dM[0] = p->Ms0[c] * (a - m[0]); dM[1] = p->Ms0[c] * (b - m[1]); dM[2] = p->Ms0[c] * (d - m[2]);
+        mx[c] = a; my[c] = b; mz[c] = d;
+        #pragma omp parallel for schedule(static)
+        for (int64_t ci = 0; ci < P; ++ci) {
+            int ii = (int)(ci % nx), jj = (int)((ci / nx) % ny), kk = (int)(ci / ((int64_t)nx * ny));
+            int ox = ii - i, oy = jj - j, oz = kk - k;
+            double sx = ox < 0 ? -1.0 : 1.0, sy = oy < 0 ? -1.0 : 1.0, sz = oz < 0 ? -1.0 : 1.0;
+            int64_t o = ((int64_t)abs(oz) * ny + abs(oy)) * nx + abs(ox);
+            double nxx = tab[o], nyy = tab[P + o], nzz = tab[2 * P + o];
+            double nxy = sx * sy * tab[3 * P + o], nxz = sx * sz * tab[4 * P + o], nyz = sy * sz * tab[5 * P + o];
+            bx[ci] -= ORC_MU0 * (nxx * dM[0] + nxy * dM[1] + nxz * dM[2]);
+            by[ci] -= ORC_MU0 * (nxy * dM[0] + nyy * dM[1] + nyz * dM[2]);
+            bz[ci] -= ORC_MU0 * (nxz * dM[0] + nyz * dM[1] + nzz * dM[2]);
+        }
+    }
+    if (trials_out) *trials_out = trials;
+    return accepted;
+}
+
 /*
  * Parity plumbing (stage 2): O4 evaluated for every active cell of one colour with trial
  * vectors supplied by the caller (dm_in[3c+a]) instead of O3's own, so that the energy arithmetic of another
