@@ -43,6 +43,7 @@ struct mmc_ctx {
     float* Ms0_split = nullptr;
     uint32_t* cw = nullptr;                       // per-cell mode: class << 7 | mask (colour-split)
     float* table = nullptr; size_t table_cap = 0; // per-cell mode: kClassFloats floats per class
+    float* table_cubic = nullptr;                 // ... and the cubic-anisotropy table of the same stride
     size_t n_classes = 0;
     Control* ctl = nullptr;
     unsigned long long* run_sums = nullptr;       // [4] fixed-point running sums (kSumScale)
@@ -167,7 +168,7 @@ int ensure_setup(mmc_ctx* c)
     Coef cf{};
     cf.Bx = (float)c->B[0]; cf.By = (float)c->B[1]; cf.Bz = (float)c->B[2];
     // one table entry (kClassFloats floats, ClassSlot order) per class
-    auto class_values = [&](const Cls& k, double beta, float* out) {
+    auto class_values = [&](const Cls& k, double beta, float* out, float* outc) {
         const mmc_material& mt = c->regions[k.region];
         double al = std::sqrt(mt.ax * mt.ax + mt.ay * mt.ay + mt.az * mt.az);
         double ex = 0, ey = 0, ez = 1;
@@ -180,8 +181,9 @@ int ensure_setup(mmc_ctx* c)
         out[CS_K1T] = (float)(beta * V * mt.K1 * k.th.me * k.th.me * k.th.me);
         out[CS_C0] = (float)((k.th.me > 0 || k.th.mu2 == 0) ? 0.0 : -k.th.c4 * k.th.mu2 * k.th.mu2);
         // cubic anisotropy: K(T) = K me^(l(l+1)/2), l = 4, 6; axes by Gram-Schmidt, e3 = e1 x e2
-        out[CS_BK1C] = (float)(beta * V * mt.K1c * std::pow(k.th.me, 10.0));
-        out[CS_BK2C] = (float)(beta * V * mt.K2c * std::pow(k.th.me, 21.0));
+        outc[CS_BK1C] = (float)(beta * V * mt.K1c * std::pow(k.th.me, 10.0));
+        outc[CS_BK2C] = (float)(beta * V * mt.K2c * std::pow(k.th.me, 21.0));
+        outc[11] = 0.f;
         double e1[3] = { mt.c1x, mt.c1y, mt.c1z }, e2[3] = { mt.c2x, mt.c2y, mt.c2z };
         double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
         if (!(n1 > 0)) { e1[0] = 1; e1[1] = e1[2] = 0; n1 = 1; }
@@ -193,21 +195,21 @@ int ensure_setup(mmc_ctx* c)
             const double p2 = e1[a]; for (int q = 0; q < 3; ++q) e2[q] -= p2 * e1[q]; n2 = std::sqrt(e2[0] * e2[0] + e2[1] * e2[1] + e2[2] * e2[2]); }
         for (int q = 0; q < 3; ++q) e2[q] /= n2;
         const double e3[3] = { e1[1] * e2[2] - e1[2] * e2[1], e1[2] * e2[0] - e1[0] * e2[2], e1[0] * e2[1] - e1[1] * e2[0] };
-        for (int q = 0; q < 3; ++q) { out[CS_CUB + q] = (float)e1[q]; out[CS_CUB + 3 + q] = (float)e2[q]; out[CS_CUB + 6 + q] = (float)e3[q]; }
+        for (int q = 0; q < 3; ++q) { outc[CS_CUB + q] = (float)e1[q]; outc[CS_CUB + 3 + q] = (float)e2[q]; outc[CS_CUB + 6 + q] = (float)e3[q]; }
     };
     c->n_classes = classes.size();
     if (!c->percell) {
         if (!classes.empty()) {
             const Cls& k = classes[0];
             const double beta = 1.0 / (kB * (double)k.T);
-            float v[kClassFloats];
-            class_values(k, beta, v);
+            float v[kClassFloats], vc[kClassFloats];
+            class_values(k, beta, v, vc);
             cf.kx = (float)(beta * Jd[0]); cf.ky = (float)(beta * Jd[1]); cf.kz = (float)(beta * Jd[2]);
             cf.gx = (float)(beta * D0 * V / c->dx); cf.gy = (float)(beta * D0 * V / c->dy);
             cf.c4 = v[CS_C4]; cf.mu2 = k.th.mu2; cf.bKq = v[CS_BKQ]; cf.bzee = v[CS_BZEE]; cf.sigma = v[CS_SIGMA];
             cf.ax = v[CS_AX]; cf.ay = v[CS_AY]; cf.az = v[CS_AZ];
-            cf.bK1c = v[CS_BK1C]; cf.bK2c = v[CS_BK2C];
-            for (int q = 0; q < 9; ++q) cf.cub[q] = v[CS_CUB + q];
+            cf.bK1c = vc[CS_BK1C]; cf.bK2c = vc[CS_BK2C];
+            for (int q = 0; q < 9; ++q) cf.cub[q] = vc[CS_CUB + q];
             c->K1T_u = v[CS_K1T]; c->c0_u = v[CS_C0];
             c->sigma_first = v[CS_SIGMA];
         }
@@ -216,11 +218,15 @@ int ensure_setup(mmc_ctx* c)
         const double b1 = 1.0 / kB;                   // beta at T = 1 K; the kernel multiplies by the class's 1/T
         cf.kx = (float)(b1 * Jd[0]); cf.ky = (float)(b1 * Jd[1]); cf.kz = (float)(b1 * Jd[2]);
         cf.gx = (float)(b1 * D0 * V / c->dx); cf.gy = (float)(b1 * D0 * V / c->dy);
-        std::vector<float> tab(classes.size() * kClassFloats);
-        for (size_t q = 0; q < classes.size(); ++q) class_values(classes[q], 1.0 / (kB * (double)classes[q].T), &tab[kClassFloats * q]);
+        std::vector<float> tab(classes.size() * kClassFloats), tabc(classes.size() * kClassFloats);
+        for (size_t q = 0; q < classes.size(); ++q)
+            class_values(classes[q], 1.0 / (kB * (double)classes[q].T), &tab[kClassFloats * q], &tabc[kClassFloats * q]);
         c->sigma_first = tab[CS_SIGMA];
-        if (tab.size() > c->table_cap) { cudaFree(c->table); c->table = nullptr; c->table_cap = tab.size(); }
+        if (tab.size() > c->table_cap) { cudaFree(c->table); cudaFree(c->table_cubic); c->table = c->table_cubic = nullptr; c->table_cap = tab.size(); }
         rc = upload(c, &c->table, tab); if (rc) return rc;
+        bool cubic = false;
+        for (const auto& r : c->regions) if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0)) cubic = true;
+        if (cubic) { rc = upload(c, &c->table_cubic, tabc); if (rc) return rc; }
         std::vector<uint32_t> cw(S, 0u);
         for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
             const long long cell = (long long)i + (long long)g.nx * (j + (long long)g.ny * k);
@@ -267,6 +273,7 @@ SweepArgs make_args(mmc_ctx* c, int colour)
     a.mask = c->mask; a.coef = c->coef;
     a.coef.Bx = (float)c->B[0]; a.coef.By = (float)c->B[1]; a.coef.Bz = (float)c->B[2];
     a.cw = c->percell ? c->cw : nullptr; a.table = c->percell ? reinterpret_cast<const float4*>(c->table) : nullptr;
+    a.table_cubic = (c->percell && (c->features & F_CUBIC)) ? reinterpret_cast<const float4*>(c->table_cubic) : nullptr;
     a.ctl = c->ctl; a.seed_lo = (unsigned)c->seed; a.seed_hi = (unsigned)(c->seed >> 32);
     a.colour = colour; a.run_sums = c->run_sums;
     return a;
@@ -363,7 +370,7 @@ int mmc_destroy(mmc_ctx* c)
     DeviceGuard dg(c->device);
     cudaStreamSynchronize(c->stream);
     for (int q = 0; q < 3; ++q) { cudaFree(c->m[q]); cudaFree(c->bd[q]); }
-    cudaFree(c->cw); cudaFree(c->table);
+    cudaFree(c->cw); cudaFree(c->table); cudaFree(c->table_cubic);
     cudaFree(c->mask); cudaFree(c->Ms0_split); cudaFree(c->ctl); cudaFree(c->run_sums); cudaFree(c->obs_scratch);
     cudaFree(c->d_obs); cudaFree(c->d_flag); cudaFree(c->stage);
     demag_destroy(c->demag);

@@ -116,8 +116,11 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
         acc[5] += kT * ((double)K1T - (double)bKq * me_ * me_);
         {   // cubic anisotropy, Eq. (12): direction cosines with respect to the class's cubic axes
             const float* cb; float bK1c, bK2c;
-            if (PERCELL) { const float* t = reinterpret_cast<const float*>(a.table) + (size_t)kClassFloats * (a.cw[s] >> 7);
-                           cb = t + CS_CUB; bK1c = t[CS_BK1C]; bK2c = t[CS_BK2C]; }
+            if (PERCELL) {
+                if (a.table_cubic) { const float* t = reinterpret_cast<const float*>(a.table_cubic) + (size_t)kClassFloats * (a.cw[s] >> 7);
+                                     cb = t + CS_CUB; bK1c = t[CS_BK1C]; bK2c = t[CS_BK2C]; }
+                else { cb = a.coef.cub; bK1c = 0.f; bK2c = 0.f; }
+            }
             else { cb = a.coef.cub; bK1c = a.coef.bK1c; bK2c = a.coef.bK2c; }
             if (bK1c != 0.f || bK2c != 0.f) {
                 const double il = 1.0 / sqrt(l2);

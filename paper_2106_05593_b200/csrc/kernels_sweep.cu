@@ -72,10 +72,10 @@ struct CellCoef {
     float bK1c, bK2c, cub[9];          // cubic anisotropy (only read when CUBIC)
 };
 
-// class table slots CS_BK1C .. CS_CUB + 8 (floats 12 .. 22 of a class)
+// cubic table slots CS_BK1C, CS_BK2C, CS_CUB .. CS_CUB + 8 of a class
 __device__ __forceinline__ void load_cubic(const float4* t, CellCoef& cf)
 {
-    const float4 t3 = __ldg(t + 3), t4 = __ldg(t + 4), t5 = __ldg(t + 5);
+    const float4 t3 = __ldg(t), t4 = __ldg(t + 1), t5 = __ldg(t + 2);
     cf.bK1c = t3.x; cf.bK2c = t3.y; cf.cub[0] = t3.z; cf.cub[1] = t3.w;
     cf.cub[2] = t4.x; cf.cub[3] = t4.y; cf.cub[4] = t4.z; cf.cub[5] = t4.w;
     cf.cub[6] = t5.x; cf.cub[7] = t5.y; cf.cub[8] = t5.z;
@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
             kscale = t0.x; cf.c4 = t0.y;
             cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
             cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
-            if (CUBIC) load_cubic(t, cf);
+            if (CUBIC) load_cubic(a.table_cubic + (kClassFloats / 4) * cls, cf);
         } else {
             cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
             cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
@@ -481,7 +481,7 @@ __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_ke
                 kscale = t0.x; cf.c4 = t0.y;
                 cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
                 cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
-                if (CUBIC) load_cubic(tb, cf);
+                if (CUBIC) load_cubic(a.table_cubic + (kClassFloats / 4) * cls[t], cf);
             } else {
                 cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
                 cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;

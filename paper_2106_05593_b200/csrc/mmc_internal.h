@@ -53,13 +53,14 @@ struct Coef {
 
 // Per-cell mode (more than one coefficient class, e.g. cfg 4: one class per distinct (region, T) pair): every cell
 // carries one 32-bit word  cw = class << 7 | mask byte  (colour-split, 2*H entries), and the coefficients of a
-// class sit in a table of kClassFloats floats per class (96 B; the passes read the first 40 B, 96 B with cubic anisotropy).  The table is a few MB for
+// class sit in a table of kClassFloats floats per class (48 B = three 16-byte loads); cubic anisotropy adds a second
+// table of the same stride, so that meshes without it keep the small footprint in L2.  The table is a few MB for
 // the paper's granular film and stays L2-resident; the HBM cost per cell is the 4-byte word.
-constexpr int kClassFloats = 24;      // six 16-byte loads; the last three only with cubic anisotropy
+constexpr int kClassFloats = 12;      // three 16-byte loads per class and table (main table; cubic table only with F_CUBIC)
 enum ClassSlot { CS_INVT = 0, CS_C4 = 1, CS_MU2 = 2 /* double in slots 2,3 */, CS_BKQ = 4, CS_BZEE = 5, CS_SIGMA = 6,
                  CS_AX = 7, CS_AY = 8, CS_AZ = 9, CS_K1T = 10 /* beta V K1(T), read-out only */,
                  CS_C0 = 11 /* c0 - c4 mu2^2, read-out only */,
-                 CS_BK1C = 12, CS_BK2C = 13, CS_CUB = 14 /* 9 floats */ };
+                 /* second table (cubic anisotropy), same stride: */ CS_BK1C = 0, CS_BK2C = 1, CS_CUB = 2 /* 9 floats */ };
 constexpr unsigned kMaxClasses = 1u << 25;
 constexpr float kSumScale = 4194304.f;              // 2^22: fixed-point scale of the running sums (a warp's sum fits int32 for |m| < 8; blocks add in 64 bits)
 
@@ -93,6 +94,7 @@ struct SweepArgs {
     const uint8_t* mask;         // colour-split; bits 0..5 bonded +x,-x,+y,-y,+z,-z; bit 6 active
     const uint32_t* cw;          // per-cell mode: class << 7 | mask (colour-split), else NULL
     const float4* table;         // per-cell mode: kClassFloats floats per class, else NULL
+    const float4* table_cubic;   // per-cell mode with cubic anisotropy: kClassFloats floats per class (CS_BK1C ...), else NULL
     Coef coef;
     Control* ctl;
     unsigned seed_lo, seed_hi;
