@@ -80,9 +80,9 @@ def demag_kernel_bytes(wl, ms0_per_cell):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/), cfg 4
-NCU_TRAFFIC_CFG4 = {   # profiles/r1e_summary.md
-    "colour_pass_kernel": 112.1e6, "demag_rows_fwd_kernel": 103.7e6, "demag_columns_kernel": 451.8e6,
-    "demag_z_inverse_kernel": 226.7e6, "demag_rows_inv_kernel": 127.7e6,
+NCU_TRAFFIC_CFG4 = {   # profiles/r1f_summary.md
+    "colour_pass_kernel": 114.4e6, "demag_rows_fwd_kernel": 100.2e6, "demag_columns_kernel": 452.9e6,
+    "demag_z_inverse_kernel": 226.8e6, "demag_rows_inv_kernel": 128.6e6,
 }
 
 
