@@ -121,7 +121,7 @@ int mmc_sweep_timed(mmc_ctx* ctx, int n_sweeps, double* phase_ms);
  * in tesla; any of them may be NULL (then the field is only computed).  Works with demag disabled too. */
 int mmc_demag_field(mmc_ctx* ctx, float* bx, float* by, float* bz);
 int mmc_get_observables(mmc_ctx* ctx, mmc_obs* host_out);      /* synchronises */
-int mmc_reset_counters(mmc_ctx* ctx);                          /* accepted/trials := 0 */
+int mmc_reset_counters(mmc_ctx* ctx);                          /* accepted/trials := 0; the cone controller's window is not touched */
 int mmc_reset_averages(mmc_ctx* ctx);                          /* run_mean_* := 0 */
 /* Histograms of the current state over the non-empty cells, the paper's verification read-outs (PAPER.md:108 length
  * distribution, PAPER.md:114 angular deviation from the mean direction).  kind 0: x = |m|; kind 1: x =

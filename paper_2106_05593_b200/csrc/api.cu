@@ -635,7 +635,9 @@ int mmc_reset_counters(mmc_ctx* c)
     Control h;
     CU(c, cudaMemcpyAsync(&h, c->ctl, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
-    h.accepted = h.trials = 0; h.win_accepted = h.win_trials = 0; h.win_sweeps = 0;
+    // the read-out is accepted + win_accepted: zero it without disturbing the cone controller's 100-iteration window
+    // (unsigned wrap-around: the window's counts are added back when it closes)
+    h.accepted = 0ull - h.win_accepted; h.trials = 0ull - h.win_trials;
     CU(c, cudaMemcpyAsync(c->ctl, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     return MMC_OK;
