@@ -158,8 +158,14 @@ def _peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def _workload(cfg: int, small: bool):
+def _workload(cfg: int, small: bool, shape=None):
     import workloads as W
+    if shape:                                     # same recipe on another mesh (the L2-exceeding stand-in); not a bench line
+        dims = [int(x) for x in shape.split(",")]
+        kw = dict(nx=dims[0], ny=dims[1])
+        if len(dims) > 2 and cfg in (4, 6):
+            kw["nz"] = dims[2]
+        return W.make(cfg, **kw)
     if small:
         kw = {1: {}, 2: dict(nx=64, ny=64), 3: dict(nx=64, ny=64), 4: dict(nx=64, ny=64, nz=4), 5: dict(nx=140, ny=140),
               6: dict(nx=64, ny=64, nz=4)}[cfg]
@@ -227,7 +233,7 @@ def run_ours(args):
     import paper_2106_05593_b200 as P
     import workloads as W
     cfg = args.config
-    wl = _workload(cfg, args.small)
+    wl = _workload(cfg, args.small, args.shape)
     wl.adaptive_cone = False                      # fixed cone/sigma for throughput runs (SURVEY 8(d) timing protocol)
     wl.seed = replica_seed(wl.seed, rank)
     g = P.MMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, device=local)
@@ -308,7 +314,7 @@ def run_ours(args):
             d["share_of_step"] = d["launch_ms"] * d["launches_per_step"] / step_ms if step_ms > 0 else None
             if "flops" in d:
                 d["achieved_TFLOPs"] = d["flops"] / t / 1e12 if t > 0 else 0.0
-            d["ncu_traffic_bytes"] = NCU_TRAFFIC_CFG4.get(k) if (cfg == 4 and not args.small) else None
+            d["ncu_traffic_bytes"] = NCU_TRAFFIC_CFG4.get(k) if (cfg == 4 and not args.small and not args.shape) else None
         dom = max(kern, key=lambda k: kern[k]["launch_ms"])          # the dominant kernel = longest single launch
         dk = kern[dom]
         demag_ms = sum(phases[k] for k in ("pack", "rows_fwd", "columns", "rows_inv", "z_inverse")) / K
@@ -363,6 +369,7 @@ def main():
                     help="BASELINE.json config (default 4: the largest fully magnetic mesh, 1024x1024x4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--small", action="store_true", help="reduced mesh (debugging only; not a bench number)")
+    ap.add_argument("--shape", default=None, help="nx,ny[,nz]: the config's recipe on another mesh (exploration; not a bench number)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     if args.impl == "reference":
