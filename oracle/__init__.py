@@ -55,6 +55,7 @@ class _Problem(C.Structure):
         ("bdx", C.c_void_p), ("bdy", C.c_void_p), ("bdz", C.c_void_p),
         ("one_minus_cos_cone", C.c_double), ("seed", C.c_uint64),
         ("K1cT", C.c_void_p), ("K2cT", C.c_void_p), ("cub", C.c_void_p),
+        ("K2T", C.c_void_p), ("me2", C.c_void_p),
     ]
 
 
@@ -215,6 +216,7 @@ class Material:
     K1c: float = 0.0; K2c: float = 0.0
     c1x: float = 1.0; c1y: float = 0.0; c1z: float = 0.0
     c2x: float = 0.0; c2y: float = 1.0; c2z: float = 0.0
+    K2: float = 0.0          # 4th-order uniaxial constant of Eq. (11), J/m^3, same axis as K1
 
 
 def cubic_axes(r):
@@ -252,6 +254,7 @@ class OracleMMC:
         self.demag_r_near = 32
         self._demag = None
         self.has_cubic = False
+        self.has_k2 = False
         self.seed = 0
         self.sweep = 0
         self.accepted = 0; self.trials = 0
@@ -345,6 +348,12 @@ class OracleMMC:
                     k1[q] = r.K1c * cls["me"][q] ** 10; k2[q] = r.K2c * cls["me"][q] ** 21
             arr["K1cT"] = np.ascontiguousarray(k1[inv]); arr["K2cT"] = np.ascontiguousarray(k2[inv])
             arr["cub"] = np.ascontiguousarray(ax9[inv])
+        # 4th-order uniaxial term of Eq. (11): K2(T) = K2 me^10 (l = 4); zero at and above Tc (me = 0)
+        self.has_k2 = any(r.Ms0 > 0 and r.K2 != 0 for r in self.regions)
+        if self.has_k2:
+            k2 = np.array([self.regions[reg[first[q]]].K2 * cls["me"][q] ** 10 for q in range(uniq.size)])
+            arr["K2T"] = np.ascontiguousarray(k2[inv])
+            arr["me2"] = np.ascontiguousarray(np.where(cls["me"] > 0, cls["me"] ** 2, 1.0)[inv])
         self.coef = arr
         self._dirty = False
 
@@ -370,6 +379,10 @@ class OracleMMC:
             p.K1cT, p.K2cT, p.cub = (self.coef[k].ctypes.data for k in ("K1cT", "K2cT", "cub"))
         else:
             p.K1cT = p.K2cT = p.cub = None
+        if self.has_k2:
+            p.K2T, p.me2 = self.coef["K2T"].ctypes.data, self.coef["me2"].ctypes.data
+        else:
+            p.K2T = p.me2 = None
         return p
 
     # -- demag ----------------------------------------------------------------------------

@@ -157,6 +157,9 @@ typedef struct {
     /* cubic anisotropy, Eq. (12): NULL = none */
     const double *K1cT, *K2cT;    /* N, K1c me^10 and K2c me^21 (me^(l(l+1)/2), l = 4, 6), 0 for T >= Tc */
     const double *cub;            /* 9N: the three orthonormal cubic axes of the cell, cub[9c + 3a + q] */
+    /* 4th-order uniaxial term of Eq. (11), reading G5 (m_i there = M/Ms(T) = m/me): NULL = none */
+    const double *K2T;            /* N, K2 me^10 (l = 4 in me^(l(l+1)/2)), 0 for T >= Tc */
+    const double *me2;            /* N, me^2 */
 } orc_problem;
 
 /* Eq. (12): alpha^2 beta^2 + alpha^2 gamma^2 + beta^2 gamma^2 and alpha^2 beta^2 gamma^2 of the DIRECTION of v          */
@@ -285,6 +288,13 @@ void orc_cell_dF(const orc_problem *p, const double *mx, const double *my, const
     double dme = dm[0] * e[0] + dm[1] * e[1] + dm[2] * e[2];
     double sme = (2 * m[0] + dm[0]) * e[0] + (2 * m[1] + dm[1]) * e[1] + (2 * m[2] + dm[2]) * e[2];
     terms[1] = -beta * V * p->Kq[c] * dme * sme;
+    /* Eq. (11), second term, times V (the paper's V is missing there, G5): K2(T) [1 - (m.e)^2/me^2]^2, trial minus current */
+    if (p->K2T && p->K2T[c] != 0.0) {
+        double q0 = m[0] * e[0] + m[1] * e[1] + m[2] * e[2];
+        double q1 = q0 + dme;
+        double g0 = 1.0 - q0 * q0 / p->me2[c], g1 = 1.0 - q1 * q1 / p->me2[c];
+        terms[1] += beta * V * p->K2T[c] * (g1 * g1 - g0 * g0);
+    }
     /* cubic anisotropy, Eq. (12), both terms times V: the plain difference of the energy of the trial and the current direction */
     if (p->cub) {
         double mp[3] = { m[0] + dm[0], m[1] + dm[1], m[2] + dm[2] };
@@ -421,6 +431,7 @@ void orc_observables(const orc_problem *p, const double *mx, const double *my, c
         Edmi += -p->D0 * V * (m[0] * G[0] + m[1] * G[1] + m[2] * G[2]);
         double me_ = m[0] * p->ax[c] + m[1] * p->ay[c] + m[2] * p->az[c];
         Ean += V * (p->K1T[c] - p->Kq[c] * me_ * me_);
+        if (p->K2T && p->K2T[c] != 0.0) { double g = 1.0 - me_ * me_ / p->me2[c]; Ean += V * p->K2T[c] * g * g; }
         if (p->cub) {
             double c1, c2;
             orc_cubic_invariants(p->cub + 9 * c, m, &c1, &c2);

@@ -591,3 +591,39 @@ def test_cubic_anisotropy_single_cell_distribution():
     expect = np.trapezoid(np.trapezoid(c1 * w, ph, axis=1), th) / np.trapezoid(np.trapezoid(w, ph, axis=1), th)
     assert kappa > 1.0 and expect < 0.19
     assert acc / n == pytest.approx(expect, rel=2e-2)
+
+
+def test_uniaxial_k2_term_of_eq11():
+    """Second term of Eq. (11) (reading G5: m_i = m/me, both terms times V, K2(T) = K2 me^10): the textbook
+    K2 sin^4(theta) for a vector of the equilibrium length at polar angle theta to the axis, zero along the axis, the me^10
+    temperature scaling, zero at Tc, and local dF == difference of the read-out."""
+    V = (5e-9) ** 3
+    def cell(T, K1=0.0, K2=2e5):
+        s = O.OracleMMC(2, 2, 1, 5e-9, 5e-9, 5e-9, 0, store_fp32=False)
+        s.set_material([O.Material(Ms0=8e5, A0=0.0, K1=K1, K2=K2, ax=0.0, ay=0.6, az=0.8, Tc=870.0)], None)
+        s.set_temperature(T, None)
+        return s
+    me = O.me_of_T(300.0, 870.0)
+    s = cell(300.0)
+    e = np.array([0.0, 0.6, 0.8]); perp = np.array([1.0, 0.0, 0.0])
+    for th in (0.0, 0.3, 1.0, np.pi / 2):
+        v = me * (np.cos(th) * e + np.sin(th) * perp)
+        s.set_m(*[np.full(4, x) for x in v])
+        assert s.observables()["E_an"] / 4 == pytest.approx(V * 2e5 * me ** 10 * np.sin(th) ** 4, rel=1e-11, abs=1e-30)
+    # temperature scaling and T = Tc
+    v = np.array([0.4, 0.1, 0.2])
+    Es = []
+    for T in (300.0, 700.0):
+        s = cell(T); s.set_m(*[np.full(4, x) for x in v]); Es.append(s.observables()["E_an"])
+    m3, m7 = O.me_of_T(300.0, 870.0), O.me_of_T(700.0, 870.0)
+    g = lambda me_: (1 - (v @ e) ** 2 / me_ ** 2) ** 2 * me_ ** 10
+    assert Es[1] / Es[0] == pytest.approx(g(m7) / g(m3), rel=1e-10)
+    s = cell(870.0); s.set_m(*[np.full(4, x) for x in v]); assert s.observables()["E_an"] == 0.0
+    # local dF (K1 and K2 together) = difference of the read-out
+    s = cell(300.0, K1=5e5)
+    s.set_m(*[np.full(4, x) for x in v])
+    dm = np.array([0.05, -0.2, 0.1])
+    eb = s.observables()["E_an"]; t = s.cell_dF(0, 1, 0, dm)
+    for a in range(3):
+        s.m[a][2] += dm[a]
+    assert t[1] * KB * 300.0 == pytest.approx(s.observables()["E_an"] - eb, rel=1e-10)
