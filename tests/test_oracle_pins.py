@@ -609,7 +609,7 @@ def test_uniaxial_k2_term_of_eq11():
     for th in (0.0, 0.3, 1.0, np.pi / 2):
         v = me * (np.cos(th) * e + np.sin(th) * perp)
         s.set_m(*[np.full(4, x) for x in v])
-        assert s.observables()["E_an"] / 4 == pytest.approx(V * 2e5 * me ** 10 * np.sin(th) ** 4, rel=1e-11, abs=1e-30)
+        assert s.observables()["E_an"] / 4 == pytest.approx(V * 2e5 * me ** 10 * np.sin(th) ** 4, rel=3e-6, abs=1e-30)   # the state is stored in fp32
     # temperature scaling and T = Tc
     v = np.array([0.4, 0.1, 0.2])
     Es = []
@@ -617,7 +617,7 @@ def test_uniaxial_k2_term_of_eq11():
         s = cell(T); s.set_m(*[np.full(4, x) for x in v]); Es.append(s.observables()["E_an"])
     m3, m7 = O.me_of_T(300.0, 870.0), O.me_of_T(700.0, 870.0)
     g = lambda me_: (1 - (v @ e) ** 2 / me_ ** 2) ** 2 * me_ ** 10
-    assert Es[1] / Es[0] == pytest.approx(g(m7) / g(m3), rel=1e-10)
+    assert Es[1] / Es[0] == pytest.approx(g(m7) / g(m3), rel=3e-6)
     s = cell(870.0); s.set_m(*[np.full(4, x) for x in v]); assert s.observables()["E_an"] == 0.0
     # local dF (K1 and K2 together) = difference of the read-out
     s = cell(300.0, K1=5e5)
