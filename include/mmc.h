@@ -59,6 +59,7 @@ typedef struct mmc_ctx mmc_ctx;   /* opaque, owned by the library */
 typedef struct {
     double Ms0, A0, K1, ax, ay, az, D0, Tc, mu_atom;
     double K1c, K2c, c1x, c1y, c1z, c2x, c2y, c2z;
+    double K2;      /* 4th-order uniaxial constant of Eq. (11) at T = 0, J/m^3, same axis as K1: F = V K2(T) [1 - (m.e)^2/me^2]^2, K2(T) = K2 me^10 */
 } mmc_material;
 
 /* Read-out (PAPER.md:100 acceptance rate; PAPER.md:135 average magnetisation; Appendix B energies).

@@ -38,11 +38,11 @@ class MMCError(RuntimeError):
 class Material(C.Structure):
     """mmc_material (SI units; Ms0 == 0 marks an empty region)."""
     _fields_ = [(n, C.c_double) for n in ("Ms0", "A0", "K1", "ax", "ay", "az", "D0", "Tc", "mu_atom",
-                                          "K1c", "K2c", "c1x", "c1y", "c1z", "c2x", "c2y", "c2z")]
+                                          "K1c", "K2c", "c1x", "c1y", "c1z", "c2x", "c2y", "c2z", "K2")]
 
     def __init__(self, Ms0=0.0, A0=0.0, K1=0.0, ax=0.0, ay=0.0, az=1.0, D0=0.0, Tc=1.0, mu_atom=MUB,
-                 K1c=0.0, K2c=0.0, c1x=1.0, c1y=0.0, c1z=0.0, c2x=0.0, c2y=1.0, c2z=0.0):
-        super().__init__(Ms0, A0, K1, ax, ay, az, D0, Tc, mu_atom, K1c, K2c, c1x, c1y, c1z, c2x, c2y, c2z)
+                 K1c=0.0, K2c=0.0, c1x=1.0, c1y=0.0, c1z=0.0, c2x=0.0, c2y=1.0, c2z=0.0, K2=0.0):
+        super().__init__(Ms0, A0, K1, ax, ay, az, D0, Tc, mu_atom, K1c, K2c, c1x, c1y, c1z, c2x, c2y, c2z, K2)
 
 
 class Obs(C.Structure):

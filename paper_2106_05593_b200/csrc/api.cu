@@ -183,7 +183,7 @@ int ensure_setup(mmc_ctx* c)
         // cubic anisotropy: K(T) = K me^(l(l+1)/2), l = 4, 6; axes by Gram-Schmidt, e3 = e1 x e2
         outc[CS_BK1C] = (float)(beta * V * mt.K1c * std::pow(k.th.me, 10.0));
         outc[CS_BK2C] = (float)(beta * V * mt.K2c * std::pow(k.th.me, 21.0));
-        outc[11] = 0.f;
+        outc[CS_BK2U] = (float)(k.th.me > 0 ? beta * V * mt.K2 * std::pow(k.th.me, 6.0) : 0.0);
         double e1[3] = { mt.c1x, mt.c1y, mt.c1z }, e2[3] = { mt.c2x, mt.c2y, mt.c2z };
         double n1 = std::sqrt(e1[0] * e1[0] + e1[1] * e1[1] + e1[2] * e1[2]);
         if (!(n1 > 0)) { e1[0] = 1; e1[1] = e1[2] = 0; n1 = 1; }
@@ -210,6 +210,7 @@ int ensure_setup(mmc_ctx* c)
             cf.ax = v[CS_AX]; cf.ay = v[CS_AY]; cf.az = v[CS_AZ];
             cf.bK1c = vc[CS_BK1C]; cf.bK2c = vc[CS_BK2C];
             for (int q = 0; q < 9; ++q) cf.cub[q] = vc[CS_CUB + q];
+            cf.bK2u = vc[CS_BK2U];
             c->K1T_u = v[CS_K1T]; c->c0_u = v[CS_C0];
             c->sigma_first = v[CS_SIGMA];
         }
@@ -225,7 +226,7 @@ int ensure_setup(mmc_ctx* c)
         if (tab.size() > c->table_cap) { cudaFree(c->table); cudaFree(c->table_cubic); c->table = c->table_cubic = nullptr; c->table_cap = tab.size(); }
         rc = upload(c, &c->table, tab); if (rc) return rc;
         bool cubic = false;
-        for (const auto& r : c->regions) if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0)) cubic = true;
+        for (const auto& r : c->regions) if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0 || r.K2 != 0.0)) cubic = true;
         if (cubic) { rc = upload(c, &c->table_cubic, tabc); if (rc) return rc; }
         std::vector<uint32_t> cw(S, 0u);
         for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
@@ -245,7 +246,7 @@ int ensure_setup(mmc_ctx* c)
     if (c->demag_enabled) f |= F_DEMAG;
     if (n_active == (unsigned long long)N) f |= F_DENSE;
     for (const auto& r : c->regions)
-        if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0)) f |= F_CUBIC;
+        if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0 || r.K2 != 0.0)) f |= F_CUBIC;
     c->features = f;
     c->dirty = false;
     return MMC_OK;
@@ -339,7 +340,7 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     c->g.H = (int64_t)c->g.hx * ny * nz;
     c->dx = dx; c->dy = dy; c->dz = dz; c->V = dx * dy * dz;
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
-    c->regions.push_back(mmc_material{ 0, 0, 0, 0, 0, 1, 0, 1, 9.2740100783e-24, 0, 0, 1, 0, 0, 0, 1, 0 });
+    c->regions.push_back(mmc_material{ 0, 0, 0, 0, 0, 1, 0, 1, 9.2740100783e-24, 0, 0, 1, 0, 0, 0, 1, 0, 0 });
     DeviceGuard dg(device);
     auto bail = [&](int code) { mmc_destroy(c); return code; };
     if (!dg.ok) return bail(MMC_E_CUDA);

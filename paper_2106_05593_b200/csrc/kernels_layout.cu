@@ -115,13 +115,14 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
         const double me_ = m[0] * ax + m[1] * ay + m[2] * az;
         acc[5] += kT * ((double)K1T - (double)bKq * me_ * me_);
         {   // cubic anisotropy, Eq. (12): direction cosines with respect to the class's cubic axes
-            const float* cb; float bK1c, bK2c;
+            const float* cb; float bK1c, bK2c, bK2u = 0.f;
             if (PERCELL) {
                 if (a.table_cubic) { const float* t = reinterpret_cast<const float*>(a.table_cubic) + (size_t)kClassFloats * (a.cw[s] >> 7);
-                                     cb = t + CS_CUB; bK1c = t[CS_BK1C]; bK2c = t[CS_BK2C]; }
+                                     cb = t + CS_CUB; bK1c = t[CS_BK1C]; bK2c = t[CS_BK2C]; bK2u = t[CS_BK2U]; }
                 else { cb = a.coef.cub; bK1c = 0.f; bK2c = 0.f; }
             }
-            else { cb = a.coef.cub; bK1c = a.coef.bK1c; bK2c = a.coef.bK2c; }
+            else { cb = a.coef.cub; bK1c = a.coef.bK1c; bK2c = a.coef.bK2c; bK2u = a.coef.bK2u; }
+            if (bK2u != 0.f) { const double gq = mu2 - me_ * me_; acc[5] += kT * (double)bK2u * gq * gq; }      // V K2(T) [1 - (m.e)^2/me^2]^2
             if (bK1c != 0.f || bK2c != 0.f) {
                 const double il = 1.0 / sqrt(l2);
                 const double al = (m[0] * cb[0] + m[1] * cb[1] + m[2] * cb[2]) * il, be = (m[0] * cb[3] + m[1] * cb[4] + m[2] * cb[5]) * il,

@@ -69,7 +69,7 @@ __device__ __forceinline__ void sincos_2pi(float u, float* sn, float* cs)
 struct CellCoef {
     float kx, ky, kz, gx, gy, bKq, bzee, c4, sigma, ax, ay, az;
     double mu2;
-    float bK1c, bK2c, cub[9];          // cubic anisotropy (only read when CUBIC)
+    float bK1c, bK2c, cub[9], bK2u;    // higher-order anisotropy (only read when CUBIC)
 };
 
 // cubic table slots CS_BK1C, CS_BK2C, CS_CUB .. CS_CUB + 8 of a class
@@ -78,7 +78,7 @@ __device__ __forceinline__ void load_cubic(const float4* t, CellCoef& cf)
     const float4 t3 = __ldg(t), t4 = __ldg(t + 1), t5 = __ldg(t + 2);
     cf.bK1c = t3.x; cf.bK2c = t3.y; cf.cub[0] = t3.z; cf.cub[1] = t3.w;
     cf.cub[2] = t4.x; cf.cub[3] = t4.y; cf.cub[4] = t4.z; cf.cub[5] = t4.w;
-    cf.cub[6] = t5.x; cf.cub[7] = t5.y; cf.cub[8] = t5.z;
+    cf.cub[6] = t5.x; cf.cub[7] = t5.y; cf.cub[8] = t5.z; cf.bK2u = t5.w;
 }
 
 struct CellResult { float dm[3]; float f, L; float terms[6]; float margin; bool accept; };
@@ -133,6 +133,13 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
     const float sme = fmaf(fmaf(2.f, m[0], dm0), cf.ax, fmaf(fmaf(2.f, m[1], dm1), cf.ay, fmaf(2.f, m[2], dm2) * cf.az));
     float an = -cf.bKq * dme * sme;
     if (CUBIC) {
+        // Eq. (11), second term: V K2(T) [1 - q/me^2]^2 with q = (m.e)^2; its change is -dq (2 (me^2 - q) - dq) K2(T)/me^4,
+        // dq = (dm.e)((2m+dm).e); bK2u = beta V K2(T)/me^4, mu2 = me^2 below Tc (bK2u = 0 above)
+        {
+            const float qe = fmaf(m[0], cf.ax, fmaf(m[1], cf.ay, m[2] * cf.az));
+            const float dq = dme * sme;
+            an = fmaf(-cf.bK2u * dq, fmaf(2.f, (float)cf.mu2 - qe * qe, -dq), an);
+        }
         // Eq. (12) for the directions n and n' = n + dn (the trial vector is L f (n + dn)): squares of the direction cosines
         // A, B, G and their changes dA = d(alpha)(2 alpha + d(alpha)), ...; both invariants as differences without cancellation
         const float al = fmaf(n0, cf.cub[0], fmaf(n1, cf.cub[1], n2 * cf.cub[2]));
@@ -322,7 +329,7 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
         } else {
             cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
             cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
-            if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; }
+            if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; cf.bK2u = a.coef.bK2u; }
         }
         cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
         cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
@@ -485,7 +492,7 @@ __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_ke
             } else {
                 cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
                 cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
-                if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; }
+                if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; cf.bK2u = a.coef.bK2u; }
             }
             cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
             cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;

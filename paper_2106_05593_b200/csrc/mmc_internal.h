@@ -49,6 +49,7 @@ struct Coef {
     float Bx, By, Bz;       // applied field, tesla
     float bK1c, bK2c;       // beta V K1c me^10, beta V K2c me^21  (cubic anisotropy, Eq. (12))
     float cub[9];           // the three orthonormal cubic axes
+    float bK2u;             // beta V K2 me^6 = beta V K2(T) / me^4  (4th-order uniaxial term of Eq. (11))
 };
 
 // Per-cell mode (more than one coefficient class, e.g. cfg 4: one class per distinct (region, T) pair): every cell
@@ -60,7 +61,7 @@ constexpr int kClassFloats = 12;      // three 16-byte loads per class and table
 enum ClassSlot { CS_INVT = 0, CS_C4 = 1, CS_MU2 = 2 /* double in slots 2,3 */, CS_BKQ = 4, CS_BZEE = 5, CS_SIGMA = 6,
                  CS_AX = 7, CS_AY = 8, CS_AZ = 9, CS_K1T = 10 /* beta V K1(T), read-out only */,
                  CS_C0 = 11 /* c0 - c4 mu2^2, read-out only */,
-                 /* second table (cubic anisotropy), same stride: */ CS_BK1C = 0, CS_BK2C = 1, CS_CUB = 2 /* 9 floats */ };
+                 /* second table (cubic anisotropy), same stride: */ CS_BK1C = 0, CS_BK2C = 1, CS_CUB = 2 /* 9 floats */, CS_BK2U = 11 };
 constexpr unsigned kMaxClasses = 1u << 25;
 constexpr float kSumScale = 4194304.f;              // 2^22: fixed-point scale of the running sums (a warp's sum fits int32 for |m| < 8; blocks add in 64 bits)
 
@@ -84,7 +85,7 @@ enum Feature : unsigned {
     F_DMI = 8u,
     F_DEMAG = 16u,
     F_DENSE = 32u,
-    F_CUBIC = 64u,    // cubic anisotropy, Eq. (12)    // no empty cell: every in-mesh cell is active, so no load has to wait for the mask / class word
+    F_CUBIC = 64u,    // higher-order anisotropy: cubic, Eq. (12), and the K2 term of Eq. (11) (second class table)    // no empty cell: every in-mesh cell is active, so no load has to wait for the mask / class word
 };
 
 struct SweepArgs {

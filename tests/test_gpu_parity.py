@@ -99,6 +99,13 @@ def _small(cfg, **kw):
     return W.make(cfg, **kw)
 
 
+def _with_k2(wl, K2):
+    for r in wl.regions:
+        if r["Ms0"] > 0:
+            r["K2"] = K2                              # 4th-order uniaxial term of Eq. (11)
+    return wl
+
+
 CASES = {
     "cfg1_32x32": lambda: W.cfg1(),
     "cfg1_paper_regime": lambda: W.cfg1(paper_regime=True),
@@ -115,6 +122,9 @@ CASES = {
     # cubic anisotropy (Eq. (12), K1c + K2c, random cubic axes per grain), periodic in the plane, phase-separated grains
     "fe_film_cubic_48x40x3": lambda: W.fe_film(nx=48, ny=40, nz=3),
     "fe_film_cubic_36x22x10": lambda: W.fe_film(nx=36, ny=22, nz=10),
+    # K1 + K2 of Eq. (11): uniform film (kernel arguments) and granular film (class tables, tilted axes, T > Tc in the hot spot)
+    "cfg1_k2_32x32": lambda: _with_k2(W.cfg1(paper_regime=True), -1.5e5),
+    "cfg4_k2_30x21x3": lambda: _with_k2(W.cfg4(nx=30, ny=21, nz=3), 4e5),
 }
 
 
@@ -137,7 +147,7 @@ def test_colour_pass_parity(name):
 
 
 @pytest.mark.parametrize("name", ["cfg1_paper_regime", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150",
-                                  "fe_film_cubic_48x40x3"])
+                                  "fe_film_cubic_48x40x3", "cfg4_k2_30x21x3"])
 def test_sweep_matches_replayed_oracle(name):
     """mmc_sweep(n) (demag -> red -> black -> counter++) against the oracle replaying the same iterations.  A cell whose
     decision flips inside the margin window makes the two trajectories differ from there on, so the bar is: the first
@@ -206,7 +216,7 @@ def test_demag_field_parity(shape, d):
 
 
 @pytest.mark.parametrize("name", ["cfg1_32x32", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg3_48x40_800K", "cfg4_30x21x3", "cfg5_160x150",
-                                  "fe_film_cubic_48x40x3"])
+                                  "fe_film_cubic_48x40x3", "cfg1_k2_32x32", "cfg4_k2_30x21x3"])
 def test_observables_parity(name):
     wl = CASES[name]()
     g, o = _gpu(wl), _orc(wl)
