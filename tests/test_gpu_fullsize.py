@@ -252,3 +252,46 @@ def test_gpu_angular_distribution_is_langevin():
         expect = 1.0 / np.tanh(xi) - 1.0 / xi
         assert ob["run_mean_m"][2] / L == pytest.approx(expect, abs=3e-4), f"xi = {xi}"
         assert abs(ob["run_mean_m"][0]) < 3e-4 and abs(ob["run_mean_m"][1]) < 3e-4
+
+
+# ------------------------------------------------------------------------------------------------ whole schedules (soak)
+def test_cfg2_hysteresis_branch_full_size():
+    """BASELINE.json config 2 as written: 256x256x1 permalloy film, demag, B_x from +100 mT to -100 mT in 2 mT steps, 200
+    iterations per step (20 200 iterations with the adaptive cone).  Sanity of the physics over a long run: the film starts
+    and ends saturated along the field, the branch is monotone within noise, reverses in one piece, |m| stays at me(300 K), the
+    acceptance rate is held near 0.5 by the cone controller, nothing leaves the physical range."""
+    import paper_2106_05593_b200 as P
+    from paper_2106_05593_b200.schedule import run_schedule
+    wl = W.make(2)
+    g = _gpu(wl)
+    rows = run_schedule(g, wl)
+    mx = np.array([r["mean_m"][0] for r in rows]); ml = np.array([r["mean_len"] for r in rows])
+    assert len(rows) == 101 and g.observables()["sweeps_done"] == 20200
+    assert mx[0] > 0.8 and mx[-1] < -0.5                              # 200 iterations per step: the reversal is under way, not complete
+    assert np.all(np.diff(mx) < 5e-3)                                  # decreasing field: m_x never climbs back
+    assert np.all(np.abs(ml - 0.8675) < 2e-3) and np.all(np.isfinite(mx))
+    acc = np.array([r["acceptance"] for r in rows[20:]])
+    assert np.all((acc > 0.35) & (acc < 0.65))
+    m = _np(g.get_m())
+    L = np.sqrt(m[0] ** 2 + m[1] ** 2 + m[2] ** 2)
+    assert L.max() < 1.0 and L.min() > 0.5
+    g.close()
+
+
+def test_cfg3_temperature_sweep_tracks_the_length_curve():
+    """BASELINE.json config 3 (reduced to 128x128 and 1000 iterations per temperature): T from 200 K to 800 K through Tc = 700 K
+    with the state carried over.  <|m|> follows me(T) far below Tc, stays ABOVE me near and above Tc (the mean
+    of the length distribution is not me), decreases monotonically, and the T = Tc step (reading G10) runs."""
+    from paper_2106_05593_b200.schedule import run_schedule
+    wl = W.cfg3(nx=128, ny=128)
+    wl.schedule = [("T", T, 1000) for (_, T, _) in wl.schedule]
+    g = _gpu(wl)
+    rows = run_schedule(g, wl)
+    T = np.array([r["value"] for r in rows]); ml = np.array([r["mean_len"] for r in rows])
+    assert 700.0 in T and T[0] == 200.0 and T[-1] == 800.0
+    assert np.all(np.diff(ml) < 0)
+    me = np.array([O.me_of_T(float(t), 700.0) for t in T])
+    assert abs(ml[0] - me[0]) < 2e-3                                   # 200 K: the chain sits at me
+    assert np.all(ml[T >= 650.0] > me[T >= 650.0] + 0.01)              # near and above Tc: mean length > me (0 above Tc)
+    assert ml[-1] < 0.2                                                # 800 K, 2 nm cells: a broad distribution around 0.14
+    g.close()
