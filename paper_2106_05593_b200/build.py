@@ -25,8 +25,9 @@ def _newer(target, deps):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
-    hdrs = [os.path.join(CSRC, "mmc_internal.h"), os.path.join(HERE, "..", "include", "mmc.h")]
+    hdrs = [os.path.join(CSRC, h) for h in ("mmc_internal.h", "fft_reg.cuh", "fft_smem.cuh")] + [os.path.join(HERE, "..", "include", "mmc.h")]
     objs = []
+    jobs = []
     for f in CU + CPP:
         src = os.path.join(CSRC, f)
         obj = os.path.join(OBJ, f.rsplit(".", 1)[0] + ".o")
@@ -36,10 +37,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
                 cmd = [NVCC] + NVFLAGS + ["-c", src, "-o", obj]
             else:
                 cmd = ["g++", "-O2", "-std=gnu++17", "-fPIC", "-I/usr/local/cuda/include", "-c", src, "-o", obj]
-            r = subprocess.run(cmd, capture_output=True, text=True)
-            log = os.path.join(OBJ, f + ".log")
-            with open(log, "w") as fh:
-                fh.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+            jobs.append((f, cmd))
+
+    def compile_one(job):
+        f, cmd = job
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        with open(os.path.join(OBJ, f + ".log"), "w") as fh:
+            fh.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+        return f, cmd, r
+
+    from concurrent.futures import ThreadPoolExecutor
+    with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 1))) as ex:     # the translation units compile side by side
+        for f, cmd, r in ex.map(compile_one, jobs):
             if verbose or r.returncode:
                 sys.stderr.write(r.stdout + r.stderr)
             if r.returncode:
