@@ -532,6 +532,11 @@ static int sweep_impl(mmc_ctx* c, int n_sweeps, PhaseTimer* timer)
     DeviceGuard dg(c->device);
     int rc = ready(c); if (rc) return rc;
     if (c->demag_enabled) { rc = ensure_demag(c); if (rc) return rc; }
+    if (!timer && !c->demag_enabled && n_sweeps > 0) {            // small meshes: all iterations in one launch
+        rc = launch_small_mesh_sweeps(make_args(c, 0), c->features, n_sweeps, c->stream);
+        if (rc == MMC_OK) return MMC_OK;
+        if (rc != MMC_E_UNSUPPORTED) return fail(c, rc, "small-mesh launch failed");
+    }
     if (timer) timer->mark(-1, c->stream);
     for (int it = 0; it < n_sweeps; ++it) {
         if (c->demag_enabled) { rc = compute_demag(c, timer); if (rc) return rc; }

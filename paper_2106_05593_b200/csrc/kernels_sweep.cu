@@ -252,25 +252,24 @@ __device__ __forceinline__ void pass_tail(const SweepArgs& a, PassTailSmem& sm, 
 #define MMC_PASS_THREADS 512
 #endif
 constexpr int kPassThreads = MMC_PASS_THREADS;      // CTA = 32 x BY x BZ brick of this many cells
-template <unsigned F, bool DEBUG>
-__global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads) colour_pass_kernel(const SweepArgs a)
+// coherent load for the persistent single-CTA kernel, whose passes read what earlier passes of the same launch wrote;
+// read-only path otherwise
+template <bool COHERENT> __device__ __forceinline__ float ldc(const float* p) { return COHERENT ? __ldcg(p) : __ldg(p); }   // .cg: from L2, never a stale line
+
+// One cell of the active colour: compact index q of row (j, k).  The body of the one-cell-per-thread pass.
+template <unsigned F, bool DEBUG, bool COHERENT>
+__device__ __forceinline__ void pass_one_cell(const SweepArgs& a, int col, int q, int j, int k, unsigned long long sweep, float omc,
+                                              bool& active, bool& accept, float& fs0, float& fs1, float& fs2, float& fs3)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0, CUBIC = (F & F_CUBIC) != 0;
-    __shared__ PassTailSmem s_tail;
-    pass_tail_init(s_tail);
-
     const int nx = a.g.nx, ny = a.g.ny, nz = a.g.nz, hx = a.g.hx;
     const unsigned pbc = a.g.pbc;
-    const int q = blockIdx.x * 32 + threadIdx.x;
-    const int j = blockIdx.y * blockDim.y + threadIdx.y;
-    const int k = HASZ ? blockIdx.z * blockDim.z + threadIdx.z : 0;
-    const int col = a.colour;
     const int s = ((j + k) & 1) ^ col;               // active cells of this row sit at i = 2q + s
     const int i = 2 * q + s;
-    bool active = i < nx && j < ny && k < nz;
-    bool accept = false;
-    float fs0 = 0.f, fs1 = 0.f, fs2 = 0.f, fs3 = 0.f;   // the cell's final vector and length (running sums)
+    active = i < nx && j < ny && k < nz;
+    accept = false;
+    fs0 = fs1 = fs2 = fs3 = 0.f;                      // the cell's final vector and length (running sums)
 
     // 32-bit element offsets: mmc_create guarantees 2 H < 2^31
     const unsigned H = (unsigned)a.g.H;
@@ -309,11 +308,11 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
         for (int c = 0; c < 3; ++c) {
             const float* __restrict__ P = a.m[c];
             m[c] = a.m[c][ownb];
-            xa[c] = __ldg(P + othb);
-            xb[c] = __ldg(P + oX);
-            yn[c] = __ldg(P + oN);
-            ys[c] = __ldg(P + oS);
-            if (HASZ) { zu[c] = __ldg(P + oU); zd[c] = __ldg(P + oD); }
+            xa[c] = ldc<COHERENT>(P + othb);
+            xb[c] = ldc<COHERENT>(P + oX);
+            yn[c] = ldc<COHERENT>(P + oN);
+            ys[c] = ldc<COHERENT>(P + oS);
+            if (HASZ) { zu[c] = ldc<COHERENT>(P + oU); zd[c] = ldc<COHERENT>(P + oD); }
             if (DEMAG) Bd[c] = __ldg(a.bd[c] + ownb);
         }
         CellCoef cf;
@@ -362,8 +361,6 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
             dxx = bE * e[0] - bW * wv[0];
             dyy = bN * yn[1] - bS * ys[1];
         }
-        const unsigned long long sweep = a.ctl->sweep;
-        const float omc = a.ctl->one_minus_cos_cone;
         const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
         const unsigned cell = (unsigned)row * nx + i;                     // natural cell index (< 2^31)
         const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
@@ -383,6 +380,20 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
         }
     }
 
+}
+
+template <unsigned F, bool DEBUG>
+__global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads) colour_pass_kernel(const SweepArgs a)
+{
+    constexpr bool HASZ = (F & F_Z) != 0;
+    __shared__ PassTailSmem s_tail;
+    pass_tail_init(s_tail);
+    const int q = blockIdx.x * 32 + threadIdx.x;
+    const int j = blockIdx.y * blockDim.y + threadIdx.y;
+    const int k = HASZ ? blockIdx.z * blockDim.z + threadIdx.z : 0;
+    bool active, accept;
+    float fs0, fs1, fs2, fs3;
+    pass_one_cell<F, DEBUG, false>(a, a.colour, q, j, k, a.ctl->sweep, a.ctl->one_minus_cos_cone, active, accept, fs0, fs1, fs2, fs3);
     pass_tail(a, s_tail, accept ? 1u : 0u, active ? 1u : 0u, fs0, fs1, fs2, fs3, kPassThreads / 32);
 }
 
@@ -541,7 +552,7 @@ __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_ke
 
 // S11 + bookkeeping, one thread: advance the sweep counter; every 100 iterations compare the acceptance rate with
 // 0.5 +- 0.05 and move the cone by one degree, clamped to [1, 180] degrees.
-__global__ void end_sweep_kernel(Control* ctl)
+__device__ __forceinline__ void end_sweep(Control* ctl)
 {
     ctl->sweep += 1ull;
     ctl->run_sweeps += 1ull;
@@ -558,6 +569,65 @@ __global__ void end_sweep_kernel(Control* ctl)
             ctl->one_minus_cos_cone = (float)(2.0 * h * h);
         }
         ctl->win_accepted = 0ull; ctl->win_trials = 0ull; ctl->win_sweeps = 0u;
+    }
+}
+__global__ void end_sweep_kernel(Control* ctl) { end_sweep(ctl); }
+
+// ------------------------------------------------------------------------------------------------ small meshes: all iterations in one launch
+// Meshes of a few thousand cells without demag (BASELINE.json config 1: 1024 cells) are bound by launch latency: three
+// launches per iteration take ~12 us while the arithmetic of a pass takes ~1 us.  Here ONE CTA runs n iterations in one
+// launch (SURVEY 8(d) "Config 1"): red pass, barrier, black pass, barrier, end-of-sweep bookkeeping by thread 0, barrier.
+// The cell arithmetic is pass_one_cell, the same function the one-cell pass uses, with coherent loads (a pass reads what
+// the previous pass of the same launch wrote; the state lives in this SM's L1/L2); counters and running sums are reduced
+// per pass with the same integer arithmetic, so the results are bit-identical to the launch-per-pass path.
+constexpr int kSmallThreads = 1024;
+constexpr int kSmallMaxCells = 1 << 13;         // <= 4 cells per thread and colour: a warp's fixed-point sum stays inside int32 for |m| < 2
+
+template <unsigned F>
+__global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(const SweepArgs a, int n_sweeps)
+{
+    __shared__ unsigned s_cnt;                        // accepted | trials << 16 would overflow: two words
+    __shared__ unsigned s_tri;
+    __shared__ long long s_sum[4];
+    const int tid = threadIdx.x;
+    const int hxr = (a.g.nx + 1) >> 1, rows = a.g.ny * a.g.nz, slots = hxr * rows;
+    Control* ctl = a.ctl;
+    for (int it = 0; it < n_sweeps; ++it) {
+        const unsigned long long sweep = *reinterpret_cast<volatile unsigned long long*>(&ctl->sweep);
+        const float omc = *reinterpret_cast<volatile float*>(&ctl->one_minus_cos_cone);
+        for (int col = 0; col < 2; ++col) {
+            if (tid == 0) { s_cnt = 0u; s_tri = 0u; s_sum[0] = s_sum[1] = s_sum[2] = s_sum[3] = 0; }
+            __syncthreads();
+            unsigned n_acc = 0u, n_tri = 0u;
+            int i0 = 0, i1 = 0, i2 = 0, i3 = 0;       // fixed point per thread: <= 32 cells of |m| < 2 stay inside int32
+            for (int idx = tid; idx < slots; idx += kSmallThreads) {
+                const int q = idx % hxr, row = idx / hxr, j = row % a.g.ny, k = row / a.g.ny;
+                bool active, accept;
+                float f0, f1, f2, f3;
+                pass_one_cell<F, false, true>(a, col, q, j, k, sweep, omc, active, accept, f0, f1, f2, f3);
+                n_acc += accept ? 1u : 0u; n_tri += active ? 1u : 0u;
+                i0 += __float2int_rn(f0 * kSumScale); i1 += __float2int_rn(f1 * kSumScale);
+                i2 += __float2int_rn(f2 * kSumScale); i3 += __float2int_rn(f3 * kSumScale);
+            }
+            const unsigned wa = __reduce_add_sync(0xffffffffu, n_acc), wt = __reduce_add_sync(0xffffffffu, n_tri);
+            const long long w0 = (long long)__reduce_add_sync(0xffffffffu, i0), w1 = (long long)__reduce_add_sync(0xffffffffu, i1),
+                            w2 = (long long)__reduce_add_sync(0xffffffffu, i2), w3 = (long long)__reduce_add_sync(0xffffffffu, i3);
+            if ((tid & 31) == 0) {
+                atomicAdd(&s_cnt, wa); atomicAdd(&s_tri, wt);
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[0]), (unsigned long long)w0);
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[1]), (unsigned long long)w1);
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[2]), (unsigned long long)w2);
+                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[3]), (unsigned long long)w3);
+            }
+            __syncthreads();                          // the pass is complete and visible to the whole CTA
+            if (tid == 0) {
+                ctl->win_accepted += s_cnt; ctl->win_trials += s_tri;
+                if (a.run_sums) for (int t = 0; t < 4; ++t) a.run_sums[t] += (unsigned long long)s_sum[t];
+                if (col == 1) end_sweep(ctl);
+                __threadfence_block();
+            }
+        }
+        __syncthreads();                              // the new sweep counter and cone are visible
     }
 }
 
@@ -601,6 +671,21 @@ static int launch_variant(const SweepArgs& a, bool debug, cudaStream_t st)
 // Instantiated variants: the smallest instantiated superset of the requested features is used.  F_PERCELL must
 // match exactly (its word array and table exist only in per-cell mode); the mask and B_d arrays always exist
 // (B_d = 0 when the demag term is off), so the other flags may be over-approximated.
+// n whole iterations in one launch for small meshes without demag; returns MMC_E_UNSUPPORTED when the mesh does not qualify
+// (the caller then takes the launch-per-pass path).  Variants: uniform coefficients only.
+int launch_small_mesh_sweeps(const SweepArgs& a, unsigned f, int n_sweeps, void* stream)
+{
+    cudaStream_t st = (cudaStream_t)stream;
+    const long long cells = (long long)a.g.nx * a.g.ny * a.g.nz;
+    if (cells > kSmallMaxCells || (f & (F_PERCELL | F_DEMAG | F_CUBIC))) return MMC_E_UNSUPPORTED;
+    f &= ~F_DENSE;
+    constexpr unsigned U = F_MASK | F_Z | F_DMI;
+    if (f == 0u) small_mesh_sweeps_kernel<0u><<<1, kSmallThreads, 0, st>>>(a, n_sweeps);
+    else if ((f & ~F_MASK) == 0u) small_mesh_sweeps_kernel<F_MASK><<<1, kSmallThreads, 0, st>>>(a, n_sweeps);
+    else small_mesh_sweeps_kernel<U><<<1, kSmallThreads, 0, st>>>(a, n_sweeps);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+
 int launch_colour_pass(const SweepArgs& a, unsigned f, bool debug, void* stream)
 {
     cudaStream_t st = (cudaStream_t)stream;

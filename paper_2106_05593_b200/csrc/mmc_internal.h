@@ -110,6 +110,7 @@ struct Observables { double sum[4]; double E[6]; unsigned long long n_active; };
 // kernels_sweep.cu
 int launch_colour_pass(const SweepArgs& a, unsigned features, bool debug, void* stream);
 int launch_end_sweep(Control* ctl, void* stream);
+int launch_small_mesh_sweeps(const SweepArgs& a, unsigned features, int n_sweeps, void* stream);
 // kernels_layout.cu
 int launch_to_split(const Geometry& g, const float* nat, float* split, void* stream);
 int launch_from_split(const Geometry& g, const float* split, float* nat, void* stream);

@@ -386,3 +386,25 @@ def test_histograms_parity(name):
     with pytest.raises(P.MMCError):
         g.histogram("length", 10, 1.0, 1.0)
     g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg1_32x32", "cfg1_paper_regime", "cfg1_ragged_40x24", "cfg1_ragged_periodic_12x6", "cfg1_k2_32x32"])
+def test_single_launch_small_mesh_path_is_bitwise_the_launch_per_pass_path(name):
+    """Small meshes without demag run all iterations of mmc_sweep in ONE launch (one CTA, SURVEY 8(d) "Config 1"); mmc_sweep_timed
+    keeps the launch-per-pass kernels.  Same cell arithmetic, integer reductions: states, counters, energies and the
+    adaptive cone must agree bit for bit after 230 iterations (two cone-controller windows and a partial one)."""
+    wl = CASES[name]()
+    wl.adaptive_cone = True
+    a, b = _gpu(wl), _gpu(wl)
+    a.sweep(230)
+    b.sweep_timed(230)
+    ma, mb = a.get_m(), b.get_m()
+    assert all(bool((ma[q] == mb[q]).all()) for q in range(3))
+    oa, ob = a.observables(), b.observables()
+    for k in ("accepted", "trials", "sweeps_done", "cone_deg", "run_sweeps", "E_ex", "E_an", "E_long"):
+        assert oa[k] == ob[k], k
+    # running means: both paths add 2^-22 fixed-point values; the launch-per-pass kernel rounds the sum of a thread's two
+    # cells, this one every cell: they agree to that quantum
+    assert abs(oa["run_mean_len"] - ob["run_mean_len"]) < 2.0 ** -22 and np.abs(oa["run_mean_m"] - ob["run_mean_m"]).max() < 2.0 ** -22
+    assert oa["sweeps_done"] == 230
+    a.close(); b.close()
