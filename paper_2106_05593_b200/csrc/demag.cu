@@ -478,8 +478,14 @@ struct ColFastArgs {
 #ifndef MMC_COLS_MINB
 #define MMC_COLS_MINB 3
 #endif
-template <int LGN, bool HALF>
-__global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G, fftr::Shape<LGN>::T >= 256 ? 2 : MMC_COLS_MINB)
+#ifndef MMC_COLS_MINB_PLANAR
+#define MMC_COLS_MINB_PLANAR 3
+#endif
+// PLANAR (one layer, Pz == 1, no xz / yz spectrum): B_z = K_zz M_z decouples from (B_x, B_y), so the in-plane pair and the
+// z component go through the transforms one after the other and a thread holds two components instead of three.
+template <int LGN, bool HALF, bool PLANAR>
+__global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G,
+                                  fftr::Shape<LGN>::T >= 256 ? 2 : (PLANAR ? MMC_COLS_MINB_PLANAR : MMC_COLS_MINB))
 columns_fast_kernel(const ColFastArgs a)
 {
     using S = fftr::Shape<LGN>;
@@ -488,6 +494,76 @@ columns_fast_kernel(const ColFastArgs a)
     float2* s1 = sm + threadIdx.y * S::SMEM;
     float2* s2 = s1 + S::S1;
     const int tid = threadIdx.x;
+    if constexpr (PLANAR) {
+        const int kxr = blockIdx.x * S::G + threadIdx.y;
+        const bool live = kxr < a.Cx;
+        const int kx = live ? kxr : a.Cx - 1;
+        const int ny = a.ny;
+        const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), a.tw1, a.tw2 };
+        const size_t nb = (size_t)kx * N + tid;
+        float2 v[2][16];
+        // in-plane pair: load, the xx / yy / xy spectrum into L2 meanwhile, two forward transforms, 2x2 multiply, two inverse
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const float2* __restrict__ col = a.Tin + ((size_t)c * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const int j = tid + n1 * T;
+                v[c][n1] = (n1 < NL && (HALF || j < ny)) ? col[j] : make_float2(0.f, 0.f);
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+#pragma unroll
+            for (int e = 0; e < 16; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
+        }
+#pragma unroll
+        for (int c = 0; c < 2; ++c) fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float2 u = v[0][e], w1 = v[1][e];
+            const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T), xy = __ldg(a.nhat[3] + nb + e * T);
+            v[0][e].x = fmaf(xx, u.x, xy * w1.x); v[0][e].y = fmaf(xx, u.y, xy * w1.y);
+            v[1][e].x = fmaf(xy, u.x, yy * w1.x); v[1][e].y = fmaf(xy, u.y, yy * w1.y);
+        }
+        __syncthreads();                               // every thread is done reading exchange buffer 2
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
+            float2* __restrict__ col = a.Tout + ((size_t)c * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < NL; ++n1) {
+                const int j = tid + n1 * T;
+                if (live && (HALF || j < ny)) col[j] = v[c][n1];
+            }
+        }
+        // z component in the registers of the first
+        {
+            float2 (&z)[16] = v[0];
+            const float2* __restrict__ cin = a.Tin + ((size_t)2 * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const int j = tid + n1 * T;
+                z[n1] = (n1 < NL && (HALF || j < ny)) ? cin[j] : make_float2(0.f, 0.f);
+            }
+            __syncthreads();                           // the last inverse transform read exchange buffer 1
+            fftr::forward<LGN, HALF, true>(z, s1, s2, tw, tid);
+#pragma unroll
+            for (int e = 0; e < 16; ++e) {
+                const float zz = __ldg(a.nhat[2] + nb + e * T);
+                z[e].x *= zz; z[e].y *= zz;
+            }
+            __syncthreads();
+            fftr::inverse<LGN, true>(z, s1, s2, tw, tid);
+            float2* __restrict__ col = a.Tout + ((size_t)2 * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < NL; ++n1) {
+                const int j = tid + n1 * T;
+                if (live && (HALF || j < ny)) col[j] = z[n1];
+            }
+        }
+        return;
+    }
     // with the fused z-DFT the Pz CTAs of one kx read the same layers: kz is the fastest block index so that they run
     // together and all but the first find them in L2
     const bool zf = a.nz > 0;
@@ -660,9 +736,15 @@ static int launch_columns_fast_h(const DemagPlan* p, const ColFastArgs& ca, cuda
 {
     using S = fftr::Shape<LGN>;
     const size_t smem = (size_t)S::G * S::SMEM * sizeof(float2);
-    auto kern = columns_fast_kernel<LGN, HALF>;
-    if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
     const unsigned nbx = (p->Cx + S::G - 1) / S::G;
+    if (ca.nz == 0 && p->Pz == 1 && ca.nhat[4] == nullptr && ca.nhat[5] == nullptr) {      // one layer: the planar variant
+        auto kp = columns_fast_kernel<LGN, HALF, true>;
+        if (smem > 48 * 1024 && cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+        kp<<<dim3(nbx, 1), dim3(S::T, S::G), smem, st>>>(ca);
+        return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+    }
+    auto kern = columns_fast_kernel<LGN, HALF, false>;
+    if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
     const dim3 grid = ca.nz > 0 ? dim3(p->Pz, nbx) : dim3(nbx, p->Pz), block(S::T, S::G);
     if (grid.y > 65535u) return MMC_E_UNSUPPORTED;
     kern<<<grid, block, smem, st>>>(ca);
