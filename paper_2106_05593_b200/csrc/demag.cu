@@ -481,11 +481,14 @@ struct ColFastArgs {
 #ifndef MMC_COLS_MINB_PLANAR
 #define MMC_COLS_MINB_PLANAR 3
 #endif
+#ifndef MMC_COLS_MINB_PLANAR_T256
+#define MMC_COLS_MINB_PLANAR_T256 2
+#endif
 // PLANAR (one layer, Pz == 1, no xz / yz spectrum): B_z = K_zz M_z decouples from (B_x, B_y), so the in-plane pair and the
 // z component go through the transforms one after the other and a thread holds two components instead of three.
 template <int LGN, bool HALF, bool PLANAR>
 __global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G,
-                                  fftr::Shape<LGN>::T >= 256 ? 2 : (PLANAR ? MMC_COLS_MINB_PLANAR : MMC_COLS_MINB))
+                                  fftr::Shape<LGN>::T >= 256 ? (PLANAR ? MMC_COLS_MINB_PLANAR_T256 : 2) : (PLANAR ? MMC_COLS_MINB_PLANAR : MMC_COLS_MINB))
 columns_fast_kernel(const ColFastArgs a)
 {
     using S = fftr::Shape<LGN>;
