@@ -100,7 +100,11 @@ int mmc_set_move(mmc_ctx* ctx, double cone_deg, double sigma, int adaptive_cone)
 int mmc_set_demag(mmc_ctx* ctx, int enabled, int updates_per_sweep);
 int mmc_set_seed(mmc_ctx* ctx, uint64_t seed);
 int mmc_set_sweep_counter(mmc_ctx* ctx, uint64_t sweep);
-/* device pointers, N floats each, natural cell order.  Fails with MMC_E_ZERO_LENGTH if a non-empty cell is 0. */
+/* device pointers, N floats each, natural cell order.  m = M/Ms0.  Fails with MMC_E_ZERO_LENGTH if a non-empty
+ * cell is 0 or not finite (reading G13) and with MMC_E_INVALID if a non-empty cell has |m| >= 2 (the running sums of the
+ * pass are exact fixed-point numbers for |m| < 2; |m| ~ 1000 means M in A/m was passed).  Values in EMPTY cells are
+ * ignored, whatever they are (NaN markers included): the library stores 0 there and mmc_get_m returns 0 for them.
+ * The check runs when material and temperature are known (here, or at the first call that needs the state). */
 int mmc_set_m(mmc_ctx* ctx, const float* mx, const float* my, const float* mz);
 int mmc_get_m(mmc_ctx* ctx, float* mx, float* my, float* mz);
 /* The same with HOST pointers (N floats each; pinned memory makes the copies asynchronous): the library does the

@@ -417,14 +417,15 @@ class OracleMMC:
         self._win_acc += acc; self._win_tri += tri.value
         return d
 
-    def sweep_once(self):
-        """O6: [demag] -> red -> [demag iff updates_per_sweep == 2] -> black -> counter++; then S11."""
+    def sweep_once(self, dump=False):
+        """O6: [demag] -> red -> [demag iff updates_per_sweep == 2] -> black -> counter++; then S11.
+        With dump=True returns the per-cell dumps of the two passes (see colour_pass)."""
         if self.demag_enabled:
             self.bd = self.demag_field()
-        self.colour_pass(0)
+        dumps = [self.colour_pass(0, dump=dump)]
         if self.demag_enabled and self.demag_updates == 2:
             self.bd = self.demag_field()
-        self.colour_pass(1)
+        dumps.append(self.colour_pass(1, dump=dump))
         self.sweep += 1
         self._win_sweeps += 1
         if self._win_sweeps == 100:
@@ -434,6 +435,7 @@ class OracleMMC:
                 if rate > 0.55: self.cone_deg = min(180.0, self.cone_deg + 1.0)
                 elif rate < 0.45: self.cone_deg = max(1.0, self.cone_deg - 1.0)
             self._win_acc = self._win_tri = self._win_sweeps = 0
+        return dumps if dump else None
 
     def run(self, n_sweeps):
         for _ in range(n_sweeps):

@@ -23,8 +23,25 @@ def _newer(target, deps):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def _flags_changed() -> bool:
+    """The full compile command lines are part of the build's identity: a change of MMC_NVCC_FLAGS (the -D tuning knobs of
+    csrc/) or of the compiler must rebuild everything, or an A/B run would time the same binary twice."""
+    stamp = os.path.join(OBJ, "flags.stamp")
+    ident = " ".join([NVCC] + NVFLAGS) + "\n"
+    try:
+        with open(stamp) as fh:
+            same = fh.read() == ident
+    except OSError:
+        same = False
+    if not same:
+        with open(stamp, "w") as fh:
+            fh.write(ident)
+    return not same
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    force = _flags_changed() or force
     hdrs = [os.path.join(CSRC, h) for h in ("mmc_internal.h", "fft_reg.cuh", "fft_smem.cuh")] + [os.path.join(HERE, "..", "include", "mmc.h")]
     objs = []
     jobs = []

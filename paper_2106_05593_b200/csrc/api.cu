@@ -29,6 +29,9 @@ struct mmc_ctx {
     uint64_t seed = 0;
     // derived (host)
     bool dirty = true, m_needs_check = false;
+    // B_d bookkeeping: state_version counts every change of m (or of Ms0), bd_version is the state_version whose field sits in
+    // bd[] (0 = none): a read-out or the first iteration of a sweep does not repeat a convolution of an unchanged state
+    uint64_t state_version = 1, bd_version = 0;
     bool percell = false;
     unsigned features = 0;
     double A0 = 0, D0 = 0, sigma_first = 0;
@@ -39,11 +42,12 @@ struct mmc_ctx {
     // device
     float* m[3] = { nullptr, nullptr, nullptr };
     float* bd[3] = { nullptr, nullptr, nullptr };
-    uint8_t* mask = nullptr;
-    float* Ms0_split = nullptr;
-    uint32_t* cw = nullptr;                       // per-cell mode: class << 7 | mask (colour-split)
+    // every uploaded buffer carries its own capacity (elements); upload() grows it when needed
+    uint8_t* mask = nullptr; size_t mask_cap = 0;
+    float* Ms0_split = nullptr; size_t ms0_cap = 0;
+    uint32_t* cw = nullptr; size_t cw_cap = 0;    // per-cell mode: class << 7 | mask (colour-split)
     float* table = nullptr; size_t table_cap = 0; // per-cell mode: kClassFloats floats per class
-    float* table_cubic = nullptr;                 // ... and the cubic-anisotropy table of the same stride
+    float* table_cubic = nullptr; size_t table_cubic_cap = 0;   // ... and the cubic-anisotropy table of the same stride
     size_t n_classes = 0;
     Control* ctl = nullptr;
     unsigned long long* run_sums = nullptr;       // [4] fixed-point running sums (kSumScale)
@@ -72,10 +76,18 @@ inline long long split_index_h(const Geometry& g, int i, int j, int k)
     return (long long)col * g.H + ((long long)k * g.ny + j) * g.hx + (i >> 1);
 }
 
+// Host vector -> device buffer that grows to fit: *cap is the allocation of *dptr in elements (0 = none).  A buffer is
+// never written beyond its own allocation, whatever the order of set_material / set_temperature calls on a long-lived ctx.
 template <class T>
-int upload(mmc_ctx* c, T** dptr, const std::vector<T>& h)
+int upload(mmc_ctx* c, T** dptr, size_t* cap, const std::vector<T>& h)
 {
-    if (!*dptr) CU(c, cudaMalloc(dptr, h.size() * sizeof(T)));
+    if (h.empty()) return MMC_OK;
+    if (h.size() > *cap) {
+        CU(c, cudaStreamSynchronize(c->stream));     // kernels in flight may still read the old buffer
+        cudaFree(*dptr); *dptr = nullptr; *cap = 0;
+        if (cudaMalloc(dptr, h.size() * sizeof(T)) != cudaSuccess) { *dptr = nullptr; return fail(c, MMC_E_NOMEM, "device allocation failed"); }
+        *cap = h.size();
+    }
     CU(c, cudaMemcpyAsync(*dptr, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     return MMC_OK;
@@ -160,8 +172,8 @@ int ensure_setup(mmc_ctx* c)
     }
     c->Ms0_uniform = ms0_uniform && n_active == (unsigned long long)N;   // empty cells need per-cell weights to zero their M
     c->Ms0_u = ms0_first > 0 ? (float)ms0_first : 0.f;
-    int rc = upload(c, &c->mask, mask); if (rc) return rc;
-    if (!c->Ms0_uniform) { rc = upload(c, &c->Ms0_split, ms0); if (rc) return rc; }
+    int rc = upload(c, &c->mask, &c->mask_cap, mask); if (rc) return rc;
+    if (!c->Ms0_uniform) { rc = upload(c, &c->Ms0_split, &c->ms0_cap, ms0); if (rc) return rc; }
     // coefficients
     const double V = c->V, kB = kBoltzmann;
     const double Jd[3] = { 2.0 * A0 * V / (c->dx * c->dx), 2.0 * A0 * V / (c->dy * c->dy), 2.0 * A0 * V / (c->dz * c->dz) };
@@ -223,11 +235,10 @@ int ensure_setup(mmc_ctx* c)
         for (size_t q = 0; q < classes.size(); ++q)
             class_values(classes[q], 1.0 / (kB * (double)classes[q].T), &tab[kClassFloats * q], &tabc[kClassFloats * q]);
         c->sigma_first = tab[CS_SIGMA];
-        if (tab.size() > c->table_cap) { cudaFree(c->table); cudaFree(c->table_cubic); c->table = c->table_cubic = nullptr; c->table_cap = tab.size(); }
-        rc = upload(c, &c->table, tab); if (rc) return rc;
+        rc = upload(c, &c->table, &c->table_cap, tab); if (rc) return rc;
         bool cubic = false;
         for (const auto& r : c->regions) if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0 || r.K2 != 0.0)) cubic = true;
-        if (cubic) { rc = upload(c, &c->table_cubic, tabc); if (rc) return rc; }
+        if (cubic) { rc = upload(c, &c->table_cubic, &c->table_cubic_cap, tabc); if (rc) return rc; }
         std::vector<uint32_t> cw(S, 0u);
         for (int k = 0; k < g.nz; ++k) for (int j = 0; j < g.ny; ++j) for (int i = 0; i < g.nx; ++i) {
             const long long cell = (long long)i + (long long)g.nx * (j + (long long)g.ny * k);
@@ -235,7 +246,7 @@ int ensure_setup(mmc_ctx* c)
             const size_t sidx = (size_t)split_index_h(g, i, j, k);
             if (id >= 0) cw[sidx] = ((uint32_t)id << 7) | mask[sidx];
         }
-        rc = upload(c, &c->cw, cw); if (rc) return rc;
+        rc = upload(c, &c->cw, &c->cw_cap, cw); if (rc) return rc;
     }
     c->coef = cf;
     unsigned f = 0;
@@ -249,6 +260,7 @@ int ensure_setup(mmc_ctx* c)
         if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0 || r.K2 != 0.0)) f |= F_CUBIC;
     c->features = f;
     c->dirty = false;
+    c->bd_version = 0;                                   // Ms0 or the set of non-empty cells may have changed
     return MMC_OK;
 }
 
@@ -294,20 +306,23 @@ int compute_demag(mmc_ctx* c, PhaseTimer* timer = nullptr)
     int rc = ensure_demag(c); if (rc) return rc;
     std::string e;
     rc = demag_compute(c->demag, c->m, c->Ms0_uniform ? nullptr : c->Ms0_split, c->Ms0_u, c->bd, c->stream, &e, timer);
-    if (rc != MMC_OK) return fail(c, rc, "demag: " + e);
+    if (rc != MMC_OK) { c->bd_version = 0; return fail(c, rc, "demag: " + e); }
+    c->bd_version = c->state_version;
     return MMC_OK;
 }
 
 int check_m(mmc_ctx* c)
 {
     CU(c, cudaMemsetAsync(c->d_flag, 0, sizeof(int), c->stream));
-    int rc = launch_check_zero(c->g, c->m, c->mask, c->d_flag, c->stream);
-    if (rc) return fail(c, rc, "check_zero launch failed");
+    int rc = launch_check_state(c->g, c->m, c->mask, c->d_flag, c->stream);
+    if (rc) return fail(c, rc, "check_state launch failed");
     int flag = 0;
     CU(c, cudaMemcpyAsync(&flag, c->d_flag, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CU(c, cudaStreamSynchronize(c->stream));
     c->m_needs_check = false;
-    if (flag) return fail(c, MMC_E_ZERO_LENGTH, "a non-empty cell has zero (or non-finite) magnetisation");
+    c->state_version++;
+    if (flag & 1) return fail(c, MMC_E_ZERO_LENGTH, "a non-empty cell has zero (or non-finite) magnetisation");
+    if (flag & 2) return fail(c, MMC_E_INVALID, "a non-empty cell has |m| >= 2: m is M/Ms0 (PAPER.md:32), not M in A/m");
     return MMC_OK;
 }
 
@@ -445,8 +460,10 @@ int mmc_set_demag(mmc_ctx* c, int enabled, int updates_per_sweep)
     if (!c) return MMC_E_INVALID;
     if (updates_per_sweep != 1 && updates_per_sweep != 2) return fail(c, MMC_E_INVALID, "updates_per_sweep must be 1 or 2");
     DeviceGuard dg(c->device);
-    if (c->demag_enabled && !enabled)
+    if (c->demag_enabled && !enabled) {
         for (int q = 0; q < 3; ++q) cudaMemsetAsync(c->bd[q], 0, (size_t)(2 * c->g.H) * sizeof(float), c->stream);
+        c->bd_version = 0;
+    }
     c->demag_enabled = enabled ? 1 : 0; c->demag_updates = updates_per_sweep; c->dirty = true;
     return MMC_OK;
 }
@@ -473,7 +490,7 @@ int mmc_set_m(mmc_ctx* c, const float* mx, const float* my, const float* mz)
         int rc = launch_to_split(c->g, src[q], c->m[q], c->stream);
         if (rc) return fail(c, rc, "to_split launch failed");
     }
-    c->m_set = true;
+    c->m_set = true; c->state_version++;
     if (c->material_set && c->T_set) {
         int rc = ensure_setup(c); if (rc) return rc;
         return check_m(c);
@@ -494,7 +511,7 @@ int mmc_set_m_host(mmc_ctx* c, const float* mx, const float* my, const float* mz
         int rc = launch_to_split(c->g, c->stage, c->m[q], c->stream);
         if (rc) return fail(c, rc, "to_split launch failed");
     }
-    c->m_set = true;
+    c->m_set = true; c->state_version++;
     if (c->material_set && c->T_set) {
         int rc = ensure_setup(c); if (rc) return rc;
         return check_m(c);
@@ -534,16 +551,20 @@ static int sweep_impl(mmc_ctx* c, int n_sweeps, PhaseTimer* timer)
     if (c->demag_enabled) { rc = ensure_demag(c); if (rc) return rc; }
     if (!timer && !c->demag_enabled && n_sweeps > 0) {            // small meshes: all iterations in one launch
         rc = launch_small_mesh_sweeps(make_args(c, 0), c->features, n_sweeps, c->stream);
-        if (rc == MMC_OK) return MMC_OK;
+        if (rc == MMC_OK) { c->state_version++; return MMC_OK; }
         if (rc != MMC_E_UNSUPPORTED) return fail(c, rc, "small-mesh launch failed");
     }
     if (timer) timer->mark(-1, c->stream);
     for (int it = 0; it < n_sweeps; ++it) {
-        if (c->demag_enabled) { rc = compute_demag(c, timer); if (rc) return rc; }
+        // the field is fully computed at the start of the iteration (skipped when bd[] already holds the
+        // field of exactly this state, e.g. straight after a read-out) and frozen for the passes
+        if (c->demag_enabled && (timer || c->bd_version != c->state_version)) { rc = compute_demag(c, timer); if (rc) return rc; }
+        c->state_version++;
         rc = launch_colour_pass(make_args(c, 0), c->features, false, c->stream);
         if (rc) return fail(c, rc, "red pass launch failed");
         if (timer) timer->mark(PH_RED, c->stream);
         if (c->demag_enabled && c->demag_updates == 2) { rc = compute_demag(c, timer); if (rc) return rc; }
+        c->state_version++;
         rc = launch_colour_pass(make_args(c, 1), c->features, false, c->stream);
         if (rc) return fail(c, rc, "black pass launch failed");
         if (timer) timer->mark(PH_BLACK, c->stream);
@@ -570,6 +591,7 @@ int mmc_sweep_timed(mmc_ctx* c, int n_sweeps, double* phase_ms)
             phase_ms[t.phase[i]] += (double)ms;
     }
     for (void* e : t.events) cudaEventDestroy((cudaEvent_t)e);
+    if (rc == MMC_OK && t.failed) return fail(c, MMC_E_CUDA, "mmc_sweep_timed: a timing event could not be created or recorded");
     return rc;
 }
 
@@ -582,8 +604,10 @@ int mmc_demag_field(mmc_ctx* c, float* bx, float* by, float* bz)
     float* dst[3] = { bx, by, bz };
     for (int q = 0; q < 3; ++q)
         if (dst[q]) { rc = launch_from_split(c->g, c->bd[q], dst[q], c->stream); if (rc) return fail(c, rc, "from_split launch failed"); }
-    if (!c->demag_enabled)                       // keep the sweep's field term off
+    if (!c->demag_enabled) {                     // keep the sweep's field term off
         for (int q = 0; q < 3; ++q) CU(c, cudaMemsetAsync(c->bd[q], 0, (size_t)(2 * c->g.H) * sizeof(float), c->stream));
+        c->bd_version = 0;
+    }
     return MMC_OK;
 }
 
@@ -592,7 +616,7 @@ int mmc_get_observables(mmc_ctx* c, mmc_obs* out)
     if (!c || !out) return fail(c, MMC_E_INVALID, "NULL pointer");
     DeviceGuard dg(c->device);
     int rc = ready(c); if (rc) return rc;
-    if (c->demag_enabled) { rc = compute_demag(c); if (rc) return rc; }
+    if (c->demag_enabled && c->bd_version != c->state_version) { rc = compute_demag(c); if (rc) return rc; }   // E_demag: field of the current state
     SweepArgs a = make_args(c, 0);
     if (!c->demag_enabled) a.bd[0] = a.bd[1] = a.bd[2] = nullptr;
     ObsParams op{};
@@ -723,6 +747,7 @@ int mmc_debug_pass(mmc_ctx* c, int colour, float* dm, float* dF_terms, float* ma
     a.run_sums = nullptr;
     a.dbg_dm = dm; a.dbg_terms = dF_terms; a.dbg_margin = margin; a.dbg_acc = accepted;
     rc = launch_colour_pass(a, c->features, true, c->stream);
+    c->state_version++;
     if (rc) return fail(c, rc, "debug pass launch failed");
     return MMC_OK;
 }

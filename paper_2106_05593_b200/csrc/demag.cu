@@ -442,10 +442,10 @@ static int launch_rows_fast(const DemagPlan* p, const RowFastArgs& ra, bool inve
     const dim3 grid((p->g.ny + R::RJ - 1) / R::RJ, 3 * p->g.nz), block(R::RJ, R::T);
     const size_t smem = (size_t)R::RJ * R::ES * sizeof(float2);
     if (inverse) {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_inv_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (smem > 48 * 1024 && cudaFuncSetAttribute(rows_inv_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
         rows_inv_fast_kernel<LGH><<<grid, block, smem, st>>>(ra);
     } else {
-        if (smem > 48 * 1024) cudaFuncSetAttribute(rows_fwd_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (smem > 48 * 1024 && cudaFuncSetAttribute(rows_fwd_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
         rows_fwd_fast_kernel<LGH><<<grid, block, smem, st>>>(ra);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
@@ -776,10 +776,10 @@ static int launch_rows(const DemagPlan* p, const RowArgs& ra, bool inverse, cuda
 {
     const dim3 grid((p->g.ny + p->RJ - 1) / p->RJ, 3);
     if (inverse) {
-        if (p->smemA > 48 * 1024) cudaFuncSetAttribute(rows_inv_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA);
+        if (p->smemA > 48 * 1024 && cudaFuncSetAttribute(rows_inv_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA) != cudaSuccess) return MMC_E_CUDA;
         rows_inv_kernel<PZ><<<grid, p->threadsA, p->smemA, st>>>(ra);
     } else {
-        if (p->smemA > 48 * 1024) cudaFuncSetAttribute(rows_fwd_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA);
+        if (p->smemA > 48 * 1024 && cudaFuncSetAttribute(rows_fwd_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA) != cudaSuccess) return MMC_E_CUDA;
         rows_fwd_kernel<PZ><<<grid, p->threadsA, p->smemA, st>>>(ra);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
@@ -900,8 +900,7 @@ void demag_destroy(DemagPlan* p)
 void PhaseTimer::mark(int ph, void* stream)
 {
     cudaEvent_t e;
-    if (cudaEventCreate(&e) != cudaSuccess) return;
-    cudaEventRecord(e, (cudaStream_t)stream);
+    if (cudaEventCreate(&e) != cudaSuccess || cudaEventRecord(e, (cudaStream_t)stream) != cudaSuccess) { failed = true; return; }   // mmc_sweep_timed reports it
     events.push_back((void*)e); phase.push_back(ph);
 }
 

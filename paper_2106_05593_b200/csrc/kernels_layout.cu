@@ -45,18 +45,23 @@ int launch_from_split(const Geometry& g, const float* split, float* nat, void* s
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 
-__global__ void check_zero_kernel(Geometry g, const float* mx, const float* my, const float* mz, const uint8_t* mask, int* flag)
+// State check of mmc_set_m over the storage slots.  Non-empty cells: flag bit 0 when |m| = 0 or not finite (G13: rotation
+// undefined, a multiplicative length move cannot leave 0), bit 1 when |m| >= 2 (m = M/Ms0; the fixed-point
+// running sums of the pass are exact for |m| < 2).  Empty cells and padding slots: set to 0, whatever the caller passed
+// (NaN markers included), so that the 0/1 bond weights and Ms0 = 0 factors that multiply them can never produce a NaN.
+__global__ void check_state_kernel(Geometry g, float* mx, float* my, float* mz, const uint8_t* mask, int* flag)
 {
     const long long n = 2 * g.H;
     for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
-        if (!(mask[s] & 0x40u)) continue;
+        if (!(mask[s] & 0x40u)) { mx[s] = 0.f; my[s] = 0.f; mz[s] = 0.f; continue; }
         const float l2 = mx[s] * mx[s] + my[s] * my[s] + mz[s] * mz[s];
-        if (!(l2 > 0.f) || !isfinite(l2)) atomicExch(flag, 1);
+        if (!(l2 > 0.f) || !isfinite(l2)) atomicOr(flag, 1);
+        else if (!(l2 < 4.f)) atomicOr(flag, 2);
     }
 }
-int launch_check_zero(const Geometry& g, const float* const m[3], const uint8_t* mask, int* flag, void* stream)
+int launch_check_state(const Geometry& g, float* const m[3], const uint8_t* mask, int* flag, void* stream)
 {
-    check_zero_kernel<<<grid_for(2 * g.H), 256, 0, (cudaStream_t)stream>>>(g, m[0], m[1], m[2], mask, flag);
+    check_state_kernel<<<grid_for(2 * g.H), 256, 0, (cudaStream_t)stream>>>(g, m[0], m[1], m[2], mask, flag);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 

@@ -114,7 +114,7 @@ int launch_small_mesh_sweeps(const SweepArgs& a, unsigned features, int n_sweeps
 // kernels_layout.cu
 int launch_to_split(const Geometry& g, const float* nat, float* split, void* stream);
 int launch_from_split(const Geometry& g, const float* split, float* nat, void* stream);
-int launch_check_zero(const Geometry& g, const float* const m[3], const uint8_t* mask, int* flag, void* stream);
+int launch_check_state(const Geometry& g, float* const m[3], const uint8_t* mask, int* flag, void* stream);
 struct ObsParams {
     float K1T_u;                           // beta V K1(T), uniform mode (units of kB T); per-cell mode: class table
     float c0_u;                            // c0 - c4 mu2^2, uniform mode (units of kB T)
@@ -135,6 +135,7 @@ enum Phase { PH_PACK = 0, PH_FFT_FWD, PH_MULTIPLY, PH_FFT_INV, PH_CROP, PH_RED, 
 struct PhaseTimer {
     std::vector<void*> events;     // cudaEvent_t
     std::vector<int> phase;        // phase ended by events[i]; -1 = start marker
+    bool failed = false;           // an event could not be created / recorded: the phase times would be wrong
     void mark(int ph, void* stream);
 };
 

@@ -8,11 +8,21 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 
+def pytest_addoption(parser):
+    parser.addoption("--runslow", action="store_true", default=False, help="also run the tests marked slow (minutes each)")
+
+
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
+    config.addinivalue_line("markers", "slow: minutes of CPU time; skipped unless --runslow is given")
 
 
 def pytest_collection_modifyitems(config, items):
+    if not config.getoption("--runslow"):
+        skip_slow = pytest.mark.skip(reason="slow: run with --runslow")
+        for it in items:
+            if "slow" in it.keywords:
+                it.add_marker(skip_slow)
     try:
         import torch
         has_gpu = torch.cuda.is_available()

@@ -41,15 +41,52 @@ def test_no_gpu_means_loud_failure(P):
 
 
 def test_product_does_not_import_the_oracle():
-    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2106_05593_b200")):
+    """Product and oracle are independent: no file of the package names the oracle package or its library in code, the
+    binding never imports it, and the oracle never names the package."""
+    pkg = os.path.join(ROOT, "paper_2106_05593_b200")
+    pat = re.compile(r"import\s+oracle|from\s+oracle|oracle\.|libmmc_oracle|mmc_oracle\.c|orc_[a-z_0-9]+\s*\(|[\"'/]oracle[\"'/]")
+    for dirpath, _, files in os.walk(pkg):
         for fn in files:
-            if fn.endswith((".py", ".cu", ".cpp", ".h")):
+            if fn.endswith((".py", ".cu", ".cuh", ".cpp", ".h")):
                 src = open(os.path.join(dirpath, fn)).read()
-                assert "oracle" not in src.replace("oracle/", "").lower() or fn == "mmc_host.cpp" and "import" not in src, fn
-    src = open(os.path.join(ROOT, "paper_2106_05593_b200", "__init__.py")).read()
-    assert "import oracle" not in src and "from oracle" not in src
-    osrc = open(os.path.join(ROOT, "oracle", "__init__.py")).read()
-    assert "import paper_2106_05593_b200" not in osrc and "from paper_2106_05593_b200" not in osrc
+                hits = pat.findall(src)
+                assert not hits, (fn, hits)
+    for fn in ("include/mmc.h",):
+        assert not pat.findall(open(os.path.join(ROOT, fn)).read()), fn
+    opat = re.compile(r"(?:import|from)\s+paper_2106_05593_b200|libmmc_b200|#\s*include\s*[\"<][^\">]*mmc(?:_internal)?\.h")
+    for fn in os.listdir(os.path.join(ROOT, "oracle")):
+        if fn.endswith((".py", ".c", ".h")):
+            assert not opat.findall(open(os.path.join(ROOT, "oracle", fn)).read()), fn
+    wsrc = open(os.path.join(ROOT, "workloads", "__init__.py")).read()          # the shared input generators import neither
+    assert not re.findall(r"^\s*(?:import|from)\s+(?:oracle|paper_2106_05593_b200)", wsrc, flags=re.M)
+
+
+def test_explain_iteration_classifies_flips():
+    """tests/parity_util.py on the oracle alone: an exact replay has no flips; a decision forced the other way in a cell
+    whose margin is far from zero is reported as unexplained; a state that is neither candidate is reported as such."""
+    import oracle as O
+    import workloads as W
+    from parity_util import explain_iteration
+    wl = W.cfg2(nx=20, ny=14); wl.adaptive_cone = False
+
+    def orc():
+        s = O.OracleMMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, store_fp32=True)
+        W.configure(s, wl, O.Material)
+        return s
+    a = orc(); a.run(1)
+    r = explain_iteration(wl, orc(), a.get_m())
+    assert r["flips"] == 0 and r["neither"] == 0 and r["unexplained"] == 0 and r["active"] == wl.N and r["untouched_ok"]
+    b = orc(); d_red, _ = b.sweep_once(dump=True)
+    red = np.flatnonzero(~np.isnan(d_red["margin"]))
+    c = red[np.argmax(np.abs(d_red["margin"][red]))]                 # the red cell furthest from the decision boundary
+    m = a.get_m()
+    m0 = orc().get_m()
+    for q in range(3):                                               # force the other decision there
+        m[q][c] = m0[q][c] if d_red["accepted"][c] else np.float32(m0[q][c] + d_red["dm"][c, q])
+    r = explain_iteration(wl, orc(), m)
+    assert r["flips"] >= 1 and r["unexplained"] >= 1 and c in r["flip_cells"]
+    m = a.get_m(); m[0][c] += 1e-3
+    assert explain_iteration(wl, orc(), m)["neither"] == 1
 
 
 def test_thermal_setup_matches_oracle(P):

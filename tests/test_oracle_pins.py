@@ -627,3 +627,26 @@ def test_uniaxial_k2_term_of_eq11():
     for a in range(3):
         s.m[a][2] += dm[a]
     assert t[1] * KB * 300.0 == pytest.approx(s.observables()["E_an"] - eb, rel=1e-10)
+
+
+def test_uniaxial_k1_readout_constant_is_textbook_k1_sin2():
+    """First term of Eq. (11) in the read-out (reading G5): E_an = V K1(T) [1 - (m.e)^2/me^2] with
+    K1(T) = K1 me^3 (l = 2), i.e. the textbook K1(T) sin^2(theta) for a vector of the equilibrium length at
+    polar angle theta to the axis -- in particular exactly zero along the axis, which pins the constant V K1 me^3 that no
+    energy DIFFERENCE can see -- and zero at and above Tc."""
+    V = (5e-9) ** 3
+    e = np.array([0.0, 0.6, 0.8]); perp = np.array([1.0, 0.0, 0.0])
+    for T in (300.0, 700.0):
+        me = O.me_of_T(T, 870.0)
+        s = O.OracleMMC(2, 2, 1, 5e-9, 5e-9, 5e-9, 0, store_fp32=False)
+        s.set_material([O.Material(Ms0=8e5, A0=0.0, K1=5e5, ax=0.0, ay=0.6, az=0.8, Tc=870.0)], None)
+        s.set_temperature(T, None)
+        for th in (0.0, 0.4, 1.1, np.pi / 2, 2.5):
+            v = me * (np.cos(th) * e + np.sin(th) * perp)
+            s.m = [np.full(4, x) for x in v]                       # fp64 state: no storage rounding in this pin
+            assert s.observables()["E_an"] / 4 == pytest.approx(V * 5e5 * me ** 3 * np.sin(th) ** 2, rel=1e-12, abs=1e-12 * V * 5e5)
+    s = O.OracleMMC(2, 2, 1, 5e-9, 5e-9, 5e-9, 0, store_fp32=False)
+    s.set_material([O.Material(Ms0=8e5, A0=0.0, K1=5e5, ax=0.0, ay=0.6, az=0.8, Tc=870.0)], None)
+    for T in (870.0, 900.0):
+        s.set_temperature(T, None); s.m = [np.full(4, x) for x in (0.02, 0.01, 0.03)]
+        assert s.observables()["E_an"] == 0.0
