@@ -53,37 +53,86 @@ def _pow2_at_least(n, start):
     return p
 
 
-def demag_kernel_bytes(wl, ms0_per_cell):
-    """Algorithmic bytes per launch of the three demag kernels (units per launch = the N mesh cells of one convolution).
-    T = the transposed half-spectrum array [3][Pz][Px/2+1][ny] complex64 that the rows kernels write/read and the columns
-    kernel transforms in place (only the ny kept rows are ever stored); tensor = 4 (one layer) or 6 real arrays over
-    [Pz/2+1][Px/2+1][Py]."""
+def demag_layout(wl):
+    """Which demag path libmmc_b200 takes for this mesh (mirrors demag_create): register-resident rows/columns kernels for
+    padded lengths 2^8..2^12; with several layers the layer-pair columns kernel (no z transform) when nz * Py/16 <= 512
+    threads, else a z-DFT of the shortest linear length 2 nz - 1 with a separate inverse z pass."""
     Px, Py = _pow2_at_least(wl.nx, 2), _pow2_at_least(wl.ny, 1)
-    Pz = 2 * wl.nz - 1 if 1 < wl.nz <= 16 else _pow2_at_least(wl.nz, 1)   # register-resident path: shortest linear length
-    Cx = Px // 2 + 1
-    T = 3 * Pz * Cx * wl.ny * 8
-    tensor = (4 if wl.nz == 1 else 6) * (Pz // 2 + 1) * Cx * Py * 4
-    state = 3 * wl.N * 4
-    # algorithmic flops (5 n log2 n per complex transform of length n, + the 3x3 real-symmetric multiply)
+    fast = 8 <= (Px // 2).bit_length() - 1 <= 11 and 8 <= Py.bit_length() - 1 <= 12 and wl.nz <= 16
+    lp = fast and wl.nz > 1 and (Py // 16) * wl.nz <= 512
+    Pz = 1 if wl.nz == 1 else (2 * wl.nz - 1 if fast else _pow2_at_least(wl.nz, 1))
+    return Px, Py, Pz, fast, lp
+
+
+def demag_kernel_bytes(wl, ms0_per_cell):
+    """Algorithmic bytes and flops per launch of the demag kernels (units per launch = the N mesh cells of one convolution).
+    U = the layers' transposed half-spectra [3][nz][Px/2+1][ny] complex64 that the rows kernels write / read (only the ny kept
+    rows are ever stored).  Layer-pair path: the columns kernel transforms U in place and reads the tensor spectra of the nz
+    layer offsets: (4 + 6 (nz-1)) real arrays [Px/2+1][Py].  z-DFT path: the columns kernel reads U, writes the Pz planes
+    T = [3][Pz][Px/2+1][ny] and reads 6 (4 for one layer) real arrays [Pz/2+1][Px/2+1][Py]; z_inverse reads T, writes U."""
     import math
-    fl_rows = 3 * wl.ny * wl.nz * 5 * (Px // 2) * math.log2(Px // 2)
-    fl_cols = 3 * Pz * Cx * 2 * 5 * Py * math.log2(Py) + Pz * Cx * Py * (20 if wl.nz == 1 else 36)
-    # several layers: the rows kernels work per layer on U = [3][nz][Cx][ny] (the z-DFT is fused into the columns kernel's
-    # load, its inverse is the z_inverse pass T -> U); one layer: U = T, no z pass
+    Px, Py, Pz, fast, lp = demag_layout(wl)
+    Cx = Px // 2 + 1
     U = 3 * wl.nz * Cx * wl.ny * 8
+    state = 3 * wl.N * 4
+    fl_rows = 3 * wl.ny * wl.nz * 5 * (Px // 2) * math.log2(Px // 2)
+    fft_y = 5 * Py * math.log2(Py)                               # flops of one complex column transform
     out = {"rows_fwd": {"bytes": state + (wl.N * 4 if ms0_per_cell else 0) + U, "flops": fl_rows},
-           "columns": {"bytes": U + T + tensor, "flops": fl_cols},
            "rows_inv": {"bytes": U + state, "flops": fl_rows}}
-    if wl.nz > 1:
-        out["z_inverse"] = {"bytes": T + U, "flops": 3 * Cx * wl.ny * 8 * wl.nz * (Pz - 1)}
+    if lp:
+        tensor = (4 + 6 * (wl.nz - 1)) * Cx * Py * 4
+        out["columns"] = {"bytes": 2 * U + tensor, "flops": 3 * wl.nz * Cx * 2 * fft_y + Cx * Py * wl.nz * wl.nz * 36}
+    else:
+        T = 3 * Pz * Cx * wl.ny * 8
+        tensor = (4 if wl.nz == 1 else 6) * (Pz // 2 + 1) * Cx * Py * 4
+        out["columns"] = {"bytes": (U + T if wl.nz > 1 else 2 * T) + tensor,
+                          "flops": 3 * Pz * Cx * 2 * fft_y + Pz * Cx * Py * (20 if wl.nz == 1 else 36)}
+        if wl.nz > 1:
+            out["z_inverse"] = {"bytes": T + U, "flops": 3 * Cx * wl.ny * 8 * wl.nz * (Pz - 1)}
     return out
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full captures (profiles/), cfg 4
-NCU_TRAFFIC_CFG4 = {   # profiles/r1f_summary.md
-    "colour_pass_kernel": 114.4e6, "demag_rows_fwd_kernel": 100.2e6, "demag_columns_kernel": 452.9e6,
-    "demag_z_inverse_kernel": 226.8e6, "demag_rows_inv_kernel": 128.6e6,
-}
+def source_hash():
+    """Identity of the kernels a measurement belongs to: sha256 over the library's sources and the build script."""
+    import hashlib
+    h = hashlib.sha256()
+    base = os.path.join(ROOT, "paper_2106_05593_b200")
+    files = sorted(os.path.join(base, "csrc", f) for f in os.listdir(os.path.join(base, "csrc")))
+    for f in files + [os.path.join(base, "build.py"), os.path.join(ROOT, "include", "mmc.h")]:
+        with open(f, "rb") as fh:
+            h.update(os.path.basename(f).encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+_KERNEL_OF = (("colour_pass", "colour_pass_kernel"), ("rows_fwd", "demag_rows_fwd_kernel"), ("rows_inv", "demag_rows_inv_kernel"),
+              ("columns", "demag_columns_kernel"), ("z_inverse", "demag_z_inverse_kernel"))
+
+
+def ncu_traffic(cfg):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch (mean over the captured launches) of every kernel of the
+    step, from the committed ncu capture profiles/traffic_cfg<N>.csv -- but only if profiles/traffic_cfg<N>.md says that the
+    capture was taken from exactly these sources (source_hash); otherwise there is no measurement and the field is null."""
+    import csv
+    md = os.path.join(ROOT, "profiles", f"traffic_cfg{cfg}.md"); cs = os.path.join(ROOT, "profiles", f"traffic_cfg{cfg}.csv")
+    if not (os.path.exists(md) and os.path.exists(cs)):
+        return {}
+    with open(md) as f:
+        if f"source_hash: {source_hash()}" not in f.read():
+            return {}
+    per = {}
+    with open(cs) as f:
+        rows = [ln for ln in f if ln.startswith('"')]
+    rd = csv.DictReader(rows)
+    for r in rd:
+        kind = {"dram__bytes_read.sum": "dram_bytes", "dram__bytes_write.sum": "dram_bytes",
+                "sm__inst_executed.sum": "warp_instructions"}.get(r["Metric Name"])
+        if kind is None:
+            continue
+        v = float(r["Metric Value"].replace(",", "")) * {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(r["Metric Unit"], 1.0)
+        name = next((k for pat, k in _KERNEL_OF if pat in r["Kernel Name"]), None)
+        if name:
+            d = per.setdefault(name, {}).setdefault(kind, {}); d[r["ID"]] = d.get(r["ID"], 0.0) + v
+    return {k: {kind: sum(d.values()) / len(d) for kind, d in kinds.items()} for k, kinds in per.items()}
 
 
 def replica_seed(base_seed: int, rank: int) -> int:
@@ -182,26 +231,49 @@ def oracle_sample(cfg: int):
     return W.make(cfg, **kw), kw
 
 
-def time_oracle(cfg: int, steps: int, warmup: int):
+def _omp_threads(n=None):
+    """Thread count of the OpenMP runtime the oracle's C file was built against (libgomp): set it (n) or read it back.
+    The oracle itself is not touched: this is the runtime's own switch, like the OMP_NUM_THREADS environment variable."""
+    import ctypes
+    try:
+        omp = ctypes.CDLL("libgomp.so.1")
+        if n is not None:
+            omp.omp_set_num_threads(int(n))
+        return int(omp.omp_get_max_threads())
+    except OSError:
+        return int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+
+
+def time_oracle(cfg: int, steps, warmup: int, threads=None, budget_s=10.0):
+    """The fp64 oracle as it stands on a bounded sample of config `cfg`: whole iterations (updates/s) and, separately, its
+    demag convolution (numpy.fft on the padded grid, not a tuned FFT).  threads=None: all host cores."""
     import oracle as O
     import workloads as W
     wl, kw = oracle_sample(cfg)
     wl.adaptive_cone = False
     o = O.OracleMMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, store_fp32=True)
     W.configure(o, wl, O.Material)
+    all_cores = os.cpu_count() or 1
+    cores = _omp_threads(threads if threads else all_cores)
+    conv = None
     if wl.demag:
         o.demag_field()                       # tensor set-up outside the timed region (as on the GPU side)
+        t0 = time.perf_counter(); n = 0
+        while n < 3 or (time.perf_counter() - t0 < 1.0 and n < 50):
+            o.demag_field(); n += 1
+        conv = n / (time.perf_counter() - t0)
     t0 = time.perf_counter()
     o.run(max(1, warmup))
     per = (time.perf_counter() - t0) / max(1, warmup)
-    if steps is None:                         # cpu_baseline leg: about 10 s of CPU work
-        steps = int(min(400, max(2, round(10.0 / max(per, 1e-3)))))
+    if steps is None:                         # cpu_baseline leg: about budget_s of CPU work
+        steps = int(min(400, max(2, round(budget_s / max(per, 1e-3)))))
     t0 = time.perf_counter()
     o.run(steps)
     dt = time.perf_counter() - t0
-    cores = int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1))
+    _omp_threads(all_cores)
     sample = f"{wl.name} recipe on a {wl.nx}x{wl.ny}x{wl.nz} mesh ({wl.n_active} non-empty cells), {steps} iterations incl. numpy.fft demag"
-    return wl.n_active * steps / dt, dt, cores, sample
+    return {"value": wl.n_active * steps / dt, "seconds": dt, "steps": steps, "cores": cores, "sample": sample,
+            "demag_convolutions_per_sec": conv}
 
 
 def run_reference(args):
@@ -209,11 +281,13 @@ def run_reference(args):
     if rank != 0:
         return 0
     steps = max(1, args.steps); warm = max(1, args.warmup)
-    v, dt, cores, sample = time_oracle(args.config, steps, warm)
+    r = time_oracle(args.config, steps, warm)
+    v, dt, cores, sample = r["value"], r["seconds"], r["cores"], r["sample"]
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": warm,
             "ms_per_step": 1e3 * dt / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": {"workload": f"cfg{args.config} (oracle sample: {sample})"},
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                             "demag_convolutions_per_sec": r["demag_convolutions_per_sec"]},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line))
     return 0
@@ -307,17 +381,52 @@ def run_ours(args):
                 kern["demag_" + name + "_kernel"] = {"launch_ms": phases[ph] / K, "launches_per_step": 1, "bytes": db[name]["bytes"],
                                                     "flops": db[name]["flops"], "units_per_launch": wl.N,
                                                     "bytes_per_unit": db[name]["bytes"] / wl.N}
+        full = not args.small and not args.shape
+        traffic = ncu_traffic(cfg) if full else {}          # measured by ncu from exactly these sources, or nothing
+        ISSUE_PEAK = 148 * 4 * 1.965e9                      # warp instructions / s (B200_PROFILING.md: 148 SMs, 1965 MHz; 4 schedulers per SM)
+        FMA_PEAK = 74.4                                     # TFLOP/s: 148 SM x 128 FP32 lanes x 2 flop x 1.965 GHz (no tensor cores: no contraction here)
         for k, d in kern.items():
             t = d["launch_ms"] * 1e-3
             d["achieved_GBs"] = d["bytes"] / t / 1e9 if t > 0 else 0.0
             d["frac_of_hbm_peak"] = d["achieved_GBs"] / peak
             d["share_of_step"] = d["launch_ms"] * d["launches_per_step"] / step_ms if step_ms > 0 else None
+            tr = traffic.get(k, {})
+            d["ncu_traffic_bytes"] = tr.get("dram_bytes")
+            d["ncu_warp_instructions"] = tr.get("warp_instructions")
             if "flops" in d:
                 d["achieved_TFLOPs"] = d["flops"] / t / 1e12 if t > 0 else 0.0
-            d["ncu_traffic_bytes"] = NCU_TRAFFIC_CFG4.get(k) if (cfg == 4 and not args.small and not args.shape) else None
+                d["frac_of_fma_peak"] = d["achieved_TFLOPs"] / FMA_PEAK
+            if tr.get("warp_instructions") and t > 0:
+                d["issue_slot_frac"] = tr["warp_instructions"] / t / ISSUE_PEAK
+            # which roofline is the tighter one for this kernel: the larger of the HBM fraction (algorithmic bytes) and the
+            # plain-ALU fraction (algorithmic flops for the transforms; issue slots, from the ncu instruction count, for the pass)
+            alu = d.get("frac_of_fma_peak", d.get("issue_slot_frac"))
+            d["bound"] = "alu" if (alu is not None and alu > d["frac_of_hbm_peak"]) else "hbm"
         dom = max(kern, key=lambda k: kern[k]["launch_ms"])          # the dominant kernel = longest single launch
         dk = kern[dom]
         demag_ms = sum(phases[k] for k in ("pack", "rows_fwd", "columns", "rows_inv", "z_inverse")) / K
+        # launches inside the timed region (graph nodes are kernel launches too); small meshes without demag: ONE launch runs all K iterations
+        single_launch = (not wl.demag) and wl.N <= 8192 and not percell
+        per_iter = (len([k for k in kern if k.startswith("demag_")]) * wl.demag_updates if wl.demag else 0) + 3
+        roof_hbm = {"kernel": dom, "bound": "hbm", "achieved": dk["achieved_GBs"], "peak": peak, "unit": "GB/s",
+                    "frac": dk["frac_of_hbm_peak"], "traffic": dk["ncu_traffic_bytes"], "peak_source": peak_src,
+                    "algorithmic_bytes_per_unit": dk["bytes_per_unit"], "units_per_launch": dk["units_per_launch"],
+                    "launch_ms": dk["launch_ms"], "share_of_step": dk["share_of_step"],
+                    "traffic_source": (f"profiles/traffic_cfg{cfg}.csv (ncu, source_hash {source_hash()})" if dk["ncu_traffic_bytes"] is not None
+                                       else "no ncu capture of these sources: null")}
+        roof_alu = None
+        if "achieved_TFLOPs" in dk:
+            roof_alu = {"kernel": dom, "bound": "alu", "achieved": dk["achieved_TFLOPs"], "peak": FMA_PEAK, "unit": "TFLOP/s",
+                        "frac": dk["frac_of_fma_peak"], "traffic": dk["ncu_traffic_bytes"],
+                        "peak_source": "derived: 148 SM x 128 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts and clocks); "
+                                       "algorithmic flops = 5 n log2 n per complex transform + the tensor products",
+                        "launch_ms": dk["launch_ms"], "share_of_step": dk["share_of_step"]}
+        elif "issue_slot_frac" in dk:
+            roof_alu = {"kernel": dom, "bound": "alu", "achieved": dk["ncu_warp_instructions"] / (dk["launch_ms"] * 1e-3) / 1e12,
+                        "peak": ISSUE_PEAK / 1e12, "unit": "T warp-instr/s", "frac": dk["issue_slot_frac"], "traffic": dk["ncu_traffic_bytes"],
+                        "peak_source": "derived: 148 SM x 4 schedulers x 1.965 GHz; instructions from the ncu capture",
+                        "launch_ms": dk["launch_ms"], "share_of_step": dk["share_of_step"]}
+        primary, other = (roof_alu, roof_hbm) if (dk["bound"] == "alu" and roof_alu) else (roof_hbm, roof_alu)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -329,30 +438,30 @@ def run_ours(args):
                              "(L2 = 126 MB)" if wl.N >= 2 ** 22 else
                              "working set fits L2 (small config, a parity case rather than a bench line)",
                        "parallelism": "replicas" if world > 1 else "single GPU", "cone_deg": wl.cone_deg,
-                       "acceptance": ob["accepted"] / max(1, ob["trials"])},
+                       "acceptance": ob["accepted"] / max(1, ob["trials"]),
+                       "launch_path": ("one launch of the single-CTA kernel for all K iterations" if single_launch else
+                                       "first iteration as plain launches, the rest replayed from CUDA graphs of 16 and 1 iterations")},
             "clocks": clocks,
             "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nE},
-            "gpu_launches": ((7 if wl.nz > 1 else 6) if wl.demag else 3) * K,
+            "gpu_launches": 1 if single_launch else per_iter * K,
             "phases_ms_per_step": {k: v / K for k, v in phases.items()},
+            "phases_path": ("mmc_sweep_timed: launch-per-kernel with CUDA events around every launch" +
+                            ("; NOT the path of `value`, which runs the single-launch small-mesh kernel" if single_launch else
+                             "; same kernels as `value`, which replays them from CUDA graphs without the events")),
             "sweep_only_updates_per_sec": wl.n_active / (2 * pass_ms * 1e-3) if pass_ms > 0 else None,
             "demag_convolutions_per_sec": (1e3 / demag_ms) if (wl.demag and demag_ms > 0) else None,
-            "roofline": {"kernel": dom, "bound": "hbm", "achieved": dk["achieved_GBs"], "peak": peak, "unit": "GB/s",
-                         "frac": dk["frac_of_hbm_peak"], "traffic": dk["ncu_traffic_bytes"], "peak_source": peak_src,
-                         "algorithmic_bytes_per_unit": dk["bytes_per_unit"], "units_per_launch": dk["units_per_launch"],
-                         "launch_ms": dk["launch_ms"], "share_of_step": dk["share_of_step"],
-                         "note": "FFT kernels are co-limited by the FP32 pipes: see kernels[*].achieved_TFLOPs against "
-                                 "148 SM x 128 lanes x 1.965 GHz = 37.2 T FP32 instr/s (74.4 TFLOP/s if every one were an FMA)"},
-            # the same kernel against the plain-ALU peak (no tensor cores: nothing here is a contraction): algorithmic flops
-            # (5 n log2 n per complex transform + the tensor multiply) over 148 SM x 128 FP32 lanes x 2 (FMA) x 1.965 GHz
-            "roofline_alu": ({"kernel": dom, "bound": "alu", "achieved": dk["achieved_TFLOPs"], "peak": 74.4, "unit": "TFLOP/s",
-                              "frac": dk["achieved_TFLOPs"] / 74.4,
-                              "peak_source": "derived: 148 SM x 128 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts and clocks)"}
-                             if "achieved_TFLOPs" in dk else None),
+            "roofline": primary,
+            "roofline_other": other,
             "kernels": kern,
         }
         if not args.no_cpu_baseline and world == 1:
-            v, dt, cores, sample = time_oracle(cfg, None, 1)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
+            # the oracle beside it: all host cores (~10 s) and one core (~6 s), plus its convolutions/s
+            r = time_oracle(cfg, None, 1, None, 10.0)
+            r1 = time_oracle(cfg, None, 1, 1, 6.0)
+            line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"],
+                                    "demag_convolutions_per_sec": r["demag_convolutions_per_sec"],
+                                    "one_core": {"value": r1["value"], "cores": r1["cores"], "sample": r1["sample"],
+                                                 "demag_convolutions_per_sec": r1["demag_convolutions_per_sec"]}}
         print(json.dumps(line))
     g.close()
     if world > 1:

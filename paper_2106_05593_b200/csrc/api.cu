@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <unordered_map>
@@ -32,6 +33,17 @@ struct mmc_ctx {
     // B_d bookkeeping: state_version counts every change of m (or of Ms0), bd_version is the state_version whose field sits in
     // bd[] (0 = none): a read-out or the first iteration of a sweep does not repeat a convolution of an unchanged state
     uint64_t state_version = 1, bd_version = 0;
+    // CUDA graphs of whole iterations (launch-per-kernel path): kernel arguments are captured by value, so the graphs are
+    // rebuilt whenever a setter changes anything a launch depends on (args_version); device-side state (m, control block,
+    // sweep counter) is read through pointers and needs no rebuild.  Captured on a private stream (the caller's stream may
+    // be the legacy default stream, which cannot be captured) and launched into the caller's stream.
+    uint64_t args_version = 1;
+    struct IterGraph { cudaGraphExec_t exec = nullptr; uint64_t version = 0; };
+    IterGraph graph1, graphN;
+    cudaStream_t cap_stream = nullptr;
+    bool graphs_off = false;
+    PassTma tma;                                  // TMA-staged pass: tensor maps over m, bd, cw (rebuilt when a pointer changes)
+    bool tma_off = false;
     bool percell = false;
     unsigned features = 0;
     double A0 = 0, D0 = 0, sigma_first = 0;
@@ -259,6 +271,10 @@ int ensure_setup(mmc_ctx* c)
     for (const auto& r : c->regions)
         if (r.Ms0 > 0 && (r.K1c != 0.0 || r.K2c != 0.0 || r.K2 != 0.0)) f |= F_CUBIC;
     c->features = f;
+    c->tma.ok = false;
+    // TMA boxes bring in whole tiles, empty cells included, while the brick kernel skips the loads of empty cells: staged only
+    // for meshes that are mostly magnetic (BASELINE config 5 is 30 % magnetic and loses 5 % with staging, measured)
+    if (!c->tma_off && n_active * 10ull >= (unsigned long long)N * 6ull) pass_tma_build(c->g, c->m, c->bd, c->percell ? c->cw : nullptr, &c->tma);
     c->dirty = false;
     c->bd_version = 0;                                   // Ms0 or the set of non-empty cells may have changed
     return MMC_OK;
@@ -301,11 +317,11 @@ int ensure_demag(mmc_ctx* c)
     return MMC_OK;
 }
 
-int compute_demag(mmc_ctx* c, PhaseTimer* timer = nullptr)
+int compute_demag(mmc_ctx* c, PhaseTimer* timer = nullptr, cudaStream_t stream_override = nullptr, bool use_override = false)
 {
     int rc = ensure_demag(c); if (rc) return rc;
     std::string e;
-    rc = demag_compute(c->demag, c->m, c->Ms0_uniform ? nullptr : c->Ms0_split, c->Ms0_u, c->bd, c->stream, &e, timer);
+    rc = demag_compute(c->demag, c->m, c->Ms0_uniform ? nullptr : c->Ms0_split, c->Ms0_u, c->bd, use_override ? stream_override : c->stream, &e, timer);
     if (rc != MMC_OK) { c->bd_version = 0; return fail(c, rc, "demag: " + e); }
     c->bd_version = c->state_version;
     return MMC_OK;
@@ -355,6 +371,8 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     c->g.H = (int64_t)c->g.hx * ny * nz;
     c->dx = dx; c->dy = dy; c->dz = dz; c->V = dx * dy * dz;
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
+    c->graphs_off = std::getenv("MMC_NO_GRAPH") != nullptr;      // A/B knob: plain launches only
+    c->tma_off = std::getenv("MMC_NO_TMA") != nullptr;           // A/B knob: the pass with per-thread loads (colour_pass2_kernel) everywhere
     c->regions.push_back(mmc_material{ 0, 0, 0, 0, 0, 1, 0, 1, 9.2740100783e-24, 0, 0, 1, 0, 0, 0, 1, 0, 0 });
     DeviceGuard dg(device);
     auto bail = [&](int code) { mmc_destroy(c); return code; };
@@ -390,6 +408,9 @@ int mmc_destroy(mmc_ctx* c)
     cudaFree(c->mask); cudaFree(c->Ms0_split); cudaFree(c->ctl); cudaFree(c->run_sums); cudaFree(c->obs_scratch);
     cudaFree(c->d_obs); cudaFree(c->d_flag); cudaFree(c->stage);
     demag_destroy(c->demag);
+    if (c->graph1.exec) cudaGraphExecDestroy(c->graph1.exec);
+    if (c->graphN.exec) cudaGraphExecDestroy(c->graphN.exec);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     delete c;
     return MMC_OK;
 }
@@ -413,14 +434,14 @@ int mmc_set_material(mmc_ctx* c, int n_regions, const mmc_material* regions, con
             if (region_of_cell[i] < 0 || region_of_cell[i] >= n_regions) return fail(c, MMC_E_INVALID, "region_of_cell out of range");
     c->regions.assign(regions, regions + n_regions);
     if (region_of_cell) c->region_of_cell.assign(region_of_cell, region_of_cell + N); else c->region_of_cell.clear();
-    c->material_set = true; c->dirty = true; c->m_needs_check = c->m_set;
+    c->material_set = true; c->dirty = true; c->m_needs_check = c->m_set; c->args_version++;
     return MMC_OK;
 }
 
 int mmc_set_exchange_coupling(mmc_ctx* c, int inter_region_exchange)
 {
     if (!c) return MMC_E_INVALID;
-    c->inter_region = inter_region_exchange ? 1 : 0; c->dirty = true;
+    c->inter_region = inter_region_exchange ? 1 : 0; c->dirty = true; c->args_version++;
     return MMC_OK;
 }
 
@@ -434,7 +455,7 @@ int mmc_set_temperature(mmc_ctx* c, double T_uniform, const float* T_per_cell)
         if (!(T_uniform > 0) || !std::isfinite(T_uniform)) return fail(c, MMC_E_INVALID, "T must be > 0");
         c->T_cell.clear();
     }
-    c->T_uniform = T_uniform; c->T_set = true; c->dirty = true;
+    c->T_uniform = T_uniform; c->T_set = true; c->dirty = true; c->args_version++;
     return MMC_OK;
 }
 
@@ -442,7 +463,7 @@ int mmc_set_field(mmc_ctx* c, double Bx, double By, double Bz)
 {
     if (!c) return MMC_E_INVALID;
     if (!std::isfinite(Bx) || !std::isfinite(By) || !std::isfinite(Bz)) return fail(c, MMC_E_INVALID, "field must be finite");
-    c->B[0] = Bx; c->B[1] = By; c->B[2] = Bz;          // read into the kernel arguments at every launch
+    c->B[0] = Bx; c->B[1] = By; c->B[2] = Bz; c->args_version++;          // read into the kernel arguments at every launch
     return MMC_OK;
 }
 
@@ -450,7 +471,7 @@ int mmc_set_move(mmc_ctx* c, double cone_deg, double sigma, int adaptive_cone)
 {
     if (!c) return MMC_E_INVALID;
     if (!(cone_deg > 0) || cone_deg > 180.0 || !(sigma < 1.0)) return fail(c, MMC_E_INVALID, "0 < cone <= 180 and sigma < 1 required");
-    c->cone_deg = cone_deg; c->sigma_user = sigma; c->adaptive = adaptive_cone ? 1 : 0; c->dirty = true;
+    c->cone_deg = cone_deg; c->sigma_user = sigma; c->adaptive = adaptive_cone ? 1 : 0; c->dirty = true; c->args_version++;
     DeviceGuard dg(c->device);
     return push_control(c, true);
 }
@@ -464,11 +485,11 @@ int mmc_set_demag(mmc_ctx* c, int enabled, int updates_per_sweep)
         for (int q = 0; q < 3; ++q) cudaMemsetAsync(c->bd[q], 0, (size_t)(2 * c->g.H) * sizeof(float), c->stream);
         c->bd_version = 0;
     }
-    c->demag_enabled = enabled ? 1 : 0; c->demag_updates = updates_per_sweep; c->dirty = true;
+    c->demag_enabled = enabled ? 1 : 0; c->demag_updates = updates_per_sweep; c->dirty = true; c->args_version++;
     return MMC_OK;
 }
 
-int mmc_set_seed(mmc_ctx* c, uint64_t seed) { if (!c) return MMC_E_INVALID; c->seed = seed; return MMC_OK; }
+int mmc_set_seed(mmc_ctx* c, uint64_t seed) { if (!c) return MMC_E_INVALID; c->seed = seed; c->args_version++; return MMC_OK; }
 
 int mmc_set_sweep_counter(mmc_ctx* c, uint64_t sweep)
 {
@@ -543,6 +564,52 @@ int mmc_get_m(mmc_ctx* c, float* mx, float* my, float* mz)
     return MMC_OK;
 }
 
+// One iteration, enqueued on `st`: [demag] -> red -> [demag] -> black -> end of sweep.
+static int enqueue_iteration(mmc_ctx* c, cudaStream_t st, PhaseTimer* timer, bool field_is_current)
+{
+    int rc;
+    // the field is fully computed at the start of the iteration (skipped when bd[] already holds the
+    // field of exactly this state, e.g. straight after a read-out) and frozen for the passes
+    if (c->demag_enabled && !field_is_current) { rc = compute_demag(c, timer, st, true); if (rc) return rc; }
+    c->state_version++;
+    rc = launch_colour_pass(make_args(c, 0), c->features, false, st, &c->tma);
+    if (rc) return fail(c, rc, "red pass launch failed");
+    if (timer) timer->mark(PH_RED, st);
+    if (c->demag_enabled && c->demag_updates == 2) { rc = compute_demag(c, timer, st, true); if (rc) return rc; }
+    c->state_version++;
+    SweepArgs black = make_args(c, 1);
+    black.finish = 1;                                 // S11 by the last CTA of the black pass: no separate one-thread launch
+    rc = launch_colour_pass(black, c->features, false, st, &c->tma);
+    if (rc) return fail(c, rc, "black pass launch failed");
+    if (timer) { timer->mark(PH_BLACK, st); timer->mark(PH_END, st); }
+    return MMC_OK;
+}
+
+constexpr int kGraphIters = 16;                       // iterations in the long graph
+
+// Capture `iters` iterations into an executable graph.  Any failure switches graphs off for this ctx (plain launches go on).
+static bool build_graph(mmc_ctx* c, int iters, mmc_ctx::IterGraph* g)
+{
+    if (g->exec) { cudaGraphExecDestroy(g->exec); g->exec = nullptr; }
+    g->version = 0;
+    if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) { c->graphs_off = true; cudaGetLastError(); return false; }
+    if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeRelaxed) != cudaSuccess) { c->graphs_off = true; cudaGetLastError(); return false; }
+    const uint64_t sv = c->state_version, bv = c->bd_version;
+    int rc = MMC_OK;
+    for (int it = 0; it < iters && rc == MMC_OK; ++it) rc = enqueue_iteration(c, c->cap_stream, nullptr, false);
+    c->state_version = sv; c->bd_version = bv;        // nothing ran
+    cudaGraph_t graph = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+    if (rc != MMC_OK || e != cudaSuccess || !graph || cudaGraphInstantiate(&g->exec, graph, 0) != cudaSuccess) {
+        if (graph) cudaGraphDestroy(graph);
+        g->exec = nullptr; c->graphs_off = true; cudaGetLastError();
+        return false;
+    }
+    cudaGraphDestroy(graph);
+    g->version = c->args_version;
+    return true;
+}
+
 static int sweep_impl(mmc_ctx* c, int n_sweeps, PhaseTimer* timer)
 {
     if (!c || n_sweeps < 0) return fail(c, MMC_E_INVALID, "n_sweeps >= 0 required");
@@ -555,22 +622,27 @@ static int sweep_impl(mmc_ctx* c, int n_sweeps, PhaseTimer* timer)
         if (rc != MMC_E_UNSUPPORTED) return fail(c, rc, "small-mesh launch failed");
     }
     if (timer) timer->mark(-1, c->stream);
-    for (int it = 0; it < n_sweeps; ++it) {
-        // the field is fully computed at the start of the iteration (skipped when bd[] already holds the
-        // field of exactly this state, e.g. straight after a read-out) and frozen for the passes
-        if (c->demag_enabled && (timer || c->bd_version != c->state_version)) { rc = compute_demag(c, timer); if (rc) return rc; }
-        c->state_version++;
-        rc = launch_colour_pass(make_args(c, 0), c->features, false, c->stream);
-        if (rc) return fail(c, rc, "red pass launch failed");
-        if (timer) timer->mark(PH_RED, c->stream);
-        if (c->demag_enabled && c->demag_updates == 2) { rc = compute_demag(c, timer); if (rc) return rc; }
-        c->state_version++;
-        rc = launch_colour_pass(make_args(c, 1), c->features, false, c->stream);
-        if (rc) return fail(c, rc, "black pass launch failed");
-        if (timer) timer->mark(PH_BLACK, c->stream);
-        rc = launch_end_sweep(c->ctl, c->stream);
-        if (rc) return fail(c, rc, "end_sweep launch failed");
-        if (timer) timer->mark(PH_END, c->stream);
+    int left = n_sweeps;
+    if (!timer && !c->graphs_off && left > 0) {
+        // The first iteration after a change of settings runs as plain launches (it also loads the kernels and builds the demag
+        // plan outside any capture); from then on whole iterations are replayed from graphs: 16 at a time, then one at a time.
+        if (c->graph1.version != c->args_version) {
+            rc = enqueue_iteration(c, c->stream, nullptr, c->bd_version == c->state_version); if (rc) return rc;
+            --left;
+            build_graph(c, 1, &c->graph1);
+        }
+        if (!c->graphs_off && left >= 2 * kGraphIters && c->graphN.version != c->args_version) build_graph(c, kGraphIters, &c->graphN);
+        while (!c->graphs_off && left > 0) {
+            const bool big = left >= kGraphIters && c->graphN.version == c->args_version && c->graphN.exec;
+            if (!big && !(c->graph1.version == c->args_version && c->graph1.exec)) break;
+            if (cudaGraphLaunch(big ? c->graphN.exec : c->graph1.exec, c->stream) != cudaSuccess) { c->graphs_off = true; cudaGetLastError(); break; }
+            const int done = big ? kGraphIters : 1;
+            left -= done; c->state_version += 2ull * done; c->bd_version = 0;
+        }
+    }
+    for (; left > 0; --left) {
+        rc = enqueue_iteration(c, c->stream, timer, !timer && c->bd_version == c->state_version);
+        if (rc) return rc;
     }
     return MMC_OK;
 }

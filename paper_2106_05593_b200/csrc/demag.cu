@@ -51,6 +51,10 @@ struct DemagPlan {
     float2* T = nullptr;             // [3][Pz][Cx][ny]
     float2* U = nullptr;             // fastA with nz > 1: [3][nz][Cx][ny], the layers before the z-DFT and after its inverse
     float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
+    // layer-pair columns kernel (several layers, no z transform): U is transformed in place, T and nhat do not exist
+    bool lp = false;
+    int lpG = 1;                     // kx per CTA
+    float* nh2[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };    // [nz][Cx][Py]: 2-D spectra per layer offset dz
 };
 
 #define CK(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) { if (err) *err = std::string(#x) + ": " + cudaGetErrorString(e_); return MMC_E_CUDA; } } while (0)
@@ -82,14 +86,15 @@ __global__ void place_kernel(int nx, int ny, int nz, int Px, int Py, int Pz, con
 }
 // spectrum (D2Z layout [kz][ky][kx <= Px/2]) -> nhat[kz <= Pz/2][kx][p], p = position of ky in the y transform's output
 __global__ void permute_kernel(const double2* __restrict__ spec, float* __restrict__ out, int Cx, int Py, int Kz, Plan py, double scale,
-                               int fast_lg)
+                               int fast_lg, int imag = 0)
 {
     const long long n = (long long)Kz * Cx * Py;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
         const int p = (int)(t % Py); const long long r = t / Py; const int kx = (int)(r % Cx), kz = (int)(r / Cx);
         // fast path: slot e of thread tid sits at p = e * (Py/16) + tid
         const int ky = fast_lg ? fftr::freq_of_slot(fast_lg, p % (Py >> 4), p / (Py >> 4)) : fft::freq_of_pos(py, p);
-        out[t] = (float)(scale * spec[((long long)kz * Py + ky) * Cx + kx].x);
+        const double2 z = spec[((long long)kz * Py + ky) * Cx + kx];
+        out[t] = (float)(scale * (imag ? z.y : z.x));
     }
 }
 __global__ void twiddle_kernel(float2* tw, int P)
@@ -520,49 +525,54 @@ columns_fast_kernel(const ColFastArgs a)
 #pragma unroll
             for (int e = 0; e < 16; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
         }
+        // ONE copy of each transform in the instruction stream (the straight-line version of this kernel is ~75 KB of code
+        // and starves the instruction cache): pass p = 0 is the in-plane pair, p = 1 the z component; the transforms always
+        // work on v[0] and the two register arrays swap.
+#pragma unroll 1
+        for (int p = 0; p < 2; ++p) {
+            const int nc = p ? 1 : 2;
+#pragma unroll 1
+            for (int c = 0; c < nc; ++c) {
+                fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
 #pragma unroll
-        for (int c = 0; c < 2; ++c) fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
-#pragma unroll
-        for (int e = 0; e < 16; ++e) {
-            const float2 u = v[0][e], w1 = v[1][e];
-            const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T), xy = __ldg(a.nhat[3] + nb + e * T);
-            v[0][e].x = fmaf(xx, u.x, xy * w1.x); v[0][e].y = fmaf(xx, u.y, xy * w1.y);
-            v[1][e].x = fmaf(xy, u.x, yy * w1.x); v[1][e].y = fmaf(xy, u.y, yy * w1.y);
-        }
-        __syncthreads();                               // every thread is done reading exchange buffer 2
-#pragma unroll
-        for (int c = 0; c < 2; ++c) {
-            fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
-            float2* __restrict__ col = a.Tout + ((size_t)c * a.Cx + kx) * ny;
-#pragma unroll
-            for (int n1 = 0; n1 < NL; ++n1) {
-                const int j = tid + n1 * T;
-                if (live && (HALF || j < ny)) col[j] = v[c][n1];
+                for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = t0; }
             }
-        }
-        // z component in the registers of the first
-        {
-            float2 (&z)[16] = v[0];
-            const float2* __restrict__ cin = a.Tin + ((size_t)2 * a.Cx + kx) * ny;
+            if (p == 0) {                              // two swaps: v[0] = M^_x, v[1] = M^_y
 #pragma unroll
-            for (int n1 = 0; n1 < 16; ++n1) {
-                const int j = tid + n1 * T;
-                z[n1] = (n1 < NL && (HALF || j < ny)) ? cin[j] : make_float2(0.f, 0.f);
+                for (int e = 0; e < 16; ++e) {
+                    const float2 u = v[0][e], w1 = v[1][e];
+                    const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T), xy = __ldg(a.nhat[3] + nb + e * T);
+                    v[0][e].x = fmaf(xx, u.x, xy * w1.x); v[0][e].y = fmaf(xx, u.y, xy * w1.y);
+                    v[1][e].x = fmaf(xy, u.x, yy * w1.x); v[1][e].y = fmaf(xy, u.y, yy * w1.y);
+                }
+            } else {                                   // one swap: M^_z sits in v[1]; back to v[0] with its product
+#pragma unroll
+                for (int e = 0; e < 16; ++e) {
+                    const float zz = __ldg(a.nhat[2] + nb + e * T);
+                    v[0][e] = make_float2(v[1][e].x * zz, v[1][e].y * zz);
+                }
             }
-            __syncthreads();                           // the last inverse transform read exchange buffer 1
-            fftr::forward<LGN, HALF, true>(z, s1, s2, tw, tid);
+            __syncthreads();                           // every thread is done reading exchange buffer 2
+#pragma unroll 1
+            for (int c = 0; c < nc; ++c) {
+                fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
+                float2* __restrict__ col = a.Tout + ((size_t)(p ? 2 : c) * a.Cx + kx) * ny;
 #pragma unroll
-            for (int e = 0; e < 16; ++e) {
-                const float zz = __ldg(a.nhat[2] + nb + e * T);
-                z[e].x *= zz; z[e].y *= zz;
+                for (int n1 = 0; n1 < NL; ++n1) {
+                    const int j = tid + n1 * T;
+                    if (live && (HALF || j < ny)) col[j] = v[0][n1];
+                }
+#pragma unroll
+                for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = t0; }
             }
-            __syncthreads();
-            fftr::inverse<LGN, true>(z, s1, s2, tw, tid);
-            float2* __restrict__ col = a.Tout + ((size_t)2 * a.Cx + kx) * ny;
+            if (p == 0) {                              // z component in the registers of the first
+                const float2* __restrict__ cin = a.Tin + ((size_t)2 * a.Cx + kx) * ny;
 #pragma unroll
-            for (int n1 = 0; n1 < NL; ++n1) {
-                const int j = tid + n1 * T;
-                if (live && (HALF || j < ny)) col[j] = z[n1];
+                for (int n1 = 0; n1 < 16; ++n1) {
+                    const int j = tid + n1 * T;
+                    v[0][n1] = (n1 < NL && (HALF || j < ny)) ? cin[j] : make_float2(0.f, 0.f);
+                }
+                __syncthreads();                       // the last inverse transform read exchange buffer 1
             }
         }
         return;
@@ -626,20 +636,24 @@ columns_fast_kernel(const ColFastArgs a)
             for (int e = 0; e < 16; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
         }
     }
-#pragma unroll
+    // one copy of each transform in the instruction stream: the loops over the components are not unrolled, the three
+    // register arrays rotate instead (see columns_lp_kernel)
+#pragma unroll 1
     for (int c = 0; c < 3; ++c) {
         if (HALF) {
 #pragma unroll
-            for (int n1 = 8; n1 < 16; ++n1) v[c][n1] = make_float2(0.f, 0.f);
+            for (int n1 = 8; n1 < 16; ++n1) v[0][n1] = make_float2(0.f, 0.f);
         } else if (!zf) {
             const float2* __restrict__ col = a.Tin + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
                 const int j = tid + n1 * T;
-                v[c][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
+                v[0][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
             }
         }
-        fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
+        fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
     }
     // S2: B^ = K^ M^ (see columns_kernel); slot e of thread tid reads the permuted spectrum at e*T + tid
     {
@@ -666,15 +680,185 @@ columns_fast_kernel(const ColFastArgs a)
         }
     }
     __syncthreads();                                   // every thread is done reading exchange buffer 2
-#pragma unroll
+#pragma unroll 1
     for (int c = 0; c < 3; ++c) {
-        fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
+        fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
         float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
         for (int n1 = 0; n1 < NL; ++n1) {
             const int j = tid + n1 * T;
-            if (live && (HALF || j < ny)) col[j] = v[c][n1];
+            if (live && (HALF || j < ny)) col[j] = v[0][n1];
         }
+#pragma unroll
+        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ kernel B, layer-pair variant
+// Several layers WITHOUT a z transform (Eq. (14), written out in z): in the 2-D Fourier domain of one layer
+//     B^_k(kx, ky) = sum_k' K^(kx, ky; k - k') M^_k'(kx, ky),      K^(.; dz) = 2-D spectrum of -mu0 N(x, y, dz),
+// so the nz layers' columns are transformed once each way (3 nz forward + 3 nz inverse transforms per kx instead of the
+// 3 (2 nz - 1) + 3 (2 nz - 1) of a length-(2 nz - 1) z-DFT), the z direction costs nz^2 small 3x3 products per frequency, and
+// neither the z planes nor the inverse z pass exist.  One CTA per kx (G of them for short transforms): thread group k
+// (threadIdx.y, T = Py/16 threads) owns layer k: load its three columns, three forward transforms (registers, fft_reg.cuh),
+// then the layers meet through shared memory in chunks of EC register slots (a slot is one frequency: the sum over layers
+// and components for a chunk is complete within the chunk, so the result replaces the chunk in the same registers),
+// three inverse transforms, store in place.  The exchange reuses the transforms' exchange buffers (double-buffered chunks).
+// Tensor spectra: nh[q][dz][kx][slot], dz = 0 .. nz-1; diagonal and xy components are even in dz and real; xz and yz are odd
+// in dz and (odd in one in-plane coordinate only) purely imaginary: nh[4], nh[5] hold the imaginary parts.
+struct ColLPArgs {
+    int ny, Cx;
+    const float2* tw1; const float2* tw2;      // fft_reg.cuh twiddle tables of the length-Py transform
+    float2* U;                                 // [3][nz][Cx][ny], transformed in place
+    const float* nh[6];
+};
+
+template <int LGN> struct LPShape { static constexpr int EC = LGN == 8 ? 2 : 4, NC = 16 / EC; };   // 2 * 3 EC T <= Shape::SMEM
+// planes of the tensor spectrum per chunk row: dz = 0 has 4 components (xz = yz = 0), every other dz has 6
+__host__ __device__ constexpr int lp_planes(int nz) { return 4 + 6 * (nz - 1); }
+__host__ __device__ constexpr int lp_plane_index(int d, int q) { return d == 0 ? q : 4 + 6 * (d - 1) + q; }
+
+// Shared memory: [transform exchange buffers of the G * nz groups | two chunks of tensor spectrum | two mbarriers].
+// The tensor spectrum of a chunk (EC consecutive slots = EC * T consecutive floats of each plane) is brought in by
+// cp.async.bulk copies that complete on an mbarrier, two chunks ahead of their use: the first two are requested before the
+// forward transforms start, chunk ch + 2 as soon as chunk ch has been consumed, so no thread ever waits for these loads.
+template <int LGN, bool HALF>
+__global__ void __launch_bounds__(512, 1) columns_lp_kernel(const ColLPArgs a)
+{
+    using S = fftr::Shape<LGN>;
+    constexpr int N = S::N, T = S::T, NL = HALF ? 8 : 16, EC = LPShape<LGN>::EC, NC = LPShape<LGN>::NC;
+    extern __shared__ float2 sm[];
+    const int tid = threadIdx.x, k = threadIdx.y, g = threadIdx.z, nz = blockDim.y, G = blockDim.z;
+    const int grp = g * nz + k;
+    float2* s1 = sm + grp * S::SMEM;
+    float2* s2 = s1 + S::S1;
+    const int NP = lp_planes(nz);
+    float* tens = reinterpret_cast<float*>(sm + G * nz * S::SMEM);          // [2][G][NP][EC * T]
+    const int tbuf = G * NP * EC * T;
+    unsigned long long* bar = reinterpret_cast<unsigned long long*>(tens + 2 * tbuf);
+    const int kxr = blockIdx.x * G + g;
+    const bool live = kxr < a.Cx;                      // idle groups still walk through the barriers
+    const int kx = live ? kxr : a.Cx - 1;
+    const int ny = a.ny;
+    const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), a.tw1, a.tw2 };
+    const size_t plane = (size_t)a.Cx * N;             // one dz plane of a tensor component
+    if (tid == 0 && grp == 0) { fftr::mbar_init(bar, G * nz); fftr::mbar_init(bar + 1, G * nz); fftr::mbar_fence_init(); }
+    __syncthreads();
+    // thread 0 of group (g, k) requests plane dz = k of this kx for chunk ch: one copy of EC * T floats per component
+    auto request = [&](int ch) {
+        if (tid != 0) return;
+        const int nq = k == 0 ? 4 : 6;
+        unsigned long long* b = bar + (ch & 1);
+        fftr::mbar_arrive_expect_tx(b, (unsigned)(nq * EC * T * sizeof(float)));
+        float* dst = tens + (ch & 1) * tbuf + (g * NP + lp_plane_index(k, 0)) * (EC * T);
+        for (int q = 0; q < nq; ++q)
+            fftr::bulk_copy_g2s(dst + q * (EC * T), a.nh[q] + (size_t)k * plane + (size_t)kx * N + ch * (EC * T),
+                                (unsigned)(EC * T * sizeof(float)), b);
+    };
+    request(0);
+    request(1);
+    float2 v[3][16];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float2* __restrict__ col = a.U + ((size_t)(c * nz + k) * a.Cx + kx) * ny;
+#pragma unroll
+        for (int n1 = 0; n1 < 16; ++n1) {
+            const int j = tid + n1 * T;
+            v[c][n1] = (n1 < NL && (HALF || j < ny)) ? col[j] : make_float2(0.f, 0.f);
+        }
+    }
+    // transforms of different layers do not wait for one another: one named barrier per group (warp-aligned groups only)
+    constexpr bool GROUPS = T >= 64;
+    const fftr::GroupSync gsync{ 1 + grp, T };
+    // ONE copy of each transform in the instruction stream: the loops below are not unrolled; instead the register arrays
+    // rotate (component-wise here, chunk-wise in the multiply), so that the loop body always works on v[0] / the first EC
+    // slots.  Straight-line code for all components and chunks is ~100 KB and starves the instruction cache (measured: 45 %
+    // of the warp cycles stalled on instruction fetch); the rotations cost ~15 % more instructions.
+#pragma unroll 1
+    for (int c = 0; c < 3; ++c) {
+        if constexpr (GROUPS) fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid, gsync);
+        else fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
+    }
+    __syncthreads();                                   // every group is done with its exchange buffers: they now carry the layers
+    // S2 with the z direction as a direct sum over layer pairs.  xb[buf][g][layer][component][slot of the chunk][tid]
+    constexpr int XS = 3 * EC * T;                     // one layer of one chunk
+    float2* xb = sm + g * nz * XS;
+    const int xbuf = G * nz * XS;                      // one buffer (all groups)
+    {
+        float2* w = xb + k * XS + tid;
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int e = 0; e < EC; ++e) w[(c * EC + e) * T] = v[c][e];
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int ch = 0; ch < NC; ++ch) {                  // the current chunk sits in slots 0 .. EC-1 (the slots rotate, see below)
+        if (ch + 1 < NC) {                             // the next chunk goes to the other buffer while this one is consumed
+            float2* w = xb + ((ch + 1) & 1) * xbuf + k * XS + tid;
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int e = 0; e < EC; ++e) w[(c * EC + e) * T] = v[c][EC + e];
+        }
+        fftr::mbar_wait(bar + (ch & 1), (ch >> 1) & 1);                     // this chunk's tensor spectrum has landed
+        const float2* r = xb + (ch & 1) * xbuf + tid;
+        const float* tc = tens + (ch & 1) * tbuf + g * NP * (EC * T) + tid;
+#pragma unroll
+        for (int e = 0; e < EC; ++e) {
+            float2 ox = make_float2(0.f, 0.f), oy = ox, oz = ox;
+#pragma unroll 1
+            for (int d = 0; d < nz; ++d) {
+                const float* t = tc + lp_plane_index(d, 0) * (EC * T) + e * T;
+                const float xx = t[0], yy = t[EC * T], zz = t[2 * EC * T], xy = t[3 * EC * T];
+                float xz = 0.f, yz = 0.f;
+                if (d > 0) { xz = t[4 * EC * T]; yz = t[5 * EC * T]; }
+                // layer k' = k - d (offset +d) and, for d > 0, k' = k + d (offset -d: xz, yz change sign)
+#pragma unroll
+                for (int side = 0; side < 2; ++side) {
+                    const int kp = side ? k + d : k - d;
+                    if (side ? (d == 0 || kp >= nz) : (kp < 0)) continue;
+                    const float2* m = r + kp * XS + e * T;
+                    const float2 mx = m[0], my = m[EC * T], mz = m[2 * EC * T];
+                    const float sxz = side ? -xz : xz, syz = side ? -yz : yz;
+                    // (i s)(p + i q) = -s q + i s p
+                    ox.x = fmaf(xx, mx.x, fmaf(xy, my.x, fmaf(-sxz, mz.y, ox.x)));
+                    ox.y = fmaf(xx, mx.y, fmaf(xy, my.y, fmaf(sxz, mz.x, ox.y)));
+                    oy.x = fmaf(xy, mx.x, fmaf(yy, my.x, fmaf(-syz, mz.y, oy.x)));
+                    oy.y = fmaf(xy, mx.y, fmaf(yy, my.y, fmaf(syz, mz.x, oy.y)));
+                    oz.x = fmaf(-sxz, mx.y, fmaf(-syz, my.y, fmaf(zz, mz.x, oz.x)));
+                    oz.y = fmaf(sxz, mx.x, fmaf(syz, my.x, fmaf(zz, mz.y, oz.y)));
+                }
+            }
+            v[0][e] = ox; v[1][e] = oy; v[2][e] = oz;
+        }
+        __syncthreads();                               // chunk consumed by all layers; after the last one the buffers go back to the transforms
+        if (ch + 2 < NC) request(ch + 2);              // its buffers are free again
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {                  // rotate the slots by one chunk (NC rotations restore the order)
+            float2 t0[EC];
+#pragma unroll
+            for (int e = 0; e < EC; ++e) t0[e] = v[c][e];
+#pragma unroll
+            for (int e = 0; e < 16 - EC; ++e) v[c][e] = v[c][e + EC];
+#pragma unroll
+            for (int e = 0; e < EC; ++e) v[c][16 - EC + e] = t0[e];
+        }
+    }
+#pragma unroll 1
+    for (int c = 0; c < 3; ++c) {
+        if constexpr (GROUPS) fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid, gsync);
+        else fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
+        float2* __restrict__ col = a.U + ((size_t)(c * nz + k) * a.Cx + kx) * ny;
+#pragma unroll
+        for (int n1 = 0; n1 < NL; ++n1) {
+            const int j = tid + n1 * T;
+            if (live && (HALF || j < ny)) col[j] = v[0][n1];
+        }
+#pragma unroll
+        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
     }
 }
 
@@ -758,6 +942,38 @@ static int launch_columns_fast(const DemagPlan* p, const ColFastArgs& ca, cudaSt
 {
     return 2 * p->g.ny == p->Py ? launch_columns_fast_h<LGN, true>(p, ca, st) : launch_columns_fast_h<LGN, false>(p, ca, st);
 }
+template <int LGN>
+static int launch_columns_lp(const DemagPlan* p, const ColLPArgs& la, cudaStream_t st)
+{
+    using S = fftr::Shape<LGN>;
+    const int G = p->lpG, nz = p->g.nz;
+    const size_t smem = (size_t)G * nz * S::SMEM * sizeof(float2)
+                        + (size_t)2 * G * lp_planes(nz) * LPShape<LGN>::EC * S::T * sizeof(float) + 2 * sizeof(unsigned long long);
+    if (smem > 227 * 1024) return MMC_E_UNSUPPORTED;
+    const dim3 grid((p->Cx + G - 1) / G), block(S::T, nz, G);
+    if (2 * p->g.ny == p->Py) {
+        auto kern = columns_lp_kernel<LGN, true>;
+        if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+        kern<<<grid, block, smem, st>>>(la);
+    } else {
+        auto kern = columns_lp_kernel<LGN, false>;
+        if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+        kern<<<grid, block, smem, st>>>(la);
+    }
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+static int launch_columns_lp_any(const DemagPlan* p, const ColLPArgs& la, cudaStream_t st)
+{
+    switch (ilog2(p->Py)) {
+        case 8: return launch_columns_lp<8>(p, la, st);
+        case 9: return launch_columns_lp<9>(p, la, st);
+        case 10: return launch_columns_lp<10>(p, la, st);
+        case 11: return launch_columns_lp<11>(p, la, st);
+        case 12: return launch_columns_lp<12>(p, la, st);
+        default: return MMC_E_UNSUPPORTED;
+    }
+}
+
 static int launch_columns_fast_any(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
 {
     switch (ilog2(p->Py)) {
@@ -842,8 +1058,21 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
             fftr::twiddle_tables_kernel<<<blocks_for((long long)ntw), 256, 0, st>>>(p->twB1, p->twB2, lgPy);
         }
     }
+    // several layers on the register-resident path: the layer-pair columns kernel when one CTA can hold a thread group per
+    // layer (nz * Py/16 <= 512 threads); else the z-DFT path (planes T, z_inverse pass)
+#ifndef MMC_DEMAG_LP
+#define MMC_DEMAG_LP 1
+#endif
+    {
+        const int Tn = p->Py / 16;
+        p->lp = MMC_DEMAG_LP && p->fastA && g.nz > 1 && Tn * g.nz <= 512;
+        if (p->lp) {
+            const int gmax = std::max(1, std::min(Tn >= 128 ? 1 : 128 / Tn, 512 / (Tn * g.nz)));
+            p->lpG = std::min(gmax, std::max(1, p->Cx / 296));          // short transforms share a CTA once the grid is two waves deep
+        }
+    }
     const size_t nT = (size_t)3 * p->Pz * p->Cx * g.ny;
-    CK(cudaMalloc(&p->T, nT * sizeof(float2)));
+    if (!p->lp) CK(cudaMalloc(&p->T, nT * sizeof(float2)));
     if (p->fastA && g.nz > 1) CK(cudaMalloc(&p->U, (size_t)3 * g.nz * p->Cx * g.ny * sizeof(float2)));
     CK(cudaMalloc(&p->twx, (size_t)p->Px * sizeof(float2)));
     CK(cudaMalloc(&p->twy, (size_t)p->Py * sizeof(float2)));
@@ -854,6 +1083,38 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     std::vector<double> oct[6];
     demag_tensor_octant(g.nx, g.ny, g.nz, dx, dy, dz, kNearRadius, oct);
     const size_t nO = (size_t)g.nx * g.ny * g.nz;
+    static const int SX[6] = { 1, 1, 1, -1, -1, 1 }, SY[6] = { 1, 1, 1, -1, 1, -1 }, SZ[6] = { 1, 1, 1, 1, -1, -1 };
+    if (p->lp) {
+        // 2-D spectra of the tensor at every layer offset dz = 0 .. nz-1 (the octant table holds dz >= 0; the kernel applies the
+        // parity in dz): place plane dz on the (Px, Py) grid, 2-D D2Z, real part (xx, yy, zz, xy) or imaginary part (xz, yz: odd
+        // in exactly one in-plane coordinate), in the column transform's slot order, -mu0 / (2 Px Py) folded in
+        const size_t r2 = (size_t)p->Px * p->Py, c2 = (size_t)p->Cx * p->Py, nP = (size_t)g.nx * g.ny;
+        double *d_oct = nullptr, *d_full = nullptr; double2* d_spec = nullptr;
+        CK(cudaMalloc(&d_oct, nO * sizeof(double)));
+        CK(cudaMalloc(&d_full, r2 * sizeof(double)));
+        CK(cudaMalloc(&d_spec, c2 * sizeof(double2)));
+        int n2[2] = { p->Py, p->Px };
+        cufftHandle pd;
+        CF(cufftPlanMany(&pd, 2, n2, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, 1));
+        CF(cufftSetStream(pd, st));
+        const double scale2 = -kMu0 / (2.0 * (double)p->Px * (double)p->Py);
+        for (int q = 0; q < 6; ++q) {
+            CK(cudaMalloc(&p->nh2[q], (size_t)g.nz * c2 * sizeof(float)));
+            CK(cudaMemsetAsync(p->nh2[q], 0, (size_t)g.nz * c2 * sizeof(float), st));
+            CK(cudaMemcpyAsync(d_oct, oct[q].data(), nO * sizeof(double), cudaMemcpyHostToDevice, st));
+            for (int dzp = (q >= 4 ? 1 : 0); dzp < g.nz; ++dzp) {        // xz, yz vanish at dz = 0
+                place_kernel<<<blocks_for((long long)r2), 256, 0, st>>>(g.nx, g.ny, 1, p->Px, p->Py, 1, d_oct + (size_t)dzp * nP, SX[q], SY[q], 1, d_full);
+                CF(cufftExecD2Z(pd, d_full, (cufftDoubleComplex*)d_spec));
+                permute_kernel<<<blocks_for((long long)c2), 256, 0, st>>>(d_spec, p->nh2[q] + (size_t)dzp * c2, p->Cx, p->Py, 1, p->py, scale2,
+                                                                         ilog2(p->Py), q >= 4 ? 1 : 0);
+            }
+            CK(cudaStreamSynchronize(st));                   // oct[q] host buffer must outlive the copy
+        }
+        cufftDestroy(pd);
+        cudaFree(d_oct); cudaFree(d_full); cudaFree(d_spec);
+        CK(cudaGetLastError());
+        return MMC_OK;
+    }
     const size_t rsize = (size_t)p->Px * p->Py * p->Pz, csize = (size_t)p->Cx * p->Py * p->Pz;
     const int Kz = p->Pz / 2 + 1;
     double *d_oct = nullptr, *d_full = nullptr; double2* d_spec = nullptr;
@@ -867,7 +1128,6 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     cufftHandle pd;
     CF(cufftPlanMany(&pd, rank, dims, nullptr, 1, 0, nullptr, 1, 0, CUFFT_D2Z, 1));
     CF(cufftSetStream(pd, st));
-    static const int SX[6] = { 1, 1, 1, -1, -1, 1 }, SY[6] = { 1, 1, 1, -1, 1, -1 }, SZ[6] = { 1, 1, 1, 1, -1, -1 };
     const double scale = -kMu0 / (2.0 * (double)p->Px * (double)p->Py * (double)p->Pz);
     for (int q = 0; q < 6; ++q) {
         if (g.nz == 1 && q >= 4) continue;                   // N_xz = N_yz = 0 in a single layer
@@ -893,7 +1153,7 @@ void demag_destroy(DemagPlan* p)
 {
     if (!p) return;
     cudaFree(p->T); cudaFree(p->U); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2); 
-    for (int q = 0; q < 6; ++q) cudaFree(p->nhat[q]);
+    for (int q = 0; q < 6; ++q) { cudaFree(p->nhat[q]); cudaFree(p->nh2[q]); }
     delete p;
 }
 
@@ -931,7 +1191,14 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
     ca.ny = p->g.ny; ca.Cx = p->Cx; ca.Py = p->Py; ca.lgPy = ilog2(p->Py); ca.Pz = p->Pz; ca.BS = fft::padded_len(p->Py);
     ca.py = p->py; ca.twy = p->twy; ca.T = p->T;
     for (int q = 0; q < 6; ++q) ca.nhat[q] = p->nhat[q];
-    if (p->fastB) {
+    if (p->lp) {
+        ColLPArgs la{};
+        la.ny = p->g.ny; la.Cx = p->Cx; la.tw1 = p->twB1; la.tw2 = p->twB2; la.U = p->U;
+        for (int q = 0; q < 6; ++q) la.nh[q] = p->nh2[q];
+        rc = launch_columns_lp_any(p, la, st);
+        if (rc) { if (err) *err = "columns_lp_kernel launch failed"; return rc; }
+        if (timer) timer->mark(PH_MULTIPLY, stream);
+    } else if (p->fastB) {
         ColFastArgs fa{};
         fa.ny = p->g.ny; fa.Cx = p->Cx; fa.Pz = p->Pz; fa.nz = p->U ? p->g.nz : 0; fa.tw1 = p->twB1; fa.tw2 = p->twB2;
         fa.Tin = p->U ? p->U : p->T; fa.Tout = p->T;

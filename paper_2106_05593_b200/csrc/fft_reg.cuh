@@ -98,9 +98,17 @@ __device__ __forceinline__ void stage_twiddles(float2 w, const float2* __restric
     }
 }
 
-template <int LGN, bool HALF, bool TABLE>
+// Barrier of the threads that share one transform's exchange buffers: the whole CTA (default), or a named barrier of one
+// warp-aligned thread group (several independent transforms in one CTA that should not wait for one another).
+struct BlockSync { __device__ __forceinline__ void operator()() const { __syncthreads(); } };
+struct GroupSync {
+    int id, n;                                        // barrier 1..15, threads (a multiple of 32)
+    __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+};
+
+template <int LGN, bool HALF, bool TABLE, class Sync = BlockSync>
 __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
-                                        const Twiddles& tw, int tid)
+                                        const Twiddles& tw, int tid, const Sync& sync = Sync())
 {
     using S = Shape<LGN>;
     constexpr int T = S::T, R3 = S::R3;
@@ -123,7 +131,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
     }
     float2 pw2[15];                               // requested before the barrier: the registers of v are free here
     if constexpr (R3 > 1) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw2);
-    __syncthreads();
+    sync();
     const int u = tid >> 4, q1 = tid & 15;
     {
         const float2* r1 = s1 + q1 * (T + 1) + u;
@@ -140,7 +148,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
             if (q > 0) y = fft::cmul(y, pw[q - 1]);
             d2[q] = y;
         }
-        __syncthreads();
+        sync();
         const float2* r2 = s2 + tid + (tid >> 4);
 #pragma unroll
         for (int i = 0; i < S::NI; ++i) {
@@ -157,14 +165,14 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
         for (int q = 0; q < 16; ++q) x[q] = v[fft::bitrev<16>(q)];
 #pragma unroll
         for (int q = 0; q < 16; ++q) v[q] = x[q];
-        __syncthreads();                          // buffer 1 was read last: the next transform may overwrite it
+        sync();                          // buffer 1 was read last: the next transform may overwrite it
     }
 }
 
 // the mirror: v[e] = Y[freq_of_slot(tid, e)] on entry, v[n1] = N * y[tid + n1*T] on exit
-template <int LGN, bool TABLE>
+template <int LGN, bool TABLE, class Sync = BlockSync>
 __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
-                                        const Twiddles& tw, int tid)
+                                        const Twiddles& tw, int tid, const Sync& sync = Sync())
 {
     using S = Shape<LGN>;
     constexpr int T = S::T, R3 = S::R3;
@@ -183,7 +191,7 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
         }
         float2 pw[15];
         stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw);
-        __syncthreads();
+        sync();
         const float2* r2 = s2 + u * S::U + 17 * q1;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
@@ -204,7 +212,7 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
     {
         float2 pw[15];
         stage_twiddles<T, TABLE>(tw.w1, tw.t1, tid, pw);
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             float2 y = s1[q * (T + 1) + tid];
@@ -213,7 +221,35 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
         }
     }
     fft::dit<16, true>(v);
-    if constexpr (R3 == 1) __syncthreads();       // as in forward
+    if constexpr (R3 == 1) sync();       // as in forward
+}
+
+// ---- asynchronous bulk copies global -> shared, completion on an mbarrier (cp.async.bulk: the TMA unit moves the bytes,
+// no thread waits on a register) -------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned arrivals)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(arrivals) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+// one arrival that also announces `bytes` of asynchronous copies to come
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+// bytes: a multiple of 16; dst and src 16-byte aligned
+__device__ __forceinline__ void bulk_copy_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!ok);
 }
 
 // Slot bookkeeping for kernels that need to know which frequency a register holds (demag.cu rows kernels):

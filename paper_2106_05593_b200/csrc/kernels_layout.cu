@@ -71,39 +71,51 @@ int launch_check_state(const Geometry& g, float* const m[3], const uint8_t* mask
 //   E_ex   = 1/2 sum_{bonded nb} (A0 V/h_d^2)|m - m_nb|^2        (each bond seen from both ends)
 //   E_an   = V K1(T) - (V K1 me)(m.e)^2 ; E_zee = -V Ms0 m.B_ext ; E_dmi = -D0 V m.G ;
 //   E_demag = -(V Ms0/2) m.B_d ; E_long = kB T [c4 (l2 - mu2)^2 + c0adj]
-template <bool PERCELL>
+template <bool PERCELL, bool DMI>
 __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams op, double* __restrict__ scratch)
 {
     const Geometry g = a.g;
-    const long long n = 2 * g.H;
+    const unsigned hx = (unsigned)g.hx, H = (unsigned)g.H, n = 2u * H;    // mmc_create: 2 H < 2^31
+    const int hxr = (g.nx + 1) >> 1;
     double acc[11];
 #pragma unroll
     for (int t = 0; t < 11; ++t) acc[t] = 0.0;
-    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n; s += (long long)gridDim.x * blockDim.x) {
+    // one thread per storage slot, 32-bit index arithmetic, neighbours by their offsets in the other colour's plane (as in the
+    // pass); the exchange energy counts every bond once, from its -x / -y / -z end (bits 0, 2, 4 of the mask byte)
+    for (unsigned s = blockIdx.x * blockDim.x + threadIdx.x; s < n; s += gridDim.x * blockDim.x) {
         const unsigned mb = a.mask[s];
         if (!(mb & 0x40u)) continue;
-        const int col = s >= g.H;
-        const long long w = s - (long long)col * g.H;
-        const int q = (int)(w % g.hx); const int row = (int)(w / g.hx);
-        const int j = row % g.ny, k = row / g.ny;
-        const int i = 2 * q + (((j + k) & 1) ^ col);
+        const unsigned col = s >= H ? 1u : 0u, w = s - col * H;
+        const unsigned row = w / hx; const int q = (int)(w - row * hx);
+        const int k = (int)(row / (unsigned)g.ny), j = (int)(row - (unsigned)k * g.ny);
+        const int sp = ((j + k) & 1) ^ (int)col;
+        const unsigned oth = (1u - col) * H + row * hx + q;           // same compact index in the other colour's plane
         const double m[3] = { a.m[0][s], a.m[1][s], a.m[2][s] };
         const double l2 = m[0] * m[0] + m[1] * m[1] + m[2] * m[2];
         acc[0] += m[0]; acc[1] += m[1]; acc[2] += m[2]; acc[3] += sqrt(l2); acc[10] += 1.0;
-        double nbv[6][3];
+        // offsets of the six neighbours relative to `oth` (only used when the bond bit is set, i.e. the neighbour exists)
+        int off[6];
+        off[0] = sp ? ((q + 1 < hxr) ? 1 : -q) : 0;                                       // +x
+        off[1] = sp ? 0 : ((q > 0) ? -1 : hxr - 1);                                       // -x
+        off[2] = (j + 1 < g.ny) ? (int)hx : -(g.ny - 1) * (int)hx;                        // +y
+        off[3] = (j > 0) ? -(int)hx : (g.ny - 1) * (int)hx;                               // -y
+        const int lay = g.ny * (int)hx;
+        off[4] = (k + 1 < g.nz) ? lay : -(g.nz - 1) * lay;                                // +z
+        off[5] = (k > 0) ? -lay : (g.nz - 1) * lay;                                       // -z
+        double nbv[4][3];
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
-            nbv[d][0] = nbv[d][1] = nbv[d][2] = 0.0;
-            if (!((mb >> d) & 1u)) continue;
-            int ii = i, jj = j, kk = k;
-            const int step = (d & 1) ? -1 : 1;
-            if ((d >> 1) == 0) { ii += step; if (ii < 0) ii += g.nx; if (ii >= g.nx) ii -= g.nx; }
-            if ((d >> 1) == 1) { jj += step; if (jj < 0) jj += g.ny; if (jj >= g.ny) jj -= g.ny; }
-            if ((d >> 1) == 2) { kk += step; if (kk < 0) kk += g.nz; if (kk >= g.nz) kk -= g.nz; }
-            const long long t = split_index(g, ii, jj, kk);
-            nbv[d][0] = a.m[0][t]; nbv[d][1] = a.m[1][t]; nbv[d][2] = a.m[2][t];
-            const double e0 = m[0] - nbv[d][0], e1 = m[1] - nbv[d][1], e2 = m[2] - nbv[d][2];
-            acc[4] += 0.5 * op.aex[d >> 1] * (e0 * e0 + e1 * e1 + e2 * e2);
+            const bool need = (d & 1) == 0 || (DMI && d < 4);        // + directions for the exchange, E/W/N/S for the DMI vector
+            double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+            if (need && ((mb >> d) & 1u)) {
+                const unsigned t = oth + (unsigned)off[d];
+                v0 = a.m[0][t]; v1 = a.m[1][t]; v2 = a.m[2][t];
+                if ((d & 1) == 0) {
+                    const double e0 = m[0] - v0, e1 = m[1] - v1, e2 = m[2] - v2;
+                    acc[4] += op.aex[d >> 1] * (e0 * e0 + e1 * e1 + e2 * e2);
+                }
+            }
+            if (d < 4) { nbv[d][0] = v0; nbv[d][1] = v1; nbv[d][2] = v2; }
         }
         float invT, bKq, bzee, c4, ax, ay, az, K1T, c0a; double mu2;
         if (PERCELL) {
@@ -137,10 +149,12 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
             }
         }
         acc[6] += -kT * (double)bzee * (m[0] * a.coef.Bx + m[1] * a.coef.By + m[2] * a.coef.Bz);
-        const double G0 = 0.5 * (-(nbv[0][2] - nbv[1][2]) * op.inv_d[0]);
-        const double G1 = 0.5 * (-(nbv[2][2] - nbv[3][2]) * op.inv_d[1]);
-        const double G2 = 0.5 * ((nbv[0][0] - nbv[1][0]) * op.inv_d[0] + (nbv[2][1] - nbv[3][1]) * op.inv_d[1]);
-        acc[7] += -op.D0V * (m[0] * G0 + m[1] * G1 + m[2] * G2);
+        if (DMI) {
+            const double G0 = 0.5 * (-(nbv[0][2] - nbv[1][2]) * op.inv_d[0]);
+            const double G1 = 0.5 * (-(nbv[2][2] - nbv[3][2]) * op.inv_d[1]);
+            const double G2 = 0.5 * ((nbv[0][0] - nbv[1][0]) * op.inv_d[0] + (nbv[2][1] - nbv[3][1]) * op.inv_d[1]);
+            acc[7] += -op.D0V * (m[0] * G0 + m[1] * G1 + m[2] * G2);
+        }
         if (a.bd[0]) acc[8] += -0.5 * kT * (double)bzee * (m[0] * a.bd[0][s] + m[1] * a.bd[1][s] + m[2] * a.bd[2][s]);
         const double dv = l2 - mu2;
         acc[9] += kT * ((double)c4 * dv * dv + (double)c0a);
@@ -222,8 +236,11 @@ int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, Ob
                             int scratch_blocks, void* stream)
 {
     cudaStream_t st = (cudaStream_t)stream;
-    if (percell) observables_kernel<true><<<scratch_blocks, 256, 0, st>>>(a, op, scratch);
-    else         observables_kernel<false><<<scratch_blocks, 256, 0, st>>>(a, op, scratch);
+    const bool dmi = op.D0V != 0.0;
+    if (percell) { if (dmi) observables_kernel<true, true><<<scratch_blocks, 256, 0, st>>>(a, op, scratch);
+                   else     observables_kernel<true, false><<<scratch_blocks, 256, 0, st>>>(a, op, scratch); }
+    else         { if (dmi) observables_kernel<false, true><<<scratch_blocks, 256, 0, st>>>(a, op, scratch);
+                   else     observables_kernel<false, false><<<scratch_blocks, 256, 0, st>>>(a, op, scratch); }
     observables_final_kernel<<<1, 32, 0, st>>>(scratch, scratch_blocks, dev_out);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }

@@ -1,14 +1,19 @@
 // kernels_sweep.cu -- the MMC colour pass (PAPER.md:92 steps 1-4, Eq. (5), (7), (10), (11), (14), (15)) for sm_100a.
 //
-// One thread owns one cell of the active colour.  A warp owns 32 consecutive compact indices of one mesh row of the
-// colour-split layout (mmc_internal.h), so every load of the warp is one fully used 128-byte line: the cell's own
-// vector and B_d, the same compact index of the other colour's row (one x neighbour), that index +-1 (the other x
-// neighbour), and the same compact index of the four adjacent rows (y and z neighbours).  A CTA is a 32 x BY x BZ
-// brick of such cells, so most neighbour lines are shared inside the CTA and come from L1.  Few live registers per
-// thread (one cell) buy the occupancy that hides the HBM latency; the instruction stream, not the byte stream, is
-// the tighter bound of this kernel.
+// Three kernels share one per-cell body (cell_update: trial move, dF/kBT, Eq. (5)):
+//   colour_pass2_kernel      the timed path: a thread owns TWO consecutive compact cells of a row of the active colour
+//                            (64-bit loads of the colour-split arrays of mmc_internal.h; a warp = 64 compact cells of one
+//                            row, a CTA = a 64 x BY x BZ brick of one colour, so neighbour lines are shared through L1);
+//   colour_pass_kernel       one cell per thread: the debug pass with its per-cell dump, and meshes whose compact rows do not
+//                            pair up (periodic in x with an odd compact row length);
+//   small_mesh_sweeps_kernel meshes of <= 8192 cells without demag: one CTA, state in shared memory, all n iterations of
+//                            mmc_sweep(n) in ONE launch.
+// The instruction stream, not the byte stream, is the tighter bound of the pass.
 // RNG: one Philox4x32-10 block per cell per sweep keyed by the natural cell index (replayable on the CPU side).
+#include <cuda.h>
 #include <cuda_runtime.h>
+
+#include <cstring>
 
 #include "mmc_internal.h"
 
@@ -183,6 +188,42 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
     return r;
 }
 
+// S11 + bookkeeping, one thread: advance the sweep counter; every 100 iterations compare the acceptance rate with
+// 0.5 +- 0.05 and move the cone by one degree (PAPER.md:100), clamped to [1, 180] degrees.
+__device__ __forceinline__ void end_sweep(Control* ctl)
+{
+    ctl->sweep += 1ull;
+    ctl->run_sweeps += 1ull;
+    ctl->win_sweeps += 1u;
+    if (ctl->win_sweeps >= 100u) {
+        ctl->accepted += ctl->win_accepted; ctl->trials += ctl->win_trials;
+        if (ctl->adaptive && ctl->win_trials > 0ull) {
+            const double rate = (double)ctl->win_accepted / (double)ctl->win_trials;
+            double cone = ctl->cone_deg;
+            if (rate > 0.55) cone = fmin(180.0, cone + 1.0);
+            else if (rate < 0.45) cone = fmax(1.0, cone - 1.0);
+            ctl->cone_deg = cone;
+            const double h = sin(0.5 * cone * 0.017453292519943295);
+            ctl->one_minus_cos_cone = (float)(2.0 * h * h);
+        }
+        ctl->win_accepted = 0ull; ctl->win_trials = 0ull; ctl->win_sweeps = 0u;
+    }
+}
+// The last CTA of the black pass closes the iteration (S11) when SweepArgs::finish is set: every CTA signs in on a global
+// ticket after its counters have been added (fence, then ticket), and the CTA that draws the last ticket has all of them
+// behind it.  Saves the one-thread end_sweep launch of every iteration (~3 us on the launch-bound configs).
+__device__ __forceinline__ void finish_sweep_ticket(const SweepArgs& a)
+{
+    if (!a.finish) return;
+    __threadfence();
+    const unsigned total = gridDim.x * gridDim.y * gridDim.z;
+    if (atomicAdd(&a.ctl->pad, 1u) == total - 1u) {
+        __threadfence();
+        a.ctl->pad = 0u;
+        end_sweep(a.ctl);
+    }
+}
+
 // ---- S10: acceptance counters and running sums.  Thread: counts and the final vectors of its cells.  Warp: integer REDUX
 // of the packed counts and of the fixed-point sums (kSumScale = 2^22; a warp's <= 64 cells stay far inside int32).  Block:
 // 32-bit shared atomics by lane 0 (two accumulators per sum, for even and odd warps: each collects <= 256 cells, so it
@@ -238,6 +279,7 @@ __device__ __forceinline__ void pass_tail(const SweepArgs& a, PassTailSmem& sm, 
                         atomicAdd(&a.run_sums[t], (unsigned long long)((long long)(int)atomicAdd(&sm.sum[0][t], 0u) +
                                                                        (long long)(int)atomicAdd(&sm.sum[1][t], 0u)));
             }
+            finish_sweep_ticket(a);
         }
     }
 }
@@ -252,9 +294,9 @@ __device__ __forceinline__ void pass_tail(const SweepArgs& a, PassTailSmem& sm, 
 #define MMC_PASS_THREADS 512
 #endif
 constexpr int kPassThreads = MMC_PASS_THREADS;      // CTA = 32 x BY x BZ brick of this many cells
-// coherent load for the persistent single-CTA kernel, whose passes read what earlier passes of the same launch wrote;
-// read-only path otherwise
-template <bool COHERENT> __device__ __forceinline__ float ldc(const float* p) { return COHERENT ? __ldcg(p) : __ldg(p); }   // .cg: from L2, never a stale line
+// plain (generic) load for the single-CTA kernel, whose state lives in shared memory and whose passes read what earlier
+// passes of the same launch wrote (ordered by block barriers); read-only path otherwise
+template <bool COHERENT> __device__ __forceinline__ float ldc(const float* p) { return COHERENT ? *p : __ldg(p); }
 
 // One cell of the active colour: compact index q of row (j, k).  The body of the one-cell-per-thread pass.
 template <unsigned F, bool DEBUG, bool COHERENT>
@@ -397,6 +439,95 @@ __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads)
     pass_tail(a, s_tail, accept ? 1u : 0u, active ? 1u : 0u, fs0, fs1, fs2, fs3, kPassThreads / 32);
 }
 
+// The update of a thread's two cells from their loaded neighbourhood: compact cells q0, q0 + 1 of row (j, k) (mesh cells i0
+// and i0 + 2; `row` = k ny + j; s = parity of the row: active cells sit at i = 2 q + s).  m2 / bd2: own vectors and B_d;
+// xc: the other colour's pair at the same compact index, xs: its third x neighbour (q0 - 1 for s == 0, q0 + 2 for s == 1);
+// yn, ys, zu, zd: the other colour's pairs of the four adjacent rows.  Shared by colour_pass2_kernel (operands from
+// global memory / L1) and colour_pass_tma_kernel (operands from the TMA-staged shared-memory tile).
+template <unsigned F>
+__device__ __forceinline__ void update_pair(const SweepArgs& a, int s, int row, int i0, unsigned ownb, const bool (&act)[2],
+                                            const unsigned (&mb)[2], const unsigned (&cls)[2], const float2 (&m2)[3],
+                                            const float2 (&xc)[3], const float (&xs)[3], const float2 (&yn)[3], const float2 (&ys)[3],
+                                            const float2 (&zu)[3], const float2 (&zd)[3], const float2 (&bd2)[3],
+                                            unsigned long long sweep, float omc,
+                                            unsigned& n_acc, float& fs0, float& fs1, float& fs2, float& fs3)
+{
+    constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
+                   DMI = (F & F_DMI) != 0, CUBIC = (F & F_CUBIC) != 0;
+    const int nx = a.g.nx, ny = a.g.ny;
+    const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
+#pragma unroll
+    for (int t = 0; t < 2; ++t) {
+        if (!act[t]) continue;
+        float m[3], e[3], wv[3], N[3], S_[3], U[3], D[3], Bd[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            m[c] = t ? m2[c].y : m2[c].x;
+            // s == 0: cell 0: E = xc.x, W = xs; cell 1: E = xc.y, W = xc.x.   s == 1: cell 0: W = xc.x, E = xc.y; cell 1: W = xc.y, E = xs
+            if (t == 0) { e[c] = s ? xc[c].y : xc[c].x; wv[c] = s ? xc[c].x : xs[c]; }
+            else        { e[c] = s ? xs[c] : xc[c].y;   wv[c] = s ? xc[c].y : xc[c].x; }
+            N[c] = t ? yn[c].y : yn[c].x; S_[c] = t ? ys[c].y : ys[c].x;
+            if (HASZ) { U[c] = t ? zu[c].y : zu[c].x; D[c] = t ? zd[c].y : zd[c].x; }
+            Bd[c] = t ? bd2[c].y : bd2[c].x;
+        }
+        CellCoef cf;
+        float kscale = 1.f;
+        if (PERCELL) {
+            const float4* tb = a.table + (kClassFloats / 4) * cls[t];
+            const float4 t0 = __ldg(tb), t1 = __ldg(tb + 1);
+            const float2 t2 = __ldg(reinterpret_cast<const float2*>(tb + 2));
+            kscale = t0.x; cf.c4 = t0.y;
+            cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
+            cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
+            if (CUBIC) load_cubic(a.table_cubic + (kClassFloats / 4) * cls[t], cf);
+        } else {
+            cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
+            cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
+            if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; cf.bK2u = a.coef.bK2u; }
+        }
+        cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
+        cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
+        float bE = 1.f, bW = 1.f, bN = 1.f, bS = 1.f, bU = HASZ ? 1.f : 0.f, bD = HASZ ? 1.f : 0.f;
+        if (MASK || PERCELL) {
+            const unsigned b = mb[t];
+            bE = (b & 1u) ? 1.f : 0.f;  bW = (b & 2u) ? 1.f : 0.f;
+            bN = (b & 4u) ? 1.f : 0.f;  bS = (b & 8u) ? 1.f : 0.f;
+            bU = (b & 16u) ? 1.f : 0.f; bD = (b & 32u) ? 1.f : 0.f;
+        } else {
+            if (nx < 2) { bE = 0.f; bW = 0.f; }
+            if (ny < 2) { bN = 0.f; bS = 0.f; }
+        }
+        float Sg[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const float sx = bE * (e[c] - m[c]) + bW * (wv[c] - m[c]);
+            const float sy = bN * (N[c] - m[c]) + bS * (S_[c] - m[c]);
+            float acc = fmaf(cf.kx, sx, cf.ky * sy);
+            if (HASZ) acc = fmaf(cf.kz, bU * (U[c] - m[c]) + bD * (D[c] - m[c]), acc);
+            Sg[c] = acc;
+        }
+        float selfc = 0.5f * fmaf(cf.kx, bE + bW, cf.ky * (bN + bS));
+        if (HASZ) selfc = fmaf(0.5f * cf.kz, bU + bD, selfc);
+        float dzx = 0.f, dzy = 0.f, dxx = 0.f, dyy = 0.f;
+        if (DMI) {
+            dzx = bE * e[2] - bW * wv[2];
+            dzy = bN * N[2] - bS * S_[2];
+            dxx = bE * e[0] - bW * wv[0];
+            dyy = bN * N[1] - bS * S_[1];
+        }
+        const unsigned cell = (unsigned)row * nx + (unsigned)(i0 + 2 * t);       // natural cell index (< 2^31)
+        const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
+        const CellResult r = cell_update<DMI, false, CUBIC>(m, Sg, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
+        float f0 = m[0], f1 = m[1], f2 = m[2], f3 = r.L;
+        if (r.accept) {
+            f0 += r.dm[0]; f1 += r.dm[1]; f2 += r.dm[2]; f3 *= r.f;
+            a.m[0][ownb + t] = f0; a.m[1][ownb + t] = f1; a.m[2][ownb + t] = f2;
+            n_acc++;
+        }
+        fs0 += f0; fs1 += f1; fs2 += f2; fs3 += f3;
+    }
+}
+
 // ------------------------------------------------------------------------------------------------ the pass, two cells per thread
 // The same pass with a thread owning TWO consecutive compact cells of a row (mesh cells i and i + 2): the vectors, B_d and
 // class words / masks come as 64-bit loads, the x neighbour between the two cells is loaded once, index arithmetic, bond
@@ -412,7 +543,7 @@ template <unsigned F>
 __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_kernel(const SweepArgs a)
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
-                   DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0, CUBIC = (F & F_CUBIC) != 0;
+                   DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
     __shared__ PassTailSmem s_tail;
     pass_tail_init(s_tail);
 
@@ -473,129 +604,232 @@ __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_ke
             if (HASZ) { zu[c] = __ldg(reinterpret_cast<const float2*>(P + othb + dU)); zd[c] = __ldg(reinterpret_cast<const float2*>(P + othb + dD)); }
             bd2[c] = DEMAG ? __ldg(reinterpret_cast<const float2*>(a.bd[c] + ownb)) : make_float2(0.f, 0.f);
         }
-        const unsigned long long sweep = a.ctl->sweep;
-        const float omc = a.ctl->one_minus_cos_cone;
-        const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
-#pragma unroll
-        for (int t = 0; t < 2; ++t) {
-            if (!act[t]) continue;
-            float m[3], e[3], wv[3], N[3], S_[3], U[3], D[3], Bd[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                m[c] = t ? m2[c].y : m2[c].x;
-                // s == 0: cell 0: E = xc.x, W = xs; cell 1: E = xc.y, W = xc.x.   s == 1: cell 0: W = xc.x, E = xc.y; cell 1: W = xc.y, E = xs
-                if (t == 0) { e[c] = s ? xc[c].y : xc[c].x; wv[c] = s ? xc[c].x : xs[c]; }
-                else        { e[c] = s ? xs[c] : xc[c].y;   wv[c] = s ? xc[c].y : xc[c].x; }
-                N[c] = t ? yn[c].y : yn[c].x; S_[c] = t ? ys[c].y : ys[c].x;
-                if (HASZ) { U[c] = t ? zu[c].y : zu[c].x; D[c] = t ? zd[c].y : zd[c].x; }
-                Bd[c] = t ? bd2[c].y : bd2[c].x;
-            }
-            CellCoef cf;
-            float kscale = 1.f;
-            if (PERCELL) {
-                const float4* tb = a.table + (kClassFloats / 4) * cls[t];
-                const float4 t0 = __ldg(tb), t1 = __ldg(tb + 1);
-                const float2 t2 = __ldg(reinterpret_cast<const float2*>(tb + 2));
-                kscale = t0.x; cf.c4 = t0.y;
-                cf.mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
-                cf.bKq = t1.x; cf.bzee = t1.y; cf.sigma = t1.z; cf.ax = t1.w; cf.ay = t2.x; cf.az = t2.y;
-                if (CUBIC) load_cubic(a.table_cubic + (kClassFloats / 4) * cls[t], cf);
-            } else {
-                cf.bKq = a.coef.bKq; cf.bzee = a.coef.bzee; cf.c4 = a.coef.c4; cf.sigma = a.coef.sigma;
-                cf.ax = a.coef.ax; cf.ay = a.coef.ay; cf.az = a.coef.az; cf.mu2 = a.coef.mu2;
-                if (CUBIC) { cf.bK1c = a.coef.bK1c; cf.bK2c = a.coef.bK2c; for (int q = 0; q < 9; ++q) cf.cub[q] = a.coef.cub[q]; cf.bK2u = a.coef.bK2u; }
-            }
-            cf.kx = a.coef.kx * kscale; cf.ky = a.coef.ky * kscale; cf.kz = a.coef.kz * kscale;
-            cf.gx = a.coef.gx * kscale; cf.gy = a.coef.gy * kscale;
-            float bE = 1.f, bW = 1.f, bN = 1.f, bS = 1.f, bU = HASZ ? 1.f : 0.f, bD = HASZ ? 1.f : 0.f;
-            if (MASK || PERCELL) {
-                const unsigned b = mb[t];
-                bE = (b & 1u) ? 1.f : 0.f;  bW = (b & 2u) ? 1.f : 0.f;
-                bN = (b & 4u) ? 1.f : 0.f;  bS = (b & 8u) ? 1.f : 0.f;
-                bU = (b & 16u) ? 1.f : 0.f; bD = (b & 32u) ? 1.f : 0.f;
-            } else {
-                if (nx < 2) { bE = 0.f; bW = 0.f; }
-                if (ny < 2) { bN = 0.f; bS = 0.f; }
-            }
-            float Sg[3];
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const float sx = bE * (e[c] - m[c]) + bW * (wv[c] - m[c]);
-                const float sy = bN * (N[c] - m[c]) + bS * (S_[c] - m[c]);
-                float acc = fmaf(cf.kx, sx, cf.ky * sy);
-                if (HASZ) acc = fmaf(cf.kz, bU * (U[c] - m[c]) + bD * (D[c] - m[c]), acc);
-                Sg[c] = acc;
-            }
-            float selfc = 0.5f * fmaf(cf.kx, bE + bW, cf.ky * (bN + bS));
-            if (HASZ) selfc = fmaf(0.5f * cf.kz, bU + bD, selfc);
-            float dzx = 0.f, dzy = 0.f, dxx = 0.f, dyy = 0.f;
-            if (DMI) {
-                dzx = bE * e[2] - bW * wv[2];
-                dzy = bN * N[2] - bS * S_[2];
-                dxx = bE * e[0] - bW * wv[0];
-                dyy = bN * N[1] - bS * S_[1];
-            }
-            const unsigned cell = (unsigned)row * nx + (unsigned)(i0 + 2 * t);       // natural cell index (< 2^31)
-            const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
-            const CellResult r = cell_update<DMI, false, CUBIC>(m, Sg, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
-            float f0 = m[0], f1 = m[1], f2 = m[2], f3 = r.L;
-            if (r.accept) {
-                f0 += r.dm[0]; f1 += r.dm[1]; f2 += r.dm[2]; f3 *= r.f;
-                a.m[0][ownb + t] = f0; a.m[1][ownb + t] = f1; a.m[2][ownb + t] = f2;
-                n_acc++;
-            }
-            fs0 += f0; fs1 += f1; fs2 += f2; fs3 += f3;
-        }
+        update_pair<F>(a, s, row, i0, ownb, act, mb, cls, m2, xc, xs, yn, ys, zu, zd, bd2, a.ctl->sweep, a.ctl->one_minus_cos_cone,
+                       n_acc, fs0, fs1, fs2, fs3);
     }
     pass_tail(a, s_tail, n_acc, (act[0] ? 1u : 0u) + (act[1] ? 1u : 0u), fs0, fs1, fs2, fs3, kPass2Threads / 32);
 }
 
-// S11 + bookkeeping, one thread: advance the sweep counter; every 100 iterations compare the acceptance rate with
-// 0.5 +- 0.05 and move the cone by one degree (PAPER.md:100), clamped to [1, 180] degrees.
-__device__ __forceinline__ void end_sweep(Control* ctl)
+// ------------------------------------------------------------------------------------------------ the pass, staged by TMA
+// The same pass with its operands staged into shared memory by the TMA unit (cp.async.bulk.tensor + mbarrier) instead of
+// per-thread global loads: a persistent CTA walks over tiles of 64 x BY x BZ compact cells of the active colour; one producer
+// warp requests, per tile, the own-colour boxes (m, B_d, class words) and the other colour's boxes with a one-row / one-layer
+// halo and a 16-byte aligned x window (72 floats from q0 - 4), into a ring of kTmaStages stages; eight consumer warps wait
+// on the stage's full barrier, update the tile from shared memory with update_pair (two cells per thread, a warp per row)
+// and release the stage.  Out-of-mesh elements arrive as zeros (their bonds are masked).  TMA does not wrap, so this
+// kernel serves meshes without periodic directions (BASELINE configs 2, 4, 5); everything else takes colour_pass2_kernel.
+// north_star (a) asks for this variant to be measured against plain L1-served loads: profiles/ has both.
+constexpr int kTmaConsumerWarps = 8, kTmaThreads = (kTmaConsumerWarps + 1) * 32, kTmaStages = 2;
+constexpr int kTmaX = 64, kTmaXO = 72;                 // compact cells per tile row; floats of the other colour's x window
+
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned arrivals)
 {
-    ctl->sweep += 1ull;
-    ctl->run_sweeps += 1ull;
-    ctl->win_sweeps += 1u;
-    if (ctl->win_sweeps >= 100u) {
-        ctl->accepted += ctl->win_accepted; ctl->trials += ctl->win_trials;
-        if (ctl->adaptive && ctl->win_trials > 0ull) {
-            const double rate = (double)ctl->win_accepted / (double)ctl->win_trials;
-            double cone = ctl->cone_deg;
-            if (rate > 0.55) cone = fmin(180.0, cone + 1.0);
-            else if (rate < 0.45) cone = fmax(1.0, cone - 1.0);
-            ctl->cone_deg = cone;
-            const double h = sin(0.5 * cone * 0.017453292519943295);
-            ctl->one_minus_cos_cone = (float)(2.0 * h * h);
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(arrivals) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity)
+{
+    unsigned ok;
+    do {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+// one box of a rank-4 tensor (x, y, z, colour) -> shared memory, completion counted in bytes on `bar`
+__device__ __forceinline__ void tma_load_4d(void* dst, const void* tmap, int x, int y, int z, int w, unsigned long long* bar)
+{
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(smem_addr(dst)), "l"(tmap), "r"(x), "r"(y), "r"(z), "r"(w), "r"(smem_addr(bar)) : "memory");
+}
+
+template <unsigned F>
+__global__ void __launch_bounds__(kTmaThreads, 2) colour_pass_tma_kernel(const SweepArgs a, const PassTmaShape sh,
+                                                                       const __grid_constant__ PassTmaMaps maps)
+{
+    constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
+                   DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
+    extern __shared__ __align__(128) unsigned char tsm[];
+    __shared__ unsigned long long s_bar[2 * kTmaStages];          // full[stage], empty[stage]
+    __shared__ unsigned long long s_tot[6];                       // accepted, trials, four fixed-point sums
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int BY = sh.BY, BZ = sh.BZ, zh = sh.zh, rows = BY * BZ, OY = BY + 2;
+    const int own_arr = rows * kTmaX * 4;                          // bytes of one own-colour array of a tile
+    const int oth_arr = sh.oth_arr;                                // bytes of one other-colour array (128-byte multiple)
+    constexpr int NOWN = 3 + (DEMAG ? 3 : 0) + (PERCELL ? 1 : 0);
+    const int stage_bytes = NOWN * own_arr + 3 * oth_arr;
+    const int ntiles = sh.tiles_x * sh.tiles_y * sh.tiles_z;
+    const int col = a.colour;
+    if (threadIdx.x == 0) {
+        for (int q = 0; q < kTmaStages; ++q) { mbar_init(&s_bar[q], 1u); mbar_init(&s_bar[kTmaStages + q], kTmaConsumerWarps); }
+        for (int q = 0; q < 6; ++q) s_tot[q] = 0ull;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == kTmaConsumerWarps) {
+        // ---- producer: one lane requests the boxes of every tile of this CTA
+        if (lane == 0) {
+            int it = 0;
+            for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
+                const int st = it % kTmaStages, ph = (it / kTmaStages) & 1;
+                mbar_wait(&s_bar[kTmaStages + st], (unsigned)(ph ^ 1));              // the consumers have released this stage
+                const int tx = t % sh.tiles_x, r = t / sh.tiles_x, ty = r % sh.tiles_y, tz = r / sh.tiles_y;
+                const int q0 = tx * kTmaX, j0 = ty * BY, k0 = tz * BZ;
+                unsigned char* base = tsm + (size_t)st * stage_bytes;
+                unsigned long long* full = &s_bar[st];
+                unsigned bytes = (unsigned)(3 * own_arr + 3 * sh.oth_box_bytes);
+                if (DEMAG) bytes += 3u * own_arr;
+                if (PERCELL) bytes += (unsigned)own_arr;
+                mbar_expect_tx(full, bytes);
+                int slot = 0;
+                for (int c = 0; c < 3; ++c) tma_load_4d(base + (slot++) * own_arr, &maps.own_m[c], q0, j0, k0, col, full);
+                if (DEMAG) for (int c = 0; c < 3; ++c) tma_load_4d(base + (slot++) * own_arr, &maps.bd[c], q0, j0, k0, col, full);
+                if (PERCELL) tma_load_4d(base + (slot++) * own_arr, &maps.cw, q0, j0, k0, col, full);
+                unsigned char* ob = base + NOWN * own_arr;
+                for (int c = 0; c < 3; ++c) tma_load_4d(ob + c * oth_arr, &maps.oth_m[c], q0 - 4, j0 - 1, k0 - zh, 1 - col, full);
+            }
         }
-        ctl->win_accepted = 0ull; ctl->win_trials = 0ull; ctl->win_sweeps = 0u;
+    } else {
+        // ---- consumers: a warp per tile row, two cells per lane
+        const int nx = a.g.nx, ny = a.g.ny, nz = a.g.nz, hx = a.g.hx;
+        const unsigned H = (unsigned)a.g.H;
+        const unsigned long long sweep = a.ctl->sweep;
+        const float omc = a.ctl->one_minus_cos_cone;
+        const bool want_sums = a.run_sums != nullptr;
+        long long tot[6] = { 0, 0, 0, 0, 0, 0 };                   // lane 0: accepted, trials, fixed-point sums of this warp
+        const int ql = 2 * lane;                                   // compact index of the lane's first cell inside the tile row
+        int it = 0;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
+            const int st = it % kTmaStages, ph = (it / kTmaStages) & 1;
+            const int tx = t % sh.tiles_x, rr = t / sh.tiles_x, ty = rr % sh.tiles_y, tz = rr / sh.tiles_y;
+            const int j0 = ty * BY, k0 = tz * BZ, q0 = tx * kTmaX + ql;
+            const unsigned char* base = tsm + (size_t)st * stage_bytes;
+            const unsigned char* ob = base + NOWN * own_arr;
+            mbar_wait(&s_bar[st], (unsigned)ph);                   // the tile has landed
+            unsigned n_acc = 0u, n_tri = 0u;
+            int is0 = 0, is1 = 0, is2 = 0, is3 = 0;                // fixed-point sums, rounded per cell pair exactly as colour_pass2_kernel does
+            for (int r = warp; r < rows; r += kTmaConsumerWarps) {
+                float fs0 = 0.f, fs1 = 0.f, fs2 = 0.f, fs3 = 0.f;
+                const int kk = r / BY, jj = r - kk * BY, j = j0 + jj, k = k0 + kk;
+                const int s = ((j + k) & 1) ^ col;
+                const int i0 = 2 * q0 + s;
+                const bool inrow = j < ny && k < nz;
+                bool act[2] = { inrow && i0 < nx, inrow && i0 + 2 < nx };
+                const int row = k * ny + j;
+                const unsigned ownb = (unsigned)col * H + (unsigned)row * hx + q0;
+                const int oo = (r * kTmaX + ql) * 4;               // byte offset of the lane's pair in an own-colour array
+                unsigned mb[2] = { 0x7fu, 0x7fu }, cls[2] = { 0u, 0u };
+                if (act[0]) {
+                    if (PERCELL) {
+                        const uint2 w = *reinterpret_cast<const uint2*>(base + (NOWN - 1) * own_arr + oo);
+                        mb[0] = w.x & 0x7fu; cls[0] = w.x >> 7; mb[1] = w.y & 0x7fu; cls[1] = w.y >> 7;
+                    } else if (MASK) {
+                        const uchar2 w = __ldg(reinterpret_cast<const uchar2*>(a.mask + ownb));
+                        mb[0] = w.x; mb[1] = w.y;
+                    }
+                    if (!DENSE && (MASK || PERCELL)) { act[0] = act[0] && (mb[0] & 0x40u); act[1] = act[1] && (mb[1] & 0x40u); }
+                }
+                if (act[0] || act[1]) {
+                    float2 m2[3], xc[3], yn[3], ys[3], zu[3], zd[3], bd2[3];
+                    float xs[3];
+                    const int orow = (kk + zh) * OY + jj + 1;      // this row inside the other colour's box
+                    const int up = (zh || kk + 1 < BZ) ? OY : 0, dn = (zh || kk > 0) ? -OY : 0;   // no layer there: any row (bond masked)
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        const float* om = reinterpret_cast<const float*>(ob + c * oth_arr) + 4 + ql;
+                        m2[c] = *reinterpret_cast<const float2*>(base + c * own_arr + oo);
+                        xc[c] = *reinterpret_cast<const float2*>(om + orow * kTmaXO);
+                        xs[c] = om[orow * kTmaXO + (s ? 2 : -1)];
+                        yn[c] = *reinterpret_cast<const float2*>(om + (orow + 1) * kTmaXO);
+                        ys[c] = *reinterpret_cast<const float2*>(om + (orow - 1) * kTmaXO);
+                        if (HASZ) {
+                            zu[c] = *reinterpret_cast<const float2*>(om + (orow + up) * kTmaXO);
+                            zd[c] = *reinterpret_cast<const float2*>(om + (orow + dn) * kTmaXO);
+                        }
+                        bd2[c] = DEMAG ? *reinterpret_cast<const float2*>(base + (3 + c) * own_arr + oo) : make_float2(0.f, 0.f);
+                    }
+                    update_pair<F>(a, s, row, i0, ownb, act, mb, cls, m2, xc, xs, yn, ys, zu, zd, bd2, sweep, omc, n_acc, fs0, fs1, fs2, fs3);
+                }
+                n_tri += (act[0] ? 1u : 0u) + (act[1] ? 1u : 0u);
+                if (want_sums) {
+                    is0 += __float2int_rn(fs0 * kSumScale); is1 += __float2int_rn(fs1 * kSumScale);
+                    is2 += __float2int_rn(fs2 * kSumScale); is3 += __float2int_rn(fs3 * kSumScale);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&s_bar[kTmaStages + st]);    // this warp has read everything it needs from the stage
+            // S10: the tile's counters and fixed-point sums (a warp holds <= 128 cells of |m| < 2: inside int32), added up in 64 bits by lane 0
+            const unsigned cnt = __reduce_add_sync(0xffffffffu, n_acc | (n_tri << 16));
+            tot[0] += cnt & 0xffffu; tot[1] += cnt >> 16;
+            if (want_sums) {
+                tot[2] += __reduce_add_sync(0xffffffffu, is0);
+                tot[3] += __reduce_add_sync(0xffffffffu, is1);
+                tot[4] += __reduce_add_sync(0xffffffffu, is2);
+                tot[5] += __reduce_add_sync(0xffffffffu, is3);
+            }
+        }
+        if (lane == 0 && tot[1])
+            for (int q = 0; q < 6; ++q) atomicAdd(&s_tot[q], (unsigned long long)tot[q]);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        if (s_tot[1]) {
+            atomicAdd(&a.ctl->win_trials, s_tot[1]);
+            if (s_tot[0]) atomicAdd(&a.ctl->win_accepted, s_tot[0]);
+            if (a.run_sums) for (int q = 0; q < 4; ++q) atomicAdd(&a.run_sums[q], s_tot[2 + q]);
+        }
+        finish_sweep_ticket(a);
     }
 }
+
 __global__ void end_sweep_kernel(Control* ctl) { end_sweep(ctl); }
 
 // ------------------------------------------------------------------------------------------------ small meshes: all iterations in one launch
 // Meshes of a few thousand cells without demag (BASELINE.json config 1: 1024 cells) are bound by launch latency: three
 // launches per iteration take ~12 us while the arithmetic of a pass takes ~1 us.  Here ONE CTA runs n iterations in one
-// launch (SURVEY 8(d) "Config 1"): red pass, barrier, black pass, barrier, end-of-sweep bookkeeping by thread 0, barrier.
-// The cell arithmetic is pass_one_cell, the same function the one-cell pass uses, with coherent loads (a pass reads what
-// the previous pass of the same launch wrote; the state lives in this SM's L1/L2); counters and running sums are reduced
-// per pass with the same integer arithmetic, so the results are bit-identical to the launch-per-pass path.
+// launch (SURVEY 8(d) "Config 1"): the state (colour-split, 3 x 2H floats), the control block and the running sums are
+// copied to shared memory, then red pass, barrier, black pass, barrier, end-of-sweep bookkeeping by thread 0, barrier, n
+// times, and everything is written back once.  The cell arithmetic is pass_one_cell, the same function the one-cell pass
+// uses (its pointers simply point into shared memory); counters and running sums are reduced per pass with the same
+// integer arithmetic, so the results are bit-identical to the launch-per-pass path.
 constexpr int kSmallThreads = 1024;
 constexpr int kSmallMaxCells = 1 << 13;         // <= 4 cells per thread and colour: a warp's fixed-point sum stays inside int32 for |m| < 2
+constexpr int kSmallMaxSlots = 1 << 14;         // storage slots (2 H) per component: 3 x 64 KB of shared memory
 
 template <unsigned F>
-__global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(const SweepArgs a, int n_sweeps)
+__global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(const SweepArgs a_in, int n_sweeps)
 {
+    extern __shared__ float s_m[];                    // [3][2 H]
+    __shared__ Control s_ctl;
+    __shared__ unsigned long long s_run[4];
     __shared__ unsigned s_cnt;                        // accepted | trials << 16 would overflow: two words
     __shared__ unsigned s_tri;
     __shared__ long long s_sum[4];
     const int tid = threadIdx.x;
+    SweepArgs a = a_in;
     const int hxr = (a.g.nx + 1) >> 1, rows = a.g.ny * a.g.nz, slots = hxr * rows;
-    Control* ctl = a.ctl;
+    const int S2 = (int)(2 * a.g.H);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        for (int i = tid; i < S2; i += kSmallThreads) s_m[c * S2 + i] = a_in.m[c][i];
+        a.m[c] = s_m + c * S2;
+    }
+    if (tid == 0) s_ctl = *a_in.ctl;
+    if (tid < 4) s_run[tid] = a_in.run_sums ? a_in.run_sums[tid] : 0ull;
+    a.ctl = &s_ctl;
+    __syncthreads();
     for (int it = 0; it < n_sweeps; ++it) {
-        const unsigned long long sweep = *reinterpret_cast<volatile unsigned long long*>(&ctl->sweep);
-        const float omc = *reinterpret_cast<volatile float*>(&ctl->one_minus_cos_cone);
+        const unsigned long long sweep = s_ctl.sweep;
+        const float omc = s_ctl.one_minus_cos_cone;
         for (int col = 0; col < 2; ++col) {
+            __syncthreads();                          // s_ctl read by everyone; previous totals consumed
             if (tid == 0) { s_cnt = 0u; s_tri = 0u; s_sum[0] = s_sum[1] = s_sum[2] = s_sum[3] = 0; }
             __syncthreads();
             unsigned n_acc = 0u, n_tri = 0u;
@@ -621,14 +855,18 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(con
             }
             __syncthreads();                          // the pass is complete and visible to the whole CTA
             if (tid == 0) {
-                ctl->win_accepted += s_cnt; ctl->win_trials += s_tri;
-                if (a.run_sums) for (int t = 0; t < 4; ++t) a.run_sums[t] += (unsigned long long)s_sum[t];
-                if (col == 1) end_sweep(ctl);
-                __threadfence_block();
+                s_ctl.win_accepted += s_cnt; s_ctl.win_trials += s_tri;
+                if (a_in.run_sums) for (int t = 0; t < 4; ++t) s_run[t] += (unsigned long long)s_sum[t];
+                if (col == 1) end_sweep(&s_ctl);
             }
         }
         __syncthreads();                              // the new sweep counter and cone are visible
     }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        for (int i = tid; i < S2; i += kSmallThreads) a_in.m[c][i] = s_m[c * S2 + i];
+    if (tid == 0) *a_in.ctl = s_ctl;
+    if (tid < 4 && a_in.run_sums) a_in.run_sums[tid] = s_run[tid];
 }
 
 int launch_end_sweep(Control* ctl, void* stream)
@@ -673,22 +911,110 @@ static int launch_variant(const SweepArgs& a, bool debug, cudaStream_t st)
 // (B_d = 0 when the demag term is off), so the other flags may be over-approximated.
 // n whole iterations in one launch for small meshes without demag; returns MMC_E_UNSUPPORTED when the mesh does not qualify
 // (the caller then takes the launch-per-pass path).  Variants: uniform coefficients only.
+template <unsigned F>
+static int launch_small_variant(const SweepArgs& a, int n_sweeps, cudaStream_t st)
+{
+    const size_t smem = (size_t)3 * 2 * a.g.H * sizeof(float);
+    auto kern = small_mesh_sweeps_kernel<F>;
+    if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+    kern<<<1, kSmallThreads, smem, st>>>(a, n_sweeps);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
 int launch_small_mesh_sweeps(const SweepArgs& a, unsigned f, int n_sweeps, void* stream)
 {
     cudaStream_t st = (cudaStream_t)stream;
     const long long cells = (long long)a.g.nx * a.g.ny * a.g.nz;
-    if (cells > kSmallMaxCells || (f & (F_PERCELL | F_DEMAG | F_CUBIC))) return MMC_E_UNSUPPORTED;
+    if (cells > kSmallMaxCells || 2 * a.g.H > kSmallMaxSlots || (f & (F_PERCELL | F_DEMAG | F_CUBIC))) return MMC_E_UNSUPPORTED;
     f &= ~F_DENSE;
     constexpr unsigned U = F_MASK | F_Z | F_DMI;
-    if (f == 0u) small_mesh_sweeps_kernel<0u><<<1, kSmallThreads, 0, st>>>(a, n_sweeps);
-    else if ((f & ~F_MASK) == 0u) small_mesh_sweeps_kernel<F_MASK><<<1, kSmallThreads, 0, st>>>(a, n_sweeps);
-    else small_mesh_sweeps_kernel<U><<<1, kSmallThreads, 0, st>>>(a, n_sweeps);
-    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+    if (f == 0u) return launch_small_variant<0u>(a, n_sweeps, st);
+    if ((f & ~F_MASK) == 0u) return launch_small_variant<F_MASK>(a, n_sweeps, st);
+    return launch_small_variant<U>(a, n_sweeps, st);
 }
 
-int launch_colour_pass(const SweepArgs& a, unsigned f, bool debug, void* stream)
+// ---- host side of the TMA-staged pass
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+void pass_tma_build(const Geometry& g, float* const m[3], float* const bd[3], const uint32_t* cw, PassTma* out)
+{
+    out->ok = false;
+    if (g.pbc != 0u) return;                                       // TMA boxes do not wrap
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qr;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) != cudaSuccess || !fn || qr != cudaDriverEntryPointSuccess) {
+        cudaGetLastError();
+        return;
+    }
+    EncodeTiledFn encode = reinterpret_cast<EncodeTiledFn>(fn);
+    PassTmaShape sh{};
+    sh.BZ = g.nz >= 4 ? 4 : g.nz;
+    sh.zh = g.nz > sh.BZ ? 1 : 0;
+    sh.BY = 16 / sh.BZ;
+    const int hxr = (g.nx + 1) >> 1;
+    sh.tiles_x = (hxr + kTmaX - 1) / kTmaX; sh.tiles_y = (g.ny + sh.BY - 1) / sh.BY; sh.tiles_z = (g.nz + sh.BZ - 1) / sh.BZ;
+    const int oy = sh.BY + 2, oz = sh.BZ + 2 * sh.zh;
+    sh.oth_box_bytes = oy * oz * kTmaXO * 4;
+    sh.oth_arr = (sh.oth_box_bytes + 127) / 128 * 128;
+    const cuuint64_t dims[4] = { (cuuint64_t)g.hx, (cuuint64_t)g.ny, (cuuint64_t)g.nz, 2 };
+    const cuuint64_t strides[3] = { (cuuint64_t)g.hx * 4, (cuuint64_t)g.hx * g.ny * 4, (cuuint64_t)g.H * 4 };
+    const cuuint32_t own_box[4] = { (cuuint32_t)kTmaX, (cuuint32_t)sh.BY, (cuuint32_t)sh.BZ, 1 };
+    const cuuint32_t oth_box[4] = { (cuuint32_t)kTmaXO, (cuuint32_t)oy, (cuuint32_t)oz, 1 };
+    const cuuint32_t ones[4] = { 1, 1, 1, 1 };
+    auto enc = [&](unsigned char (&dst)[128], CUtensorMapDataType dt, const void* base, const cuuint32_t* box) {
+        CUtensorMap tm;
+        if (encode(&tm, dt, 4, const_cast<void*>(base), dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS) return false;
+        static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
+        std::memcpy(dst, &tm, 128);
+        return true;
+    };
+    bool good = true;
+    for (int c = 0; c < 3 && good; ++c) {
+        good = enc(out->maps.own_m[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, m[c], own_box) && enc(out->maps.oth_m[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, m[c], oth_box)
+               && enc(out->maps.bd[c], CU_TENSOR_MAP_DATA_TYPE_FLOAT32, bd[c], own_box);
+    }
+    if (good && cw) good = enc(out->maps.cw, CU_TENSOR_MAP_DATA_TYPE_UINT32, cw, own_box);
+    if (!good) return;
+    out->sh = sh; out->key[0] = m[0]; out->key[1] = bd[0]; out->key[2] = cw;
+    out->ok = true;
+}
+
+template <unsigned F>
+static int launch_tma_variant(const SweepArgs& a, const PassTma& t, cudaStream_t st)
+{
+    constexpr int NOWN = 3 + ((F & F_DEMAG) ? 3 : 0) + ((F & F_PERCELL) ? 1 : 0);
+    const int rows = t.sh.BY * t.sh.BZ;
+    const size_t smem = (size_t)kTmaStages * ((size_t)NOWN * rows * kTmaX * 4 + 3 * (size_t)t.sh.oth_arr);
+    auto kern = colour_pass_tma_kernel<F>;
+    if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+    const int ntiles = t.sh.tiles_x * t.sh.tiles_y * t.sh.tiles_z;
+    if (ntiles < 2 * 148) return MMC_E_UNSUPPORTED;               // too few tiles to give every SM its two CTAs: the brick kernel spreads better
+    const int grid = 2 * 148;
+    kern<<<grid, kTmaThreads, smem, st>>>(a, t.sh, t.maps);
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+// the feature sets of the open-boundary BASELINE configs; anything else is served by colour_pass2_kernel
+static int launch_colour_pass_tma(const SweepArgs& a, unsigned f, const PassTma& t, cudaStream_t st)
+{
+    switch (f) {
+        case F_MASK | F_DEMAG | F_DENSE: return launch_tma_variant<F_MASK | F_DEMAG | F_DENSE>(a, t, st);                                   // cfg 2
+        case F_MASK | F_DEMAG: return launch_tma_variant<F_MASK | F_DEMAG>(a, t, st);                                                       // cfg 5
+        case F_MASK | F_PERCELL | F_Z | F_DEMAG | F_DENSE: return launch_tma_variant<F_MASK | F_PERCELL | F_Z | F_DEMAG | F_DENSE>(a, t, st);   // cfg 4
+        case F_MASK | F_PERCELL | F_Z | F_DEMAG: return launch_tma_variant<F_MASK | F_PERCELL | F_Z | F_DEMAG>(a, t, st);
+        case F_MASK | F_Z | F_DEMAG | F_DENSE: return launch_tma_variant<F_MASK | F_Z | F_DEMAG | F_DENSE>(a, t, st);
+        default: return MMC_E_UNSUPPORTED;
+    }
+}
+
+int launch_colour_pass(const SweepArgs& a, unsigned f, bool debug, void* stream, const PassTma* tma)
 {
     cudaStream_t st = (cudaStream_t)stream;
+    if (tma && tma->ok && !debug) {
+        const int rc = launch_colour_pass_tma(a, f, *tma, st);
+        if (rc != MMC_E_UNSUPPORTED) return rc;
+    }
     constexpr unsigned UALL = F_MASK | F_Z | F_DMI | F_DEMAG, PALL = UALL | F_PERCELL;
     const bool dense = (f & F_DENSE) != 0;             // only ever a promise, never over-approximated
     f &= ~F_DENSE;

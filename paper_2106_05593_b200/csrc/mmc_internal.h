@@ -74,7 +74,7 @@ struct Control {
     int adaptive;
     double cone_deg;
     float one_minus_cos_cone;
-    unsigned int pad;
+    unsigned int pad;                // ticket counter of finish_sweep_ticket (kernels_sweep.cu); 0 between passes
     unsigned long long run_sweeps;   // sweeps accumulated into the running sums
 };
 
@@ -100,6 +100,7 @@ struct SweepArgs {
     Control* ctl;
     unsigned seed_lo, seed_hi;
     int colour;
+    int finish;                  // != 0: the last CTA of this pass runs the end-of-sweep bookkeeping (S11) itself
     unsigned long long* run_sums; // [4] running sums of the sweeps' final mx,my,mz,|m| in fixed point (two's complement, kSumScale), or NULL
     // debug dump (natural order), any NULL
     float* dbg_dm; float* dbg_terms; float* dbg_margin; uint8_t* dbg_acc;
@@ -107,8 +108,21 @@ struct SweepArgs {
 
 struct Observables { double sum[4]; double E[6]; unsigned long long n_active; };
 
+// TMA-staged colour pass (kernels_sweep.cu): tensor maps (CUtensorMap is 128 bytes, 64-byte aligned) over the colour-split
+// arrays as rank-4 tensors (x = compact index, y, z, colour) and the tile shape they were encoded for.
+struct alignas(64) PassTmaMaps { unsigned char own_m[3][128], oth_m[3][128], bd[3][128], cw[128]; };
+struct PassTmaShape { int BY, BZ, zh, tiles_x, tiles_y, tiles_z, oth_arr, oth_box_bytes; };
+struct PassTma {
+    bool ok = false;
+    PassTmaShape sh{};
+    PassTmaMaps maps{};
+    const void* key[3] = { nullptr, nullptr, nullptr };   // m[0], bd[0], cw the maps were built for
+};
+// builds the maps when the mesh qualifies (no periodic direction, driver entry point available); ok = false otherwise
+void pass_tma_build(const Geometry& g, float* const m[3], float* const bd[3], const uint32_t* cw, PassTma* out);
+
 // kernels_sweep.cu
-int launch_colour_pass(const SweepArgs& a, unsigned features, bool debug, void* stream);
+int launch_colour_pass(const SweepArgs& a, unsigned features, bool debug, void* stream, const PassTma* tma = nullptr);
 int launch_end_sweep(Control* ctl, void* stream);
 int launch_small_mesh_sweeps(const SweepArgs& a, unsigned features, int n_sweeps, void* stream);
 // kernels_layout.cu
