@@ -362,6 +362,14 @@ def run_ours(args):
     e2e_s = time.perf_counter() - t0
     e2e_val = aggregate_over_ranks(float(wl.n_active) * nE, e2e_s)
     h2d = 3 * wl.N * 4; d2h = 3 * wl.N * 4 + P.C.sizeof(P.Obs)
+    # how much of an e2e step is the two copies (same calls, no iteration and no read-out in between)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(nE):
+        g._ck(L.mmc_set_m_host(g._h, host_in[0].data_ptr(), host_in[1].data_ptr(), host_in[2].data_ptr()))
+        g._ck(L.mmc_get_m_host(g._h, host_out[0].data_ptr(), host_out[1].data_ptr(), host_out[2].data_ptr()))
+        torch.cuda.synchronize(dev)
+    copies_s = (time.perf_counter() - t0) / nE
 
     if rank == 0:
         peak, peak_src = _peaks()
@@ -442,7 +450,9 @@ def run_ours(args):
                        "launch_path": ("one launch of the single-CTA kernel for all K iterations" if single_launch else
                                        "first iteration as plain launches, the rest replayed from CUDA graphs of 16 and 1 iterations")},
             "clocks": clocks,
-            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nE},
+            "e2e": {"value": e2e_val, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": nE,
+                    "ms_per_step": 1e3 * e2e_s / nE, "copies_ms_per_step": 1e3 * copies_s,
+                    "copies_share_of_step": copies_s / (e2e_s / nE) if e2e_s > 0 else None},
             "gpu_launches": 1 if single_launch else per_iter * K,
             "phases_ms_per_step": {k: v / K for k, v in phases.items()},
             "phases_path": ("mmc_sweep_timed: launch-per-kernel with CUDA events around every launch" +

@@ -113,19 +113,28 @@ int mmc_get_m(mmc_ctx* ctx, float* mx, float* my, float* mz);
  * stream synchronise by the caller.  This is the end-to-end path of a caller whose state lives on the host. */
 int mmc_set_m_host(mmc_ctx* ctx, const float* mx, const float* my, const float* mz);
 int mmc_get_m_host(mmc_ctx* ctx, float* mx, float* my, float* mz);
-/* n iterations, asynchronous on the ctx stream. */
+/* n iterations, asynchronous on the ctx stream.  Launch structure (results do not depend on it, bit for bit):
+ * meshes of <= 8192 cells without demag run all n iterations in ONE launch of a single-CTA kernel (state in shared memory);
+ * otherwise the first iteration after a change of settings is enqueued kernel by kernel and the rest are replayed from CUDA
+ * graphs of 16 and 1 iterations (rebuilt when a setter changes a kernel argument), with programmatic dependent launch
+ * between the kernels.  Environment knobs, read when the ctx (or its demag plan) is created, for A/B measurements:
+ * MMC_NO_GRAPH (plain launches), MMC_NO_PDL (no programmatic dependent launch), MMC_TMA=1 (TMA-staged colour pass on meshes
+ * without periodic directions), MMC_LP=1 (layer-pair columns kernel of the demag convolution on multi-layer meshes). */
 int mmc_sweep(mmc_ctx* ctx, int n_sweeps);
 /* Same as mmc_sweep, but brackets every phase of every iteration with CUDA events on the ctx stream, synchronises, and
  * returns the summed device time per phase in milliseconds: phase_ms[8] (host) = [0] unused (pack+pad is fused into
  * the rows kernel), [1] rows kernel (S0 + x transform + z-DFT), [2] columns kernel (y transform, tensor multiply S2,
  * inverse y transform), [3] inverse rows kernel (S3, writes B_d), [4] inverse z-DFT pass (several layers only; it runs
  * between [2] and [3]), [5] red pass, [6] black
- * pass, [7] end-of-sweep bookkeeping. */
+ * pass, [7] end-of-sweep bookkeeping (on meshes of <= 2^20 cells the last CTA of the black pass
+ * does it, so [7] is ~0 there).  Launch-per-kernel with events: the kernels of mmc_sweep, not its graphs. */
 int mmc_sweep_timed(mmc_ctx* ctx, int n_sweeps, double* phase_ms);
 /* One demag convolution of the current state; bx/by/bz device float[N] (natural order) receive B_d = mu0 H_d
  * in tesla; any of them may be NULL (then the field is only computed).  Works with demag disabled too. */
 int mmc_demag_field(mmc_ctx* ctx, float* bx, float* by, float* bz);
-int mmc_get_observables(mmc_ctx* ctx, mmc_obs* host_out);      /* synchronises */
+/* Synchronises.  E_demag needs the field of the CURRENT state: a convolution is run for it only if the state has changed since
+ * the last one (mmc_demag_field, or a previous read-out); the means, counters and running averages never need one. */
+int mmc_get_observables(mmc_ctx* ctx, mmc_obs* host_out);
 int mmc_reset_counters(mmc_ctx* ctx);                          /* accepted/trials := 0; the cone controller's window is not touched */
 int mmc_reset_averages(mmc_ctx* ctx);                          /* run_mean_* := 0 */
 /* Histograms of the current state over the non-empty cells, the paper's verification read-outs (PAPER.md:108 length

@@ -12,6 +12,8 @@
 
 using namespace mmc;
 
+namespace mmc { bool g_pdl = true; }     // see mmc_internal.h, launch_pdl
+
 struct mmc_ctx {
     Geometry g{};
     double dx = 0, dy = 0, dz = 0, V = 0;
@@ -372,7 +374,10 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     c->dx = dx; c->dy = dy; c->dz = dz; c->V = dx * dy * dz;
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
     c->graphs_off = std::getenv("MMC_NO_GRAPH") != nullptr;      // A/B knob: plain launches only
-    c->tma_off = std::getenv("MMC_NO_TMA") != nullptr;           // A/B knob: the pass with per-thread loads (colour_pass2_kernel) everywhere
+    mmc::g_pdl = std::getenv("MMC_NO_PDL") == nullptr;           // A/B knob (process-wide, read at every create): no programmatic dependent launch
+    // the TMA-staged pass runs at the speed of the L1-served brick kernel on the meshes it serves (both
+    // ncu tables in profiles/): the brick kernel, which serves every mesh, is the default; MMC_TMA=1 selects the staged variant
+    { const char* e = std::getenv("MMC_TMA"); c->tma_off = !(e && e[0] == '1'); }
     c->regions.push_back(mmc_material{ 0, 0, 0, 0, 0, 1, 0, 1, 9.2740100783e-24, 0, 0, 1, 0, 0, 0, 1, 0, 0 });
     DeviceGuard dg(device);
     auto bail = [&](int code) { mmc_destroy(c); return code; };
@@ -384,7 +389,7 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
         cudaMemsetAsync(c->m[q], 0, S * sizeof(float), c->stream);
         cudaMemsetAsync(c->bd[q], 0, S * sizeof(float), c->stream);
     }
-    c->obs_blocks = 148 * 4;
+    c->obs_blocks = 148 * 12;                     // whole waves at 3 or 4 resident CTAs per SM; ~9 slots per thread on the 4 M-cell meshes
     if (cudaMalloc(&c->ctl, sizeof(Control)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->run_sums, 4 * sizeof(unsigned long long)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->obs_scratch, (size_t)c->obs_blocks * 11 * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);
@@ -577,11 +582,17 @@ static int enqueue_iteration(mmc_ctx* c, cudaStream_t st, PhaseTimer* timer, boo
     if (timer) timer->mark(PH_RED, st);
     if (c->demag_enabled && c->demag_updates == 2) { rc = compute_demag(c, timer, st, true); if (rc) return rc; }
     c->state_version++;
+    // S11: on launch-bound meshes the last CTA of the black pass does the end-of-sweep bookkeeping itself (one launch less per
+    // iteration: ~3 us of the ~22 us of BASELINE config 2); on large meshes the per-CTA fence + ticket costs more than the
+    // one-thread launch it saves (config 4, 4096 CTAs: +6 us on the pass against a 3 us launch), so the separate kernel stays
+    const bool fuse_end = (long long)c->g.nx * c->g.ny * c->g.nz <= (1ll << 20);
     SweepArgs black = make_args(c, 1);
-    black.finish = 1;                                 // S11 by the last CTA of the black pass: no separate one-thread launch
+    black.finish = fuse_end ? 1 : 0;
     rc = launch_colour_pass(black, c->features, false, st, &c->tma);
     if (rc) return fail(c, rc, "black pass launch failed");
-    if (timer) { timer->mark(PH_BLACK, st); timer->mark(PH_END, st); }
+    if (timer) timer->mark(PH_BLACK, st);
+    if (!fuse_end) { rc = launch_end_sweep(c->ctl, st); if (rc) return fail(c, rc, "end_sweep launch failed"); }
+    if (timer) timer->mark(PH_END, st);
     return MMC_OK;
 }
 

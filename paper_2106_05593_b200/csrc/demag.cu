@@ -14,9 +14,14 @@
 //                       real/imaginary parts go straight to the even/odd cells of the colour-split B_d.
 // Each kernel exists twice: the generic shared-memory variant described above (fft_smem.cuh, any length) and the
 // register-resident variant (fft_reg.cuh: 16 points per thread, compile-time lengths 2^8 .. 2^12) that the paper-sized
-// meshes use.  In the latter the rows kernels work layer by layer (several CTAs per SM instead of one holding all layers):
-// the forward z-DFT is fused into the columns kernel's load (CTA (kx, kz) sums its plane from the nz layers, which the
-// Pz CTAs of one kx read together and find in L2), the inverse z-DFT is a streaming pass of its own (z_inverse_kernel).
+// meshes use.  In the latter the rows kernels work layer by layer (several CTAs per SM instead of one holding all layers)
+// and the z direction belongs to the columns kernel, in one of two ways:
+//   layer-pair sum  (columns_lp_kernel; several layers, nz * Py/16 <= 512 threads and the shared memory fits): no z transform
+//                   at all; the nz layers' columns are transformed once each way and combined per frequency with the 2-D
+//                   tensor spectra of the nz layer offsets, in place in U;
+//   z-DFT           (columns_fast_kernel; otherwise, and the one-layer PLANAR case): CTA (kx, kz) sums plane kz of a DFT of the
+//                   shortest linear length 2 nz - 1 from the nz layers in its loader, and the inverse z-DFT is a streaming
+//                   pass of its own (z_inverse_kernel).
 // Padded lengths are powers of two >= 2n-1 (any mesh size works).  All normalisation and -mu0 are folded into the
 // tensor spectrum, which is built once at set-up in fp64 (host Newell/moment table -> device placement -> cuFFT D2Z).
 #include <cuda_runtime.h>
@@ -24,6 +29,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 
 #include "fft_reg.cuh"
 #include "fft_smem.cuh"
@@ -123,6 +129,7 @@ struct RowArgs {
 template <int PZ>
 __global__ void __launch_bounds__(512) rows_fwd_kernel(const RowArgs a)
 {
+    pdl_enter();
     extern __shared__ float2 sm[];
     const Geometry g = a.g;
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -186,6 +193,7 @@ __global__ void __launch_bounds__(512) rows_fwd_kernel(const RowArgs a)
 template <int PZ>
 __global__ void __launch_bounds__(512) rows_inv_kernel(const RowArgs a)
 {
+    pdl_enter();
     extern __shared__ float2 sm[];
     const Geometry g = a.g;
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -250,6 +258,7 @@ struct ColArgs {
 template <bool THREE_D>
 __global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
 {
+    pdl_enter();
     extern __shared__ float2 sm[];
     const int tid = threadIdx.x, nt = blockDim.x;
     const int kx = blockIdx.x, kz = blockIdx.y;
@@ -293,7 +302,7 @@ __global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
 
 // ------------------------------------------------------------------------------------------------ kernels A and C, register-resident
 // The x direction with the length-Hx transform of fft_reg.cuh (Hx = 2^LGH, 8 <= LGH <= 11), one (component, layer) per
-// CTA: the z-DFT lives in the columns kernel (cluster), so these kernels have no coupling between layers and
+// CTA: the z direction lives in the columns kernel (layer-pair sum, or z-DFT in its loader), so these kernels have no coupling between layers and
 // T[c][k][kx][j] holds nz planes per component.
 // block (RJ = 4, T = Hx/16): threadIdx.x = row of the tile (fastest, so that the four rows' values of one frequency are
 // one 32-byte sector of the transposed array), threadIdx.y = thread of the row's transform.
@@ -304,10 +313,13 @@ __global__ void __launch_bounds__(256) columns_kernel(const ColArgs a)
 #ifndef MMC_ROWS_RJ11
 #define MMC_ROWS_RJ11 4
 #endif
+#ifndef MMC_ROWS_RJ10
+#define MMC_ROWS_RJ10 4
+#endif
 template <int LGH> struct RowShape {
     using S = fftr::Shape<LGH>;
     static constexpr int Hx = S::N, T = S::T;
-    static constexpr int RJ = LGH >= 11 ? MMC_ROWS_RJ11 : 4;   // mesh rows per CTA
+    static constexpr int RJ = LGH >= 11 ? MMC_ROWS_RJ11 : (LGH == 10 ? MMC_ROWS_RJ10 : 4);   // mesh rows per CTA
     static constexpr int CP = Hx + Hx / 16;              // pad(k) + pad(Hx - k) (+1 when k & 15 != 0); = pad(Hx)
     static constexpr int ES = (S::SMEM > CP ? S::SMEM : CP) + 16 / RJ;   // row stride: RJ rows of a half-warp in different bank groups
 };
@@ -323,6 +335,7 @@ struct RowFastArgs {
 template <int LGH>
 __global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape<LGH>::RJ * RowShape<LGH>::T > 256 ? 1 : 2) rows_fwd_fast_kernel(const RowFastArgs a)
 {
+    pdl_enter();
     using R = RowShape<LGH>;
     constexpr int T = R::T, Hx = R::Hx;
     extern __shared__ float2 sm[];
@@ -387,6 +400,7 @@ __global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape
 template <int LGH>
 __global__ void __launch_bounds__(RowShape<LGH>::RJ * RowShape<LGH>::T, RowShape<LGH>::RJ * RowShape<LGH>::T > 256 ? 1 : MMC_ROWS_INV_MINB) rows_inv_fast_kernel(const RowFastArgs a)
 {
+    pdl_enter();
     using R = RowShape<LGH>;
     constexpr int T = R::T, Hx = R::Hx;
     extern __shared__ float2 sm[];
@@ -448,10 +462,10 @@ static int launch_rows_fast(const DemagPlan* p, const RowFastArgs& ra, bool inve
     const size_t smem = (size_t)R::RJ * R::ES * sizeof(float2);
     if (inverse) {
         if (smem > 48 * 1024 && cudaFuncSetAttribute(rows_inv_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
-        rows_inv_fast_kernel<LGH><<<grid, block, smem, st>>>(ra);
+        launch_pdl(rows_inv_fast_kernel<LGH>, dim3(grid), dim3(block), (size_t)(smem), st, ra);
     } else {
         if (smem > 48 * 1024 && cudaFuncSetAttribute(rows_fwd_fast_kernel<LGH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
-        rows_fwd_fast_kernel<LGH><<<grid, block, smem, st>>>(ra);
+        launch_pdl(rows_fwd_fast_kernel<LGH>, dim3(grid), dim3(block), (size_t)(smem), st, ra);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
@@ -496,6 +510,7 @@ __global__ void __launch_bounds__(fftr::Shape<LGN>::T * fftr::Shape<LGN>::G,
                                   fftr::Shape<LGN>::T >= 256 ? (PLANAR ? MMC_COLS_MINB_PLANAR_T256 : 2) : (PLANAR ? MMC_COLS_MINB_PLANAR : MMC_COLS_MINB))
 columns_fast_kernel(const ColFastArgs a)
 {
+    pdl_enter();
     using S = fftr::Shape<LGN>;
     constexpr int N = S::N, T = S::T, NL = HALF ? 8 : 16;
     extern __shared__ float2 sm[];
@@ -525,54 +540,49 @@ columns_fast_kernel(const ColFastArgs a)
 #pragma unroll
             for (int e = 0; e < 16; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
         }
-        // ONE copy of each transform in the instruction stream (the straight-line version of this kernel is ~75 KB of code
-        // and starves the instruction cache): pass p = 0 is the in-plane pair, p = 1 the z component; the transforms always
-        // work on v[0] and the two register arrays swap.
-#pragma unroll 1
-        for (int p = 0; p < 2; ++p) {
-            const int nc = p ? 1 : 2;
-#pragma unroll 1
-            for (int c = 0; c < nc; ++c) {
-                fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
 #pragma unroll
-                for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = t0; }
+        for (int c = 0; c < 2; ++c) fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) {
+            const float2 u = v[0][e], w1 = v[1][e];
+            const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T), xy = __ldg(a.nhat[3] + nb + e * T);
+            v[0][e].x = fmaf(xx, u.x, xy * w1.x); v[0][e].y = fmaf(xx, u.y, xy * w1.y);
+            v[1][e].x = fmaf(xy, u.x, yy * w1.x); v[1][e].y = fmaf(xy, u.y, yy * w1.y);
+        }
+        __syncthreads();                               // every thread is done reading exchange buffer 2
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
+            float2* __restrict__ col = a.Tout + ((size_t)c * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < NL; ++n1) {
+                const int j = tid + n1 * T;
+                if (live && (HALF || j < ny)) col[j] = v[c][n1];
             }
-            if (p == 0) {                              // two swaps: v[0] = M^_x, v[1] = M^_y
+        }
+        // z component in the registers of the first
+        {
+            float2 (&z)[16] = v[0];
+            const float2* __restrict__ cin = a.Tin + ((size_t)2 * a.Cx + kx) * ny;
 #pragma unroll
-                for (int e = 0; e < 16; ++e) {
-                    const float2 u = v[0][e], w1 = v[1][e];
-                    const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T), xy = __ldg(a.nhat[3] + nb + e * T);
-                    v[0][e].x = fmaf(xx, u.x, xy * w1.x); v[0][e].y = fmaf(xx, u.y, xy * w1.y);
-                    v[1][e].x = fmaf(xy, u.x, yy * w1.x); v[1][e].y = fmaf(xy, u.y, yy * w1.y);
-                }
-            } else {                                   // one swap: M^_z sits in v[1]; back to v[0] with its product
-#pragma unroll
-                for (int e = 0; e < 16; ++e) {
-                    const float zz = __ldg(a.nhat[2] + nb + e * T);
-                    v[0][e] = make_float2(v[1][e].x * zz, v[1][e].y * zz);
-                }
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const int j = tid + n1 * T;
+                z[n1] = (n1 < NL && (HALF || j < ny)) ? cin[j] : make_float2(0.f, 0.f);
             }
-            __syncthreads();                           // every thread is done reading exchange buffer 2
-#pragma unroll 1
-            for (int c = 0; c < nc; ++c) {
-                fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
-                float2* __restrict__ col = a.Tout + ((size_t)(p ? 2 : c) * a.Cx + kx) * ny;
+            __syncthreads();                           // the last inverse transform read exchange buffer 1
+            fftr::forward<LGN, HALF, true>(z, s1, s2, tw, tid);
 #pragma unroll
-                for (int n1 = 0; n1 < NL; ++n1) {
-                    const int j = tid + n1 * T;
-                    if (live && (HALF || j < ny)) col[j] = v[0][n1];
-                }
-#pragma unroll
-                for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = t0; }
+            for (int e = 0; e < 16; ++e) {
+                const float zz = __ldg(a.nhat[2] + nb + e * T);
+                z[e].x *= zz; z[e].y *= zz;
             }
-            if (p == 0) {                              // z component in the registers of the first
-                const float2* __restrict__ cin = a.Tin + ((size_t)2 * a.Cx + kx) * ny;
+            __syncthreads();
+            fftr::inverse<LGN, true>(z, s1, s2, tw, tid);
+            float2* __restrict__ col = a.Tout + ((size_t)2 * a.Cx + kx) * ny;
 #pragma unroll
-                for (int n1 = 0; n1 < 16; ++n1) {
-                    const int j = tid + n1 * T;
-                    v[0][n1] = (n1 < NL && (HALF || j < ny)) ? cin[j] : make_float2(0.f, 0.f);
-                }
-                __syncthreads();                       // the last inverse transform read exchange buffer 1
+            for (int n1 = 0; n1 < NL; ++n1) {
+                const int j = tid + n1 * T;
+                if (live && (HALF || j < ny)) col[j] = z[n1];
             }
         }
         return;
@@ -636,24 +646,20 @@ columns_fast_kernel(const ColFastArgs a)
             for (int e = 0; e < 16; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
         }
     }
-    // one copy of each transform in the instruction stream: the loops over the components are not unrolled, the three
-    // register arrays rotate instead (see columns_lp_kernel)
-#pragma unroll 1
+#pragma unroll
     for (int c = 0; c < 3; ++c) {
         if (HALF) {
 #pragma unroll
-            for (int n1 = 8; n1 < 16; ++n1) v[0][n1] = make_float2(0.f, 0.f);
+            for (int n1 = 8; n1 < 16; ++n1) v[c][n1] = make_float2(0.f, 0.f);
         } else if (!zf) {
             const float2* __restrict__ col = a.Tin + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
             for (int n1 = 0; n1 < 16; ++n1) {
                 const int j = tid + n1 * T;
-                v[0][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
+                v[c][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
             }
         }
-        fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
-#pragma unroll
-        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
+        fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
     }
     // S2: B^ = K^ M^ (see columns_kernel); slot e of thread tid reads the permuted spectrum at e*T + tid
     {
@@ -680,17 +686,15 @@ columns_fast_kernel(const ColFastArgs a)
         }
     }
     __syncthreads();                                   // every thread is done reading exchange buffer 2
-#pragma unroll 1
+#pragma unroll
     for (int c = 0; c < 3; ++c) {
-        fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
+        fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
         float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
         for (int n1 = 0; n1 < NL; ++n1) {
             const int j = tid + n1 * T;
-            if (live && (HALF || j < ny)) col[j] = v[0][n1];
+            if (live && (HALF || j < ny)) col[j] = v[c][n1];
         }
-#pragma unroll
-        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
     }
 }
 
@@ -713,18 +717,22 @@ struct ColLPArgs {
     const float* nh[6];
 };
 
-template <int LGN> struct LPShape { static constexpr int EC = LGN == 8 ? 2 : 4, NC = 16 / EC; };   // 2 * 3 EC T <= Shape::SMEM
+template <int LGN> struct LPShape { static constexpr int EC = 2, NC = 16 / EC; };   // slots per chunk; 2 * 3 EC T <= Shape::SMEM
 // planes of the tensor spectrum per chunk row: dz = 0 has 4 components (xz = yz = 0), every other dz has 6
 __host__ __device__ constexpr int lp_planes(int nz) { return 4 + 6 * (nz - 1); }
 __host__ __device__ constexpr int lp_plane_index(int d, int q) { return d == 0 ? q : 4 + 6 * (d - 1) + q; }
 
-// Shared memory: [transform exchange buffers of the G * nz groups | two chunks of tensor spectrum | two mbarriers].
+// Shared memory: [transform exchange buffers of the G * nz groups | the two twiddle tables | two chunks of tensor spectrum |
+// two mbarriers]: ~210 KB for four layers of Py = 2048, so there is no L1 to speak of: the twiddle tables live in shared
+// memory too (read where they are used: no 15-entry register staging), and the kernel must not spill (a CTA's spill
+// footprint would be L2 traffic).
 // The tensor spectrum of a chunk (EC consecutive slots = EC * T consecutive floats of each plane) is brought in by
 // cp.async.bulk copies that complete on an mbarrier, two chunks ahead of their use: the first two are requested before the
 // forward transforms start, chunk ch + 2 as soon as chunk ch has been consumed, so no thread ever waits for these loads.
 template <int LGN, bool HALF>
 __global__ void __launch_bounds__(512, 1) columns_lp_kernel(const ColLPArgs a)
 {
+    pdl_enter();
     using S = fftr::Shape<LGN>;
     constexpr int N = S::N, T = S::T, NL = HALF ? 8 : 16, EC = LPShape<LGN>::EC, NC = LPShape<LGN>::NC;
     extern __shared__ float2 sm[];
@@ -733,16 +741,19 @@ __global__ void __launch_bounds__(512, 1) columns_lp_kernel(const ColLPArgs a)
     float2* s1 = sm + grp * S::SMEM;
     float2* s2 = s1 + S::S1;
     const int NP = lp_planes(nz);
-    float* tens = reinterpret_cast<float*>(sm + G * nz * S::SMEM);          // [2][G][NP][EC * T]
+    float2* tws1 = sm + G * nz * S::SMEM;                                    // fft_reg.cuh twiddle tables, 15 T entries each
+    float2* tws2 = tws1 + 15 * T;
+    float* tens = reinterpret_cast<float*>(tws2 + 15 * T);                   // [2][G][NP][EC * T]
     const int tbuf = G * NP * EC * T;
     unsigned long long* bar = reinterpret_cast<unsigned long long*>(tens + 2 * tbuf);
     const int kxr = blockIdx.x * G + g;
     const bool live = kxr < a.Cx;                      // idle groups still walk through the barriers
     const int kx = live ? kxr : a.Cx - 1;
     const int ny = a.ny;
-    const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), a.tw1, a.tw2 };
+    const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), tws1, tws2 };
     const size_t plane = (size_t)a.Cx * N;             // one dz plane of a tensor component
     if (tid == 0 && grp == 0) { fftr::mbar_init(bar, G * nz); fftr::mbar_init(bar + 1, G * nz); fftr::mbar_fence_init(); }
+    for (int i = grp * T + tid; i < 15 * T; i += G * nz * T) { tws1[i] = __ldg(a.tw1 + i); tws2[i] = __ldg(a.tw2 + i); }
     __syncthreads();
     // thread 0 of group (g, k) requests plane dz = k of this kx for chunk ch: one copy of EC * T floats per component
     auto request = [&](int ch) {
@@ -776,8 +787,8 @@ __global__ void __launch_bounds__(512, 1) columns_lp_kernel(const ColLPArgs a)
     // of the warp cycles stalled on instruction fetch); the rotations cost ~15 % more instructions.
 #pragma unroll 1
     for (int c = 0; c < 3; ++c) {
-        if constexpr (GROUPS) fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid, gsync);
-        else fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
+        if constexpr (GROUPS) fftr::forward<LGN, HALF, 2>(v[0], s1, s2, tw, tid, gsync);
+        else fftr::forward<LGN, HALF, 2>(v[0], s1, s2, tw, tid);
 #pragma unroll
         for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
     }
@@ -849,8 +860,8 @@ __global__ void __launch_bounds__(512, 1) columns_lp_kernel(const ColLPArgs a)
     }
 #pragma unroll 1
     for (int c = 0; c < 3; ++c) {
-        if constexpr (GROUPS) fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid, gsync);
-        else fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
+        if constexpr (GROUPS) fftr::inverse<LGN, 2>(v[0], s1, s2, tw, tid, gsync);
+        else fftr::inverse<LGN, 2>(v[0], s1, s2, tw, tid);
         float2* __restrict__ col = a.U + ((size_t)(c * nz + k) * a.Cx + kx) * ny;
 #pragma unroll
         for (int n1 = 0; n1 < NL; ++n1) {
@@ -869,6 +880,7 @@ constexpr int kMaxFastLayers = 16;
 template <int NZ>
 __global__ void __launch_bounds__(256) z_inverse_kernel(const float2* __restrict__ in, float2* __restrict__ out, size_t plane)
 {
+    pdl_enter();
     constexpr int PZ = 2 * NZ - 1;
     __shared__ float2 w[PZ];                               // exp(+2 pi i q / Pz)
     if (threadIdx.x < PZ) { const float2 r = fftr::root(threadIdx.x, PZ); w[threadIdx.x] = make_float2(r.x, -r.y); }
@@ -898,21 +910,21 @@ static int launch_z_inverse(const DemagPlan* p, const float2* in, float2* out, c
     const size_t plane = (size_t)p->Cx * p->g.ny;
     const int blocks = (int)std::min<size_t>((plane + 255) / 256, (size_t)148 * 16);
     switch (p->g.nz) {
-        case 2: z_inverse_kernel<2><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 3: z_inverse_kernel<3><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 4: z_inverse_kernel<4><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 5: z_inverse_kernel<5><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 6: z_inverse_kernel<6><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 7: z_inverse_kernel<7><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 8: z_inverse_kernel<8><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 9: z_inverse_kernel<9><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 10: z_inverse_kernel<10><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 11: z_inverse_kernel<11><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 12: z_inverse_kernel<12><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 13: z_inverse_kernel<13><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 14: z_inverse_kernel<14><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 15: z_inverse_kernel<15><<<blocks, 256, 0, st>>>(in, out, plane); break;
-        case 16: z_inverse_kernel<16><<<blocks, 256, 0, st>>>(in, out, plane); break;
+        case 2: launch_pdl(z_inverse_kernel<2>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 3: launch_pdl(z_inverse_kernel<3>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 4: launch_pdl(z_inverse_kernel<4>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 5: launch_pdl(z_inverse_kernel<5>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 6: launch_pdl(z_inverse_kernel<6>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 7: launch_pdl(z_inverse_kernel<7>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 8: launch_pdl(z_inverse_kernel<8>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 9: launch_pdl(z_inverse_kernel<9>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 10: launch_pdl(z_inverse_kernel<10>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 11: launch_pdl(z_inverse_kernel<11>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 12: launch_pdl(z_inverse_kernel<12>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 13: launch_pdl(z_inverse_kernel<13>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 14: launch_pdl(z_inverse_kernel<14>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 15: launch_pdl(z_inverse_kernel<15>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
+        case 16: launch_pdl(z_inverse_kernel<16>, dim3(blocks), dim3(256), (size_t)(0), st, in, out, plane); break;
         default: return MMC_E_UNSUPPORTED;
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
@@ -927,14 +939,14 @@ static int launch_columns_fast_h(const DemagPlan* p, const ColFastArgs& ca, cuda
     if (ca.nz == 0 && p->Pz == 1 && ca.nhat[4] == nullptr && ca.nhat[5] == nullptr) {      // one layer: the planar variant
         auto kp = columns_fast_kernel<LGN, HALF, true>;
         if (smem > 48 * 1024 && cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
-        kp<<<dim3(nbx, 1), dim3(S::T, S::G), smem, st>>>(ca);
+        launch_pdl(kp, dim3(nbx, 1), dim3(S::T, S::G), smem, st, ca);
         return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
     }
     auto kern = columns_fast_kernel<LGN, HALF, false>;
     if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
     const dim3 grid = ca.nz > 0 ? dim3(p->Pz, nbx) : dim3(nbx, p->Pz), block(S::T, S::G);
     if (grid.y > 65535u) return MMC_E_UNSUPPORTED;
-    kern<<<grid, block, smem, st>>>(ca);
+    launch_pdl(kern, dim3(grid), dim3(block), (size_t)(smem), st, ca);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 template <int LGN>
@@ -943,22 +955,39 @@ static int launch_columns_fast(const DemagPlan* p, const ColFastArgs& ca, cudaSt
     return 2 * p->g.ny == p->Py ? launch_columns_fast_h<LGN, true>(p, ca, st) : launch_columns_fast_h<LGN, false>(p, ca, st);
 }
 template <int LGN>
+static size_t lp_smem_bytes(int nz, int G)
+{
+    using S = fftr::Shape<LGN>;
+    return (size_t)G * nz * S::SMEM * sizeof(float2) + (size_t)2 * 15 * S::T * sizeof(float2)
+           + (size_t)2 * G * lp_planes(nz) * LPShape<LGN>::EC * S::T * sizeof(float) + 2 * sizeof(unsigned long long);
+}
+static size_t lp_smem_bytes_any(int lgN, int nz, int G)
+{
+    switch (lgN) {
+        case 8: return lp_smem_bytes<8>(nz, G);
+        case 9: return lp_smem_bytes<9>(nz, G);
+        case 10: return lp_smem_bytes<10>(nz, G);
+        case 11: return lp_smem_bytes<11>(nz, G);
+        case 12: return lp_smem_bytes<12>(nz, G);
+        default: return ~(size_t)0;
+    }
+}
+template <int LGN>
 static int launch_columns_lp(const DemagPlan* p, const ColLPArgs& la, cudaStream_t st)
 {
     using S = fftr::Shape<LGN>;
     const int G = p->lpG, nz = p->g.nz;
-    const size_t smem = (size_t)G * nz * S::SMEM * sizeof(float2)
-                        + (size_t)2 * G * lp_planes(nz) * LPShape<LGN>::EC * S::T * sizeof(float) + 2 * sizeof(unsigned long long);
+    const size_t smem = lp_smem_bytes<LGN>(nz, G);
     if (smem > 227 * 1024) return MMC_E_UNSUPPORTED;
     const dim3 grid((p->Cx + G - 1) / G), block(S::T, nz, G);
     if (2 * p->g.ny == p->Py) {
         auto kern = columns_lp_kernel<LGN, true>;
         if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
-        kern<<<grid, block, smem, st>>>(la);
+        launch_pdl(kern, dim3(grid), dim3(block), (size_t)(smem), st, la);
     } else {
         auto kern = columns_lp_kernel<LGN, false>;
         if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
-        kern<<<grid, block, smem, st>>>(la);
+        launch_pdl(kern, dim3(grid), dim3(block), (size_t)(smem), st, la);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
@@ -993,10 +1022,10 @@ static int launch_rows(const DemagPlan* p, const RowArgs& ra, bool inverse, cuda
     const dim3 grid((p->g.ny + p->RJ - 1) / p->RJ, 3);
     if (inverse) {
         if (p->smemA > 48 * 1024 && cudaFuncSetAttribute(rows_inv_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA) != cudaSuccess) return MMC_E_CUDA;
-        rows_inv_kernel<PZ><<<grid, p->threadsA, p->smemA, st>>>(ra);
+        launch_pdl(rows_inv_kernel<PZ>, dim3(grid), dim3(p->threadsA), p->smemA, st, ra);
     } else {
         if (p->smemA > 48 * 1024 && cudaFuncSetAttribute(rows_fwd_kernel<PZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)p->smemA) != cudaSuccess) return MMC_E_CUDA;
-        rows_fwd_kernel<PZ><<<grid, p->threadsA, p->smemA, st>>>(ra);
+        launch_pdl(rows_fwd_kernel<PZ>, dim3(grid), dim3(p->threadsA), p->smemA, st, ra);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
@@ -1061,14 +1090,20 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     // several layers on the register-resident path: the layer-pair columns kernel when one CTA can hold a thread group per
     // layer (nz * Py/16 <= 512 threads); else the z-DFT path (planes T, z_inverse pass)
 #ifndef MMC_DEMAG_LP
-#define MMC_DEMAG_LP 1
+#define MMC_DEMAG_LP 0
 #endif
     {
         const int Tn = p->Py / 16;
-        p->lp = MMC_DEMAG_LP && p->fastA && g.nz > 1 && Tn * g.nz <= 512;
+        // Measured on BASELINE config 4 (1024 x 1024 x 4): layer-pair 0.314 ms against 0.240 + 0.045 ms for the z-DFT columns kernel
+        // + inverse z pass: the z-DFT path is the default, the layer-pair kernel is selected with MMC_LP=1
+        const char* lp_env = std::getenv("MMC_LP");
+        const bool lp_on = lp_env ? lp_env[0] == '1' : (MMC_DEMAG_LP != 0);
+        p->lp = lp_on && p->fastA && g.nz > 1 && Tn * g.nz <= 512;
         if (p->lp) {
             const int gmax = std::max(1, std::min(Tn >= 128 ? 1 : 128 / Tn, 512 / (Tn * g.nz)));
             p->lpG = std::min(gmax, std::max(1, p->Cx / 296));          // short transforms share a CTA once the grid is two waves deep
+            while (p->lpG > 1 && lp_smem_bytes_any(ilog2(p->Py), g.nz, p->lpG) > 227 * 1024) p->lpG >>= 1;
+            if (lp_smem_bytes_any(ilog2(p->Py), g.nz, p->lpG) > 227 * 1024) p->lp = false;      // does not fit one SM: the z-DFT path
         }
     }
     const size_t nT = (size_t)3 * p->Pz * p->Cx * g.ny;
@@ -1213,8 +1248,8 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
         }
     } else {
         const dim3 gridB(p->Cx, p->Pz);
-        if (p->g.nz > 1) columns_kernel<true><<<gridB, p->threadsB, p->smemB, st>>>(ca);
-        else             columns_kernel<false><<<gridB, p->threadsB, p->smemB, st>>>(ca);
+        if (p->g.nz > 1) launch_pdl(columns_kernel<true>, dim3(gridB), dim3(p->threadsB), p->smemB, st, ca);
+        else             launch_pdl(columns_kernel<false>, dim3(gridB), dim3(p->threadsB), p->smemB, st, ca);
         if (timer) timer->mark(PH_MULTIPLY, stream);
     }
     rc = p->fastA ? launch_rows_fast_any(p, rf, true, st) : launch_rows_any(p, ra, true, st);

@@ -87,12 +87,18 @@ __global__ void twiddle_tables_kernel(float2* t1, float2* t2, int lgN)
     }
 }
 
-template <int T, bool TABLE>
+// TABLE: 0 = computed in registers, 1 = table in global memory read through L1 (__ldg), 2 = table in shared memory
+// (kernels whose shared memory leaves no L1; the short latency also lets the compiler fetch each twiddle where it is used
+// instead of holding 15 of them in registers)
+template <int T, int TABLE>
 __device__ __forceinline__ void stage_twiddles(float2 w, const float2* __restrict__ tab, int tid, float2 (&pw)[15])
 {
-    if (TABLE) {
+    if (TABLE == 1) {
 #pragma unroll
         for (int q = 0; q < 15; ++q) pw[q] = __ldg(tab + q * T + tid);
+    } else if (TABLE == 2) {
+#pragma unroll
+        for (int q = 0; q < 15; ++q) pw[q] = tab[q * T + tid];
     } else {
         powers15(w, pw);
     }
@@ -106,7 +112,7 @@ struct GroupSync {
     __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 };
 
-template <int LGN, bool HALF, bool TABLE, class Sync = BlockSync>
+template <int LGN, bool HALF, int TABLE, class Sync = BlockSync>
 __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
                                         const Twiddles& tw, int tid, const Sync& sync = Sync())
 {
@@ -130,7 +136,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
         }
     }
     float2 pw2[15];                               // requested before the barrier: the registers of v are free here
-    if constexpr (R3 > 1) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw2);
+    if constexpr (R3 > 1 && TABLE != 2) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw2);
     sync();
     const int u = tid >> 4, q1 = tid & 15;
     {
@@ -141,6 +147,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
     fft::dif<16, false>(v);
     if constexpr (R3 > 1) {
         float2* d2 = s2 + u * S::U + 17 * q1;
+        if constexpr (TABLE == 2) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw2);      // shared-memory table: fetched where it is used
         float2 (&pw)[15] = pw2;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
@@ -170,7 +177,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
 }
 
 // the mirror: v[e] = Y[freq_of_slot(tid, e)] on entry, v[n1] = N * y[tid + n1*T] on exit
-template <int LGN, bool TABLE, class Sync = BlockSync>
+template <int LGN, int TABLE, class Sync = BlockSync>
 __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
                                         const Twiddles& tw, int tid, const Sync& sync = Sync())
 {
@@ -190,8 +197,9 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
             for (int uu = 0; uu < R3; ++uu) d2[uu * S::U + i * (T + R3)] = x[uu];
         }
         float2 pw[15];
-        stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw);
+        if constexpr (TABLE != 2) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw);
         sync();
+        if constexpr (TABLE == 2) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw);
         const float2* r2 = s2 + u * S::U + 17 * q1;
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
@@ -211,8 +219,9 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
     }
     {
         float2 pw[15];
-        stage_twiddles<T, TABLE>(tw.w1, tw.t1, tid, pw);
+        if constexpr (TABLE != 2) stage_twiddles<T, TABLE>(tw.w1, tw.t1, tid, pw);
         sync();
+        if constexpr (TABLE == 2) stage_twiddles<T, TABLE>(tw.w1, tw.t1, tid, pw);
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
             float2 y = s1[q * (T + 1) + tid];

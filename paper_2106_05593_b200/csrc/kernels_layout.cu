@@ -90,9 +90,12 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
         const int k = (int)(row / (unsigned)g.ny), j = (int)(row - (unsigned)k * g.ny);
         const int sp = ((j + k) & 1) ^ (int)col;
         const unsigned oth = (1u - col) * H + row * hx + q;           // same compact index in the other colour's plane
-        const double m[3] = { a.m[0][s], a.m[1][s], a.m[2][s] };
+        // fp32 per-cell terms (differences, dot products: a few 1e-7 relative), fp64 where a bracket cancels (l2 - mu2, the
+        // anisotropy constant against its (m.e)^2 term) and for every accumulation
+        const float mf[3] = { a.m[0][s], a.m[1][s], a.m[2][s] };
+        const double m[3] = { mf[0], mf[1], mf[2] };
         const double l2 = m[0] * m[0] + m[1] * m[1] + m[2] * m[2];
-        acc[0] += m[0]; acc[1] += m[1]; acc[2] += m[2]; acc[3] += sqrt(l2); acc[10] += 1.0;
+        acc[0] += m[0]; acc[1] += m[1]; acc[2] += m[2]; acc[3] += (double)sqrtf((float)l2); acc[10] += 1.0;
         // offsets of the six neighbours relative to `oth` (only used when the bond bit is set, i.e. the neighbour exists)
         int off[6];
         off[0] = sp ? ((q + 1 < hxr) ? 1 : -q) : 0;                                       // +x
@@ -102,21 +105,23 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
         const int lay = g.ny * (int)hx;
         off[4] = (k + 1 < g.nz) ? lay : -(g.nz - 1) * lay;                                // +z
         off[5] = (k > 0) ? -lay : (g.nz - 1) * lay;                                       // -z
-        double nbv[4][3];
+        float nbv[4][3];
+        double eex = 0.0;
 #pragma unroll
         for (int d = 0; d < 6; ++d) {
             const bool need = (d & 1) == 0 || (DMI && d < 4);        // + directions for the exchange, E/W/N/S for the DMI vector
-            double v0 = 0.0, v1 = 0.0, v2 = 0.0;
+            float v0 = 0.f, v1 = 0.f, v2 = 0.f;
             if (need && ((mb >> d) & 1u)) {
                 const unsigned t = oth + (unsigned)off[d];
                 v0 = a.m[0][t]; v1 = a.m[1][t]; v2 = a.m[2][t];
                 if ((d & 1) == 0) {
-                    const double e0 = m[0] - v0, e1 = m[1] - v1, e2 = m[2] - v2;
-                    acc[4] += op.aex[d >> 1] * (e0 * e0 + e1 * e1 + e2 * e2);
+                    const float e0 = mf[0] - v0, e1 = mf[1] - v1, e2 = mf[2] - v2;
+                    eex += op.aex[d >> 1] * (double)fmaf(e0, e0, fmaf(e1, e1, e2 * e2));
                 }
             }
             if (d < 4) { nbv[d][0] = v0; nbv[d][1] = v1; nbv[d][2] = v2; }
         }
+        acc[4] += eex;
         float invT, bKq, bzee, c4, ax, ay, az, K1T, c0a; double mu2;
         if (PERCELL) {
             const float* t = reinterpret_cast<const float*>(a.table) + (size_t)kClassFloats * (a.cw[s] >> 7);
@@ -148,14 +153,15 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
                 acc[5] += kT * ((double)bK1c * (A * B + A * G + B * G) + (double)bK2c * A * B * G);
             }
         }
-        acc[6] += -kT * (double)bzee * (m[0] * a.coef.Bx + m[1] * a.coef.By + m[2] * a.coef.Bz);
+        acc[6] += -kT * (double)(bzee * fmaf(mf[0], a.coef.Bx, fmaf(mf[1], a.coef.By, mf[2] * a.coef.Bz)));
         if (DMI) {
-            const double G0 = 0.5 * (-(nbv[0][2] - nbv[1][2]) * op.inv_d[0]);
-            const double G1 = 0.5 * (-(nbv[2][2] - nbv[3][2]) * op.inv_d[1]);
-            const double G2 = 0.5 * ((nbv[0][0] - nbv[1][0]) * op.inv_d[0] + (nbv[2][1] - nbv[3][1]) * op.inv_d[1]);
-            acc[7] += -op.D0V * (m[0] * G0 + m[1] * G1 + m[2] * G2);
+            const float ix = (float)op.inv_d[0], iy = (float)op.inv_d[1];
+            const float G0 = 0.5f * (-(nbv[0][2] - nbv[1][2]) * ix);
+            const float G1 = 0.5f * (-(nbv[2][2] - nbv[3][2]) * iy);
+            const float G2 = 0.5f * ((nbv[0][0] - nbv[1][0]) * ix + (nbv[2][1] - nbv[3][1]) * iy);
+            acc[7] += -op.D0V * (double)fmaf(mf[0], G0, fmaf(mf[1], G1, mf[2] * G2));
         }
-        if (a.bd[0]) acc[8] += -0.5 * kT * (double)bzee * (m[0] * a.bd[0][s] + m[1] * a.bd[1][s] + m[2] * a.bd[2][s]);
+        if (a.bd[0]) acc[8] += -0.5 * kT * (double)(bzee * fmaf(mf[0], a.bd[0][s], fmaf(mf[1], a.bd[1][s], mf[2] * a.bd[2][s])));
         const double dv = l2 - mu2;
         acc[9] += kT * ((double)c4 * dv * dv + (double)c0a);
     }
@@ -174,12 +180,15 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
     }
 }
 
+// warp w sums quantity w over the blocks: lane l takes blocks l, l + 32, ... in order, then a fixed shuffle tree: deterministic
 __global__ void observables_final_kernel(const double* __restrict__ scratch, int blocks, Observables* out)
 {
-    const int t = threadIdx.x;
+    const int t = threadIdx.x >> 5, lane = threadIdx.x & 31;
     if (t >= 11) return;
     double v = 0.0;
-    for (int b = 0; b < blocks; ++b) v += scratch[11ll * b + t];      // fixed order: deterministic
+    for (int b = lane; b < blocks; b += 32) v += scratch[11ll * b + t];
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    if (lane) return;
     if (t < 4) out->sum[t] = v;
     else if (t < 10) out->E[t - 4] = v;
     else out->n_active = (unsigned long long)(v + 0.5);
@@ -241,7 +250,7 @@ int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, Ob
                    else     observables_kernel<true, false><<<scratch_blocks, 256, 0, st>>>(a, op, scratch); }
     else         { if (dmi) observables_kernel<false, true><<<scratch_blocks, 256, 0, st>>>(a, op, scratch);
                    else     observables_kernel<false, false><<<scratch_blocks, 256, 0, st>>>(a, op, scratch); }
-    observables_final_kernel<<<1, 32, 0, st>>>(scratch, scratch_blocks, dev_out);
+    observables_final_kernel<<<1, 11 * 32, 0, st>>>(scratch, scratch_blocks, dev_out);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 

@@ -88,18 +88,15 @@ __device__ __forceinline__ void load_cubic(const float4* t, CellCoef& cf)
 
 struct CellResult { float dm[3]; float f, L; float terms[6]; float margin; bool accept; };
 
-// The per-cell body: trial move (O3), dF/kBT (O4), Eq. (5) in the log domain (O5).
-//   m      : current vector          S  : sum_d k_d sum_{bonded nb in d}(m_nb - m)   (beta J_d folded into k_d)
-//   selfc  : sum_d k_d n_d / 2       dzx, dzy, dxx, dyy : E-W / N-S differences of m_z, m_x, m_y for the DMI vector
-//   B      : B_ext + B_d (tesla); TERMS (debug) keeps Zeeman and demag apart for the per-term dump
-template <bool DMI, bool TERMS, bool CUBIC>
-__device__ __forceinline__ CellResult cell_update(const float m[3], const float S[3], float selfc,
-                                                  float dzx, float dzy, float dxx, float dyy,
-                                                  const float Bext[3], const float Bd[3],
-                                                  const CellCoef& cf, uint4 rnd, float omc)
+// The part of the trial move (O3) that needs nothing but the cell's own vector and its random numbers: unit vector, tangent
+// frame, rotation inside the cone.  Kept apart from the energies so that a kernel can run it for all of a thread's cells BEFORE
+// it touches anything that comes from a dependent load (class table, neighbours): ~250 instructions per cell of cover.
+struct Trial { float n0, n1, n2, dn0, dn1, dn2, L, l2, u_len, u_acc; };
+__device__ __forceinline__ Trial trial_direction(const float m[3], uint4 rnd, float omc)
 {
-    CellResult r;
-    const float u_cos = u01(rnd.x), u_phi = u01(rnd.y), u_len = u01(rnd.z), u_acc = u01(rnd.w);
+    Trial tr;
+    const float u_cos = u01(rnd.x), u_phi = u01(rnd.y);
+    tr.u_len = u01(rnd.z); tr.u_acc = u01(rnd.w);
     const float l2 = fmaf(m[0], m[0], fmaf(m[1], m[1], m[2] * m[2]));
     const float iL = rsqrt_1ulp(l2), L = l2 * iL;
     const float n0 = m[0] * iL, n1 = m[1] * iL, n2 = m[2] * iL;
@@ -123,9 +120,26 @@ __device__ __forceinline__ CellResult cell_update(const float m[3], const float 
     const float da = fmaf(sa, p2, -w * na);
     const float db = fmaf(-ca, nc, fmaf(-sa * na, nb, -w * nb));
     const float dc = fmaf(ca, nb, fmaf(-sa * na, nc, -w * nc));
-    const float dn0 = sel2 ? db : (sel1 ? dc : da);
-    const float dn1 = sel2 ? dc : (sel1 ? da : db);
-    const float dn2 = sel2 ? da : (sel1 ? db : dc);
+    tr.dn0 = sel2 ? db : (sel1 ? dc : da);
+    tr.dn1 = sel2 ? dc : (sel1 ? da : db);
+    tr.dn2 = sel2 ? da : (sel1 ? db : dc);
+    tr.n0 = n0; tr.n1 = n1; tr.n2 = n2; tr.L = L; tr.l2 = l2;
+    return tr;
+}
+
+// The rest of the per-cell body: length factor (O3), dF/kBT (O4), Eq. (5) in the log domain (O5).
+//   m      : current vector          S  : sum_d k_d sum_{bonded nb in d}(m_nb - m)   (beta J_d folded into k_d)
+//   selfc  : sum_d k_d n_d / 2       dzx, dzy, dxx, dyy : E-W / N-S differences of m_z, m_x, m_y for the DMI vector
+//   B      : B_ext + B_d (tesla); TERMS (debug) keeps Zeeman and demag apart for the per-term dump
+template <bool DMI, bool TERMS, bool CUBIC>
+__device__ __forceinline__ CellResult cell_update(const float m[3], const float S[3], float selfc,
+                                                  float dzx, float dzy, float dxx, float dyy,
+                                                  const float Bext[3], const float Bd[3],
+                                                  const CellCoef& cf, const Trial& tr)
+{
+    CellResult r;
+    const float u_len = tr.u_len, u_acc = tr.u_acc, l2 = tr.l2, L = tr.L;
+    const float n0 = tr.n0, n1 = tr.n1, n2 = tr.n2, dn0 = tr.dn0, dn1 = tr.dn1, dn2 = tr.dn2;
     const float s = cf.sigma * fmaf(2.f, u_len, -1.f);  // f = 1 + s
     const float f = 1.f + s;
     const float dm0 = L * fmaf(f, dn0, s * n0), dm1 = L * fmaf(f, dn1, s * n1), dm2 = L * fmaf(f, dn2, s * n2);
@@ -406,7 +420,8 @@ __device__ __forceinline__ void pass_one_cell(const SweepArgs& a, int col, int q
         const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
         const unsigned cell = (unsigned)row * nx + i;                     // natural cell index (< 2^31)
         const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
-        const CellResult r = cell_update<DMI, DEBUG, CUBIC>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
+        const Trial tr = trial_direction(m, rnd, omc);
+        const CellResult r = cell_update<DMI, DEBUG, CUBIC>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, tr);
         accept = r.accept;
         fs0 = m[0]; fs1 = m[1]; fs2 = m[2]; fs3 = r.L;
         if (accept) {
@@ -427,6 +442,7 @@ __device__ __forceinline__ void pass_one_cell(const SweepArgs& a, int col, int q
 template <unsigned F, bool DEBUG>
 __global__ void __launch_bounds__(kPassThreads, DEBUG ? 1 : 1024 / kPassThreads) colour_pass_kernel(const SweepArgs a)
 {
+    pdl_enter();
     constexpr bool HASZ = (F & F_Z) != 0;
     __shared__ PassTailSmem s_tail;
     pass_tail_init(s_tail);
@@ -456,6 +472,12 @@ __device__ __forceinline__ void update_pair(const SweepArgs& a, int s, int row, 
                    DMI = (F & F_DMI) != 0, CUBIC = (F & F_CUBIC) != 0;
     const int nx = a.g.nx, ny = a.g.ny;
     const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
+    // Philox and the direction part of both trial moves first: they need only the cells' own vectors, so ~500 instructions run
+    // before anything that depends on the class table or on the neighbours is touched (their loads are in flight meanwhile)
+    const unsigned cell0 = (unsigned)row * nx + (unsigned)i0;                    // natural cell index (< 2^31); the second cell is cell0 + 2
+    const float ma[3] = { m2[0].x, m2[1].x, m2[2].x }, mb2[3] = { m2[0].y, m2[1].y, m2[2].y };
+    const Trial trial0 = trial_direction(ma, philox4x32_10(make_uint4(cell0, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi), omc);
+    const Trial trial1 = trial_direction(mb2, philox4x32_10(make_uint4(cell0 + 2u, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi), omc);
 #pragma unroll
     for (int t = 0; t < 2; ++t) {
         if (!act[t]) continue;
@@ -515,9 +537,7 @@ __device__ __forceinline__ void update_pair(const SweepArgs& a, int s, int row, 
             dxx = bE * e[0] - bW * wv[0];
             dyy = bN * N[1] - bS * S_[1];
         }
-        const unsigned cell = (unsigned)row * nx + (unsigned)(i0 + 2 * t);       // natural cell index (< 2^31)
-        const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
-        const CellResult r = cell_update<DMI, false, CUBIC>(m, Sg, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, rnd, omc);
+        const CellResult r = cell_update<DMI, false, CUBIC>(m, Sg, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, t ? trial1 : trial0);
         float f0 = m[0], f1 = m[1], f2 = m[2], f3 = r.L;
         if (r.accept) {
             f0 += r.dm[0]; f1 += r.dm[1]; f2 += r.dm[2]; f3 *= r.f;
@@ -542,6 +562,7 @@ constexpr int kPass2Threads = 256;
 template <unsigned F>
 __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_kernel(const SweepArgs a)
 {
+    pdl_enter();
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
     __shared__ PassTailSmem s_tail;
@@ -619,7 +640,7 @@ __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_ke
 // and release the stage.  Out-of-mesh elements arrive as zeros (their bonds are masked).  TMA does not wrap, so this
 // kernel serves meshes without periodic directions (BASELINE configs 2, 4, 5); everything else takes colour_pass2_kernel.
 // north_star (a) asks for this variant to be measured against plain L1-served loads: profiles/ has both.
-constexpr int kTmaConsumerWarps = 8, kTmaThreads = (kTmaConsumerWarps + 1) * 32, kTmaStages = 2;
+constexpr int kTmaConsumerWarps = 8, kTmaThreads = (kTmaConsumerWarps + 1) * 32, kTmaStages = 2;    // two CTAs per SM
 constexpr int kTmaX = 64, kTmaXO = 72;                 // compact cells per tile row; floats of the other colour's x window
 
 __device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -654,6 +675,7 @@ template <unsigned F>
 __global__ void __launch_bounds__(kTmaThreads, 2) colour_pass_tma_kernel(const SweepArgs a, const PassTmaShape sh,
                                                                        const __grid_constant__ PassTmaMaps maps)
 {
+    pdl_enter();
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0;
     extern __shared__ __align__(128) unsigned char tsm[];
@@ -674,16 +696,17 @@ __global__ void __launch_bounds__(kTmaThreads, 2) colour_pass_tma_kernel(const S
     }
     __syncthreads();
     if (warp == kTmaConsumerWarps) {
-        // ---- producer: one lane requests the boxes of every tile of this CTA
-        if (lane == 0) {
-            int it = 0;
-            for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
-                const int st = it % kTmaStages, ph = (it / kTmaStages) & 1;
+        // ---- producer warp: lane 0 requests the boxes of every tile of this CTA.  (Measured and dropped: the whole warp pulling
+        // the landed tile's coefficient-table lines into L1 with prefetch.global.L1: no effect on the consumers' gather stalls.)
+        int it = 0;
+        for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
+            const int st = it % kTmaStages, ph = (it / kTmaStages) & 1;
+            unsigned char* base = tsm + (size_t)st * stage_bytes;
+            unsigned long long* full = &s_bar[st];
+            if (lane == 0) {
                 mbar_wait(&s_bar[kTmaStages + st], (unsigned)(ph ^ 1));              // the consumers have released this stage
                 const int tx = t % sh.tiles_x, r = t / sh.tiles_x, ty = r % sh.tiles_y, tz = r / sh.tiles_y;
                 const int q0 = tx * kTmaX, j0 = ty * BY, k0 = tz * BZ;
-                unsigned char* base = tsm + (size_t)st * stage_bytes;
-                unsigned long long* full = &s_bar[st];
                 unsigned bytes = (unsigned)(3 * own_arr + 3 * sh.oth_box_bytes);
                 if (DEMAG) bytes += 3u * own_arr;
                 if (PERCELL) bytes += (unsigned)own_arr;
@@ -705,6 +728,9 @@ __global__ void __launch_bounds__(kTmaThreads, 2) colour_pass_tma_kernel(const S
         const bool want_sums = a.run_sums != nullptr;
         long long tot[6] = { 0, 0, 0, 0, 0, 0 };                   // lane 0: accepted, trials, fixed-point sums of this warp
         const int ql = 2 * lane;                                   // compact index of the lane's first cell inside the tile row
+        // (Measured and dropped, per-cell classes: fetching the NEXT row's class-table words while the current row is computed
+        // needs ~24 more registers per thread; at two CTAs of 288 threads per SM that spills 264 bytes per thread into an L1 that
+        // the stages have left 30 KB of, and one CTA of 17 warps is capped at 96 registers by the allocation granularity.)
         int it = 0;
         for (int t = blockIdx.x; t < ntiles; t += gridDim.x, ++it) {
             const int st = it % kTmaStages, ph = (it / kTmaStages) & 1;
@@ -789,7 +815,7 @@ __global__ void __launch_bounds__(kTmaThreads, 2) colour_pass_tma_kernel(const S
     }
 }
 
-__global__ void end_sweep_kernel(Control* ctl) { end_sweep(ctl); }
+__global__ void end_sweep_kernel(Control* ctl) { pdl_enter(); end_sweep(ctl); }
 
 // ------------------------------------------------------------------------------------------------ small meshes: all iterations in one launch
 // Meshes of a few thousand cells without demag (BASELINE.json config 1: 1024 cells) are bound by launch latency: three
@@ -809,10 +835,8 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(con
     extern __shared__ float s_m[];                    // [3][2 H]
     __shared__ Control s_ctl;
     __shared__ unsigned long long s_run[4];
-    __shared__ unsigned s_cnt;                        // accepted | trials << 16 would overflow: two words
-    __shared__ unsigned s_tri;
-    __shared__ long long s_sum[4];
-    const int tid = threadIdx.x;
+    __shared__ int s_w[2][kSmallThreads / 32][6];     // per pass parity, per warp: accepted, trials, four fixed-point sums
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     SweepArgs a = a_in;
     const int hxr = (a.g.nx + 1) >> 1, rows = a.g.ny * a.g.nz, slots = hxr * rows;
     const int S2 = (int)(2 * a.g.H);
@@ -824,16 +848,32 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(con
     if (tid == 0) s_ctl = *a_in.ctl;
     if (tid < 4) s_run[tid] = a_in.run_sums ? a_in.run_sums[tid] : 0ull;
     a.ctl = &s_ctl;
+    // Per pass: every warp leaves its counts and fixed-point sums in s_w (plain stores, a warp's <= 128 cells of |m| < 2 stay
+    // inside int32), one block barrier makes the pass and these visible, and warp 0 adds them up (two 16-bit halves per value
+    // through the 32-bit warp reduction) and keeps the books while the other warps are already in the next pass.  Three block
+    // barriers per iteration; no atomics.
+    auto bookkeeping = [&](int par, bool last) {
+        // warp 0 only
+        long long tot[6];
+#pragma unroll
+        for (int q = 0; q < 6; ++q) {
+            const int v = s_w[par][lane][q];
+            const int lo = __reduce_add_sync(0xffffffffu, v & 0xffff), hi = __reduce_add_sync(0xffffffffu, v >> 16);   // arithmetic shift: signed values
+            tot[q] = (long long)hi * 65536ll + (long long)lo;
+        }
+        if (lane == 0) {
+            s_ctl.win_accepted += (unsigned long long)tot[0]; s_ctl.win_trials += (unsigned long long)tot[1];
+            if (a_in.run_sums) for (int t = 0; t < 4; ++t) s_run[t] += (unsigned long long)tot[2 + t];
+            if (last) end_sweep(&s_ctl);
+        }
+    };
     __syncthreads();
     for (int it = 0; it < n_sweeps; ++it) {
         const unsigned long long sweep = s_ctl.sweep;
         const float omc = s_ctl.one_minus_cos_cone;
         for (int col = 0; col < 2; ++col) {
-            __syncthreads();                          // s_ctl read by everyone; previous totals consumed
-            if (tid == 0) { s_cnt = 0u; s_tri = 0u; s_sum[0] = s_sum[1] = s_sum[2] = s_sum[3] = 0; }
-            __syncthreads();
             unsigned n_acc = 0u, n_tri = 0u;
-            int i0 = 0, i1 = 0, i2 = 0, i3 = 0;       // fixed point per thread: <= 32 cells of |m| < 2 stay inside int32
+            int i0 = 0, i1 = 0, i2 = 0, i3 = 0;       // fixed point per thread: <= 8 cells of |m| < 2
             for (int idx = tid; idx < slots; idx += kSmallThreads) {
                 const int q = idx % hxr, row = idx / hxr, j = row % a.g.ny, k = row / a.g.ny;
                 bool active, accept;
@@ -843,22 +883,12 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(con
                 i0 += __float2int_rn(f0 * kSumScale); i1 += __float2int_rn(f1 * kSumScale);
                 i2 += __float2int_rn(f2 * kSumScale); i3 += __float2int_rn(f3 * kSumScale);
             }
-            const unsigned wa = __reduce_add_sync(0xffffffffu, n_acc), wt = __reduce_add_sync(0xffffffffu, n_tri);
-            const long long w0 = (long long)__reduce_add_sync(0xffffffffu, i0), w1 = (long long)__reduce_add_sync(0xffffffffu, i1),
-                            w2 = (long long)__reduce_add_sync(0xffffffffu, i2), w3 = (long long)__reduce_add_sync(0xffffffffu, i3);
-            if ((tid & 31) == 0) {
-                atomicAdd(&s_cnt, wa); atomicAdd(&s_tri, wt);
-                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[0]), (unsigned long long)w0);
-                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[1]), (unsigned long long)w1);
-                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[2]), (unsigned long long)w2);
-                atomicAdd(reinterpret_cast<unsigned long long*>(&s_sum[3]), (unsigned long long)w3);
-            }
-            __syncthreads();                          // the pass is complete and visible to the whole CTA
-            if (tid == 0) {
-                s_ctl.win_accepted += s_cnt; s_ctl.win_trials += s_tri;
-                if (a_in.run_sums) for (int t = 0; t < 4; ++t) s_run[t] += (unsigned long long)s_sum[t];
-                if (col == 1) end_sweep(&s_ctl);
-            }
+            const int wa = (int)__reduce_add_sync(0xffffffffu, n_acc), wt = (int)__reduce_add_sync(0xffffffffu, n_tri);
+            const int w0 = __reduce_add_sync(0xffffffffu, i0), w1 = __reduce_add_sync(0xffffffffu, i1),
+                      w2 = __reduce_add_sync(0xffffffffu, i2), w3 = __reduce_add_sync(0xffffffffu, i3);
+            if (lane == 0) { int* w = s_w[col][warp]; w[0] = wa; w[1] = wt; w[2] = w0; w[3] = w1; w[4] = w2; w[5] = w3; }
+            __syncthreads();                          // the pass and its partial sums are visible to the whole CTA
+            if (warp == 0) bookkeeping(col, col == 1);
         }
         __syncthreads();                              // the new sweep counter and cone are visible
     }
@@ -871,7 +901,7 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(con
 
 int launch_end_sweep(Control* ctl, void* stream)
 {
-    end_sweep_kernel<<<1, 1, 0, (cudaStream_t)stream>>>(ctl);
+    launch_pdl(end_sweep_kernel, dim3(1), dim3(1), (size_t)(0), (cudaStream_t)stream, ctl);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 
@@ -895,13 +925,13 @@ static int launch_variant(const SweepArgs& a, bool debug, cudaStream_t st)
 #define MMC_PASS_CELLS 2
 #endif
     const bool pairable = MMC_PASS_CELLS == 2 && !((a.g.pbc & 1u) && (hxr & 1));        // see colour_pass2_kernel
-    if (debug) colour_pass_kernel<F, true><<<gr, b, 0, st>>>(a);
-    else if (!pairable) colour_pass_kernel<F, false><<<gr, b, 0, st>>>(a);
+    if (debug) launch_pdl(colour_pass_kernel<F, true>, dim3(gr), dim3(b), (size_t)(0), st, a);
+    else if (!pairable) launch_pdl(colour_pass_kernel<F, false>, dim3(gr), dim3(b), (size_t)(0), st, a);
     else {
         const int bz = a.g.nz >= 4 ? 4 : (a.g.nz >= 2 ? 2 : 1), by = kPass2Threads / 32 / bz;
         const dim3 b2(32, by, bz), g2((hxr + 63) / 64, (a.g.ny + by - 1) / by, (a.g.nz + bz - 1) / bz);
         if (g2.y > 65535u || g2.z > 65535u) return MMC_E_UNSUPPORTED;
-        colour_pass2_kernel<F><<<g2, b2, 0, st>>>(a);
+        launch_pdl(colour_pass2_kernel<F>, dim3(g2), dim3(b2), (size_t)(0), st, a);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
@@ -992,7 +1022,7 @@ static int launch_tma_variant(const SweepArgs& a, const PassTma& t, cudaStream_t
     const int ntiles = t.sh.tiles_x * t.sh.tiles_y * t.sh.tiles_z;
     if (ntiles < 2 * 148) return MMC_E_UNSUPPORTED;               // too few tiles to give every SM its two CTAs: the brick kernel spreads better
     const int grid = 2 * 148;
-    kern<<<grid, kTmaThreads, smem, st>>>(a, t.sh, t.maps);
+    launch_pdl(kern, dim3(grid), dim3(kTmaThreads), smem, st, a, t.sh, t.maps);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 // the feature sets of the open-boundary BASELINE configs; anything else is served by colour_pass2_kernel

@@ -298,8 +298,9 @@ def test_two_demag_updates_per_iteration(name, exchange):
                                      ((1024, 10, 1), (5e-9, 5e-9, 10e-9)), ((700, 9, 4), (3e-9, 3e-9, 3e-9)),
                                      ((520, 6, 5), (3e-9, 3e-9, 3e-9)), ((2048, 7, 1), (5e-9, 5e-9, 10e-9)),
                                      ((1500, 5, 2), (3e-9, 3e-9, 3e-9)),
-                                     # register-resident rows AND columns kernels, z-DFT over a thread-block cluster of the
-                                     # columns kernel (2, 3, 4 layers: clusters of 4, 8, 8 CTAs; ragged chunks) or none (1 layer)
+                                     # register-resident rows AND columns kernels: one layer (planar columns kernel), 2 - 4 layers
+                                     # (layer-pair columns kernel, no z transform), 10 and 16 layers (z-DFT of length 2 nz - 1
+                                     # in the columns kernel's loader + the inverse z pass); ragged chunks
                                      ((256, 256, 1), (5e-9, 5e-9, 5e-9)), ((512, 128, 4), (3e-9, 3e-9, 3e-9)),
                                      ((200, 70, 1), (5e-9, 5e-9, 5e-9)), ((256, 66, 4), (3e-9, 3e-9, 3e-9)),
                                      ((301, 67, 3), (2e-9, 3e-9, 4e-9)), ((512, 72, 2), (3e-9, 3e-9, 3e-9)),
@@ -327,6 +328,73 @@ def test_demag_field_parity(shape, d):
     for a in range(3):
         assert np.abs(bg[a] - bo[a]).max() <= 2e-5 * scale
     g.close()
+
+
+class _env:
+    """Set an environment variable for the duration of a block (the library reads its A/B knobs when a context / plan is created)."""
+    def __init__(self, key, val): self.key, self.val = key, val
+    def __enter__(self):
+        import os
+        self.old = os.environ.get(self.key); os.environ[self.key] = self.val
+    def __exit__(self, *a):
+        import os
+        if self.old is None: os.environ.pop(self.key, None)
+        else: os.environ[self.key] = self.old
+
+
+@pytest.mark.parametrize("shape,d", [((64, 256, 2), (3e-9, 3e-9, 3e-9)), ((48, 1024, 2), (3e-9, 3e-9, 3e-9)), ((130, 300, 3), (3e-9, 3e-9, 3e-9)),
+                                     ((512, 128, 4), (3e-9, 3e-9, 3e-9)), ((256, 66, 4), (3e-9, 3e-9, 3e-9)), ((301, 67, 3), (2e-9, 3e-9, 4e-9)),
+                                     ((700, 69, 4), (3e-9, 3e-9, 3e-9)), ((200, 2048, 2), (3e-9, 3e-9, 3e-9))])
+def test_layer_pair_columns_kernel_parity(shape, d):
+    """The layer-pair variant of the columns kernel (MMC_LP=1: no z transform, layers combined per frequency with the 2-D tensor
+    spectra of the layer offsets; Eq. (14) written out in z) against the oracle's fp64 convolution: same bar as the default path."""
+    import paper_2106_05593_b200 as P
+    nx, ny, nz = shape; N = nx * ny * nz
+    rng = np.random.default_rng(N + 7)
+    v = rng.normal(size=(3, N)); v /= np.linalg.norm(v, axis=0)
+    m0 = (v * rng.uniform(0.3, 1.0, N)).astype(np.float32)
+    reg = (rng.uniform(size=N) > 0.2).astype(np.int32)
+    m0[:, reg == 0] = 0
+    with _env("MMC_LP", "1"):
+        g = P.MMC(nx, ny, nz, *d, 0)
+        g.set_material([P.Material(), P.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)], reg)
+        g.set_temperature(300.0); g.set_m(*m0)
+        bg = _np(g.demag_field())
+        again = _np(g.demag_field())
+    conv = O.DemagFFT(nx, ny, nz, *d)
+    M = [(8.6e5 * reg * m0[a].astype(np.float64)).reshape(nz, ny, nx) for a in range(3)]
+    bo = [b.ravel() for b in conv.field(*M)]
+    scale = max(np.abs(b).max() for b in bo)
+    for a in range(3):
+        assert np.abs(bg[a] - bo[a]).max() <= 2e-5 * scale
+        assert np.array_equal(bg[a], again[a])                       # deterministic (mbarrier / bulk-copy pipeline, shared-memory exchange)
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg2_64x48", "cfg4_48x40x4", "cfg4_30x21x3", "cfg5_160x150"])
+def test_tma_staged_pass_is_bitwise_the_default_pass(name):
+    """The TMA-staged colour pass (MMC_TMA=1: cp.async.bulk.tensor boxes into a ring of shared-memory stages, warp-specialised)
+    against the default pass (per-thread loads through L1): same cell arithmetic (update_pair), same integer reductions, so
+    states, counters and running sums must agree bit for bit.  Meshes here are stretched in x and y so that the staged variant has
+    the 296 tiles it asks for (smaller meshes fall back to the default kernel, which the test would then compare with itself)."""
+    import paper_2106_05593_b200 as P
+    base = CASES[name]()
+    big = {"cfg2": lambda: W.cfg2(nx=1300, ny=500), "cfg4": lambda: W.cfg4(nx=1290, ny=190, nz=base.nz), "cfg5": lambda: W.cfg5(nx=1300, ny=500)}[name[:4]]
+    out = []
+    for tma in ("1", "0"):
+        wl = big(); wl.adaptive_cone = False
+        if name.startswith("cfg5"):
+            wl.region_of_cell = np.ones(wl.N, np.int32); wl.m0 = np.tile(np.array([[0.5], [0.5], [0.2]], np.float32), (1, wl.N))   # mostly magnetic: staged
+        with _env("MMC_TMA", tma):
+            g = _gpu(wl)
+            g.sweep(3)
+            out.append(([x.clone() for x in g.get_m()], g.observables()))
+            g.close()
+    (ma, oa), (mb, ob) = out
+    assert all(bool((ma[q] == mb[q]).all()) for q in range(3))
+    for k in ("accepted", "trials", "run_mean_len", "E_ex", "E_demag"):
+        assert oa[k] == ob[k], k
+    assert np.array_equal(oa["run_mean_m"], ob["run_mean_m"]) and oa["trials"] == 3 * wl.n_active
 
 
 @pytest.mark.parametrize("name", ["cfg1_32x32", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg3_48x40_800K", "cfg4_30x21x3", "cfg5_160x150",
@@ -516,6 +584,35 @@ def test_demag_and_sweep_are_bitwise_reproducible(shape):
         assert og[k] == oh[k], k
     assert np.array_equal(og["run_mean_m"], oh["run_mean_m"])
     g.close(); h.close()
+
+
+@pytest.mark.parametrize("name", ["cfg2_64x48", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150"])
+def test_launch_paths_agree_bitwise(name):
+    """mmc_sweep(n) replays whole iterations from CUDA graphs (16 at a time, then one at a time) whose kernels are chained by
+    programmatic dependent launch, and on small meshes the last CTA of the black pass closes the iteration.  Plain stream
+    launches (MMC_NO_GRAPH), launches without programmatic dependencies (MMC_NO_PDL) and the event-bracketed launches of
+    mmc_sweep_timed must give the same bits: states, counters, cone, running sums after 137 iterations with the adaptive cone
+    (one controller window and a partial one; 8 x 16 + 9 iterations; a second call re-uses the cached graphs)."""
+    ref = None
+    for knob in (None, "MMC_NO_GRAPH", "MMC_NO_PDL", "timed"):
+        wl = CASES[name](); wl.adaptive_cone = True
+        import contextlib
+        with (_env(knob, "1") if knob and knob != "timed" else contextlib.nullcontext()):
+            g = _gpu(wl)
+            if knob == "timed":
+                g.sweep_timed(100); g.sweep_timed(37)
+            else:
+                g.sweep(100); g.sweep(37)
+            m = [x.clone() for x in g.get_m()]; ob = g.observables()
+            g.close()
+        if ref is None:
+            ref = (m, ob)
+            continue
+        assert all(bool((m[q] == ref[0][q]).all()) for q in range(3)), knob
+        for k in ("accepted", "trials", "sweeps_done", "cone_deg", "run_sweeps", "run_mean_len", "E_ex", "E_demag"):
+            assert ob[k] == ref[1][k], (knob, k)
+        assert np.array_equal(ob["run_mean_m"], ref[1]["run_mean_m"]), knob
+    assert ref[1]["sweeps_done"] == 137
 
 
 @pytest.mark.parametrize("name", ["cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150"])
