@@ -55,11 +55,11 @@ def _pow2_at_least(n, start):
 
 def demag_layout(wl):
     """Which demag path libmmc_b200 takes for this mesh (mirrors demag_create): register-resident rows/columns kernels for
-    padded lengths 2^8..2^12; with several layers the layer-pair columns kernel (no z transform) when nz * Py/16 <= 512
-    threads, else a z-DFT of the shortest linear length 2 nz - 1 with a separate inverse z pass."""
+    padded lengths 2^8..2^12; with several layers a z-DFT of the shortest linear length 2 nz - 1 (fused into the columns kernel's
+    loader) with a separate inverse z pass, or, with MMC_LP=1 and nz * Py/16 <= 512 threads, the layer-pair columns kernel."""
     Px, Py = _pow2_at_least(wl.nx, 2), _pow2_at_least(wl.ny, 1)
     fast = 8 <= (Px // 2).bit_length() - 1 <= 11 and 8 <= Py.bit_length() - 1 <= 12 and wl.nz <= 16
-    lp = fast and wl.nz > 1 and (Py // 16) * wl.nz <= 512
+    lp = fast and wl.nz > 1 and (Py // 16) * wl.nz <= 512 and os.environ.get("MMC_LP", "0")[:1] == "1"   # an option; the z-DFT path is the default
     Pz = 1 if wl.nz == 1 else (2 * wl.nz - 1 if fast else _pow2_at_least(wl.nz, 1))
     return Px, Py, Pz, fast, lp
 

@@ -116,9 +116,9 @@ int mmc_get_m_host(mmc_ctx* ctx, float* mx, float* my, float* mz);
 /* n iterations, asynchronous on the ctx stream.  Launch structure (results do not depend on it, bit for bit):
  * meshes of <= 8192 cells without demag run all n iterations in ONE launch of a single-CTA kernel (state in shared memory);
  * otherwise the first iteration after a change of settings is enqueued kernel by kernel and the rest are replayed from CUDA
- * graphs of 16 and 1 iterations (rebuilt when a setter changes a kernel argument), with programmatic dependent launch
- * between the kernels.  Environment knobs, read when the ctx (or its demag plan) is created, for A/B measurements:
- * MMC_NO_GRAPH (plain launches), MMC_NO_PDL (no programmatic dependent launch), MMC_TMA=1 (TMA-staged colour pass on meshes
+ * graphs of 16 and 1 iterations (rebuilt when a setter changes a kernel argument).  Environment knobs, read when the ctx (or
+ * its demag plan) is created, for A/B measurements: MMC_NO_GRAPH (plain launches), MMC_PDL=1 (programmatic dependent launch
+ * between the kernels of an iteration: measured slower, off by default), MMC_TMA=1 (TMA-staged colour pass on meshes
  * without periodic directions), MMC_LP=1 (layer-pair columns kernel of the demag convolution on multi-layer meshes). */
 int mmc_sweep(mmc_ctx* ctx, int n_sweeps);
 /* Same as mmc_sweep, but brackets every phase of every iteration with CUDA events on the ctx stream, synchronises, and

@@ -12,7 +12,7 @@
 
 using namespace mmc;
 
-namespace mmc { bool g_pdl = true; }     // see mmc_internal.h, launch_pdl
+namespace mmc { bool g_pdl = false; }     // see mmc_internal.h, launch_pdl
 
 struct mmc_ctx {
     Geometry g{};
@@ -374,7 +374,10 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     c->dx = dx; c->dy = dy; c->dz = dz; c->V = dx * dy * dz;
     c->device = device; c->stream = (cudaStream_t)cuda_stream;
     c->graphs_off = std::getenv("MMC_NO_GRAPH") != nullptr;      // A/B knob: plain launches only
-    mmc::g_pdl = std::getenv("MMC_NO_PDL") == nullptr;           // A/B knob (process-wide, read at every create): no programmatic dependent launch
+    // programmatic dependent launch between the kernels of an iteration: measured slower on every config (early-resident CTAs of
+    // the next kernel take slots from the running one: cfg 2 26.5 against 23.2 us, cfg 4 0.584 against 0.497 ms), so it is off
+    // unless MMC_PDL=1 (process-wide knob, read at every create)
+    { const char* e = std::getenv("MMC_PDL"); mmc::g_pdl = e && e[0] == '1'; }
     // the TMA-staged pass runs at the speed of the L1-served brick kernel on the meshes it serves (both
     // ncu tables in profiles/): the brick kernel, which serves every mesh, is the default; MMC_TMA=1 selects the staged variant
     { const char* e = std::getenv("MMC_TMA"); c->tma_off = !(e && e[0] == '1'); }

@@ -612,21 +612,55 @@ columns_fast_kernel(const ColFastArgs a)
         }
         const float2 wz = fftr::root(kz, a.Pz);
         float2 wk = wz;
-        for (int k = 1; k < a.nz; ++k) {
+#ifndef MMC_COLS_ZPIPE
+#define MMC_COLS_ZPIPE 1
+#endif
+        if constexpr (HALF && MMC_COLS_ZPIPE) {
+            // the upper halves of the register arrays are free until the transforms start (they hold the implied zero padding):
+            // they carry the NEXT layer's values, requested right after the previous layer's values of the same component have
+            // been consumed, i.e. two components' worth of arithmetic ahead of their use
+            if (a.nz > 1) {
 #pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + k) * a.Cx + kx) * ny;
+                for (int c = 0; c < 3; ++c) {
+                    const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + 1) * a.Cx + kx) * ny;
 #pragma unroll
-                for (int n1 = 0; n1 < NL; ++n1) {
-                    const int j = tid + n1 * T;
-                    if (HALF || j < ny) {
-                        const float2 x = col[j];
+                    for (int n1 = 0; n1 < 8; ++n1) v[c][8 + n1] = col[tid + n1 * T];
+                }
+            }
+            for (int k = 1; k < a.nz; ++k) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                    for (int n1 = 0; n1 < 8; ++n1) {
+                        const float2 x = v[c][8 + n1];
                         v[c][n1].x = fmaf(wk.x, x.x, fmaf(-wk.y, x.y, v[c][n1].x));
                         v[c][n1].y = fmaf(wk.x, x.y, fmaf(wk.y, x.x, v[c][n1].y));
                     }
+                    if (k + 1 < a.nz) {
+                        const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + k + 1) * a.Cx + kx) * ny;
+#pragma unroll
+                        for (int n1 = 0; n1 < 8; ++n1) v[c][8 + n1] = col[tid + n1 * T];
+                    }
                 }
+                wk = fft::cmul(wk, wz);
             }
-            wk = fft::cmul(wk, wz);
+        } else {
+            for (int k = 1; k < a.nz; ++k) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + k) * a.Cx + kx) * ny;
+#pragma unroll
+                    for (int n1 = 0; n1 < NL; ++n1) {
+                        const int j = tid + n1 * T;
+                        if (j < ny) {
+                            const float2 x = col[j];
+                            v[c][n1].x = fmaf(wk.x, x.x, fmaf(-wk.y, x.y, v[c][n1].x));
+                            v[c][n1].y = fmaf(wk.x, x.y, fmaf(wk.y, x.x, v[c][n1].y));
+                        }
+                    }
+                }
+                wk = fft::cmul(wk, wz);
+            }
         }
     } else if (HALF) {
 #pragma unroll
@@ -646,6 +680,31 @@ columns_fast_kernel(const ColFastArgs a)
             for (int e = 0; e < 16; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
         }
     }
+#ifndef MMC_COLS_ROLL
+#define MMC_COLS_ROLL 0
+#endif
+    // MMC_COLS_ROLL (measured and dropped, kept as a build knob): one copy of each transform in the instruction stream (the loops
+    // over the components are not unrolled, the three register arrays rotate instead), against the 14 % of the warp cycles that
+    // the 79 KB straight-line version stalls on instruction fetch: cfg 4 columns 0.265 ms rolled against 0.242 ms straight
+#if MMC_COLS_ROLL
+#pragma unroll 1
+    for (int c = 0; c < 3; ++c) {
+        if (HALF) {
+#pragma unroll
+            for (int n1 = 8; n1 < 16; ++n1) v[0][n1] = make_float2(0.f, 0.f);
+        } else if (!zf) {
+            const float2* __restrict__ col = a.Tin + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+#pragma unroll
+            for (int n1 = 0; n1 < 16; ++n1) {
+                const int j = tid + n1 * T;
+                v[0][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
+            }
+        }
+        fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
+#pragma unroll
+        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
+    }
+#else
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         if (HALF) {
@@ -661,6 +720,7 @@ columns_fast_kernel(const ColFastArgs a)
         }
         fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
     }
+#endif
     // S2: B^ = K^ M^ (see columns_kernel); slot e of thread tid reads the permuted spectrum at e*T + tid
     {
         const int kzs = (2 * kz <= a.Pz) ? kz : a.Pz - kz;
@@ -686,6 +746,20 @@ columns_fast_kernel(const ColFastArgs a)
         }
     }
     __syncthreads();                                   // every thread is done reading exchange buffer 2
+#if MMC_COLS_ROLL
+#pragma unroll 1
+    for (int c = 0; c < 3; ++c) {
+        fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
+        float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+#pragma unroll
+        for (int n1 = 0; n1 < NL; ++n1) {
+            const int j = tid + n1 * T;
+            if (live && (HALF || j < ny)) col[j] = v[0][n1];
+        }
+#pragma unroll
+        for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
+    }
+#else
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
         fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
@@ -696,6 +770,7 @@ columns_fast_kernel(const ColFastArgs a)
             if (live && (HALF || j < ny)) col[j] = v[c][n1];
         }
     }
+#endif
 }
 
 // ------------------------------------------------------------------------------------------------ kernel B, layer-pair variant

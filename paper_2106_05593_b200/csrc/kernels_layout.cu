@@ -124,11 +124,10 @@ __global__ void __launch_bounds__(256) observables_kernel(SweepArgs a, ObsParams
         acc[4] += eex;
         float invT, bKq, bzee, c4, ax, ay, az, K1T, c0a; double mu2;
         if (PERCELL) {
-            const float* t = reinterpret_cast<const float*>(a.table) + (size_t)kClassFloats * (a.cw[s] >> 7);
-            invT = t[CS_INVT]; bKq = t[CS_BKQ]; bzee = t[CS_BZEE]; c4 = t[CS_C4];
-            ax = t[CS_AX]; ay = t[CS_AY]; az = t[CS_AZ];
-            mu2 = *reinterpret_cast<const double*>(t + CS_MU2);
-            K1T = t[CS_K1T]; c0a = t[CS_C0];
+            const float4* t = a.table + (size_t)(kClassFloats / 4) * (a.cw[s] >> 7);       // three 16-byte loads (ClassSlot order)
+            const float4 t0 = __ldg(t), t1 = __ldg(t + 1), t2 = __ldg(t + 2);
+            invT = t0.x; c4 = t0.y; mu2 = __hiloint2double(__float_as_int(t0.w), __float_as_int(t0.z));
+            bKq = t1.x; bzee = t1.y; ax = t1.w; ay = t2.x; az = t2.y; K1T = t2.z; c0a = t2.w;
         } else {
             invT = 1.f / op.T_u; bKq = a.coef.bKq; bzee = a.coef.bzee; c4 = a.coef.c4;
             ax = a.coef.ax; ay = a.coef.ay; az = a.coef.az; mu2 = a.coef.mu2; K1T = op.K1T_u; c0a = op.c0_u;

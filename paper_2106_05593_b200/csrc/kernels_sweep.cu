@@ -313,9 +313,11 @@ constexpr int kPassThreads = MMC_PASS_THREADS;      // CTA = 32 x BY x BZ brick 
 template <bool COHERENT> __device__ __forceinline__ float ldc(const float* p) { return COHERENT ? *p : __ldg(p); }
 
 // One cell of the active colour: compact index q of row (j, k).  The body of the one-cell-per-thread pass.
-template <unsigned F, bool DEBUG, bool COHERENT>
+// PRE: the direction part of the trial move was computed ahead of time by cell_trial (the pipelined small-mesh kernel)
+template <unsigned F, bool DEBUG, bool COHERENT, bool PRE = false>
 __device__ __forceinline__ void pass_one_cell(const SweepArgs& a, int col, int q, int j, int k, unsigned long long sweep, float omc,
-                                              bool& active, bool& accept, float& fs0, float& fs1, float& fs2, float& fs3)
+                                              bool& active, bool& accept, float& fs0, float& fs1, float& fs2, float& fs3,
+                                              const Trial& pre = Trial())
 {
     constexpr bool MASK = (F & F_MASK) != 0, PERCELL = (F & F_PERCELL) != 0, HASZ = (F & F_Z) != 0,
                    DMI = (F & F_DMI) != 0, DEMAG = (F & F_DEMAG) != 0, DENSE = (F & F_DENSE) != 0, CUBIC = (F & F_CUBIC) != 0;
@@ -419,8 +421,9 @@ __device__ __forceinline__ void pass_one_cell(const SweepArgs& a, int col, int q
         }
         const float Bext[3] = { a.coef.Bx, a.coef.By, a.coef.Bz };
         const unsigned cell = (unsigned)row * nx + i;                     // natural cell index (< 2^31)
-        const uint4 rnd = philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi);
-        const Trial tr = trial_direction(m, rnd, omc);
+        Trial tr;
+        if (PRE) tr = pre;
+        else tr = trial_direction(m, philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi), omc);
         const CellResult r = cell_update<DMI, DEBUG, CUBIC>(m, S, selfc, dzx, dzy, dxx, dyy, Bext, Bd, cf, tr);
         accept = r.accept;
         fs0 = m[0]; fs1 = m[1]; fs2 = m[2]; fs3 = r.L;
@@ -899,6 +902,97 @@ __global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_sweeps_kernel(con
     if (tid < 4 && a_in.run_sums) a_in.run_sums[tid] = s_run[tid];
 }
 
+// Philox + direction part of the trial move of cell (q, j, k) of colour col from its CURRENT vector: everything of a cell's
+// update that does not depend on its neighbours (garbage for cells outside the mesh or empty: never used)
+__device__ __forceinline__ Trial cell_trial(const SweepArgs& a, int col, int q, int j, int k, unsigned long long sweep, float omc)
+{
+    const int s = ((j + k) & 1) ^ col, i = 2 * q + s, row = k * a.g.ny + j;
+    const unsigned ownb = (unsigned)col * (unsigned)a.g.H + (unsigned)row * a.g.hx + q;
+    const float m[3] = { a.m[0][ownb], a.m[1][ownb], a.m[2][ownb] };
+    const unsigned cell = (unsigned)row * a.g.nx + i;
+    return trial_direction(m, philox4x32_10(make_uint4(cell, 0u, (unsigned)sweep, (unsigned)(sweep >> 32)), a.seed_lo, a.seed_hi), omc);
+}
+
+// Meshes of at most 512 cells per colour (BASELINE config 1: 32 x 32): every cell has its own thread -- threads 0 .. 511 the red
+// cells, 512 .. 1023 the black ones -- and the two halves work in a two-stage pipeline: while one colour runs the neighbour-
+// dependent half of its update (gather, dF, Eq. (5), store), the other colour runs the neighbour-INDEPENDENT half of its next
+// one (Philox and the rotation of the trial move, which need only the cell's own, by then final, vector).  The dependent
+// chain of an iteration shrinks from two whole updates to two half updates.  The red cells' next trial needs the next
+// iteration's cone: in the one iteration per 100 after which the adaptive controller may change it, that half is computed after
+// the end-of-sweep bookkeeping instead.  Same arithmetic as everywhere else: results are bit-identical to the launch-per-pass path.
+template <unsigned F>
+__global__ void __launch_bounds__(kSmallThreads, 1) small_mesh_pipe_kernel(const SweepArgs a_in, int n_sweeps)
+{
+    extern __shared__ float s_m[];                    // [3][2 H]
+    __shared__ Control s_ctl;
+    __shared__ unsigned long long s_run[4];
+    __shared__ int s_w[2][kSmallThreads / 64][6];     // per colour, per warp of that colour: accepted, trials, four fixed-point sums
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int half = tid >> 9, idx = tid & 511, hwarp = idx >> 5;     // colour of this thread, its slot, its warp within the colour
+    SweepArgs a = a_in;
+    const int hxr = (a.g.nx + 1) >> 1, rows = a.g.ny * a.g.nz, slots = hxr * rows;
+    const int S2 = (int)(2 * a.g.H);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        for (int i = tid; i < S2; i += kSmallThreads) s_m[c * S2 + i] = a_in.m[c][i];
+        a.m[c] = s_m + c * S2;
+    }
+    if (tid == 0) s_ctl = *a_in.ctl;
+    if (tid < 4) s_run[tid] = a_in.run_sums ? a_in.run_sums[tid] : 0ull;
+    a.ctl = &s_ctl;
+    const bool mine = idx < slots;
+    const int q = mine ? idx % hxr : 0, row = mine ? idx / hxr : 0, j = row % a.g.ny, k = row / a.g.ny;
+    auto bookkeeping = [&](int col, bool last) {       // one warp: totals of the colour's 16 warps
+        long long tot[6];
+#pragma unroll
+        for (int t = 0; t < 6; ++t) {
+            const int v = lane < kSmallThreads / 64 ? s_w[col][lane][t] : 0;
+            const int lo = __reduce_add_sync(0xffffffffu, v & 0xffff), hi = __reduce_add_sync(0xffffffffu, v >> 16);
+            tot[t] = (long long)hi * 65536ll + (long long)lo;
+        }
+        if (lane == 0) {
+            s_ctl.win_accepted += (unsigned long long)tot[0]; s_ctl.win_trials += (unsigned long long)tot[1];
+            if (a_in.run_sums) for (int t = 0; t < 4; ++t) s_run[t] += (unsigned long long)tot[2 + t];
+            if (last) end_sweep(&s_ctl);
+        }
+    };
+    // the neighbour-dependent half of this thread's cell, and its partial sums
+    auto finish_cell = [&](const Trial& tr, unsigned long long sweep, float omc) {
+        bool active = false, accept = false;
+        float f0 = 0.f, f1 = 0.f, f2 = 0.f, f3 = 0.f;
+        if (mine) pass_one_cell<F, false, true, true>(a, half, q, j, k, sweep, omc, active, accept, f0, f1, f2, f3, tr);
+        const int wa = (int)__reduce_add_sync(0xffffffffu, accept ? 1u : 0u), wt = (int)__reduce_add_sync(0xffffffffu, active ? 1u : 0u);
+        const int w0 = __reduce_add_sync(0xffffffffu, __float2int_rn(f0 * kSumScale)), w1 = __reduce_add_sync(0xffffffffu, __float2int_rn(f1 * kSumScale)),
+                  w2 = __reduce_add_sync(0xffffffffu, __float2int_rn(f2 * kSumScale)), w3 = __reduce_add_sync(0xffffffffu, __float2int_rn(f3 * kSumScale));
+        if (lane == 0) { int* w = s_w[half][hwarp]; w[0] = wa; w[1] = wt; w[2] = w0; w[3] = w1; w[4] = w2; w[5] = w3; }
+    };
+    __syncthreads();
+    Trial tr = {};
+    if (half == 0 && mine && n_sweeps > 0) tr = cell_trial(a, 0, q, j, k, s_ctl.sweep, s_ctl.one_minus_cos_cone);   // prologue: red, first iteration
+    for (int it = 0; it < n_sweeps; ++it) {
+        const unsigned long long sweep = s_ctl.sweep;
+        const float omc = s_ctl.one_minus_cos_cone;
+        const bool cone_may_change = s_ctl.adaptive && s_ctl.win_sweeps == 99u;      // this iteration closes a controller window
+        // stage 1: red cells finish, black cells prepare (their vectors are final since the previous black stage)
+        if (half == 0) finish_cell(tr, sweep, omc);
+        else if (mine) tr = cell_trial(a, 1, q, j, k, sweep, omc);
+        __syncthreads();
+        if (tid < 32) bookkeeping(0, false);
+        // stage 2: black cells finish, red cells prepare the NEXT iteration (same cone unless the controller is about to act)
+        if (half == 1) finish_cell(tr, sweep, omc);
+        else if (mine && !cone_may_change && it + 1 < n_sweeps) tr = cell_trial(a, 0, q, j, k, sweep + 1ull, omc);
+        __syncthreads();
+        if (tid < 32) bookkeeping(1, true);
+        __syncthreads();                              // the new sweep counter and cone are visible
+        if (cone_may_change && half == 0 && mine && it + 1 < n_sweeps) tr = cell_trial(a, 0, q, j, k, s_ctl.sweep, s_ctl.one_minus_cos_cone);
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        for (int i = tid; i < S2; i += kSmallThreads) a_in.m[c][i] = s_m[c * S2 + i];
+    if (tid == 0) *a_in.ctl = s_ctl;
+    if (tid < 4 && a_in.run_sums) a_in.run_sums[tid] = s_run[tid];
+}
+
 int launch_end_sweep(Control* ctl, void* stream)
 {
     launch_pdl(end_sweep_kernel, dim3(1), dim3(1), (size_t)(0), (cudaStream_t)stream, ctl);
@@ -945,7 +1039,8 @@ template <unsigned F>
 static int launch_small_variant(const SweepArgs& a, int n_sweeps, cudaStream_t st)
 {
     const size_t smem = (size_t)3 * 2 * a.g.H * sizeof(float);
-    auto kern = small_mesh_sweeps_kernel<F>;
+    const int slots = ((a.g.nx + 1) >> 1) * a.g.ny * a.g.nz;      // cells per colour
+    auto kern = slots <= kSmallThreads / 2 ? small_mesh_pipe_kernel<F> : small_mesh_sweeps_kernel<F>;
     if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
     kern<<<1, kSmallThreads, smem, st>>>(a, n_sweeps);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;

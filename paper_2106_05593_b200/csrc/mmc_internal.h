@@ -165,12 +165,12 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
                   float* const bd[3], void* stream, std::string* err, PhaseTimer* timer = nullptr);
 
 #ifdef __CUDACC__
-// Programmatic dependent launch (PDL).  Every kernel of the iteration path starts with pdl_enter(): it lets the NEXT kernel of
-// the stream be launched right away (its CTAs become resident as slots free up and park in griddepcontrol.wait) and then waits
-// until the PREVIOUS kernel has completed and flushed its memory, before it reads or writes anything.  The kernels are launched
-// with launch_pdl (programmatic stream serialisation allowed), in streams and in captured graphs alike: the ~1.5 us between
-// dependent kernels shrinks to the dependency itself, which is what the launch-bound configs (65 k - 262 k cells) consist of.
-// MMC_NO_PDL in the environment switches the attribute off (plain stream order; pdl_enter() is then a no-op).
+// Programmatic dependent launch (PDL), an option (MMC_PDL=1).  Every kernel of the iteration path starts with pdl_enter():
+// it lets the NEXT kernel of the stream be launched right away (its CTAs become resident as slots free up and park in
+// griddepcontrol.wait) and then waits until the PREVIOUS kernel has completed and flushed its memory, before it reads or writes
+// anything; the kernels are launched with launch_pdl (programmatic stream serialisation allowed when g_pdl is set), in streams
+// and in captured graphs alike.  Measured (round 2): bit-identical results, but SLOWER on every config (the parked CTAs take
+// slots from the running kernel), so g_pdl is off by default and pdl_enter() is then a pair of no-ops.
 extern bool g_pdl;
 __device__ __forceinline__ void pdl_enter()
 {

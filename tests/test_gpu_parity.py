@@ -588,13 +588,13 @@ def test_demag_and_sweep_are_bitwise_reproducible(shape):
 
 @pytest.mark.parametrize("name", ["cfg2_64x48", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150"])
 def test_launch_paths_agree_bitwise(name):
-    """mmc_sweep(n) replays whole iterations from CUDA graphs (16 at a time, then one at a time) whose kernels are chained by
-    programmatic dependent launch, and on small meshes the last CTA of the black pass closes the iteration.  Plain stream
-    launches (MMC_NO_GRAPH), launches without programmatic dependencies (MMC_NO_PDL) and the event-bracketed launches of
+    """mmc_sweep(n) replays whole iterations from CUDA graphs (16 at a time, then one at a time), and on small meshes the last
+    CTA of the black pass closes the iteration.  Plain stream launches (MMC_NO_GRAPH), kernels chained by programmatic
+    dependent launch (MMC_PDL=1: an option, measured slower) and the event-bracketed launches of
     mmc_sweep_timed must give the same bits: states, counters, cone, running sums after 137 iterations with the adaptive cone
     (one controller window and a partial one; 8 x 16 + 9 iterations; a second call re-uses the cached graphs)."""
     ref = None
-    for knob in (None, "MMC_NO_GRAPH", "MMC_NO_PDL", "timed"):
+    for knob in (None, "MMC_NO_GRAPH", "MMC_PDL", "timed"):
         wl = CASES[name](); wl.adaptive_cone = True
         import contextlib
         with (_env(knob, "1") if knob and knob != "timed" else contextlib.nullcontext()):
@@ -647,12 +647,14 @@ def test_histograms_parity(name):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["cfg1_32x32", "cfg1_paper_regime", "cfg1_ragged_40x24", "cfg1_ragged_periodic_12x6", "cfg1_k2_32x32"])
+@pytest.mark.parametrize("name", ["cfg1_32x32", "cfg1_paper_regime", "cfg1_ragged_40x24", "cfg1_ragged_periodic_12x6", "cfg1_k2_32x32",
+                                  "cfg1_64x48_loop_kernel"])
 def test_single_launch_small_mesh_path_is_bitwise_the_launch_per_pass_path(name):
     """Small meshes without demag run all iterations of mmc_sweep in ONE launch (one CTA, SURVEY 8(d) "Config 1"); mmc_sweep_timed
     keeps the launch-per-pass kernels.  Same cell arithmetic, integer reductions: states, counters, energies and the
     adaptive cone must agree bit for bit after 230 iterations (two cone-controller windows and a partial one)."""
-    wl = CASES[name]()
+    # <= 512 cells per colour: the pipelined kernel (one thread per cell, the two colours' half updates overlap); more: the loop kernel
+    wl = W.cfg1(nx=64, ny=48, paper_regime=True) if name == "cfg1_64x48_loop_kernel" else CASES[name]()
     wl.adaptive_cone = True
     a, b = _gpu(wl), _gpu(wl)
     a.sweep(230)
