@@ -408,7 +408,7 @@ def run_ours(args):
                 d["issue_slot_frac"] = tr["warp_instructions"] / t / ISSUE_PEAK
             # which roofline is the tighter one for this kernel: the larger of the HBM fraction (algorithmic bytes) and the
             # plain-ALU fraction (algorithmic flops for the transforms; issue slots, from the ncu instruction count, for the pass)
-            alu = d.get("frac_of_fma_peak", d.get("issue_slot_frac"))
+            alu = max([x for x in (d.get("frac_of_fma_peak"), d.get("issue_slot_frac")) if x is not None], default=None)
             d["bound"] = "alu" if (alu is not None and alu > d["frac_of_hbm_peak"]) else "hbm"
         dom = max(kern, key=lambda k: kern[k]["launch_ms"])          # the dominant kernel = longest single launch
         dk = kern[dom]
@@ -425,7 +425,7 @@ def run_ours(args):
         roof_alu = None
         if "achieved_TFLOPs" in dk:
             roof_alu = {"kernel": dom, "bound": "alu", "achieved": dk["achieved_TFLOPs"], "peak": FMA_PEAK, "unit": "TFLOP/s",
-                        "frac": dk["frac_of_fma_peak"], "traffic": dk["ncu_traffic_bytes"],
+                        "frac": dk["frac_of_fma_peak"], "issue_slot_frac": dk.get("issue_slot_frac"), "traffic": dk["ncu_traffic_bytes"],
                         "peak_source": "derived: 148 SM x 128 lanes x 2 flop x 1.965 GHz (B200_PROFILING.md unit counts and clocks); "
                                        "algorithmic flops = 5 n log2 n per complex transform + the tensor products",
                         "launch_ms": dk["launch_ms"], "share_of_step": dk["share_of_step"]}

@@ -143,3 +143,38 @@ dist.destroy_process_group()
     out = json.loads(line)
     assert out["world"] == 2 and out["seed0"] != out["seed1"]
     assert out["value"] == pytest.approx((1000.0 + 2000.0) / 1.0)     # total units / max time over ranks
+
+
+def test_bench_traffic_is_measured_or_null(monkeypatch):
+    """bench.py's roofline.traffic: parsed from the committed ncu capture profiles/traffic_cfg<N>.csv only while the sources
+    are the ones the capture was taken from (profiles/traffic_cfg<N>.md carries their hash); null after any change."""
+    sys.path.insert(0, ROOT)
+    import bench
+    md = open(os.path.join(ROOT, "profiles", "traffic_cfg4.md")).read()
+    recorded = re.search(r"source_hash: ([0-9a-f]{16})", md).group(1)
+    monkeypatch.setattr(bench, "source_hash", lambda: recorded)
+    t = bench.ncu_traffic(4)
+    assert {"colour_pass_kernel", "demag_rows_fwd_kernel", "demag_columns_kernel", "demag_rows_inv_kernel"} <= set(t)
+    for k, v in t.items():
+        assert v["dram_bytes"] > 1e6 and v["warp_instructions"] > 1e5, k
+    # the columns kernel moves about what the algorithm needs (U + T + tensor = 478.6 MB for cfg 4), not multiples of it
+    assert 0.5 < t["demag_columns_kernel"]["dram_bytes"] / 478.6e6 < 1.5
+    monkeypatch.setattr(bench, "source_hash", lambda: "0" * 16)
+    assert bench.ncu_traffic(4) == {}
+    assert bench.ncu_traffic(3) == {}            # no capture committed for this config
+    assert re.fullmatch(r"[0-9a-f]{16}", __import__("importlib").reload(bench).source_hash())
+
+
+def test_bench_demag_byte_model():
+    """Algorithmic bytes of the demag kernels as DESIGN.md section 6 states them (cfg 4: U 100.8 MB, T 176.3 MB, tensor 201.5 MB)."""
+    sys.path.insert(0, ROOT)
+    import bench
+
+    class WL:
+        nx, ny, nz, N = 1024, 1024, 4, 1024 * 1024 * 4
+    b = bench.demag_kernel_bytes(WL, False)
+    assert b["columns"]["bytes"] == pytest.approx(478.6e6, rel=2e-3) and b["z_inverse"]["bytes"] == pytest.approx(277.1e6, rel=2e-3)
+    assert b["rows_fwd"]["bytes"] == pytest.approx(151.1e6, rel=2e-3) and b["rows_inv"]["bytes"] == b["rows_fwd"]["bytes"]
+    WL.nx = WL.ny = 2048; WL.nz = 1; WL.N = 2048 * 2048
+    b = bench.demag_kernel_bytes(WL, True)
+    assert "z_inverse" not in b and sum(v["bytes"] for v in b.values()) / WL.N == pytest.approx(156, abs=2)
