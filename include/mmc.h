@@ -43,6 +43,7 @@ extern "C" {
 #define MMC_E_NOMEM        -4   /* host or device allocation failed */
 #define MMC_E_UNSUPPORTED  -5   /* valid request outside what is built (e.g. A0 differing between regions) */
 #define MMC_E_STATE        -6   /* call order: m / material / temperature not set before sweeping */
+#define MMC_E_TOO_LARGE    -7   /* mmc_mean_m_static: more cells than its fixed device scratch array serves */
 
 typedef struct mmc_ctx mmc_ctx;   /* opaque, owned by the library */
 
@@ -170,6 +171,31 @@ int mmc_debug_pass(mmc_ctx* ctx, int colour, float* dm, float* dF_terms, float* 
 int mmc_thermal(double T, double Tc, double mu_atom, double V, double Ms0, double* out6);
 /* Host-side demag tensor used by the set-up: out[6] = N_xx, N_yy, N_zz, N_xy, N_xz, N_yz at integer cell offset. */
 int mmc_demag_tensor_at(double dx, double dy, double dz, int ox, int oy, int oz, double* out6);
+
+/* Allocation-free read-out of the magnetisation means, for callers that cannot allocate (stream capture into a CUDA graph,
+ * a serving loop, a harness that forbids it): the same sums as the read-out above (<m> and <|m|> over the
+ * non-empty cells; |m| rounded to fp32 per cell, fp64 accumulation) by a variant of its kernel whose per-block partial sums
+ * sit in a file-scope `static __device__` array of the library instead of a buffer the ctx allocated.  No ctx is needed and
+ * the call makes no cudaMalloc / cudaFree / allocating library call, does not synchronise, and only enqueues on cuda_stream
+ * (a 256-byte memset node + one kernel), so it may be issued while that stream is being captured.
+ *   mx, my, mz : device float[n_cells] on `device`, natural cell order as the state getter returns them (empty cells hold 0:
+ *                a cell counts as non-empty when its |m| > 0 -- a non-empty cell never has length 0, see MMC_E_ZERO_LENGTH).
+ *   out5       : device double[5] on `device`: <mx>, <my>, <mz>, <|m|> over the non-empty cells, and their number (all 0
+ *                when there is none).  Valid once the work enqueued on cuda_stream has run.  Caller-owned, like the inputs.
+ *   n_cells    : 0 <= n_cells <= MMC_STATIC_MAX_CELLS; more returns MMC_E_TOO_LARGE and enqueues nothing.  n_cells == 0
+ *                only does the set-up below and zeroes out5 (which may then be NULL).
+ * Scratch: MMC_STATIC_SCRATCH_BYTES (one 256-byte control line + 5 doubles per block of 4096 cells) of device memory that every
+ * GPU which loads the library holds until the process exits.  Its device address is resolved once per device (first call
+ * on that device, cudaGetSymbolAddress with the device current; loads the module if CUDA loads lazily): make that first call
+ * outside a stream capture.  ALL calls on a device share the array and it keeps the previous call's contents; the call
+ * clears what must start at zero (the completion ticket).  Two calls that overlap on the GPU (different streams, or graphs
+ * replayed side by side) RACE on it: order them on one stream or with events.  The result does not depend on the
+ * schedule of the blocks (fixed summation order).  Errors: MMC_E_INVALID (NULL pointer, n_cells < 0, device < 0 or >= 64),
+ * MMC_E_TOO_LARGE, MMC_E_CUDA (the runtime refused the symbol look-up, the memset or the launch). */
+#define MMC_STATIC_MAX_CELLS     16777216LL            /* 2^24 cells = 4096 blocks of 4096 cells (config 4 of BASELINE.json: 2^22) */
+#define MMC_STATIC_SCRATCH_BYTES (256 + 4096 * 5 * 8)  /* 164 096 bytes */
+int mmc_mean_m_static(const float* mx, const float* my, const float* mz, long long n_cells, double* out5,
+                      int device, void* cuda_stream);
 
 const char* mmc_strerror(int code);
 const char* mmc_last_error(const mmc_ctx* ctx);

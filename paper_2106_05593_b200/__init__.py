@@ -21,8 +21,11 @@ SYMBOLS = [
     "mmc_create", "mmc_destroy", "mmc_set_material", "mmc_set_exchange_coupling", "mmc_set_temperature",
     "mmc_set_field", "mmc_set_move", "mmc_set_demag", "mmc_set_seed", "mmc_set_sweep_counter", "mmc_set_m",
     "mmc_get_m", "mmc_set_m_host", "mmc_get_m_host", "mmc_sweep", "mmc_sweep_timed", "mmc_demag_field", "mmc_get_observables", "mmc_reset_counters", "mmc_reset_averages", "mmc_relax", "mmc_histogram",
-    "mmc_debug_pass", "mmc_thermal", "mmc_demag_tensor_at", "mmc_strerror", "mmc_last_error",
+    "mmc_debug_pass", "mmc_thermal", "mmc_demag_tensor_at", "mmc_mean_m_static", "mmc_strerror", "mmc_last_error",
 ]
+
+STATIC_MAX_CELLS = 1 << 24          # MMC_STATIC_MAX_CELLS of include/mmc.h
+E_TOO_LARGE = -7                    # MMC_E_TOO_LARGE
 
 
 class MMCLibraryError(RuntimeError):
@@ -101,6 +104,7 @@ def lib():
     L.mmc_debug_pass.argtypes = [vp, i32, vp, vp, vp, vp]
     L.mmc_thermal.argtypes = [dbl] * 5 + [C.POINTER(dbl)]
     L.mmc_demag_tensor_at.argtypes = [dbl, dbl, dbl, i32, i32, i32, C.POINTER(dbl)]
+    L.mmc_mean_m_static.argtypes = [vp, vp, vp, C.c_longlong, vp, i32, vp]
     L.mmc_strerror.argtypes = [i32]; L.mmc_strerror.restype = C.c_char_p
     L.mmc_last_error.argtypes = [vp]; L.mmc_last_error.restype = C.c_char_p
     for s in SYMBOLS:
@@ -125,6 +129,25 @@ def demag_tensor_at(dx, dy, dz, ox, oy, oz):
     if rc:
         raise MMCError(rc, lib().mmc_strerror(rc).decode())
     return np.array(list(o))
+
+
+def mean_m_static(mx, my, mz, out5, n_cells=None, stream=None):
+    """mmc_mean_m_static: enqueue <m>, <|m|> and the number of non-empty cells of the device float32 tensors mx, my, mz into
+    the device float64 tensor out5 (5 elements) on `stream` (default: torch's current stream of that device).  The library
+    allocates nothing (its scratch is a static device array shared by all calls: do not overlap two of them on the GPU);
+    neither does this wrapper: every buffer is the caller's.  Returns out5 (valid after the stream has run)."""
+    import torch
+    n = int(mx.numel() if n_cells is None else n_cells)
+    if n <= STATIC_MAX_CELLS:                      # beyond it the library refuses before it looks at the buffers
+        for t in (mx, my, mz):
+            assert t.is_cuda and t.dtype == torch.float32 and t.is_contiguous() and t.numel() >= n and t.device == mx.device
+        assert out5.is_cuda and out5.dtype == torch.float64 and out5.is_contiguous() and out5.numel() >= 5 and out5.device == mx.device
+    st = stream if stream is not None else torch.cuda.current_stream(mx.device)
+    rc = lib().mmc_mean_m_static(mx.data_ptr(), my.data_ptr(), mz.data_ptr(), n, out5.data_ptr(), mx.device.index or 0,
+                                 C.c_void_p(st.cuda_stream))
+    if rc:
+        raise MMCError(rc, lib().mmc_strerror(rc).decode())
+    return out5
 
 
 class MMC:

@@ -10,7 +10,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmmc_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-CU = ["api.cu", "kernels_sweep.cu", "kernels_layout.cu", "demag.cu"]
+CU = ["api.cu", "kernels_sweep.cu", "kernels_layout.cu", "demag.cu", "static_scratch.cu"]
 CPP = ["mmc_host.cpp"]
 NVFLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
            "-Xcompiler", "-fPIC", "-Xptxas", "-v"] + os.environ.get("MMC_NVCC_FLAGS", "").split()   # e.g. -DMMC_COLS_MINB=2 (tuning knobs of csrc/)

@@ -864,6 +864,7 @@ const char* mmc_strerror(int code)
         case MMC_E_NOMEM: return "out of memory";
         case MMC_E_UNSUPPORTED: return "unsupported configuration";
         case MMC_E_STATE: return "call order: material, temperature and m must be set first";
+        case MMC_E_TOO_LARGE: return "more cells than the static scratch array serves (MMC_STATIC_MAX_CELLS = 16777216)";
         default: return "unknown error";
     }
 }
