@@ -1132,6 +1132,8 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
         // length will do, and every plane saved is a whole set of column transforms saved.
         const int lgH = ilog2(p->Hx), lgPy = ilog2(p->Py);
         p->fastA = lgH >= 8 && lgH <= 11 && lgPy >= fftr::kMinLg && lgPy <= fftr::kMaxLg && g.nz <= kMaxFastLayers;
+        // MMC_DEMAG_GENERIC=1 (tests): the any-length shared-memory kernels on meshes the register-resident ones would serve
+        { const char* e = std::getenv("MMC_DEMAG_GENERIC"); if (e && e[0] == '1') p->fastA = false; }
         if (p->fastA && g.nz > 1) p->Pz = 2 * g.nz - 1;
     }
     p->lgPz = ilog2(p->Pz);
@@ -1155,6 +1157,7 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
     {
         const int lgPy = ilog2(p->Py);
         p->fastB = lgPy >= fftr::kMinLg && lgPy <= fftr::kMaxLg;
+        { const char* e = std::getenv("MMC_DEMAG_GENERIC"); if (e && e[0] == '1') p->fastB = false; }
         if (p->fastB) {
             const size_t ntw = (size_t)15 * (p->Py / 16);
             CK(cudaMalloc(&p->twB1, ntw * sizeof(float2)));

@@ -62,18 +62,23 @@ __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x)); }
 __device__ __forceinline__ float2 cmulc(float2 a, float2 b) { return make_float2(fmaf(a.x, b.x, a.y * b.y), fmaf(a.y, b.x, -a.x * b.y)); }   // a * conj(b)
 
-// multiply by exp(-/+ 2 pi i k / N) for compile-time k, N <= 16 (INV: conjugate root)
+// multiply by exp(-/+ 2 pi i k / N) for compile-time k < N/2, N <= 32 (INV: conjugate root)
 template <int N, bool INV>
 __device__ __forceinline__ float2 mul_root(float2 a, int k)
 {
-    // cos, sin of 2 pi j / 16, j = 0..7
-    constexpr float C[8] = { 1.f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f, 0.f,
-                             -0.38268343236508977f, -0.70710678118654752f, -0.92387953251128674f };
-    constexpr float S[8] = { 0.f, 0.38268343236508977f, 0.70710678118654752f, 0.92387953251128674f, 1.f,
-                             0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f };
-    const int j = k * (16 / N);                       // 0 <= j < 8
+    static_assert(N <= 32 && (32 % N) == 0, "mul_root: the root table covers N = 2, 4, 8, 16, 32");
+    // cos, sin of 2 pi j / 32, j = 0..15
+    constexpr float C[16] = { 1.f, 0.98078528040323044f, 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f,
+                              0.55557023301960222f, 0.38268343236508977f, 0.19509032201612827f, 0.f,
+                              -0.19509032201612827f, -0.38268343236508977f, -0.55557023301960222f, -0.70710678118654752f,
+                              -0.83146961230254524f, -0.92387953251128674f, -0.98078528040323044f };
+    constexpr float S[16] = { 0.f, 0.19509032201612827f, 0.38268343236508977f, 0.55557023301960222f, 0.70710678118654752f,
+                              0.83146961230254524f, 0.92387953251128674f, 0.98078528040323044f, 1.f,
+                              0.98078528040323044f, 0.92387953251128674f, 0.83146961230254524f, 0.70710678118654752f,
+                              0.55557023301960222f, 0.38268343236508977f, 0.19509032201612827f };
+    const int j = k * (32 / N);                       // 0 <= j < 16
     if (j == 0) return a;
-    if (j == 4) return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+    if (j == 8) return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
     const float c = C[j], s = INV ? S[j] : -S[j];     // root = c + i s
     return make_float2(fmaf(a.x, c, -a.y * s), fmaf(a.x, s, a.y * c));
 }

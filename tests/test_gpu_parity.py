@@ -307,7 +307,9 @@ def test_two_demag_updates_per_iteration(name, exchange):
                                      ((1024, 65, 1), (5e-9, 5e-9, 10e-9)), ((700, 69, 4), (3e-9, 3e-9, 3e-9)),
                                      ((2048, 66, 1), (5e-9, 5e-9, 10e-9)), ((1500, 65, 2), (3e-9, 3e-9, 3e-9)),
                                      ((130, 300, 3), (3e-9, 3e-9, 3e-9)), ((132, 70, 10), (2e-9, 2e-9, 2e-9)),
-                                     ((256, 65, 16), (2e-9, 2e-9, 2e-9))])
+                                     ((256, 65, 16), (2e-9, 2e-9, 2e-9)),
+                                     # generic shared-memory kernels (nx <= 128) with 9 .. 16 layers: padded z length 32
+                                     ((64, 48, 10), (2e-9, 2e-9, 2e-9)), ((40, 24, 16), (3e-9, 2e-9, 2e-9)), ((96, 20, 9), (2e-9, 2e-9, 4e-9))])
 def test_demag_field_parity(shape, d):
     """Eq. (14): GPU fp32 FFT convolution vs the oracle's fp64 one (itself pinned to the direct sum)."""
     import paper_2106_05593_b200 as P
@@ -340,6 +342,33 @@ class _env:
         import os
         if self.old is None: os.environ.pop(self.key, None)
         else: os.environ[self.key] = self.old
+
+
+@pytest.mark.parametrize("shape,d", [((256, 256, 1), (5e-9, 5e-9, 5e-9)), ((301, 67, 3), (2e-9, 3e-9, 4e-9)), ((512, 72, 2), (3e-9, 3e-9, 3e-9)),
+                                     ((256, 66, 4), (3e-9, 3e-9, 3e-9)), ((200, 300, 5), (3e-9, 3e-9, 3e-9)), ((132, 70, 10), (2e-9, 2e-9, 2e-9)),
+                                     ((256, 65, 16), (2e-9, 2e-9, 2e-9))])
+def test_generic_demag_kernels_on_meshes_the_fast_path_serves(shape, d):
+    """MMC_DEMAG_GENERIC=1: the any-length shared-memory kernels (rows with the z transform of padded length 1 .. 32 in registers,
+    columns per (kx, kz)) on shapes that normally take the register-resident kernels: same bar against the oracle."""
+    import paper_2106_05593_b200 as P
+    nx, ny, nz = shape; N = nx * ny * nz
+    rng = np.random.default_rng(N + 3)
+    v = rng.normal(size=(3, N)); v /= np.linalg.norm(v, axis=0)
+    m0 = (v * rng.uniform(0.3, 1.0, N)).astype(np.float32)
+    reg = (rng.uniform(size=N) > 0.2).astype(np.int32)
+    m0[:, reg == 0] = 0
+    with _env("MMC_DEMAG_GENERIC", "1"):
+        g = P.MMC(nx, ny, nz, *d, 0)
+        g.set_material([P.Material(), P.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)], reg)
+        g.set_temperature(300.0); g.set_m(*m0)
+        bg = _np(g.demag_field())
+    conv = O.DemagFFT(nx, ny, nz, *d)
+    M = [(8.6e5 * reg * m0[a].astype(np.float64)).reshape(nz, ny, nx) for a in range(3)]
+    bo = [b.ravel() for b in conv.field(*M)]
+    scale = max(np.abs(b).max() for b in bo)
+    for a in range(3):
+        assert np.abs(bg[a] - bo[a]).max() <= 2e-5 * scale
+    g.close()
 
 
 @pytest.mark.parametrize("shape,d", [((64, 256, 2), (3e-9, 3e-9, 3e-9)), ((48, 1024, 2), (3e-9, 3e-9, 3e-9)), ((130, 300, 3), (3e-9, 3e-9, 3e-9)),
