@@ -308,6 +308,11 @@ def test_two_demag_updates_per_iteration(name, exchange):
                                      ((2048, 66, 1), (5e-9, 5e-9, 10e-9)), ((1500, 65, 2), (3e-9, 3e-9, 3e-9)),
                                      ((130, 300, 3), (3e-9, 3e-9, 3e-9)), ((132, 70, 10), (2e-9, 2e-9, 2e-9)),
                                      ((256, 65, 16), (2e-9, 2e-9, 2e-9)),
+                                     # register-resident path with every other layer count up to 16 (z-DFT lengths 9 .. 29)
+                                     ((130, 65, 5), (3e-9, 3e-9, 3e-9)), ((130, 70, 6), (3e-9, 3e-9, 2e-9)), ((140, 65, 7), (3e-9, 3e-9, 3e-9)),
+                                     ((130, 66, 8), (2e-9, 3e-9, 3e-9)), ((130, 65, 9), (3e-9, 3e-9, 3e-9)), ((130, 65, 11), (3e-9, 3e-9, 3e-9)),
+                                     ((129, 65, 12), (3e-9, 3e-9, 3e-9)), ((130, 65, 13), (3e-9, 3e-9, 4e-9)), ((130, 67, 14), (3e-9, 3e-9, 3e-9)),
+                                     ((130, 65, 15), (3e-9, 3e-9, 3e-9)),
                                      # generic shared-memory kernels (nx <= 128) with 9 .. 16 layers: padded z length 32
                                      ((64, 48, 10), (2e-9, 2e-9, 2e-9)), ((40, 24, 16), (3e-9, 2e-9, 2e-9)), ((96, 20, 9), (2e-9, 2e-9, 4e-9))])
 def test_demag_field_parity(shape, d):
@@ -329,6 +334,47 @@ def test_demag_field_parity(shape, d):
     scale = max(np.abs(b).max() for b in bo)
     for a in range(3):
         assert np.abs(bg[a] - bo[a]).max() <= 2e-5 * scale
+    g.close()
+
+
+@pytest.mark.parametrize("shape,d", [((1, 1, 1), (5e-9, 5e-9, 5e-9)), ((1, 1, 5), (5e-9, 4e-9, 3e-9)), ((7, 1, 1), (2e-9, 3e-9, 4e-9)),
+                                     ((1, 9, 1), (2e-9, 3e-9, 4e-9)), ((2, 2, 2), (3e-9, 3e-9, 3e-9)), ((1, 5, 3), (3e-9, 3e-9, 5e-9)),
+                                     ((2, 1, 16), (3e-9, 3e-9, 3e-9)),
+                                     # beyond the register-resident lengths: padded nx 8192 (generic rows kernels, with generic and
+                                     # with register-resident columns), padded ny 8192 (generic columns kernel, 209 KB of shared memory)
+                                     ((2100, 6, 1), (5e-9, 5e-9, 10e-9)), ((2100, 130, 2), (3e-9, 3e-9, 3e-9)), ((12, 2100, 1), (5e-9, 5e-9, 5e-9))])
+def test_demag_field_parity_degenerate_and_oversize_meshes(shape, d):
+    """Eq. (14) on meshes with directions of length 1 or 2 (padded lengths 1, 2, 4: self-term and nearest offsets only) and on
+    meshes longer than the register-resident transforms serve; every cell magnetic."""
+    import paper_2106_05593_b200 as P
+    nx, ny, nz = shape; N = nx * ny * nz
+    rng = np.random.default_rng(1000 + N)
+    v = rng.normal(size=(3, N)); v /= np.linalg.norm(v, axis=0)
+    m0 = (v * rng.uniform(0.3, 1.0, N)).astype(np.float32)
+    g = P.MMC(nx, ny, nz, *d, 0)
+    g.set_material([P.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)])
+    g.set_temperature(300.0); g.set_m(*m0)
+    bg = _np(g.demag_field())
+    conv = O.DemagFFT(nx, ny, nz, *d)
+    M = [(8.6e5 * m0[a].astype(np.float64)).reshape(nz, ny, nx) for a in range(3)]
+    bo = [b.ravel() for b in conv.field(*M)]
+    scale = max(np.abs(b).max() for b in bo)
+    assert scale > 0.1                                                # tesla: a saturated cell's own field
+    for a in range(3):
+        assert np.abs(bg[a] - bo[a]).max() <= 2e-5 * scale
+    g.close()
+
+
+def test_demag_more_than_16_layers_is_a_clean_error():
+    import paper_2106_05593_b200 as P
+    g = P.MMC(4, 4, 17, 3e-9, 3e-9, 3e-9, 0)
+    g.set_material([P.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)]); g.set_temperature(300.0)
+    g.set_m(np.zeros(272), np.zeros(272), np.full(272, 0.9))
+    with pytest.raises(P.MMCError) as e:
+        g.demag_field()
+    assert e.value.code == -5 and "16 layers" in str(e.value)
+    g.sweep(2)                                                        # the context still works without demag
+    assert g.observables()["trials"] == 2 * 272
     g.close()
 
 
