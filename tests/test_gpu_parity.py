@@ -131,6 +131,11 @@ def _small(cfg, **kw):
     return W.make(cfg, **kw)
 
 
+def _with_pbc(wl, mask):
+    wl.pbc_mask = mask                                # exchange / DMI wrap; the demag convolution stays open-boundary
+    return wl
+
+
 def _with_k2(wl, K2):
     for r in wl.regions:
         if r["Ms0"] > 0:
@@ -157,6 +162,13 @@ CASES = {
     # K1 + K2 of Eq. (11): uniform film (kernel arguments) and granular film (class tables, tilted axes, T > Tc in the hot spot)
     "cfg1_k2_32x32": lambda: _with_k2(W.cfg1(paper_regime=True), -1.5e5),
     "cfg4_k2_30x21x3": lambda: _with_k2(W.cfg4(nx=30, ny=21, nz=3), 4e5),
+    # periodic directions not covered by the recipes: z wrap (also with the two z neighbours being the same cell), wrap in all
+    # three directions on per-cell classes, y wrap on odd nx (padded compact rows), and the shortest periodic lengths
+    "cfg4_periodic_xyz_16x12x4": lambda: _with_pbc(W.cfg4(nx=16, ny=12, nz=4), 0b111),
+    "cfg4_periodic_z_15x9x2": lambda: _with_pbc(W.cfg4(nx=15, ny=9, nz=2), 0b100),
+    "cfg2_periodic_y_37x20": lambda: _with_pbc(W.cfg2(nx=37, ny=20), 0b010),
+    "cfg3_periodic_dmi_2x2": lambda: W.cfg3(nx=2, ny=2, T=200.0),
+    "cfg1_periodic_2x6": lambda: W.cfg1(nx=2, ny=6, paper_regime=True),
 }
 
 
@@ -195,7 +207,8 @@ def _check_iteration(wl, g, o, label):
 
 
 @pytest.mark.parametrize("name", ["cfg1_paper_regime", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150",
-                                  "fe_film_cubic_48x40x3", "cfg4_k2_30x21x3"])
+                                  "fe_film_cubic_48x40x3", "cfg4_k2_30x21x3", "cfg4_periodic_xyz_16x12x4", "cfg4_periodic_z_15x9x2",
+                                  "cfg2_periodic_y_37x20", "cfg3_periodic_dmi_2x2", "cfg1_periodic_2x6"])
 def test_sweep_matches_replayed_oracle(name):
     """mmc_sweep(n) (demag -> red -> black -> counter++) against the oracle replaying the same iteration, each side with its
     own demag field.  Every active cell must hold the oracle's accepted or rejected candidate, and every cell whose decision
@@ -723,13 +736,21 @@ def test_histograms_parity(name):
 
 
 @pytest.mark.parametrize("name", ["cfg1_32x32", "cfg1_paper_regime", "cfg1_ragged_40x24", "cfg1_ragged_periodic_12x6", "cfg1_k2_32x32",
-                                  "cfg1_64x48_loop_kernel"])
+                                  "cfg1_64x48_loop_kernel", "cfg1_periodic_2x6", "cfg4_nodemag_periodic_16x12x4", "cfg4_nodemag_24x20x4",
+                                  "cfg4_nodemag_periodic_z_15x9x2", "cfg5_nodemag_90x80"])
 def test_single_launch_small_mesh_path_is_bitwise_the_launch_per_pass_path(name):
     """Small meshes without demag run all iterations of mmc_sweep in ONE launch (one CTA, SURVEY 8(d) "Config 1"); mmc_sweep_timed
     keeps the launch-per-pass kernels.  Same cell arithmetic, integer reductions: states, counters, energies and the
     adaptive cone must agree bit for bit after 230 iterations (two cone-controller windows and a partial one)."""
     # <= 512 cells per colour: the pipelined kernel (one thread per cell, the two colours' half updates overlap); more: the loop kernel
-    wl = W.cfg1(nx=64, ny=48, paper_regime=True) if name == "cfg1_64x48_loop_kernel" else CASES[name]()
+    extra = {"cfg1_64x48_loop_kernel": lambda: W.cfg1(nx=64, ny=48, paper_regime=True),
+             # several layers, per-cell classes, empty cells: the recipes of configs 4 and 5 with the demag term switched off
+             "cfg4_nodemag_periodic_16x12x4": lambda: _with_pbc(W.cfg4(nx=16, ny=12, nz=4), 0b111),
+             "cfg4_nodemag_24x20x4": lambda: W.cfg4(nx=24, ny=20, nz=4),
+             "cfg4_nodemag_periodic_z_15x9x2": lambda: _with_pbc(W.cfg4(nx=15, ny=9, nz=2), 0b100),
+             "cfg5_nodemag_90x80": lambda: W.cfg5(nx=90, ny=80)}
+    wl = extra[name]() if name in extra else CASES[name]()
+    wl.demag = False
     wl.adaptive_cone = True
     a, b = _gpu(wl), _gpu(wl)
     a.sweep(230)
