@@ -674,6 +674,36 @@ def test_demag_and_sweep_are_bitwise_reproducible(shape):
     g.close(); h.close()
 
 
+@pytest.mark.parametrize("name", ["cfg2_64x48", "cfg4_30x21x3", "cfg1_32x32"])
+def test_contexts_on_their_own_streams_agree_bitwise_with_the_default_stream(name):
+    """Every call of the library is ordered on the stream given at mmc_create (graphs are captured on a private stream and
+    launched into it): two contexts on two non-blocking streams, driven alternately without host synchronisation in between,
+    end in the state of a context on the legacy default stream, bit for bit."""
+    import paper_2106_05593_b200 as P
+    wl = CASES[name]()
+    ref = _gpu(wl); ref.sweep(40)
+    mr = [t.clone() for t in ref.get_m()]; orf = ref.observables()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    ctxs = []
+    for st in streams:
+        with torch.cuda.stream(st):
+            c = P.MMC(wl.nx, wl.ny, wl.nz, wl.dx, wl.dy, wl.dz, wl.pbc_mask, stream=st)
+            W.configure(c, wl, P.Material)
+            ctxs.append(c)
+    for chunk in (1, 17, 3, 19):                     # plain launches, graphs of 16 and of 1 iteration; alternating contexts
+        for c, st in zip(ctxs, streams):
+            with torch.cuda.stream(st):
+                c.sweep(chunk)
+    for c, st in zip(ctxs, streams):
+        with torch.cuda.stream(st):
+            m = c.get_m(); ob = c.observables()      # synchronises the context's stream
+            assert all(torch.equal(m[q], mr[q]) for q in range(3))
+            for k in ("accepted", "trials", "sweeps_done", "cone_deg", "run_mean_len", "E_ex", "E_demag", "E_long"):
+                assert ob[k] == orf[k], k
+        c.close()
+    ref.close()
+
+
 @pytest.mark.parametrize("name", ["cfg2_64x48", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150"])
 def test_launch_paths_agree_bitwise(name):
     """mmc_sweep(n) replays whole iterations from CUDA graphs (16 at a time, then one at a time), and on small meshes the last
