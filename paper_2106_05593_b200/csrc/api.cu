@@ -66,7 +66,8 @@ struct mmc_ctx {
     Control* ctl = nullptr;
     unsigned long long* run_sums = nullptr;       // [4] fixed-point running sums (kSumScale)
     double* obs_scratch = nullptr; int obs_blocks = 0;
-    Observables* d_obs = nullptr;
+    ReadOut* d_obs = nullptr;                     // device: filled by the read-out kernel
+    ReadOut* h_obs = nullptr;                     // pinned host: target of the one copy of a read-out
     int* d_flag = nullptr;
     float* stage = nullptr;                       // N floats, for natural-order outputs
     DemagPlan* demag = nullptr;
@@ -392,11 +393,13 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
         cudaMemsetAsync(c->m[q], 0, S * sizeof(float), c->stream);
         cudaMemsetAsync(c->bd[q], 0, S * sizeof(float), c->stream);
     }
-    c->obs_blocks = 148 * 12;                     // whole waves at 3 or 4 resident CTAs per SM; ~9 slots per thread on the 4 M-cell meshes
+    c->obs_blocks = 148 * 20;                     // 128-thread CTAs (kernels_layout.cu), five per SM: four whole waves; ~11 slots per thread on the 4 M-cell meshes
     if (cudaMalloc(&c->ctl, sizeof(Control)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->run_sums, 4 * sizeof(unsigned long long)) != cudaSuccess) return bail(MMC_E_NOMEM);
-    if (cudaMalloc(&c->obs_scratch, (size_t)c->obs_blocks * 11 * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);
-    if (cudaMalloc(&c->d_obs, sizeof(Observables)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaMalloc(&c->obs_scratch, ((size_t)c->obs_blocks * 11 + 1) * sizeof(double)) != cudaSuccess) return bail(MMC_E_NOMEM);   // ticket + partials
+    if (cudaMalloc(&c->d_obs, sizeof(ReadOut)) != cudaSuccess) return bail(MMC_E_NOMEM);
+    if (cudaHostAlloc(&c->h_obs, sizeof(ReadOut), cudaHostAllocDefault) != cudaSuccess) return bail(MMC_E_NOMEM);
+    cudaMemsetAsync(c->obs_scratch, 0, sizeof(double), c->stream);      // the read-out kernel's ticket
     if (cudaMalloc(&c->d_flag, sizeof(int)) != cudaSuccess) return bail(MMC_E_NOMEM);
     if (cudaMalloc(&c->stage, (size_t)nx * ny * nz * sizeof(float)) != cudaSuccess) return bail(MMC_E_NOMEM);
     cudaMemsetAsync(c->ctl, 0, sizeof(Control), c->stream);
@@ -414,7 +417,7 @@ int mmc_destroy(mmc_ctx* c)
     for (int q = 0; q < 3; ++q) { cudaFree(c->m[q]); cudaFree(c->bd[q]); }
     cudaFree(c->cw); cudaFree(c->table); cudaFree(c->table_cubic);
     cudaFree(c->mask); cudaFree(c->Ms0_split); cudaFree(c->ctl); cudaFree(c->run_sums); cudaFree(c->obs_scratch);
-    cudaFree(c->d_obs); cudaFree(c->d_flag); cudaFree(c->stage);
+    cudaFree(c->d_obs); cudaFreeHost(c->h_obs); cudaFree(c->d_flag); cudaFree(c->stage);
     demag_destroy(c->demag);
     if (c->graph1.exec) cudaGraphExecDestroy(c->graph1.exec);
     if (c->graphN.exec) cudaGraphExecDestroy(c->graphN.exec);
@@ -720,12 +723,11 @@ int mmc_get_observables(mmc_ctx* c, mmc_obs* out)
     }
     rc = launch_observables(a, c->percell, op, c->d_obs, c->obs_scratch, c->obs_blocks, c->stream);
     if (rc) return fail(c, rc, "observables launch failed");
-    Observables ho; Control hc;
-    long long fixed[4] = { 0, 0, 0, 0 };
-    CU(c, cudaMemcpyAsync(&ho, c->d_obs, sizeof(ho), cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaMemcpyAsync(&hc, c->ctl, sizeof(hc), cudaMemcpyDeviceToHost, c->stream));
-    CU(c, cudaMemcpyAsync(fixed, c->run_sums, sizeof(fixed), cudaMemcpyDeviceToHost, c->stream));
+    CU(c, cudaMemcpyAsync(c->h_obs, c->d_obs, sizeof(ReadOut), cudaMemcpyDeviceToHost, c->stream));   // sums, control block, running sums
     CU(c, cudaStreamSynchronize(c->stream));
+    const Observables ho = c->h_obs->obs; const Control hc = c->h_obs->ctl;
+    long long fixed[4];
+    for (int q = 0; q < 4; ++q) fixed[q] = (long long)c->h_obs->run_sums[q];
     std::memset(out, 0, sizeof(*out));
     const double na = ho.n_active > 0 ? (double)ho.n_active : 1.0;
     for (int q = 0; q < 3; ++q) out->mean_m[q] = ho.sum[q] / na;

@@ -110,6 +110,8 @@ struct SweepArgs {
 };
 
 struct Observables { double sum[4]; double E[6]; unsigned long long n_active; };
+// What one read-out brings to the host, gathered by the read-out kernel so that it is ONE device-to-host copy (into pinned memory)
+struct ReadOut { Observables obs; Control ctl; unsigned long long run_sums[4]; };
 
 // TMA-staged colour pass (kernels_sweep.cu): tensor maps (CUtensorMap is 128 bytes, 64-byte aligned) over the colour-split
 // arrays as rank-4 tensors (x = compact index, y, z, colour) and the tile shape they were encoded for.
@@ -141,7 +143,7 @@ struct ObsParams {
     double kB;
     float T_u;                             // uniform temperature (per-cell mode reads 1/T per cell)
 };
-int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, Observables* dev_out, double* scratch,
+int launch_observables(const SweepArgs& a, bool percell, const ObsParams& op, ReadOut* dev_out, double* scratch,
                        int scratch_blocks, void* stream);
 
 int launch_histogram(const Geometry& g, const float* const m[3], const uint8_t* mask, int kind, const double dir[3], int nbins,
