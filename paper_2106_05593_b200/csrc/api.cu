@@ -46,6 +46,7 @@ struct mmc_ctx {
     bool graphs_off = false;
     PassTma tma;                                  // TMA-staged pass: tensor maps over m, bd, cw (rebuilt when a pointer changes)
     bool tma_off = false;
+    int pass1_below = 148;                        // MMC_PASS1_BELOW: see launch_colour_pass
     bool percell = false;
     unsigned features = 0;
     double A0 = 0, D0 = 0, sigma_first = 0;
@@ -307,7 +308,7 @@ SweepArgs make_args(mmc_ctx* c, int colour)
     a.cw = c->percell ? c->cw : nullptr; a.table = c->percell ? reinterpret_cast<const float4*>(c->table) : nullptr;
     a.table_cubic = (c->percell && (c->features & F_CUBIC)) ? reinterpret_cast<const float4*>(c->table_cubic) : nullptr;
     a.ctl = c->ctl; a.seed_lo = (unsigned)c->seed; a.seed_hi = (unsigned)(c->seed >> 32);
-    a.colour = colour; a.run_sums = c->run_sums;
+    a.colour = colour; a.run_sums = c->run_sums; a.pass1_below = c->pass1_below;
     return a;
 }
 
@@ -379,6 +380,7 @@ int mmc_create(mmc_ctx** out, int nx, int ny, int nz, double dx, double dy, doub
     // the next kernel take slots from the running one: cfg 2 26.5 against 23.2 us, cfg 4 0.584 against 0.497 ms), so it is off
     // unless MMC_PDL=1 (process-wide knob, read at every create)
     { const char* e = std::getenv("MMC_PDL"); mmc::g_pdl = e && e[0] == '1'; }
+    { const char* e = std::getenv("MMC_PASS1_BELOW"); if (e) c->pass1_below = std::atoi(e); }
     // the TMA-staged pass runs at the speed of the L1-served brick kernel on the meshes it serves (both
     // ncu tables in profiles/): the brick kernel, which serves every mesh, is the default; MMC_TMA=1 selects the staged variant
     { const char* e = std::getenv("MMC_TMA"); c->tma_off = !(e && e[0] == '1'); }

@@ -58,6 +58,7 @@ struct DemagPlan {
     float2* U = nullptr;             // fastA with nz > 1: [3][nz][Cx][ny], the layers before the z-DFT and after its inverse
     float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
     // layer-pair columns kernel (several layers, no z transform): U is transformed in place, T and nhat do not exist
+    bool planar_split = false;       // one layer, fewer than two columns CTAs per SM: in-plane pair and z component in separate CTAs
     bool lp = false;
     int lpG = 1;                     // kx per CTA
     float* nh2[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };    // [nz][Cx][Py]: 2-D spectra per layer offset dz
@@ -525,7 +526,11 @@ columns_fast_kernel(const ColFastArgs a)
         const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), a.tw1, a.tw2 };
         const size_t nb = (size_t)kx * N + tid;
         float2 v[2][16];
+        // gridDim.y == 2 (small meshes, where the grid does not fill the GPU and the kernel's time is one warp's instruction
+        // chain, not throughput): the in-plane pair and the z component, which share nothing, run in different CTAs
+        const bool do_pair = gridDim.y == 1 || blockIdx.y == 0, do_z = gridDim.y == 1 || blockIdx.y == 1;
         // in-plane pair: load, the xx / yy / xy spectrum into L2 meanwhile, two forward transforms, 2x2 multiply, two inverse
+        if (do_pair) {
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
             const float2* __restrict__ col = a.Tin + ((size_t)c * a.Cx + kx) * ny;
@@ -560,8 +565,9 @@ columns_fast_kernel(const ColFastArgs a)
                 if (live && (HALF || j < ny)) col[j] = v[c][n1];
             }
         }
+        }
         // z component in the registers of the first
-        {
+        if (do_z) {
             float2 (&z)[16] = v[0];
             const float2* __restrict__ cin = a.Tin + ((size_t)2 * a.Cx + kx) * ny;
 #pragma unroll
@@ -1014,7 +1020,7 @@ static int launch_columns_fast_h(const DemagPlan* p, const ColFastArgs& ca, cuda
     if (ca.nz == 0 && p->Pz == 1 && ca.nhat[4] == nullptr && ca.nhat[5] == nullptr) {      // one layer: the planar variant
         auto kp = columns_fast_kernel<LGN, HALF, true>;
         if (smem > 48 * 1024 && cudaFuncSetAttribute(kp, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
-        launch_pdl(kp, dim3(nbx, 1), dim3(S::T, S::G), smem, st, ca);
+        launch_pdl(kp, dim3(nbx, p->planar_split ? 2 : 1), dim3(S::T, S::G), smem, st, ca);
         return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
     }
     auto kern = columns_fast_kernel<LGN, HALF, false>;
@@ -1164,6 +1170,14 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
             CK(cudaMalloc(&p->twB2, ntw * sizeof(float2)));
             fftr::twiddle_tables_kernel<<<blocks_for((long long)ntw), 256, 0, st>>>(p->twB1, p->twB2, lgPy);
         }
+    }
+    if (p->fastB && g.nz == 1) {
+        // Measured (ms per iteration, cfg 2 / cfg 3 / cfg 5): one CTA for all three components 0.0225 / 0.0293 / 0.3727; pair and z
+        // in separate CTAs 0.0209 / 0.0286 / 0.3738; every component in its own thread group of a 256-thread CTA, the pair meeting
+        // in shared memory, 0.0219 / 0.0308 / 0.412 (CTA-wide barriers over twice the warps).  MMC_COLS_SPLIT=0/1 forces the choice.
+        const int Tn = p->Py / 16, G = Tn >= 128 ? 1 : 128 / Tn;       // fftr::Shape<lgPy>::T, ::G
+        const char* e = std::getenv("MMC_COLS_SPLIT");
+        p->planar_split = e ? e[0] == '1' : (p->Cx + G - 1) / G < 2 * 148;
     }
     // several layers on the register-resident path: the layer-pair columns kernel when one CTA can hold a thread group per
     // layer (nz * Py/16 <= 512 threads); else the z-DFT path (planes T, z_inverse pass)

@@ -1025,7 +1025,10 @@ static int launch_variant(const SweepArgs& a, bool debug, cudaStream_t st)
         const int bz = a.g.nz >= 4 ? 4 : (a.g.nz >= 2 ? 2 : 1), by = kPass2Threads / 32 / bz;
         const dim3 b2(32, by, bz), g2((hxr + 63) / 64, (a.g.ny + by - 1) / by, (a.g.nz + bz - 1) / bz);
         if (g2.y > 65535u || g2.z > 65535u) return MMC_E_UNSUPPORTED;
-        launch_pdl(colour_pass2_kernel<F>, dim3(g2), dim3(b2), (size_t)(0), st, a);
+        // a grid of fewer CTAs than SMs: the pass is then as long as one thread's instruction chain, and one cell per thread halves
+        // it (cfg 2, 64 CTAs: 0.0209 -> 0.0191 ms per iteration; cfg 3, 256 CTAs: no difference).  a.pass1_below: 148, or MMC_PASS1_BELOW.
+        if ((long long)g2.x * g2.y * g2.z < a.pass1_below) launch_pdl(colour_pass_kernel<F, false>, dim3(gr), dim3(b), (size_t)(0), st, a);
+        else launch_pdl(colour_pass2_kernel<F>, dim3(g2), dim3(b2), (size_t)(0), st, a);
     }
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }

@@ -104,6 +104,7 @@ struct SweepArgs {
     unsigned seed_lo, seed_hi;
     int colour;
     int finish;                  // != 0: the last CTA of this pass runs the end-of-sweep bookkeeping (S11) itself
+    int pass1_below;              // host side only: grids of fewer CTAs take the one-cell-per-thread pass kernel (launch_colour_pass)
     unsigned long long* run_sums; // [4] running sums of the sweeps' final mx,my,mz,|m| in fixed point (two's complement, kSumScale), or NULL
     // debug dump (natural order), any NULL
     float* dbg_dm; float* dbg_terms; float* dbg_margin; uint8_t* dbg_acc;

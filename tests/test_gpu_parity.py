@@ -38,6 +38,18 @@ def _np(ts):
     return [t.detach().cpu().numpy().astype(np.float64) for t in ts]
 
 
+class _env:
+    """Set an environment variable for the duration of a block (the library reads its A/B knobs when a context / plan is created)."""
+    def __init__(self, key, val): self.key, self.val = key, val
+    def __enter__(self):
+        import os
+        self.old = os.environ.get(self.key); os.environ[self.key] = self.val
+    def __exit__(self, *a):
+        import os
+        if self.old is None: os.environ.pop(self.key, None)
+        else: os.environ[self.key] = self.old
+
+
 STATS = []          # (worst term error, worst total error, worst margin error) per checked pass, in units of their bars
 
 
@@ -209,16 +221,42 @@ def _check_iteration(wl, g, o, label):
 @pytest.mark.parametrize("name", ["cfg1_paper_regime", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150",
                                   "fe_film_cubic_48x40x3", "cfg4_k2_30x21x3", "cfg4_periodic_xyz_16x12x4", "cfg4_periodic_z_15x9x2",
                                   "cfg2_periodic_y_37x20", "cfg3_periodic_dmi_2x2", "cfg1_periodic_2x6"])
-def test_sweep_matches_replayed_oracle(name):
+@pytest.mark.parametrize("cells", ["two_cells_per_thread", "one_cell_per_thread"])
+def test_sweep_matches_replayed_oracle(name, cells):
     """mmc_sweep(n) (demag -> red -> black -> counter++) against the oracle replaying the same iteration, each side with its
     own demag field.  Every active cell must hold the oracle's accepted or rejected candidate, and every cell whose decision
-    differs must be a near-margin decision by the oracle's own margin (or a black neighbour of a red one)."""
+    differs must be a near-margin decision by the oracle's own margin (or a black neighbour of a red one).  With both pass
+    kernels: grids of fewer CTAs than SMs -- every mesh here -- take the one-cell-per-thread kernel by default, the paper-sized
+    meshes the two-cell kernel (MMC_PASS1_BELOW, include/mmc.h)."""
     wl = CASES[name]()
     wl.adaptive_cone = False
-    g, o = _gpu(wl), _orc(wl)
+    with _env("MMC_PASS1_BELOW", "0" if cells == "two_cells_per_thread" else "1000000"):
+        g = _gpu(wl)
+    o = _orc(wl)
     _check_iteration(wl, g, o, name)
     assert g.observables()["sweeps_done"] == 1
     g.close()
+
+
+@pytest.mark.parametrize("name", ["cfg2_64x48", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_48x40x4", "cfg4_30x21x3", "cfg5_160x150",
+                                  "fe_film_cubic_48x40x3", "cfg4_periodic_xyz_16x12x4", "cfg2_periodic_y_37x20", "cfg1_ragged_40x24"])
+def test_pass_kernels_with_one_and_two_cells_per_thread_agree_bitwise(name):
+    """Same cell arithmetic in both kernels: states, counters, cone and energies agree bit for bit after 25 iterations; the
+    running means to their fixed-point quantum (the two-cell kernel rounds the sum of a thread's pair, the other every cell)."""
+    wl = CASES[name]()
+    wl.adaptive_cone = True
+    with _env("MMC_PASS1_BELOW", "0"):
+        a = _gpu(wl)
+    with _env("MMC_PASS1_BELOW", "1000000"):
+        b = _gpu(wl)
+    a.sweep(25); b.sweep(25)
+    ma, mb = a.get_m(), b.get_m()
+    assert all(bool((ma[q] == mb[q]).all()) for q in range(3))
+    oa, ob = a.observables(), b.observables()
+    for k in ("accepted", "trials", "sweeps_done", "cone_deg", "run_sweeps", "E_ex", "E_an", "E_demag", "E_long"):
+        assert oa[k] == ob[k], k
+    assert abs(oa["run_mean_len"] - ob["run_mean_len"]) < 2.0 ** -22 and np.abs(oa["run_mean_m"] - ob["run_mean_m"]).max() < 2.0 ** -22
+    a.close(); b.close()
 
 
 def test_cfg1_as_written_1000_sweeps_in_lockstep():
@@ -389,18 +427,6 @@ def test_demag_more_than_16_layers_is_a_clean_error():
     g.sweep(2)                                                        # the context still works without demag
     assert g.observables()["trials"] == 2 * 272
     g.close()
-
-
-class _env:
-    """Set an environment variable for the duration of a block (the library reads its A/B knobs when a context / plan is created)."""
-    def __init__(self, key, val): self.key, self.val = key, val
-    def __enter__(self):
-        import os
-        self.old = os.environ.get(self.key); os.environ[self.key] = self.val
-    def __exit__(self, *a):
-        import os
-        if self.old is None: os.environ.pop(self.key, None)
-        else: os.environ[self.key] = self.old
 
 
 @pytest.mark.parametrize("shape,d", [((256, 256, 1), (5e-9, 5e-9, 5e-9)), ((301, 67, 3), (2e-9, 3e-9, 4e-9)), ((512, 72, 2), (3e-9, 3e-9, 3e-9)),
