@@ -727,6 +727,17 @@ columns_fast_kernel(const ColFastArgs a)
         fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
     }
 #endif
+    // MMC_COLS_NH_CS=1: the tensor spectrum, read once per convolution, as streaming (evict-first) loads so that it does not push the
+    // layers, which the Pz CTAs of a kx re-read, out of L2.  Measured: cfg 6 (10 layers, Pz = 19) 0.314 -> 0.305 ms, cfg 4 (Pz = 7)
+    // 0.240 -> 0.247 ms: off.
+#ifndef MMC_COLS_NH_CS
+#define MMC_COLS_NH_CS 0
+#endif
+#if MMC_COLS_NH_CS
+#define NH_LD(p) __ldcs(p)
+#else
+#define NH_LD(p) __ldg(p)
+#endif
     // S2: B^ = K^ M^ (see columns_kernel); slot e of thread tid reads the permuted spectrum at e*T + tid
     {
         const int kzs = (2 * kz <= a.Pz) ? kz : a.Pz - kz;
@@ -736,14 +747,14 @@ columns_fast_kernel(const ColFastArgs a)
 #pragma unroll
         for (int e = 0; e < 16; ++e) {
             const float2 u = v[0][e], w1 = v[1][e], w = v[2][e];
-            const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T),
-                        zz = __ldg(a.nhat[2] + nb + e * T), xy = __ldg(a.nhat[3] + nb + e * T);
+            const float xx = NH_LD(a.nhat[0] + nb + e * T), yy = NH_LD(a.nhat[1] + nb + e * T),
+                        zz = NH_LD(a.nhat[2] + nb + e * T), xy = NH_LD(a.nhat[3] + nb + e * T);
             float2 ox, oy, oz;
             ox.x = fmaf(xx, u.x, xy * w1.x); ox.y = fmaf(xx, u.y, xy * w1.y);
             oy.x = fmaf(xy, u.x, yy * w1.x); oy.y = fmaf(xy, u.y, yy * w1.y);
             oz.x = zz * w.x;                 oz.y = zz * w.y;
             if (three_d) {
-                const float xz = sg * __ldg(a.nhat[4] + nb + e * T), yz = sg * __ldg(a.nhat[5] + nb + e * T);
+                const float xz = sg * NH_LD(a.nhat[4] + nb + e * T), yz = sg * NH_LD(a.nhat[5] + nb + e * T);
                 ox.x = fmaf(xz, w.x, ox.x); ox.y = fmaf(xz, w.y, ox.y);
                 oy.x = fmaf(yz, w.x, oy.x); oy.y = fmaf(yz, w.y, oy.y);
                 oz.x = fmaf(xz, u.x, fmaf(yz, w1.x, oz.x)); oz.y = fmaf(xz, u.y, fmaf(yz, w1.y, oz.y));
@@ -751,6 +762,7 @@ columns_fast_kernel(const ColFastArgs a)
             v[0][e] = ox; v[1][e] = oy; v[2][e] = oz;
         }
     }
+#undef NH_LD
     __syncthreads();                                   // every thread is done reading exchange buffer 2
 #if MMC_COLS_ROLL
 #pragma unroll 1
@@ -966,7 +978,13 @@ __global__ void __launch_bounds__(256) z_inverse_kernel(const float2* __restrict
     __shared__ float2 w[PZ];                               // exp(+2 pi i q / Pz)
     if (threadIdx.x < PZ) { const float2 r = fftr::root(threadIdx.x, PZ); w[threadIdx.x] = make_float2(r.x, -r.y); }
     __syncthreads();
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < plane; i += (size_t)gridDim.x * blockDim.x) {
+#ifndef MMC_ZINV_REVERSE
+#define MMC_ZINV_REVERSE 1
+#endif
+    for (size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i0 < plane; i0 += (size_t)gridDim.x * blockDim.x) {
+        // from the end of the planes backwards: the columns kernel wrote them in ascending kx, so their tail is what L2 still holds
+        // (cfg 4: 45.8 -> 44.0 us, measured twice each way)
+        const size_t i = MMC_ZINV_REVERSE ? plane - 1 - i0 : i0;
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
             float2 x[PZ];
