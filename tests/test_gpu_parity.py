@@ -181,6 +181,10 @@ CASES = {
     "cfg2_periodic_y_37x20": lambda: _with_pbc(W.cfg2(nx=37, ny=20), 0b010),
     "cfg3_periodic_dmi_2x2": lambda: W.cfg3(nx=2, ny=2, T=200.0),
     "cfg1_periodic_2x6": lambda: W.cfg1(nx=2, ny=6, paper_regime=True),
+    # periodic in x with an ODD compact row length (nx/2 = 5, 7): the wrap neighbour of a row's last cell does not pair up, so these
+    # meshes always take the one-cell-per-thread kernel (launch_variant, "pairable")
+    "cfg1_periodic_odd_rows_10x6": lambda: W.cfg1(nx=10, ny=6, paper_regime=True),
+    "cfg3_periodic_dmi_odd_rows_14x10": lambda: W.cfg3(nx=14, ny=10, T=200.0),
 }
 
 
@@ -220,7 +224,8 @@ def _check_iteration(wl, g, o, label):
 
 @pytest.mark.parametrize("name", ["cfg1_paper_regime", "cfg2_ragged_37x19", "cfg3_64x64_200K", "cfg4_30x21x3", "cfg5_160x150",
                                   "fe_film_cubic_48x40x3", "cfg4_k2_30x21x3", "cfg4_periodic_xyz_16x12x4", "cfg4_periodic_z_15x9x2",
-                                  "cfg2_periodic_y_37x20", "cfg3_periodic_dmi_2x2", "cfg1_periodic_2x6"])
+                                  "cfg2_periodic_y_37x20", "cfg3_periodic_dmi_2x2", "cfg1_periodic_2x6", "cfg1_periodic_odd_rows_10x6",
+                                  "cfg3_periodic_dmi_odd_rows_14x10"])
 @pytest.mark.parametrize("cells", ["two_cells_per_thread", "one_cell_per_thread"])
 def test_sweep_matches_replayed_oracle(name, cells):
     """mmc_sweep(n) (demag -> red -> black -> counter++) against the oracle replaying the same iteration, each side with its
@@ -414,6 +419,26 @@ def test_demag_field_parity_degenerate_and_oversize_meshes(shape, d):
     for a in range(3):
         assert np.abs(bg[a] - bo[a]).max() <= 2e-5 * scale
     g.close()
+
+
+@pytest.mark.parametrize("shape", [(256, 256, 1), (100, 200, 1), (200, 70, 1), (1024, 65, 1)])
+def test_split_and_unsplit_planar_columns_kernel_agree_bitwise(shape):
+    """One-layer meshes: the in-plane pair and the z component of the columns kernel in one CTA (MMC_COLS_SPLIT=0) or in two (=1; the
+    default below two CTAs per SM): the same arithmetic per element, so the same bits."""
+    import paper_2106_05593_b200 as P
+    nx, ny, nz = shape; N = nx * ny * nz
+    rng = np.random.default_rng(N + 11)
+    v = rng.normal(size=(3, N)); v /= np.linalg.norm(v, axis=0)
+    m0 = (v * rng.uniform(0.3, 1.0, N)).astype(np.float32)
+    out = []
+    for split in ("0", "1"):
+        with _env("MMC_COLS_SPLIT", split):
+            g = P.MMC(nx, ny, nz, 5e-9, 5e-9, 5e-9, 0)
+            g.set_material([P.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)]); g.set_temperature(300.0); g.set_m(*m0)
+            out.append([b.clone() for b in g.demag_field()])
+            g.close()
+    assert all(torch.equal(out[0][a], out[1][a]) for a in range(3))
+    assert float(out[0][2].abs().max()) > 0.1
 
 
 def test_demag_more_than_16_layers_is_a_clean_error():
