@@ -283,15 +283,24 @@ __device__ __forceinline__ void pass_tail(const SweepArgs& a, PassTailSmem& sm, 
         __threadfence_block();
         if (atomicAdd(&sm.arrived, 1u) == (unsigned)(warps - 1)) {      // last warp of the block
             __threadfence_block();
-            const unsigned tc = atomicAdd(&sm.cnt[1], 0u);
+            // This one thread keeps the CTA's slot (registers, shared memory) occupied after every other warp has retired, so
+            // its path is kept short: the block's totals by ten independent volatile loads (the fence and the arrival counter
+            // order them after every warp's shared atomics; reading them back with atomicAdd(.., 0) was a chain of ten
+            // round trips: cfg 4 0.4972 -> 0.4952 ms per iteration, cfg 5 0.3721 -> 0.3700), then six global reductions that
+            // nobody waits for.  (Sharding those six targets over 64 lines was measured on top and brought nothing on cfg 4 / 6.)
+            const volatile unsigned* vc = sm.cnt;
+            const volatile unsigned* vs = &sm.sum[0][0];
+            const unsigned tc = vc[1], ac = vc[0];
+            const unsigned s00 = vs[0], s01 = vs[1], s02 = vs[2], s03 = vs[3], s10 = vs[4], s11 = vs[5], s12 = vs[6], s13 = vs[7];
             if (tc) {
                 atomicAdd(&a.ctl->win_trials, (unsigned long long)tc);
-                const unsigned ac = atomicAdd(&sm.cnt[0], 0u);
                 if (ac) atomicAdd(&a.ctl->win_accepted, (unsigned long long)ac);
-                if (want_sums)                         // sign-extend the two 32-bit two's-complement halves
-                    for (int t = 0; t < 4; ++t)
-                        atomicAdd(&a.run_sums[t], (unsigned long long)((long long)(int)atomicAdd(&sm.sum[0][t], 0u) +
-                                                                       (long long)(int)atomicAdd(&sm.sum[1][t], 0u)));
+                if (want_sums) {                       // sign-extend the two 32-bit two's-complement halves
+                    atomicAdd(&a.run_sums[0], (unsigned long long)((long long)(int)s00 + (long long)(int)s10));
+                    atomicAdd(&a.run_sums[1], (unsigned long long)((long long)(int)s01 + (long long)(int)s11));
+                    atomicAdd(&a.run_sums[2], (unsigned long long)((long long)(int)s02 + (long long)(int)s12));
+                    atomicAdd(&a.run_sums[3], (unsigned long long)((long long)(int)s03 + (long long)(int)s13));
+                }
             }
             finish_sweep_ticket(a);
         }
