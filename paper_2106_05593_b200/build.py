@@ -42,7 +42,7 @@ def _flags_changed() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     force = _flags_changed() or force
-    hdrs = [os.path.join(CSRC, h) for h in ("mmc_internal.h", "fft_reg.cuh", "fft_smem.cuh")] + [os.path.join(HERE, "..", "include", "mmc.h")]
+    hdrs = [os.path.join(CSRC, h) for h in ("mmc_internal.h", "fft_reg.cuh", "fft_reg8.cuh", "fft_smem.cuh")] + [os.path.join(HERE, "..", "include", "mmc.h")]
     objs = []
     jobs = []
     for f in CU + CPP:

@@ -32,6 +32,7 @@
 #include <cstdlib>
 
 #include "fft_reg.cuh"
+#include "fft_reg8.cuh"
 #include "fft_smem.cuh"
 #include "mmc_internal.h"
 
@@ -58,6 +59,8 @@ struct DemagPlan {
     float2* U = nullptr;             // fastA with nz > 1: [3][nz][Cx][ny], the layers before the z-DFT and after its inverse
     float* nhat[6] = { nullptr, nullptr, nullptr, nullptr, nullptr, nullptr };   // [Pz/2+1][Cx][Py], position order in y
     // layer-pair columns kernel (several layers, no z transform): U is transformed in place, T and nhat do not exist
+    bool cols8 = false;              // several layers, Py in 2^10 .. 2^12: columns8_kernel (8 points per thread, fft_reg8.cuh)
+    float2* tw8 = nullptr;           // its twiddle table (fftr8::Shape::NTW entries)
     bool planar_split = false;       // one layer, fewer than two columns CTAs per SM: in-plane pair and z component in separate CTAs
     bool lp = false;
     int lpG = 1;                     // kx per CTA
@@ -99,7 +102,9 @@ __global__ void permute_kernel(const double2* __restrict__ spec, float* __restri
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
         const int p = (int)(t % Py); const long long r = t / Py; const int kx = (int)(r % Cx), kz = (int)(r / Cx);
         // fast path: slot e of thread tid sits at p = e * (Py/16) + tid
-        const int ky = fast_lg ? fftr::freq_of_slot(fast_lg, p % (Py >> 4), p / (Py >> 4)) : fft::freq_of_pos(py, p);
+        // eight-point path: slot e of thread tid sits at p = e * (Py/8) + tid
+        const int ky = fast_lg < 0 ? fftr8::freq_of_slot8(-fast_lg, p % (Py >> 3), p / (Py >> 3))
+                     : fast_lg ? fftr::freq_of_slot(fast_lg, p % (Py >> 4), p / (Py >> 4)) : fft::freq_of_pos(py, p);
         const double2 z = spec[((long long)kz * Py + ky) * Cx + kx];
         out[t] = (float)(scale * (imag ? z.y : z.x));
     }
@@ -689,6 +694,13 @@ columns_fast_kernel(const ColFastArgs a)
 #ifndef MMC_COLS_ROLL
 #define MMC_COLS_ROLL 0
 #endif
+    // MMC_COLS_ROOT2 (default on): the constant roots inside the radix-16 butterflies of the three-component transforms as packed
+    // FMUL2 + FFMA2 (fft::mul_root<.., P2>; same bits).  cfg 4 columns 0.2341 -> 0.2278 ms, cfg 6 0.3047 -> 0.2980; the one-layer
+    // PLANAR instantiation (128-register cap at Py = 4096) spills with it (cfg 5 0.1457 -> 0.1522 ms) and the rows kernels do not
+    // change, so only this branch uses it
+#ifndef MMC_COLS_ROOT2
+#define MMC_COLS_ROOT2 1
+#endif
     // MMC_COLS_ROLL (measured and dropped, kept as a build knob): one copy of each transform in the instruction stream (the loops
     // over the components are not unrolled, the three register arrays rotate instead), against the 14 % of the warp cycles that
     // the 79 KB straight-line version stalls on instruction fetch: cfg 4 columns 0.265 ms rolled against 0.242 ms straight
@@ -724,7 +736,7 @@ columns_fast_kernel(const ColFastArgs a)
                 v[c][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
             }
         }
-        fftr::forward<LGN, HALF, true>(v[c], s1, s2, tw, tid);
+        fftr::forward<LGN, HALF, true, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[c], s1, s2, tw, tid);
     }
 #endif
     // MMC_COLS_NH_CS=1: the tensor spectrum, read once per convolution, as streaming (evict-first) loads so that it does not push the
@@ -780,7 +792,7 @@ columns_fast_kernel(const ColFastArgs a)
 #else
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        fftr::inverse<LGN, true>(v[c], s1, s2, tw, tid);
+        fftr::inverse<LGN, true, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[c], s1, s2, tw, tid);
         float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
         for (int n1 = 0; n1 < NL; ++n1) {
@@ -789,6 +801,125 @@ columns_fast_kernel(const ColFastArgs a)
         }
     }
 #endif
+}
+
+// kernel B, eight points per thread (fft_reg8.cuh), several layers: the z-DFT path of columns_fast_kernel with T = Py/8 threads per
+// (kx, kz) column set and 48 data registers per thread instead of 96.  grid (Pz, Cx), block T.  ColFastArgs::tw1 is the
+// fftr8 twiddle table; the tensor spectrum is stored in fftr8's slot order (slot e of thread tid at e*T + tid).
+#ifndef MMC_COLS8_MINB
+#define MMC_COLS8_MINB 2
+#endif
+template <int LGN, bool HALF>
+__global__ void __launch_bounds__(fftr8::Shape<LGN>::T, fftr8::Shape<LGN>::T >= 512 ? 1 : MMC_COLS8_MINB)
+columns8_kernel(const ColFastArgs a)
+{
+    pdl_enter();
+    using S = fftr8::Shape<LGN>;
+    constexpr int N = S::N, T = S::T, NL = HALF ? 4 : 8;
+    extern __shared__ float2 sm[];
+    float2* s1 = sm;
+    float2* s2 = sm + S::BUF;
+    const int tid = threadIdx.x;
+    const int kz = blockIdx.x, kx = blockIdx.y;        // kz fastest: the Pz CTAs of one kx find the layers in L2
+    const int ny = a.ny;
+    const float2* __restrict__ tw = a.tw1;
+    float2 v[3][8];
+    // S1, z direction: plane kz of the length-Pz DFT over the nz layers, X[kz] = sum_k w^(k kz) x[k], w = exp(-2 pi i / Pz)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz) * a.Cx + kx) * ny;
+#pragma unroll
+        for (int n1 = 0; n1 < NL; ++n1) {
+            const int j = tid + n1 * T;
+            v[c][n1] = (HALF || j < ny) ? col[j] : make_float2(0.f, 0.f);
+        }
+    }
+    const float2 wz = fftr::root(kz, a.Pz);
+    float2 wk = wz;
+    if constexpr (HALF) {
+        // the upper halves of the register arrays (the implied zero padding) carry the next layer's values, requested right
+        // after the previous layer's values of the same component have been consumed
+        if (a.nz > 1) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + 1) * a.Cx + kx) * ny;
+#pragma unroll
+                for (int n1 = 0; n1 < 4; ++n1) v[c][4 + n1] = col[tid + n1 * T];
+            }
+        }
+        for (int k = 1; k < a.nz; ++k) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                for (int n1 = 0; n1 < 4; ++n1) {
+                    const float2 x = v[c][4 + n1];
+                    v[c][n1].x = fmaf(wk.x, x.x, fmaf(-wk.y, x.y, v[c][n1].x));
+                    v[c][n1].y = fmaf(wk.x, x.y, fmaf(wk.y, x.x, v[c][n1].y));
+                }
+                if (k + 1 < a.nz) {
+                    const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + k + 1) * a.Cx + kx) * ny;
+#pragma unroll
+                    for (int n1 = 0; n1 < 4; ++n1) v[c][4 + n1] = col[tid + n1 * T];
+                }
+            }
+            wk = fft::cmul(wk, wz);
+        }
+    } else {
+        for (int k = 1; k < a.nz; ++k) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const float2* __restrict__ col = a.Tin + ((size_t)(c * a.nz + k) * a.Cx + kx) * ny;
+#pragma unroll
+                for (int n1 = 0; n1 < 8; ++n1) {
+                    const int j = tid + n1 * T;
+                    if (j < ny) {
+                        const float2 x = col[j];
+                        v[c][n1].x = fmaf(wk.x, x.x, fmaf(-wk.y, x.y, v[c][n1].x));
+                        v[c][n1].y = fmaf(wk.x, x.y, fmaf(wk.y, x.x, v[c][n1].y));
+                    }
+                }
+            }
+            wk = fft::cmul(wk, wz);
+        }
+    }
+    const int kzs = (2 * kz <= a.Pz) ? kz : a.Pz - kz;
+    const float sg = (2 * kz <= a.Pz) ? 1.f : -1.f;
+    const size_t nb = ((size_t)kzs * a.Cx + kx) * N + tid;
+#pragma unroll
+    for (int q = 0; q < 6; ++q) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.nhat[q] + nb + e * T));
+    }
+    fftr8::forward<LGN, HALF>(v[0], s1, s2, tw, tid);
+    fftr8::forward<LGN, HALF>(v[1], s2, s1, tw, tid);
+    fftr8::forward<LGN, HALF>(v[2], s1, s2, tw, tid);
+    // S2: B^ = K^ M^ (see columns_kernel)
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+        const float2 u = v[0][e], w1 = v[1][e], w = v[2][e];
+        const float xx = __ldg(a.nhat[0] + nb + e * T), yy = __ldg(a.nhat[1] + nb + e * T), zz = __ldg(a.nhat[2] + nb + e * T),
+                    xy = __ldg(a.nhat[3] + nb + e * T), xz = sg * __ldg(a.nhat[4] + nb + e * T), yz = sg * __ldg(a.nhat[5] + nb + e * T);
+        float2 ox, oy, oz;
+        ox.x = fmaf(xx, u.x, xy * w1.x); ox.y = fmaf(xx, u.y, xy * w1.y);
+        oy.x = fmaf(xy, u.x, yy * w1.x); oy.y = fmaf(xy, u.y, yy * w1.y);
+        oz.x = zz * w.x;                 oz.y = zz * w.y;
+        ox.x = fmaf(xz, w.x, ox.x); ox.y = fmaf(xz, w.y, ox.y);
+        oy.x = fmaf(yz, w.x, oy.x); oy.y = fmaf(yz, w.y, oy.y);
+        oz.x = fmaf(xz, u.x, fmaf(yz, w1.x, oz.x)); oz.y = fmaf(xz, u.y, fmaf(yz, w1.y, oz.y));
+        v[0][e] = ox; v[1][e] = oy; v[2][e] = oz;
+    }
+    __syncthreads();                                   // every thread is done reading the exchange buffers
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        if (c == 1) fftr8::inverse<LGN>(v[c], s2, s1, tw, tid);
+        else        fftr8::inverse<LGN>(v[c], s1, s2, tw, tid);
+        float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
+#pragma unroll
+        for (int n1 = 0; n1 < NL; ++n1) {
+            const int j = tid + n1 * T;
+            if (HALF || j < ny) col[j] = v[c][n1];
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ kernel B, layer-pair variant
@@ -1102,8 +1233,34 @@ static int launch_columns_lp_any(const DemagPlan* p, const ColLPArgs& la, cudaSt
     }
 }
 
+template <int LGN>
+static int launch_columns8(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
+{
+    using S = fftr8::Shape<LGN>;
+    const size_t smem = (size_t)S::SMEM * sizeof(float2);
+    const dim3 grid(p->Pz, p->Cx), block(S::T);
+    if (2 * p->g.ny == p->Py) {
+        auto kern = columns8_kernel<LGN, true>;
+        if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+        launch_pdl(kern, dim3(grid), dim3(block), (size_t)(smem), st, ca);
+    } else {
+        auto kern = columns8_kernel<LGN, false>;
+        if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+        launch_pdl(kern, dim3(grid), dim3(block), (size_t)(smem), st, ca);
+    }
+    return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
+}
+
 static int launch_columns_fast_any(const DemagPlan* p, const ColFastArgs& ca, cudaStream_t st)
 {
+    if (p->cols8) {
+        switch (ilog2(p->Py)) {
+            case 10: return launch_columns8<10>(p, ca, st);
+            case 11: return launch_columns8<11>(p, ca, st);
+            case 12: return launch_columns8<12>(p, ca, st);
+            default: return MMC_E_UNSUPPORTED;
+        }
+    }
     switch (ilog2(p->Py)) {
         case 8: return launch_columns_fast<8>(p, ca, st);
         case 9: return launch_columns_fast<9>(p, ca, st);
@@ -1216,6 +1373,21 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
             if (lp_smem_bytes_any(ilog2(p->Py), g.nz, p->lpG) > 227 * 1024) p->lp = false;      // does not fit one SM: the z-DFT path
         }
     }
+#ifndef MMC_DEMAG_COLS8
+#define MMC_DEMAG_COLS8 0
+#endif
+    {
+        // eight points per thread in the columns kernel of the z-DFT path (MMC_COLS8=0/1 forces the choice)
+        const int lgPy = ilog2(p->Py);
+        const char* e = std::getenv("MMC_COLS8");
+        const bool on = e ? e[0] == '1' : (MMC_DEMAG_COLS8 != 0);
+        p->cols8 = on && !p->lp && p->fastA && p->fastB && g.nz > 1 && lgPy >= fftr8::kMinLg && lgPy <= fftr8::kMaxLg && p->Cx <= 65535;
+        if (p->cols8) {
+            const int ntw = 7 * (p->Py / 8 + p->Py / 64 + p->Py / 512);
+            CK(cudaMalloc(&p->tw8, (size_t)ntw * sizeof(float2)));
+            fftr8::twiddle_tables8_kernel<<<blocks_for(ntw), 256, 0, st>>>(p->tw8, lgPy);
+        }
+    }
     const size_t nT = (size_t)3 * p->Pz * p->Cx * g.ny;
     if (!p->lp) CK(cudaMalloc(&p->T, nT * sizeof(float2)));
     if (p->fastA && g.nz > 1) CK(cudaMalloc(&p->U, (size_t)3 * g.nz * p->Cx * g.ny * sizeof(float2)));
@@ -1281,7 +1453,8 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
         CK(cudaMemcpyAsync(d_oct, oct[q].data(), nO * sizeof(double), cudaMemcpyHostToDevice, st));
         place_kernel<<<blocks_for((long long)rsize), 256, 0, st>>>(g.nx, g.ny, g.nz, p->Px, p->Py, p->Pz, d_oct, SX[q], SY[q], SZ[q], d_full);
         CF(cufftExecD2Z(pd, d_full, (cufftDoubleComplex*)d_spec));
-        permute_kernel<<<blocks_for((long long)nN), 256, 0, st>>>(d_spec, p->nhat[q], p->Cx, p->Py, Kz, p->py, scale, p->fastB ? ilog2(p->Py) : 0);
+        permute_kernel<<<blocks_for((long long)nN), 256, 0, st>>>(d_spec, p->nhat[q], p->Cx, p->Py, Kz, p->py, scale,
+                                                                  p->cols8 ? -ilog2(p->Py) : p->fastB ? ilog2(p->Py) : 0);
         CK(cudaStreamSynchronize(st));                       // oct[q] host buffer must outlive the copy
     }
     cufftDestroy(pd);
@@ -1297,7 +1470,7 @@ int demag_create(DemagPlan** out, const Geometry& g, double dx, double dy, doubl
 void demag_destroy(DemagPlan* p)
 {
     if (!p) return;
-    cudaFree(p->T); cudaFree(p->U); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2); 
+    cudaFree(p->T); cudaFree(p->U); cudaFree(p->twx); cudaFree(p->twy); cudaFree(p->twB1); cudaFree(p->twB2); cudaFree(p->tw8);
     for (int q = 0; q < 6; ++q) { cudaFree(p->nhat[q]); cudaFree(p->nh2[q]); }
     delete p;
 }
@@ -1347,6 +1520,7 @@ int demag_compute(DemagPlan* p, const float* const m[3], const float* Ms0_split,
         ColFastArgs fa{};
         fa.ny = p->g.ny; fa.Cx = p->Cx; fa.Pz = p->Pz; fa.nz = p->U ? p->g.nz : 0; fa.tw1 = p->twB1; fa.tw2 = p->twB2;
         fa.Tin = p->U ? p->U : p->T; fa.Tout = p->T;
+        if (p->cols8) fa.tw1 = p->tw8;
         for (int q = 0; q < 6; ++q) fa.nhat[q] = p->nhat[q];
         rc = launch_columns_fast_any(p, fa, st);
         if (rc) { if (err) *err = "columns_fast_kernel launch failed"; return rc; }

@@ -112,7 +112,7 @@ struct GroupSync {
     __device__ __forceinline__ void operator()() const { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 };
 
-template <int LGN, bool HALF, int TABLE, class Sync = BlockSync>
+template <int LGN, bool HALF, int TABLE, class Sync = BlockSync, bool P2 = false>
 __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
                                         const Twiddles& tw, int tid, const Sync& sync = Sync())
 {
@@ -120,10 +120,10 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
     constexpr int T = S::T, R3 = S::R3;
     if (HALF) {                                   // first butterfly level with a zero upper half
 #pragma unroll
-        for (int k = 0; k < 8; ++k) v[k + 8] = fft::mul_root<16, false>(v[k], k);
-        fft::dif<8, false>(v); fft::dif<8, false>(v + 8);
+        for (int k = 0; k < 8; ++k) v[k + 8] = fft::mul_root<16, false, P2>(v[k], k);
+        fft::dif<8, false, P2>(v); fft::dif<8, false, P2>(v + 8);
     } else {
-        fft::dif<16, false>(v);
+        fft::dif<16, false, P2>(v);
     }
     {
         float2 pw[15];
@@ -144,7 +144,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
 #pragma unroll
         for (int t1 = 0; t1 < 16; ++t1) v[t1] = r1[t1 * R3];
     }
-    fft::dif<16, false>(v);
+    fft::dif<16, false, P2>(v);
     if constexpr (R3 > 1) {
         float2* d2 = s2 + u * S::U + 17 * q1;
         if constexpr (TABLE == 2) stage_twiddles<T, TABLE>(tw.w2, tw.t2, tid, pw2);      // shared-memory table: fetched where it is used
@@ -162,7 +162,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
             float2 x[R3];
 #pragma unroll
             for (int uu = 0; uu < R3; ++uu) x[uu] = r2[uu * S::U + i * (T + R3)];
-            fft::dif<R3, false>(x);
+            fft::dif<R3, false, P2>(x);
 #pragma unroll
             for (int q = 0; q < R3; ++q) v[i * R3 + q] = x[fft::bitrev<R3>(q)];
         }
@@ -177,7 +177,7 @@ __device__ __forceinline__ void forward(float2 (&v)[16], float2* __restrict__ s1
 }
 
 // the mirror: v[e] = Y[freq_of_slot(tid, e)] on entry, v[n1] = N * y[tid + n1*T] on exit
-template <int LGN, int TABLE, class Sync = BlockSync>
+template <int LGN, int TABLE, class Sync = BlockSync, bool P2 = false>
 __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1, float2* __restrict__ s2,
                                         const Twiddles& tw, int tid, const Sync& sync = Sync())
 {
@@ -192,7 +192,7 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
             float2 x[R3];
 #pragma unroll
             for (int q = 0; q < R3; ++q) x[fft::bitrev<R3>(q)] = v[i * R3 + q];
-            fft::dit<R3, true>(x);
+            fft::dit<R3, true, P2>(x);
 #pragma unroll
             for (int uu = 0; uu < R3; ++uu) d2[uu * S::U + i * (T + R3)] = x[uu];
         }
@@ -211,7 +211,7 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
 #pragma unroll
         for (int q = 0; q < 16; ++q) x16[fft::bitrev<16>(q)] = v[q];
     }
-    fft::dit<16, true>(x16);
+    fft::dit<16, true, P2>(x16);
     {
         float2* d1 = s1 + q1 * (T + 1) + u;
 #pragma unroll
@@ -229,7 +229,7 @@ __device__ __forceinline__ void inverse(float2 (&v)[16], float2* __restrict__ s1
             v[fft::bitrev<16>(q)] = y;
         }
     }
-    fft::dit<16, true>(v);
+    fft::dit<16, true, P2>(v);
     if constexpr (R3 == 1) sync();       // as in forward
 }
 

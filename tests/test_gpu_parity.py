@@ -510,6 +510,41 @@ def test_layer_pair_columns_kernel_parity(shape, d):
     g.close()
 
 
+@pytest.mark.parametrize("shape,d", [((130, 1024, 2), (3e-9, 3e-9, 3e-9)), ((130, 700, 3), (3e-9, 3e-9, 3e-9)), ((130, 512, 2), (3e-9, 3e-9, 3e-9)),
+                                     ((130, 300, 3), (2e-9, 3e-9, 4e-9)), ((130, 2048, 2), (3e-9, 3e-9, 3e-9)), ((130, 1100, 2), (3e-9, 3e-9, 3e-9)),
+                                     ((256, 1024, 4), (3e-9, 3e-9, 3e-9)), ((130, 1024, 7), (3e-9, 3e-9, 3e-9))])
+def test_eight_point_columns_kernel_parity(shape, d):
+    """The columns kernel with eight points per thread (MMC_COLS8=1, fft_reg8.cuh: 8 x 8 x 8 x T3 transforms of length 2^10 .. 2^12,
+    padding exactly half and ragged, 2 - 7 layers) and the default kernel (16 points per thread) on the same mesh, both against the
+    oracle's fp64 convolution at the default path's bar."""
+    import paper_2106_05593_b200 as P
+    nx, ny, nz = shape; N = nx * ny * nz
+    rng = np.random.default_rng(N + 13)
+    v = rng.normal(size=(3, N)); v /= np.linalg.norm(v, axis=0)
+    m0 = (v * rng.uniform(0.3, 1.0, N)).astype(np.float32)
+    reg = (rng.uniform(size=N) > 0.2).astype(np.int32)
+    m0[:, reg == 0] = 0
+    out = {}
+    for k in ("0", "1"):
+        with _env("MMC_COLS8", k):
+            g = P.MMC(nx, ny, nz, *d, 0)
+            g.set_material([P.Material(), P.Material(Ms0=8.6e5, A0=1.3e-11, Tc=870.0)], reg)
+            g.set_temperature(300.0); g.set_m(*m0)
+            out[k] = _np(g.demag_field())
+            if k == "1":
+                again = _np(g.demag_field())
+            g.close()
+    conv = O.DemagFFT(nx, ny, nz, *d)
+    M = [(8.6e5 * reg * m0[a].astype(np.float64)).reshape(nz, ny, nx) for a in range(3)]
+    bo = [b.ravel() for b in conv.field(*M)]
+    scale = max(np.abs(b).max() for b in bo)
+    for a in range(3):
+        assert np.abs(out["0"][a] - bo[a]).max() <= 2e-5 * scale
+        assert np.abs(out["1"][a] - bo[a]).max() <= 2e-5 * scale
+        assert np.array_equal(out["1"][a], again[a])
+    assert any(not np.array_equal(out["0"][a], out["1"][a]) for a in range(3))      # a different transform did run
+
+
 @pytest.mark.parametrize("name", ["cfg2_64x48", "cfg4_48x40x4", "cfg4_30x21x3", "cfg5_160x150"])
 def test_tma_staged_pass_is_bitwise_the_default_pass(name):
     """The TMA-staged colour pass (MMC_TMA=1: cp.async.bulk.tensor boxes into a ring of shared-memory stages, warp-specialised)
