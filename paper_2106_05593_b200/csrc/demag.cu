@@ -606,7 +606,26 @@ columns_fast_kernel(const ColFastArgs a)
     const bool live = kxr < a.Cx;                      // idle groups still walk through the barriers
     const int kx = live ? kxr : a.Cx - 1;
     const int ny = a.ny;
+#ifndef MMC_COLS_TWS
+#define MMC_COLS_TWS 0
+#endif
+    // MMC_COLS_TWS (measured and dropped, kept as a build knob): against the instruction-fetch stalls that top this kernel's list once
+    // the additions are packed (ncu: no_instruction 1.6 of 6.2 warp cycles per instruction, instruction-cache hit rate 69 %), the
+    // rolled variant (MMC_COLS_ROLL) does fit the cache (hit rate 98.6 %, no_instruction gone) but then waits on the twiddle loads it
+    // can no longer hoist across transforms (long_scoreboard 1.2 -> 3.3: 0.302 ms); with the tables in shared memory it comes to
+    // 0.258 ms rolled and 0.261 ms unrolled, against 0.228 ms for the straight-line kernel with L1-served tables (cfg 4)
+#if MMC_COLS_TWS
+    // twiddle tables in shared memory, copied once per CTA (fft_reg.cuh TABLE = 2: fetched where they are used)
+    constexpr int TW = 2;
+    float2* tws1 = sm + S::G * S::SMEM;
+    float2* tws2 = tws1 + 15 * T;
+    for (int i = threadIdx.y * T + tid; i < 15 * T; i += S::G * T) { tws1[i] = __ldg(a.tw1 + i); tws2[i] = __ldg(a.tw2 + i); }
+    __syncthreads();
+    const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), tws1, tws2 };
+#else
+    constexpr int TW = 1;
     const fftr::Twiddles tw{ make_float2(1.f, 0.f), make_float2(1.f, 0.f), a.tw1, a.tw2 };
+#endif
     float2 v[3][16];
     // all three components' columns are requested at once, and the tensor spectrum this thread will need after the
     // forward transforms is pulled into L2 meanwhile (no registers held)
@@ -718,7 +737,7 @@ columns_fast_kernel(const ColFastArgs a)
                 v[0][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
             }
         }
-        fftr::forward<LGN, HALF, true>(v[0], s1, s2, tw, tid);
+        fftr::forward<LGN, HALF, TW, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[0], s1, s2, tw, tid);
 #pragma unroll
         for (int e = 0; e < 16; ++e) { const float2 t0 = v[0][e]; v[0][e] = v[1][e]; v[1][e] = v[2][e]; v[2][e] = t0; }
     }
@@ -736,7 +755,7 @@ columns_fast_kernel(const ColFastArgs a)
                 v[c][n1] = (j < ny) ? col[j] : make_float2(0.f, 0.f);
             }
         }
-        fftr::forward<LGN, HALF, true, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[c], s1, s2, tw, tid);
+        fftr::forward<LGN, HALF, TW, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[c], s1, s2, tw, tid);
     }
 #endif
     // MMC_COLS_NH_CS=1: the tensor spectrum, read once per convolution, as streaming (evict-first) loads so that it does not push the
@@ -779,7 +798,7 @@ columns_fast_kernel(const ColFastArgs a)
 #if MMC_COLS_ROLL
 #pragma unroll 1
     for (int c = 0; c < 3; ++c) {
-        fftr::inverse<LGN, true>(v[0], s1, s2, tw, tid);
+        fftr::inverse<LGN, TW, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[0], s1, s2, tw, tid);
         float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
         for (int n1 = 0; n1 < NL; ++n1) {
@@ -792,7 +811,7 @@ columns_fast_kernel(const ColFastArgs a)
 #else
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-        fftr::inverse<LGN, true, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[c], s1, s2, tw, tid);
+        fftr::inverse<LGN, TW, fftr::BlockSync, MMC_COLS_ROOT2 != 0>(v[c], s1, s2, tw, tid);
         float2* __restrict__ col = a.Tout + ((size_t)(c * a.Pz + kz) * a.Cx + kx) * ny;
 #pragma unroll
         for (int n1 = 0; n1 < NL; ++n1) {
@@ -1173,10 +1192,15 @@ static int launch_columns_fast_h(const DemagPlan* p, const ColFastArgs& ca, cuda
         return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
     }
     auto kern = columns_fast_kernel<LGN, HALF, false>;
-    if (smem > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) return MMC_E_CUDA;
+#if defined(MMC_COLS_TWS) && MMC_COLS_TWS
+#define MMC_COLS_TWS_EXTRA ((size_t)2 * 15 * S::T * sizeof(float2))
+#else
+#define MMC_COLS_TWS_EXTRA ((size_t)0)
+#endif
+    if (smem + MMC_COLS_TWS_EXTRA > 48 * 1024 && cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(smem + MMC_COLS_TWS_EXTRA)) != cudaSuccess) return MMC_E_CUDA;
     const dim3 grid = ca.nz > 0 ? dim3(p->Pz, nbx) : dim3(nbx, p->Pz), block(S::T, S::G);
     if (grid.y > 65535u) return MMC_E_UNSUPPORTED;
-    launch_pdl(kern, dim3(grid), dim3(block), (size_t)(smem), st, ca);
+    launch_pdl(kern, dim3(grid), dim3(block), (size_t)(smem + MMC_COLS_TWS_EXTRA), st, ca);
     return cudaGetLastError() == cudaSuccess ? MMC_OK : MMC_E_CUDA;
 }
 template <int LGN>
