@@ -120,7 +120,9 @@ int mmc_get_m_host(mmc_ctx* ctx, float* mx, float* my, float* mz);
  * graphs of 16 and 1 iterations (rebuilt when a setter changes a kernel argument).  Environment knobs, read when the ctx (or
  * its demag plan) is created, for A/B measurements: MMC_NO_GRAPH (plain launches), MMC_PDL=1 (programmatic dependent launch
  * between the kernels of an iteration: measured slower, off by default), MMC_TMA=1 (TMA-staged colour pass on meshes
- * without periodic directions), MMC_LP=1 (layer-pair columns kernel of the demag convolution on multi-layer meshes), MMC_DEMAG_GENERIC=1 (the any-length
+ * without periodic directions), MMC_LP=1 (layer-pair columns kernel of the demag convolution on multi-layer meshes), MMC_COLS8=1
+ * (multi-layer meshes, padded ny 1024 .. 4096: columns kernel with eight instead of sixteen points per thread; measured slower),
+ * MMC_DEMAG_GENERIC=1 (the any-length
  * shared-memory FFT kernels of the convolution also where the register-resident ones apply: 2 - 3 times slower, for tests),
  * MMC_PASS1_BELOW=<n> (colour passes whose grid has fewer than n CTAs run one cell per thread instead of two; default 148 = the
  * SM count: 0 forces the two-cell kernel), MMC_COLS_SPLIT=0/1 (one-layer meshes: in-plane pair and z component of the columns

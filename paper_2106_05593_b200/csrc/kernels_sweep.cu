@@ -569,7 +569,7 @@ __device__ __forceinline__ void update_pair(const SweepArgs& a, int s, int row, 
 constexpr int kPass2Threads = 256;
 
 #ifndef MMC_PASS2_MINB
-#define MMC_PASS2_MINB 4      // 64 registers (48 bytes spilled): measured 4 / 3 / 2 CTAs per SM on cfg 4: 57.5 / 61 / 72 us per pass
+#define MMC_PASS2_MINB 4      // 64 registers (48 bytes spilled): measured 5 / 4 / 3 / 2 CTAs per SM on cfg 4: 74.7 (48 registers, 292 B spilled) / 57.5 / 61 / 72 us per pass
 #endif
 template <unsigned F>
 __global__ void __launch_bounds__(kPass2Threads, MMC_PASS2_MINB) colour_pass2_kernel(const SweepArgs a)
