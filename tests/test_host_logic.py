@@ -178,3 +178,17 @@ def test_bench_demag_byte_model():
     WL.nx = WL.ny = 2048; WL.nz = 1; WL.N = 2048 * 2048
     b = bench.demag_kernel_bytes(WL, True)
     assert "z_inverse" not in b and sum(v["bytes"] for v in b.values()) / WL.N == pytest.approx(156, abs=2)
+
+
+def test_every_environment_knob_is_documented():
+    """Every MMC_* environment variable the library reads is named in include/mmc.h and in README.md."""
+    import glob
+    names = set()
+    for f in glob.glob(os.path.join(ROOT, "paper_2106_05593_b200", "csrc", "*")):
+        names |= set(re.findall(r'getenv\("(MMC_[A-Z0-9_]+)"\)', open(f).read()))
+    assert len(names) >= 8
+    hdr = open(os.path.join(ROOT, "include", "mmc.h")).read()
+    readme = open(os.path.join(ROOT, "README.md")).read()
+    for n in sorted(names):
+        assert n in hdr, f"{n} is not documented in include/mmc.h"
+        assert n in readme, f"{n} is not named in README.md"
